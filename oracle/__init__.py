@@ -1,0 +1,146 @@
+"""ctypes loader for the CPU oracle (oracle/sn_oracle.cpp).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this
+package.  It imports nothing from paper_1507_08549_b200 and the product never imports it.
+Argument marshalling only: every number comes out of sn_oracle.cpp.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sn_oracle.cpp")
+_LIB = os.path.join(_HERE, "libsn_oracle.so")
+CXXFLAGS = ["-O2", "-ffp-contract=off", "-mfma", "-fPIC", "-shared", "-std=c++17"]
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (single translation unit)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", *CXXFLAGS, "-o", _LIB, _SRC])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.sno_default_omega.restype = C.c_double
+        _lib.sno_default_omega.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int]
+        _lib.sno_ratio.restype = C.c_double
+        _lib.sno_ratio.argtypes = [C.c_double] * 5
+        _lib.sno_regular_harmonics.argtypes = [C.c_double, C.c_double, C.c_int, _dp]
+        _lib.sno_irregular_harmonics.argtypes = [C.c_double, C.c_double, C.c_int, _dp]
+        _lib.sno_moments.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, _dp, _dp]
+        _lib.sno_boundary.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, _dp, _dp, _dp, _dp]
+        _lib.sno_sweeps.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double, _dp, _dp, _dp,
+                                    _dp, _dp, C.c_int, _dp, _dp]
+        _lib.sno_solve.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, _dp,
+                                   _dp, C.c_double, C.c_int, C.POINTER(C.c_int), _dp, _dp, _dp, _dp, _dp]
+        _lib.sno_apply_operator.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp,
+                                            _dp, _dp]
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _f64(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a
+
+
+def default_omega(nr, nz, dr, dz, symmetry) -> float:
+    return lib().sno_default_omega(nr, nz, dr, dz, symmetry)
+
+
+def ratio(Rabs, P, maxf, dr, dz) -> float:
+    return lib().sno_ratio(Rabs, P, maxf, dr, dz)
+
+
+def regular_harmonics(x, y, lmax):
+    out = np.zeros(lmax + 2)
+    lib().sno_regular_harmonics(x, y, lmax, _p(out))
+    return out[: lmax + 1]
+
+
+def irregular_harmonics(x, y, lmax):
+    out = np.zeros(lmax + 2)
+    lib().sno_irregular_harmonics(x, y, lmax, _p(out))
+    return out[: lmax + 1]
+
+
+def moments(rho, dr, dz, symmetry, lmax):
+    rho = _f64(rho)
+    nz, nr = rho.shape
+    M = np.zeros(lmax + 1)
+    rc = lib().sno_moments(nr, nz, dr, dz, symmetry, lmax, _p(rho), _p(M))
+    assert rc == 0
+    return M
+
+
+def boundary(nr, nz, dr, dz, symmetry, lmax, M):
+    M = _f64(M)
+    bE, bN, bS = np.zeros(nz), np.zeros(nr), np.zeros(nr)
+    rc = lib().sno_boundary(nr, nz, dr, dz, symmetry, lmax, _p(M), _p(bE), _p(bN), _p(bS))
+    assert rc == 0
+    return bE, bN, (bS if symmetry == 0 else None)
+
+
+def sweeps(rho, phi, dr, dz, symmetry, omega, bE, bN, bS, nsweeps):
+    """nsweeps red-black SOR sweeps; returns (phi_new, Rabs[nsweeps], P[nsweeps])."""
+    rho = _f64(rho)
+    nz, nr = rho.shape
+    phi = np.array(phi, dtype=np.float64, order="C", copy=True)
+    bE, bN = _f64(bE), _f64(bN)
+    bS = _f64(bS) if bS is not None else np.zeros(nr)
+    Rabs, P = np.zeros(max(nsweeps, 1)), np.zeros(max(nsweeps, 1))
+    rc = lib().sno_sweeps(nr, nz, dr, dz, symmetry, omega, _p(rho), _p(bE), _p(bN), _p(bS), _p(phi), nsweeps,
+                          _p(Rabs), _p(P))
+    assert rc == 0
+    return phi, Rabs[:nsweeps], P[:nsweeps]
+
+
+def solve(rho, phi0, dr, dz, symmetry, lmax, tol, max_sweeps, omega=None, boundary_arrays=None,
+          history=False):
+    """Whole path.  Returns dict(phi, sweeps, residual, status[, hist])."""
+    rho = _f64(rho)
+    nz, nr = rho.shape
+    phi = np.array(phi0, dtype=np.float64, order="C", copy=True)
+    nsw, res = C.c_int(0), C.c_double(0.0)
+    hist = np.zeros(max(max_sweeps, 1)) if history else None
+    bE = bN = bS = None
+    if boundary_arrays is not None:
+        bE, bN, bS = boundary_arrays
+        bE, bN = _f64(bE), _f64(bN)
+        bS = _f64(bS) if bS is not None else np.zeros(nr)
+    rc = lib().sno_solve(nr, nz, dr, dz, symmetry, lmax, -1.0 if omega is None else float(omega), _p(rho),
+                         _p(phi), tol, max_sweeps, C.byref(nsw), C.byref(res), _p(hist), _p(bE), _p(bN), _p(bS))
+    out = {"phi": phi, "sweeps": nsw.value, "residual": res.value, "status": rc}
+    if history:
+        out["hist"] = hist[: nsw.value]
+    return out
+
+
+def apply_operator(phi, dr, dz, symmetry, bE, bN, bS):
+    phi = _f64(phi)
+    nz, nr = phi.shape
+    bS = _f64(bS) if bS is not None else np.zeros(nr)
+    out = np.zeros_like(phi)
+    lib().sno_apply_operator(nr, nz, dr, dz, symmetry, _p(phi), _p(_f64(bE)), _p(_f64(bN)), _p(bS), _p(out))
+    return out
+
+
+def solve_workload(w, phi0=None, history=False):
+    """Convenience: run the whole path on a workloads.Workload."""
+    phi0 = np.zeros_like(w.rho) if phi0 is None else phi0
+    return solve(w.rho, phi0, w.dr, w.dz, w.symmetry, w.lmax, w.tol, w.max_sweeps, omega=w.omega,
+                 history=history)
