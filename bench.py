@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- Poisson relaxation throughput (fp64 cell-updates/s) and time-to-residual per solve.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg3|cfg4a|sweep<N>] [--impl reference]
+
+One "step" = one pass of the whole hot path over one synthetic input: multipole moments -> boundary fill ->
+red-black SOR sweeps with the fused residual reduction until the device-side stopping rule fires (cold start,
+phi = 0), through the C ABI (sn_poisson_solve / _solve_batch).  Default workload: BASELINE.json configs[1]
+(256x256 n=1 polytrope, lmax 16, tol 1e-10).  Prints ONE JSON line (rank 0).
+
+Timing: W warm-up solves, then K solves each bracketed by CUDA events on the launching stream (the call
+synchronises that stream itself); L2 is flushed (a 256 MiB write) and phi re-zeroed between solves, outside the
+events; the K-step region is bracketed by barrier + torch.cuda.synchronize(); max over ranks.
+`--impl reference` times the CPU oracle (oracle/, single thread) on the same workload -- a deliberately slow
+program; parity and the roofline fraction are the headline, not that ratio.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as W  # noqa: E402
+
+METRIC = "poisson_relaxation_cell_updates_per_s"
+UNIT = "cell-updates/s"
+BYTES_PER_UPDATE = 24.0     # phi read + f read + phi write
+
+
+def make_workload(name: str):
+    """Returns (label, list of Workload members, description)."""
+    if name == "cfg1":
+        return "cfg1: 256x256 half-plane n=1 polytrope, lmax=16, tol=1e-10, cold start", [W.cfg1()]
+    if name == "cfg0":
+        return "cfg0: 64x64 uniform sphere, lmax=8, omega=1.9, 4000 fixed sweeps", [W.cfg0()]
+    if name == "cfg2":
+        return "cfg2: 512x512 half-plane n=3 WD + 20 bubbles, lmax=16, tol=1e-10, cold start", [W.cfg2()]
+    if name == "cfg3":
+        return "cfg3: 1024x2048 full-plane offset WD, lmax=32, tol=1e-10, cold solve (first of the sequence)", \
+            [W.cfg3().first]
+    if name == "cfg4a":
+        return "cfg4a: batch of 64 x 512x512 half-plane WDs, lmax=16, tol=1e-10, cold start", W.cfg4a(64)
+    if name.startswith("sweep"):
+        n = int(name[5:])
+        return f"cfg4b: {n}x{n} half-plane WD, lmax=16, 2000 fixed sweeps", [W.cfg4b(n, 2000)]
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nme, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+def l2_copy_peak_gbs(torch, mib=24, iters=40):
+    """L2-resident copy bandwidth (read + write bytes), measured live the way MEASURED_PEAKS.json measures HBM:
+    b.copy_(a) with a working set (2 x `mib` MiB) that stays in the 126 MB L2; best of several."""
+    n = mib * (1 << 20) // 8
+    a = torch.ones(n, dtype=torch.float64, device="cuda")
+    b = torch.empty_like(a)
+    for _ in range(5):
+        b.copy_(a)
+    best = 0.0
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(iters):
+            b.copy_(a)
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, 2.0 * n * 8 * iters / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return best
+
+
+def oracle_rate(members, budget_s=12.0):
+    """Times the oracle as it stands on 1 host core on a bounded sample; returns (cell-updates/s, description)."""
+    import oracle as O
+    O.build()
+    w = members[0]
+    full_cost = w.cells * 2000.0 / 1.0e8            # rough seconds for a full solve at ~1e8 updates/s
+    if full_cost <= budget_s:
+        t0 = time.perf_counter()
+        upd, n = 0, 0
+        while time.perf_counter() - t0 < budget_s * 0.8 or n == 0:
+            r = O.solve_workload(members[n % len(members)])
+            upd += r["sweeps"] * w.cells
+            n += 1
+        dt = time.perf_counter() - t0
+        return upd / dt, f"{n} full solve(s) of {w.name} ({w.nr}x{w.nz}, to tol {w.tol:g} / {w.max_sweeps} sweeps)"
+    nsw = max(4, int(budget_s * 1.0e8 / w.cells))
+    t0 = time.perf_counter()
+    O.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, w.symmetry, w.lmax, 0.0, nsw, omega=w.omega)
+    dt = time.perf_counter() - t0
+    return nsw * w.cells / dt, f"moments+boundary+{nsw} sweeps of {w.name} ({w.nr}x{w.nz})"
+
+
+def run_reference(args, label, members):
+    """--impl reference: the CPU oracle, single thread, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as O
+    O.build()
+    w = members[0]
+    per_step_sweeps = None
+    if w.cells * 2000.0 / 1.0e8 > 8.0:               # too slow for full solves: fixed-sweep sample per step
+        per_step_sweeps = max(4, int(4.0e8 / w.cells))
+
+    def one_step(i):
+        m = members[i % len(members)]
+        if per_step_sweeps is None:
+            r = O.solve_workload(m)
+            return r["sweeps"] * m.cells
+        O.solve(m.rho, np.zeros_like(m.rho), m.dr, m.dz, m.symmetry, m.lmax, 0.0, per_step_sweeps, omega=m.omega)
+        return per_step_sweeps * m.cells
+
+    for i in range(args.warmup):
+        one_step(i)
+    t0 = time.perf_counter()
+    upd = sum(one_step(i) for i in range(args.steps))
+    dt = time.perf_counter() - t0
+    value = upd / dt
+    sample = (f"{args.steps} full oracle solve(s)" if per_step_sweeps is None
+              else f"{args.steps} x (moments+boundary+{per_step_sweeps} sweeps)") + f" of {w.name}"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": label},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg1")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 streaming kernels, 2 resident kernel")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    label, members = make_workload(args.workload)
+    if args.impl == "reference":
+        run_reference(args, label, members)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_1507_08549_b200 as P
+    from paper_1507_08549_b200 import build as pbuild
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        pbuild.build()
+    if world > 1:
+        dist.barrier()
+    P.load()
+
+    # multi-GPU: batch members are sharded across ranks with no collective; a single solve runs as replicas
+    if len(members) >= world and len(members) > 1:
+        mine = members[rank::world]
+        scaling = "strong"
+    else:
+        mine = members
+        scaling = "weak"
+    w0 = mine[0]
+    nb = len(mine)
+    solver = P.PoissonSolver.for_workload(w0)
+    if args.path:
+        solver.set_option("path", args.path)
+    rho_h = np.stack([m.rho for m in mine]) if nb > 1 else w0.rho
+    rho = torch.from_numpy(rho_h).cuda()
+    phi = torch.zeros_like(rho)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    cells = w0.cells
+
+    def solve_dev():
+        res = solver.solve(rho, phi, w0.tol, w0.max_sweeps)
+        return res if isinstance(res, list) else [res]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        phi.zero_()
+        solve_dev()
+
+    sampler = ClockSampler(local_rank)
+    step_ms, sweep_ms, setup_ms, launches, updates = [], [], [], 0, 0
+    results = None
+    barrier()
+    sampler.start()
+    t_region = time.perf_counter()
+    for _ in range(args.steps):
+        phi.zero_()
+        flush.fill_(1)                                    # L2 flush between timed iterations
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        results = solve_dev()
+        e1.record()
+        torch.cuda.synchronize()
+        step_ms.append(e0.elapsed_time(e1))
+        sweep_ms.append(solver.stat("sweep_ms"))
+        setup_ms.append(solver.stat("setup_ms"))
+        launches += int(solver.stat("launches"))
+        updates += sum(r.sweeps for r in results) * cells
+    barrier()
+    region_s = time.perf_counter() - t_region
+    clocks = sampler.stop()
+    assert all(r.status == 0 for r in results), results
+
+    # end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
+    e2e = None
+    if nb == 1:
+        rho_pin = torch.from_numpy(w0.rho).pin_memory()
+        phi_pin = torch.zeros(w0.rho.shape, dtype=torch.float64).pin_memory()
+        rho_np, phi_np = rho_pin.numpy(), phi_pin.numpy()
+        e2e_ms, e2e_upd = [], 0
+        for i in range(args.warmup + args.steps):
+            phi_np[...] = 0.0
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            r = solver.solve_host(rho_np, phi_np, w0.tol, w0.max_sweeps)
+            dt = time.perf_counter() - t0
+            if i >= args.warmup:
+                e2e_ms.append(dt * 1e3)
+                e2e_upd += r.sweeps * cells
+        e2e_time = sum(e2e_ms) * 1e-3
+
+    total_ms = float(sum(step_ms))
+    t = torch.tensor([total_ms, float(updates), float(launches), e2e_time if nb == 1 else 0.0,
+                      float(e2e_upd) if nb == 1 else 0.0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        tmax = t.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone()
+        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        total_ms, updates_all, launches_all = float(tmax[0]), float(tsum[1]), int(tsum[2])
+        e2e_time_all, e2e_upd_all = float(tmax[3]), float(tsum[4])
+    else:
+        updates_all, launches_all = float(updates), launches
+        e2e_time_all, e2e_upd_all = float(t[3]), float(t[4])
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = updates_all / (total_ms * 1e-3)
+    # roofline of the dominant kernel (the relaxation sweep), from the library's own CUDA events on the stream
+    path = int(solver.stat("path"))
+    sw_ms = float(np.mean(sweep_ms))
+    sweeps_per_step = sum(r.sweeps for r in results)
+    sweep_launches = max(1, int(solver.stat("launches")) - 2 - (1 if path == 1 else 0))
+    alg_bytes_per_launch = BYTES_PER_UPDATE * sweeps_per_step * cells / sweep_launches
+    achieved = alg_bytes_per_launch / (sw_ms * 1e-3 / sweep_launches) / 1e9
+    hbm_peak, hbm_src = measured_peaks()
+    working_set = 16.0 * cells * nb
+    if working_set > 100e6:
+        bound, peak, src = "hbm", hbm_peak, hbm_src
+    else:
+        bound, peak = "l2", l2_copy_peak_gbs(torch)
+        src = "L2-resident torch copy (2 x 24 MiB, read+write bytes), measured live in this run (of measured)"
+    roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "k_halfsweep" if path == 1 else "k_sor_resident",
+                "alg_bytes_per_launch": alg_bytes_per_launch, "launch_ms": sw_ms / sweep_launches,
+                "sweep_launches_per_step": sweep_launches, "peak_source": src,
+                "frac_of_hbm_peak": achieved / hbm_peak}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": label, "grid": [w0.nr, w0.nz], "batch_per_gpu": nb, "lmax": w0.lmax,
+                   "tol": w0.tol, "l2": "flushed between timed solves (256 MiB write)",
+                   "path": {1: "streaming", 2: "resident"}.get(path, str(path)),
+                   "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"},
+        "time_to_residual_ms": total_ms / args.steps, "sweeps_per_solve": [r.sweeps for r in results][:8],
+        "final_residual": results[0].residual,
+        "setup_ms": float(np.mean(setup_ms)), "sweep_ms": sw_ms,
+        "gpu_launches": launches_all, "clocks": clocks, "roofline": roofline,
+        "region_wall_s": region_s,
+    }
+    if nb == 1:
+        out["e2e"] = {"value": e2e_upd_all / e2e_time_all, "unit": UNIT,
+                      "h2d_bytes_per_step": 2 * cells * 8, "d2h_bytes_per_step": cells * 8,
+                      "ms_per_step": e2e_time_all / args.steps * 1e3}
+    else:
+        out["e2e"] = None
+    if not args.no_cpu_baseline and world == 1:
+        v, sample = oracle_rate(mine)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                               "host_cores_available": os.cpu_count()}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,119 @@
+/* sn_poisson.h -- C ABI of the B200-native self-gravity Poisson solve of arXiv 1507.08549.
+ *
+ * What it computes (§2.1: "Phi, the gravitational potential, satisfies the Poisson Equation
+ * nabla^2 Phi = 4 pi G rho"; §2.1: "We use the successive overrelaxation method with the
+ * Gauss-Seidel method to solve the Poisson equation in cylindrical coordinates. The iteration is stopped by
+ * default when the relative changes of all grids reach below 1e-8. The inner boundaries are assumed to be
+ * reflecting and the outer boundaries are fixed by using the Roche approximation Phi(r,z) = -GM/sqrt(r^2+z^2)
+ * ... in general higher multipole terms are needed"; §2.3 / Table 2: the Poisson solver is
+ * the largest of the subroutines the paper offloads to a GPU).
+ *
+ * One solve = (a-1) multipole moments M_l = sum rho (s/L0)^l P_l(cos theta) dV, l = 0..lmax, about the origin
+ *           -> (a-1b) Dirichlet ghost values phi_b = -(1/L0) sum_l M_l P_l / (s/L0)^(l+1) one cell outside
+ *              the east / north (/ south) edges (lmax = 0 is the paper's Roche boundary)
+ *           -> (a-2) red-black SOR sweeps of the conservative cell-centred 5-point cylindrical Laplacian
+ *           -> (a-3) per-sweep fused residual maxima and an on-device stopping decision.
+ * The exact discretisation, orderings and pinned fp64 arithmetic are DESIGN.md §2-3 (readings R1..R14).
+ * G = 1: the library solves nabla^2 phi = 4 pi rho; callers scale rho or phi.
+ *
+ * Grid and layout: uniform (r,z) grid, cell centres r_i = (i+1/2) dr, i in [0,nr);
+ *   symmetry = 1 (half plane, reflecting equator): z_j = (j+1/2) dz;
+ *   symmetry = 0 (full plane): z_j = (j+1/2 - nz/2) dz;  j in [0,nz).
+ * Arrays rho and phi hold interior cells only (no ghost layer), fp64, contiguous, index j*nr + i (r fastest).
+ *
+ * Everything runs in hand-written sm_100a CUDA kernels.  There is no CPU fallback: every entry point fails
+ * (NULL / status < 0, message via sn_poisson_last_error) when no CUDA device of compute capability 10.x is
+ * usable.  No exceptions cross this boundary.  A handle supports one solve in flight at a time.
+ */
+#ifndef SN_POISSON_H
+#define SN_POISSON_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sn_poisson sn_poisson; /* opaque handle; owns all device workspace */
+
+/* Returned by value (16 bytes).
+ *   sweeps   : full sweeps (red half-sweep + black half-sweep) applied to the returned phi
+ *   status   : 0 converged (tol > 0) or fixed-sweep run completed (tol <= 0);
+ *              1 hit max_sweeps without reaching tol (not an error);
+ *             -1 bad argument / NULL (phi untouched); -2 CUDA error; -3 non-finite residual
+ *   residual : R_k of the last applied sweep k,
+ *              R_k = max|res| / (max|4 pi rho| + (2/dr^2+2/dz^2) max|phi_new|)   (R9)            */
+typedef struct {
+    int32_t sweeps;
+    int32_t status;
+    double residual;
+} sn_poisson_result;
+
+/* Create a solver for an nr x nz grid.  nr, nz >= 2; dr, dz > 0 finite; symmetry in {0,1};
+ * 0 <= lmax <= 64 (odd l are ignored when symmetry = 1; lmax = 0 reproduces PAPER.md:99's Roche boundary).
+ * Binds to the current CUDA device.  The relaxation factor defaults to the closed form of DESIGN.md R8.
+ * Returns NULL on bad arguments, allocation failure or no sm_100 device. */
+sn_poisson* sn_poisson_create(int nr, int nz, double dr, double dz, int symmetry, int lmax);
+
+/* Solve nabla^2 phi = 4 pi rho.
+ *   rho        DEVICE pointer, nr*nz fp64, read-only, never modified.
+ *   phi_inout  DEVICE pointer, nr*nz fp64: initial guess on entry (zeros = cold start, the previous potential
+ *              = warm start), the iterate after `sweeps` sweeps on exit.
+ *   tol > 0    stop after the first sweep k with R_k <= tol, or at max_sweeps.
+ *   tol <= 0   run exactly max_sweeps sweeps.
+ *   stream     cudaStream_t passed as void* (NULL = legacy default stream).  All work is enqueued on it and it
+ *              is synchronised once before returning (the result is decided on the device).
+ * Caller owns rho, phi and the stream; the handle owns everything else. */
+sn_poisson_result sn_poisson_solve(sn_poisson* h, const double* rho, double* phi_inout, double tol,
+                                   int max_sweeps, void* stream);
+
+/* Same solve with HOST buffers (pageable or pinned): copies rho and phi to device workspace, solves, copies phi
+ * back.  All copies are on `stream` and inside the call. */
+sn_poisson_result sn_poisson_solve_host(sn_poisson* h, const double* rho_host, double* phi_inout_host,
+                                        double tol, int max_sweeps, void* stream);
+
+/* nbatch independent solves on the same grid geometry ([CFG 4a]).  rho, phi_inout: DEVICE pointers to nbatch
+ * consecutive grids (member b at offset b*nr*nz).  out: HOST array of nbatch results.
+ * Returns 0, or a negative status if the call itself failed. */
+int sn_poisson_solve_batch(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double tol,
+                           int max_sweeps, void* stream, sn_poisson_result* out);
+
+void sn_poisson_destroy(sn_poisson* h);
+
+/* ---- optional, additive --------------------------------------------------------------------------------- */
+
+/* Override the relaxation factor (0 < omega < 2), e.g. [CFG 0]'s 1.9; omega <= 0 restores the default formula.
+ * Returns 0 or -1. */
+int sn_poisson_set_omega(sn_poisson* h, double omega);
+double sn_poisson_get_omega(const sn_poisson* h);
+
+/* Test hooks.  All pointers are HOST pointers.
+ * get_moments : M[0..lmax] of batch member 0 of the last solve (odd entries 0 when symmetry = 1).
+ * set_boundary: inject ghost values bE[nz], bN[nr], bS[nr] (bS ignored when symmetry = 1) and skip the moment and
+ *               boundary kernels in later solves; (NULL, NULL, NULL) restores the multipole boundary.
+ * get_boundary: the ghost arrays used by batch member 0 of the last solve.
+ * get_history : R_k for k = 1..min(n, sweeps) of batch member 0 of the last solve; returns the count copied. */
+int sn_poisson_get_moments(sn_poisson* h, double* M);
+int sn_poisson_set_boundary(sn_poisson* h, const double* bE, const double* bN, const double* bS);
+int sn_poisson_get_boundary(sn_poisson* h, double* bE, double* bN, double* bS);
+int sn_poisson_get_history(sn_poisson* h, double* R, int n);
+
+/* Tuning knobs; unknown keys return -1.
+ *   "path"        0 auto, 1 streaming kernels (phi in L2/HBM), 2 resident persistent kernel (phi on chip)
+ *   "chunk"       sweeps enqueued between host polls of the device-side decision (streaming path)
+ *   "tblock"      sweeps per halo exchange of the resident kernel (temporal blocking depth m)           */
+int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value);
+
+/* Counters of the last solve / batch: "launches" (kernels launched), "sweep_ms" (device time of the relaxation
+ * phase, CUDA events on the caller's stream), "setup_ms" (moments + boundary), "path" (1 or 2 as above),
+ * "ctas", "tile_w", "tile_h", "tblock".  Returns 0 or -1. */
+int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out);
+
+/* Message of the last failure on this thread ("" if none). */
+const char* sn_poisson_last_error(void);
+const char* sn_poisson_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SN_POISSON_H */

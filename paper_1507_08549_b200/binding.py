@@ -1,0 +1,180 @@
+"""Thin ctypes binding over libsn_poisson.so -- same names as include/sn_poisson.h, argument marshalling only.
+
+PyTorch is used by callers for device memory and streams (``tensor.data_ptr()``,
+``torch.cuda.current_stream().cuda_stream``); nothing here computes anything.  There is no CPU fallback:
+if the library is missing or no sm_100 device is usable the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsn_poisson.so")
+
+# every symbol include/sn_poisson.h declares
+EXPORTS = (
+    "sn_poisson_create", "sn_poisson_solve", "sn_poisson_solve_host", "sn_poisson_solve_batch",
+    "sn_poisson_destroy", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
+    "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
+    "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
+)
+
+
+class sn_poisson_result(C.Structure):
+    _fields_ = [("sweeps", C.c_int32), ("status", C.c_int32), ("residual", C.c_double)]
+
+    def __repr__(self):
+        return f"sn_poisson_result(sweeps={self.sweeps}, status={self.status}, residual={self.residual:.3e})"
+
+
+class SnPoissonError(RuntimeError):
+    pass
+
+
+_lib = None
+_vp = C.c_void_p
+_dp = C.POINTER(C.c_double)
+
+
+def load():
+    """dlopen the library (built in-tree by ``paper_1507_08549_b200.build``).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise SnPoissonError(f"{LIB_PATH} not found: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                             "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.sn_poisson_create.restype = _vp
+    lib.sn_poisson_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int]
+    lib.sn_poisson_solve.restype = sn_poisson_result
+    lib.sn_poisson_solve.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
+    lib.sn_poisson_solve_host.restype = sn_poisson_result
+    lib.sn_poisson_solve_host.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
+    lib.sn_poisson_solve_batch.restype = C.c_int
+    lib.sn_poisson_solve_batch.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, C.c_int, _vp,
+                                           C.POINTER(sn_poisson_result)]
+    lib.sn_poisson_destroy.restype = None
+    lib.sn_poisson_destroy.argtypes = [_vp]
+    lib.sn_poisson_set_omega.restype = C.c_int
+    lib.sn_poisson_set_omega.argtypes = [_vp, C.c_double]
+    lib.sn_poisson_get_omega.restype = C.c_double
+    lib.sn_poisson_get_omega.argtypes = [_vp]
+    lib.sn_poisson_get_moments.restype = C.c_int
+    lib.sn_poisson_get_moments.argtypes = [_vp, _dp]
+    lib.sn_poisson_set_boundary.restype = C.c_int
+    lib.sn_poisson_set_boundary.argtypes = [_vp, _dp, _dp, _dp]
+    lib.sn_poisson_get_boundary.restype = C.c_int
+    lib.sn_poisson_get_boundary.argtypes = [_vp, _dp, _dp, _dp]
+    lib.sn_poisson_get_history.restype = C.c_int
+    lib.sn_poisson_get_history.argtypes = [_vp, _dp, C.c_int]
+    lib.sn_poisson_set_option.restype = C.c_int
+    lib.sn_poisson_set_option.argtypes = [_vp, C.c_char_p, C.c_int64]
+    lib.sn_poisson_get_stat.restype = C.c_int
+    lib.sn_poisson_get_stat.argtypes = [_vp, C.c_char_p, _dp]
+    lib.sn_poisson_last_error.restype = C.c_char_p
+    lib.sn_poisson_last_error.argtypes = []
+    lib.sn_poisson_version.restype = C.c_char_p
+    lib.sn_poisson_version.argtypes = []
+    _lib = lib
+    return lib
+
+
+def sn_poisson_last_error() -> str:
+    return load().sn_poisson_last_error().decode()
+
+
+def sn_poisson_version() -> str:
+    return load().sn_poisson_version().decode()
+
+
+def sn_poisson_create(nr, nz, dr, dz, symmetry, lmax):
+    """Returns an opaque handle (int) or raises SnPoissonError with the library's message."""
+    h = load().sn_poisson_create(int(nr), int(nz), float(dr), float(dz), int(symmetry), int(lmax))
+    if not h:
+        raise SnPoissonError("sn_poisson_create failed: " + sn_poisson_last_error())
+    return h
+
+
+def sn_poisson_destroy(h):
+    load().sn_poisson_destroy(h)
+
+
+def sn_poisson_solve(h, rho_ptr, phi_ptr, tol, max_sweeps, stream=0) -> sn_poisson_result:
+    """rho_ptr / phi_ptr: DEVICE addresses (ints, e.g. tensor.data_ptr()); stream: cudaStream_t as int."""
+    return load().sn_poisson_solve(h, rho_ptr, phi_ptr, float(tol), int(max_sweeps), stream or None)
+
+
+def sn_poisson_solve_host(h, rho_ptr, phi_ptr, tol, max_sweeps, stream=0) -> sn_poisson_result:
+    """rho_ptr / phi_ptr: HOST addresses (ints, e.g. numpy ``arr.ctypes.data`` or a pinned tensor's data_ptr())."""
+    return load().sn_poisson_solve_host(h, rho_ptr, phi_ptr, float(tol), int(max_sweeps), stream or None)
+
+
+def sn_poisson_solve_batch(h, nbatch, rho_ptr, phi_ptr, tol, max_sweeps, stream=0):
+    out = (sn_poisson_result * int(nbatch))()
+    rc = load().sn_poisson_solve_batch(h, int(nbatch), rho_ptr, phi_ptr, float(tol), int(max_sweeps),
+                                       stream or None, out)
+    if rc != 0:
+        raise SnPoissonError(f"sn_poisson_solve_batch failed ({rc}): " + sn_poisson_last_error())
+    return list(out)
+
+
+def sn_poisson_set_omega(h, omega) -> int:
+    return load().sn_poisson_set_omega(h, float(omega))
+
+
+def sn_poisson_get_omega(h) -> float:
+    return load().sn_poisson_get_omega(h)
+
+
+def _check(rc, what):
+    if rc < 0:
+        raise SnPoissonError(f"{what} failed ({rc}): " + sn_poisson_last_error())
+    return rc
+
+
+def sn_poisson_get_moments(h, lmax):
+    import numpy as np
+    M = np.zeros(lmax + 1)
+    _check(load().sn_poisson_get_moments(h, M.ctypes.data_as(_dp)), "sn_poisson_get_moments")
+    return M
+
+
+def sn_poisson_set_boundary(h, bE, bN, bS=None):
+    import numpy as np
+    if bE is None:
+        return _check(load().sn_poisson_set_boundary(h, None, None, None), "sn_poisson_set_boundary")
+    bE = np.ascontiguousarray(bE, dtype=np.float64)
+    bN = np.ascontiguousarray(bN, dtype=np.float64)
+    bSp = None
+    if bS is not None:
+        bS = np.ascontiguousarray(bS, dtype=np.float64)
+        bSp = bS.ctypes.data_as(_dp)
+    return _check(load().sn_poisson_set_boundary(h, bE.ctypes.data_as(_dp), bN.ctypes.data_as(_dp), bSp),
+                  "sn_poisson_set_boundary")
+
+
+def sn_poisson_get_boundary(h, nr, nz, symmetry):
+    import numpy as np
+    bE, bN, bS = np.zeros(nz), np.zeros(nr), np.zeros(nr)
+    _check(load().sn_poisson_get_boundary(h, bE.ctypes.data_as(_dp), bN.ctypes.data_as(_dp),
+                                          bS.ctypes.data_as(_dp)), "sn_poisson_get_boundary")
+    return bE, bN, (bS if symmetry == 0 else None)
+
+
+def sn_poisson_get_history(h, n):
+    import numpy as np
+    R = np.zeros(max(int(n), 1))
+    m = _check(load().sn_poisson_get_history(h, R.ctypes.data_as(_dp), int(n)), "sn_poisson_get_history")
+    return R[:m]
+
+
+def sn_poisson_set_option(h, key: str, value: int) -> int:
+    return _check(load().sn_poisson_set_option(h, key.encode(), int(value)), f"sn_poisson_set_option({key})")
+
+
+def sn_poisson_get_stat(h, key: str) -> float:
+    out = C.c_double(0.0)
+    _check(load().sn_poisson_get_stat(h, key.encode(), C.byref(out)), f"sn_poisson_get_stat({key})")
+    return out.value

@@ -1,0 +1,76 @@
+// common.cuh -- shared device-side types of the sn_poisson library (sm_100a only).
+// Discretisation and pinned arithmetic: DESIGN.md §2-3; PAPER.md:91,99 for the physics.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace snp {
+
+constexpr double kFourPi = 12.566370614359172;   // 4*pi rounded to fp64 (R10)
+constexpr double kPi = 3.141592653589793;
+constexpr int kMaxL = 64;
+
+// Per-member control block written by the device-side stopping decision (step a-3).
+struct Ctl {
+    int done;          // 1 once the stopping rule fired (or a non-finite ratio was seen)
+    int sweeps;        // full sweeps applied when it fired
+    int status;        // 0 / 1 / -3 as in sn_poisson_result
+    int pad;
+    double residual;   // R_k of that sweep
+    double maxf;       // max |4 pi rho| (written by the moments pass)
+};
+
+// Grid geometry + coefficient tables; passed by value to every kernel.
+struct Geom {
+    int nr, nz, symmetry, lmax;
+    double dr, dz;
+    double iz2;        // 1/dz^2
+    double D, D0;      // 2/dr^2+2/dz^2 and D - 1/dz^2 (reflecting-equator row)
+    double wD, wD0;    // omega/D, omega/D0
+    double tol;
+    const double* cE;  // [nr]  ((i+1)/(i+1/2))/dr^2
+    const double* cW;  // [nr]  (i/(i+1/2))/dr^2, cW[0] = 0: regular axis
+};
+
+__device__ __forceinline__ unsigned long long dbits(double x) { return (unsigned long long)__double_as_longlong(x); }
+__device__ __forceinline__ double bits2d(unsigned long long b) { return __longlong_as_double((long long)b); }
+
+// |x| as an order-preserving unsigned key (non-negative doubles order like their bit patterns; NaN sorts highest,
+// so a NaN anywhere is sticky in a max-reduction, like the oracle's).
+__device__ __forceinline__ unsigned long long abs_key(double x) { return dbits(x) & 0x7fffffffffffffffull; }
+
+__device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long t = __shfl_xor_sync(0xffffffffu, v, o);
+        v = t > v ? t : v;
+    }
+    return v;
+}
+
+// Stopping ratio of one sweep (R9): R = Rabs / fma(D, P, maxf); Rabs == 0 -> 0.
+__device__ __forceinline__ double stop_ratio(unsigned long long rabs_key, unsigned long long p_key, double maxf,
+                                             double D) {
+    const double Rabs = bits2d(rabs_key);
+    if (Rabs == 0.0) return 0.0;
+    return __ddiv_rn(Rabs, __fma_rn(D, bits2d(p_key), maxf));
+}
+
+__device__ __forceinline__ bool is_nonfinite(double x) { return !(x == x) || x == INFINITY || x == -INFINITY; }
+
+// One SOR cell update with the pinned expression tree (R10).  Returns the new value; res_out = pre-update
+// residual f - L(phi).
+__device__ __forceinline__ double sor_update(double cE, double cW, double cN, double cS, double diag, double w,
+                                             double pE, double pW, double pN, double pS, double pC, double f,
+                                             double& res_out) {
+    double t = __dmul_rn(cE, pE);
+    t = __fma_rn(cW, pW, t);
+    t = __fma_rn(cN, pN, t);
+    t = __fma_rn(cS, pS, t);
+    t = __fma_rn(-diag, pC, t);
+    const double res = __dsub_rn(f, t);
+    res_out = res;
+    return __fma_rn(-w, res, pC);
+}
+
+}  // namespace snp

@@ -1,0 +1,449 @@
+// sn_poisson.cu -- C-ABI host side of the B200-native Poisson solve (include/sn_poisson.h).
+// Argument checks, workspace, launch sequencing; every step of the path runs in the kernels of
+// moments.cuh / sweep_stream.cuh / sweep_resident.cuh.  No CPU fallback.
+#include "../../include/sn_poisson.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+#include "moments.cuh"
+#include "sweep_stream.cuh"
+
+using namespace snp;
+
+namespace {
+
+thread_local std::string g_err;
+
+void set_err(const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+}
+
+#define CU_TRY(expr)                                                                       \
+    do {                                                                                   \
+        cudaError_t e__ = (expr);                                                          \
+        if (e__ != cudaSuccess) {                                                          \
+            set_err("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return -2;                                                                     \
+        }                                                                                  \
+    } while (0)
+
+template <typename T>
+int dev_alloc(T** p, size_t n) {
+    CU_TRY(cudaMalloc((void**)p, n * sizeof(T)));
+    return 0;
+}
+
+}  // namespace
+
+struct sn_poisson {
+    int nr = 0, nz = 0, symmetry = 0, lmax = 0;
+    double dr = 0, dz = 0;
+    double omega = 0;
+    bool omega_user = false;
+    int device = 0, num_sms = 0;
+    double L0 = 0;
+    int NL = 0;                 // moment template width (lcap + 1)
+    int mom_blocks = 0;
+
+    // options
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0;
+
+    // device workspace (sized for `cap_batch` members)
+    int cap_batch = 0, cap_sweeps = 0;
+    double *d_cE = nullptr, *d_cW = nullptr;
+    double *d_bE = nullptr, *d_bN = nullptr, *d_bS = nullptr, *d_M = nullptr, *d_partial = nullptr;
+    unsigned long long* d_slots = nullptr;
+    double* d_hist = nullptr;
+    Ctl* d_ctl = nullptr;
+    Ctl* h_ctl = nullptr;       // pinned, 2 * cap_batch (double-buffered polls)
+    double *d_rho_stage = nullptr, *d_phi_stage = nullptr;   // solve_host staging
+    bool user_boundary = false;
+    cudaEvent_t ev_poll[2] = {nullptr, nullptr};
+    cudaEvent_t ev_t[3] = {nullptr, nullptr, nullptr};
+
+    // stats of the last solve
+    double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
+    int last_sweeps0 = 0;
+};
+
+namespace {
+
+// DESIGN.md R8: default relaxation factor, closed form with only + - * / sqrt (same expression order as stated there).
+double default_omega(int nr, int nz, double dr, double dz, int symmetry) {
+    const double j01 = 2.404825557695773;
+    const double Lr = (nr + 0.5) * dr;
+    const double kz = symmetry == 1 ? kPi / (2.0 * ((nz + 0.5) * dz)) : kPi / ((nz + 1.0) * dz);
+    const double a = j01 / Lr;
+    const double lambda = a * a + kz * kz;
+    const double D = 2.0 / (dr * dr) + 2.0 / (dz * dz);
+    const double mu = 1.0 - lambda / D;
+    return 2.0 / (1.0 + std::sqrt(1.0 - mu * mu));
+}
+
+Geom make_geom(const sn_poisson* h, double tol) {
+    Geom g;
+    g.nr = h->nr; g.nz = h->nz; g.symmetry = h->symmetry; g.lmax = h->lmax;
+    g.dr = h->dr; g.dz = h->dz;
+    const double ir2 = 1.0 / (h->dr * h->dr);
+    g.iz2 = 1.0 / (h->dz * h->dz);
+    g.D = 2.0 * ir2 + 2.0 * g.iz2;
+    g.D0 = g.D - g.iz2;
+    g.wD = h->omega / g.D;
+    g.wD0 = h->omega / g.D0;
+    g.tol = tol;
+    g.cE = h->d_cE;
+    g.cW = h->d_cW;
+    return g;
+}
+
+void free_batch_ws(sn_poisson* h) {
+    cudaFree(h->d_bE); cudaFree(h->d_bN); cudaFree(h->d_bS); cudaFree(h->d_M); cudaFree(h->d_partial);
+    cudaFree(h->d_slots); cudaFree(h->d_hist); cudaFree(h->d_ctl);
+    if (h->h_ctl) cudaFreeHost(h->h_ctl);
+    h->d_bE = h->d_bN = h->d_bS = h->d_M = h->d_partial = h->d_hist = nullptr;
+    h->d_slots = nullptr; h->d_ctl = nullptr; h->h_ctl = nullptr;
+    h->cap_batch = 0; h->cap_sweeps = 0;
+}
+
+// Grow the per-member workspace.  Keeps injected boundary arrays of member 0 across a regrow.
+int ensure_ws(sn_poisson* h, int nbatch, int max_sweeps) {
+    const int need_sw = max_sweeps < 1 ? 1 : max_sweeps;
+    if (nbatch <= h->cap_batch && need_sw <= h->cap_sweeps) return 0;
+    std::vector<double> kE, kN, kS;
+    if (h->user_boundary && h->d_bE) {
+        kE.resize(h->nz); kN.resize(h->nr); kS.resize(h->nr);
+        CU_TRY(cudaMemcpy(kE.data(), h->d_bE, sizeof(double) * h->nz, cudaMemcpyDeviceToHost));
+        CU_TRY(cudaMemcpy(kN.data(), h->d_bN, sizeof(double) * h->nr, cudaMemcpyDeviceToHost));
+        CU_TRY(cudaMemcpy(kS.data(), h->d_bS, sizeof(double) * h->nr, cudaMemcpyDeviceToHost));
+    }
+    const int nb = nbatch > h->cap_batch ? nbatch : h->cap_batch;
+    const int ns = need_sw > h->cap_sweeps ? need_sw : h->cap_sweeps;
+    free_batch_ws(h);
+    if (dev_alloc(&h->d_bE, (size_t)nb * h->nz) || dev_alloc(&h->d_bN, (size_t)nb * h->nr) ||
+        dev_alloc(&h->d_bS, (size_t)nb * h->nr) || dev_alloc(&h->d_M, (size_t)nb * (kMaxL + 1)) ||
+        dev_alloc(&h->d_partial, (size_t)nb * h->mom_blocks * h->NL) || dev_alloc(&h->d_slots, (size_t)nb * 2 * ns) ||
+        dev_alloc(&h->d_hist, (size_t)nb * ns) || dev_alloc(&h->d_ctl, (size_t)nb))
+        return -2;
+    CU_TRY(cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl) * 2 * nb));
+    CU_TRY(cudaMemset(h->d_bS, 0, sizeof(double) * (size_t)nb * h->nr));
+    CU_TRY(cudaMemset(h->d_M, 0, sizeof(double) * (size_t)nb * (kMaxL + 1)));
+    h->cap_batch = nb;
+    h->cap_sweeps = ns;
+    if (!kE.empty()) {
+        for (int b = 0; b < nb; ++b) {
+            CU_TRY(cudaMemcpy(h->d_bE + (size_t)b * h->nz, kE.data(), sizeof(double) * h->nz, cudaMemcpyHostToDevice));
+            CU_TRY(cudaMemcpy(h->d_bN + (size_t)b * h->nr, kN.data(), sizeof(double) * h->nr, cudaMemcpyHostToDevice));
+            CU_TRY(cudaMemcpy(h->d_bS + (size_t)b * h->nr, kS.data(), sizeof(double) * h->nr, cudaMemcpyHostToDevice));
+        }
+    }
+    return 0;
+}
+
+int launch_moments(sn_poisson* h, const Geom& g, int nbatch, const double* rho, cudaStream_t st) {
+    dim3 grid(h->mom_blocks, nbatch);
+    switch (h->NL) {
+        case 9: k_moments<9><<<grid, kMomThreads, 0, st>>>(rho, g, h->L0, h->d_partial, h->d_ctl); break;
+        case 17: k_moments<17><<<grid, kMomThreads, 0, st>>>(rho, g, h->L0, h->d_partial, h->d_ctl); break;
+        case 33: k_moments<33><<<grid, kMomThreads, 0, st>>>(rho, g, h->L0, h->d_partial, h->d_ctl); break;
+        default: k_moments<65><<<grid, kMomThreads, 0, st>>>(rho, g, h->L0, h->d_partial, h->d_ctl); break;
+    }
+    CU_TRY(cudaGetLastError());
+    return 0;
+}
+
+// Streaming path: two launches per sweep, decision folded into the next sweep's launches, host polls per chunk.
+int run_stream(sn_poisson* h, const Geom& g, int nbatch, const double* rho, double* phi, int max_sweeps,
+               cudaStream_t st) {
+    dim3 grid((h->nr + kStreamTileW - 1) / kStreamTileW, (h->nz + kStreamTileH - 1) / kStreamTileH, nbatch);
+    const int slot_stride = 2 * h->cap_sweeps, hist_stride = h->cap_sweeps;
+    const int chunk = h->opt_chunk < 1 ? 1 : h->opt_chunk;
+    int k = 1, poll = 0;
+    bool have_poll[2] = {false, false};
+    bool all_done = false;
+    while (k <= max_sweeps && !all_done) {
+        const int kend = (max_sweeps - k + 1 < chunk) ? max_sweeps : k + chunk - 1;
+        for (; k <= kend; ++k) {
+            for (int colour = 0; colour < 2; ++colour) {
+                k_halfsweep<<<grid, kStreamWarps * 32, 0, st>>>(g, colour, k, slot_stride, hist_stride, rho, phi,
+                                                                h->d_bE, h->d_bN, h->d_bS, h->d_slots, h->d_ctl,
+                                                                h->d_hist);
+                h->st_launches += 1;
+            }
+        }
+        CU_TRY(cudaGetLastError());
+        if (g.tol > 0.0 && k <= max_sweeps) {
+            // poll the device-side decision one chunk behind, so the queue never drains
+            CU_TRY(cudaMemcpyAsync(h->h_ctl + (size_t)poll * h->cap_batch, h->d_ctl, sizeof(Ctl) * nbatch,
+                                   cudaMemcpyDeviceToHost, st));
+            CU_TRY(cudaEventRecord(h->ev_poll[poll], st));
+            have_poll[poll] = true;
+            const int prev = poll ^ 1;
+            if (have_poll[prev]) {
+                CU_TRY(cudaEventSynchronize(h->ev_poll[prev]));
+                all_done = true;
+                for (int b = 0; b < nbatch; ++b) all_done = all_done && h->h_ctl[(size_t)prev * h->cap_batch + b].done;
+            }
+            poll ^= 1;
+        }
+    }
+    k_decide_last<<<nbatch, 32, 0, st>>>(g, k - 1, slot_stride, hist_stride, h->d_slots, h->d_ctl, h->d_hist);
+    h->st_launches += 1;
+    CU_TRY(cudaGetLastError());
+    return 0;
+}
+
+int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double tol, int max_sweeps,
+               cudaStream_t st, sn_poisson_result* out) {
+    CU_TRY(cudaSetDevice(h->device));
+    if (int rc = ensure_ws(h, nbatch, max_sweeps)) return rc;
+    if (!h->omega_user) h->omega = default_omega(h->nr, h->nz, h->dr, h->dz, h->symmetry);
+    const Geom g = make_geom(h, tol);
+    h->st_launches = 0;
+    h->st_path = 1;
+
+    CU_TRY(cudaEventRecord(h->ev_t[0], st));
+    CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl) * nbatch, st));
+    CU_TRY(cudaMemsetAsync(h->d_slots, 0, sizeof(unsigned long long) * 2 * (size_t)h->cap_sweeps * nbatch, st));
+    // a-1: moments (+ max|4 pi rho|), a-1b: boundary fill (skipped when ghosts were injected by the test hook)
+    if (int rc = launch_moments(h, g, nbatch, rho, st)) return rc;
+    h->st_launches += 1;
+    if (!h->user_boundary) {
+        k_boundary<<<nbatch, 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN,
+                                           h->d_bS, 0);
+        CU_TRY(cudaGetLastError());
+        h->st_launches += 1;
+    }
+    CU_TRY(cudaEventRecord(h->ev_t[1], st));
+    // a-2 + a-3
+    if (int rc = run_stream(h, g, nbatch, rho, phi, max_sweeps, st)) return rc;
+    CU_TRY(cudaEventRecord(h->ev_t[2], st));
+    CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl) * nbatch, cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    float ms = 0;
+    CU_TRY(cudaEventElapsedTime(&ms, h->ev_t[0], h->ev_t[1]));
+    h->st_setup_ms = ms;
+    CU_TRY(cudaEventElapsedTime(&ms, h->ev_t[1], h->ev_t[2]));
+    h->st_sweep_ms = ms;
+    for (int b = 0; b < nbatch; ++b) {
+        out[b].sweeps = h->h_ctl[b].sweeps;
+        out[b].status = h->h_ctl[b].status;
+        out[b].residual = h->h_ctl[b].residual;
+    }
+    h->last_sweeps0 = out[0].sweeps;
+    return 0;
+}
+
+bool check_solve_args(sn_poisson* h, const void* rho, const void* phi, double tol, int max_sweeps) {
+    if (!h) { set_err("NULL handle"); return false; }
+    if (!rho || !phi) { set_err("NULL rho / phi pointer"); return false; }
+    if (max_sweeps < 0) { set_err("max_sweeps < 0"); return false; }
+    if (tol != tol) { set_err("tol is NaN"); return false; }
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sn_poisson_last_error(void) { return g_err.c_str(); }
+const char* sn_poisson_version(void) { return "sn_poisson 0.1 (sm_100a)"; }
+
+sn_poisson* sn_poisson_create(int nr, int nz, double dr, double dz, int symmetry, int lmax) {
+    g_err.clear();
+    if (nr < 2 || nz < 2) { set_err("nr, nz must be >= 2"); return nullptr; }
+    if (!(dr > 0) || !(dz > 0) || !std::isfinite(dr) || !std::isfinite(dz)) {
+        set_err("dr, dz must be finite and > 0");
+        return nullptr;
+    }
+    if (symmetry != 0 && symmetry != 1) { set_err("symmetry must be 0 or 1"); return nullptr; }
+    if (lmax < 0 || lmax > kMaxL) { set_err("lmax must be in [0, %d]", kMaxL); return nullptr; }
+    if ((long long)nr * nz > (1ll << 31) - 1) { set_err("grid too large"); return nullptr; }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { set_err("no CUDA device: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { set_err("cudaGetDeviceProperties failed"); return nullptr; }
+    if (prop.major != 10) {
+        set_err("device %d is sm_%d%d; this library is built for sm_100a only (no fallback)", dev, prop.major, prop.minor);
+        return nullptr;
+    }
+    sn_poisson* h = new (std::nothrow) sn_poisson();
+    if (!h) { set_err("out of host memory"); return nullptr; }
+    h->nr = nr; h->nz = nz; h->dr = dr; h->dz = dz; h->symmetry = symmetry; h->lmax = lmax;
+    h->device = dev;
+    h->num_sms = prop.multiProcessorCount;
+    h->L0 = nr * dr;
+    h->NL = lmax <= 8 ? 9 : lmax <= 16 ? 17 : lmax <= 32 ? 33 : 65;
+    const size_t ncell = (size_t)nr * nz;
+    size_t blocks = (ncell + kMomThreads * 4 - 1) / (kMomThreads * 4);
+    const size_t cap = (size_t)h->num_sms * 4;
+    h->mom_blocks = (int)(blocks < 1 ? 1 : blocks > cap ? cap : blocks);
+    h->omega = default_omega(nr, nz, dr, dz, symmetry);
+    // coefficient tables (R10): cE_i = ((i+1)/(i+1/2))/dr^2, cW_i = (i/(i+1/2))/dr^2
+    std::vector<double> cE(nr), cW(nr);
+    const double ir2 = 1.0 / (dr * dr);
+    for (int i = 0; i < nr; ++i) {
+        cE[i] = ((i + 1.0) / (i + 0.5)) * ir2;
+        cW[i] = (i / (i + 0.5)) * ir2;
+    }
+    bool ok = cudaMalloc((void**)&h->d_cE, sizeof(double) * nr) == cudaSuccess &&
+              cudaMalloc((void**)&h->d_cW, sizeof(double) * nr) == cudaSuccess &&
+              cudaMemcpy(h->d_cE, cE.data(), sizeof(double) * nr, cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaMemcpy(h->d_cW, cW.data(), sizeof(double) * nr, cudaMemcpyHostToDevice) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i) ok = cudaEventCreateWithFlags(&h->ev_poll[i], cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 3 && ok; ++i) ok = cudaEventCreate(&h->ev_t[i]) == cudaSuccess;
+    if (!ok) {
+        set_err("CUDA allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+        sn_poisson_destroy(h);
+        return nullptr;
+    }
+    return h;
+}
+
+void sn_poisson_destroy(sn_poisson* h) {
+    if (!h) return;
+    free_batch_ws(h);
+    cudaFree(h->d_cE); cudaFree(h->d_cW);
+    cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage);
+    for (auto& e : h->ev_poll) if (e) cudaEventDestroy(e);
+    for (auto& e : h->ev_t) if (e) cudaEventDestroy(e);
+    delete h;
+}
+
+sn_poisson_result sn_poisson_solve(sn_poisson* h, const double* rho, double* phi_inout, double tol, int max_sweeps,
+                                   void* stream) {
+    g_err.clear();
+    sn_poisson_result r = {0, -1, 0.0};
+    if (!check_solve_args(h, rho, phi_inout, tol, max_sweeps)) return r;
+    const int rc = solve_impl(h, 1, rho, phi_inout, tol, max_sweeps, (cudaStream_t)stream, &r);
+    if (rc) { r.sweeps = 0; r.status = rc; r.residual = 0.0; }
+    return r;
+}
+
+int sn_poisson_solve_batch(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double tol,
+                           int max_sweeps, void* stream, sn_poisson_result* out) {
+    g_err.clear();
+    if (!check_solve_args(h, rho, phi_inout, tol, max_sweeps)) return -1;
+    if (nbatch < 1 || !out) { set_err("nbatch < 1 or NULL out"); return -1; }
+    if (nbatch > 65535) { set_err("nbatch > 65535"); return -1; }
+    return solve_impl(h, nbatch, rho, phi_inout, tol, max_sweeps, (cudaStream_t)stream, out);
+}
+
+sn_poisson_result sn_poisson_solve_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
+                                        int max_sweeps, void* stream) {
+    g_err.clear();
+    sn_poisson_result r = {0, -1, 0.0};
+    if (!check_solve_args(h, rho_host, phi_inout_host, tol, max_sweeps)) return r;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = sizeof(double) * (size_t)h->nr * h->nz;
+    auto fail = [&](cudaError_t e, const char* what) {
+        set_err("%s failed: %s", what, cudaGetErrorString(e));
+        r.status = -2;
+        return r;
+    };
+    cudaError_t e;
+    if ((e = cudaSetDevice(h->device)) != cudaSuccess) return fail(e, "cudaSetDevice");
+    if (!h->d_rho_stage) {
+        if ((e = cudaMalloc((void**)&h->d_rho_stage, bytes)) != cudaSuccess) return fail(e, "cudaMalloc");
+        if ((e = cudaMalloc((void**)&h->d_phi_stage, bytes)) != cudaSuccess) return fail(e, "cudaMalloc");
+    }
+    if ((e = cudaMemcpyAsync(h->d_rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e, "H2D rho");
+    if ((e = cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e, "H2D phi");
+    const int rc = solve_impl(h, 1, h->d_rho_stage, h->d_phi_stage, tol, max_sweeps, st, &r);
+    if (rc) { r.sweeps = 0; r.status = rc; r.residual = 0.0; return r; }
+    if ((e = cudaMemcpyAsync(phi_inout_host, h->d_phi_stage, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e, "D2H phi");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return fail(e, "cudaStreamSynchronize");
+    return r;
+}
+
+int sn_poisson_set_omega(sn_poisson* h, double omega) {
+    g_err.clear();
+    if (!h) { set_err("NULL handle"); return -1; }
+    if (!(omega > 0)) {
+        h->omega_user = false;
+        h->omega = default_omega(h->nr, h->nz, h->dr, h->dz, h->symmetry);
+        return 0;
+    }
+    if (!(omega < 2.0)) { set_err("omega must be in (0, 2)"); return -1; }
+    h->omega = omega;
+    h->omega_user = true;
+    return 0;
+}
+
+double sn_poisson_get_omega(const sn_poisson* h) { return h ? h->omega : 0.0; }
+
+int sn_poisson_get_moments(sn_poisson* h, double* M) {
+    g_err.clear();
+    if (!h || !M) { set_err("NULL argument"); return -1; }
+    if (!h->d_M) { set_err("no solve has run yet"); return -1; }
+    CU_TRY(cudaMemcpy(M, h->d_M, sizeof(double) * (h->lmax + 1), cudaMemcpyDeviceToHost));
+    return 0;
+}
+
+int sn_poisson_set_boundary(sn_poisson* h, const double* bE, const double* bN, const double* bS) {
+    g_err.clear();
+    if (!h) { set_err("NULL handle"); return -1; }
+    if (!bE && !bN && !bS) { h->user_boundary = false; return 0; }
+    if (!bE || !bN || (h->symmetry == 0 && !bS)) { set_err("NULL boundary array"); return -1; }
+    if (int rc = ensure_ws(h, 1, 1)) return rc;
+    for (int b = 0; b < h->cap_batch; ++b) {
+        CU_TRY(cudaMemcpy(h->d_bE + (size_t)b * h->nz, bE, sizeof(double) * h->nz, cudaMemcpyHostToDevice));
+        CU_TRY(cudaMemcpy(h->d_bN + (size_t)b * h->nr, bN, sizeof(double) * h->nr, cudaMemcpyHostToDevice));
+        if (h->symmetry == 0)
+            CU_TRY(cudaMemcpy(h->d_bS + (size_t)b * h->nr, bS, sizeof(double) * h->nr, cudaMemcpyHostToDevice));
+    }
+    h->user_boundary = true;
+    return 0;
+}
+
+int sn_poisson_get_boundary(sn_poisson* h, double* bE, double* bN, double* bS) {
+    g_err.clear();
+    if (!h || !bE || !bN) { set_err("NULL argument"); return -1; }
+    if (!h->d_bE) { set_err("no solve has run yet"); return -1; }
+    CU_TRY(cudaMemcpy(bE, h->d_bE, sizeof(double) * h->nz, cudaMemcpyDeviceToHost));
+    CU_TRY(cudaMemcpy(bN, h->d_bN, sizeof(double) * h->nr, cudaMemcpyDeviceToHost));
+    if (bS && h->symmetry == 0) CU_TRY(cudaMemcpy(bS, h->d_bS, sizeof(double) * h->nr, cudaMemcpyDeviceToHost));
+    return 0;
+}
+
+int sn_poisson_get_history(sn_poisson* h, double* R, int n) {
+    g_err.clear();
+    if (!h || !R || n < 0) { set_err("bad argument"); return -1; }
+    if (!h->d_hist) { set_err("no solve has run yet"); return -1; }
+    const int m = n < h->last_sweeps0 ? n : h->last_sweeps0;
+    if (m > 0) CU_TRY(cudaMemcpy(R, h->d_hist, sizeof(double) * m, cudaMemcpyDeviceToHost));
+    return m;
+}
+
+int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
+    g_err.clear();
+    if (!h || !key) { set_err("NULL argument"); return -1; }
+    if (!strcmp(key, "path")) { if (value < 0 || value > 2) { set_err("path must be 0..2"); return -1; } h->opt_path = (int)value; return 0; }
+    if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
+    if (!strcmp(key, "tblock")) { if (value < 0 || value > 16) { set_err("tblock must be 0..16"); return -1; } h->opt_tblock = (int)value; return 0; }
+    set_err("unknown option '%s'", key);
+    return -1;
+}
+
+int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
+    g_err.clear();
+    if (!h || !key || !out) { set_err("NULL argument"); return -1; }
+    if (!strcmp(key, "launches")) { *out = h->st_launches; return 0; }
+    if (!strcmp(key, "sweep_ms")) { *out = h->st_sweep_ms; return 0; }
+    if (!strcmp(key, "setup_ms")) { *out = h->st_setup_ms; return 0; }
+    if (!strcmp(key, "path")) { *out = h->st_path; return 0; }
+    set_err("unknown stat '%s'", key);
+    return -1;
+}
+
+}  // extern "C"

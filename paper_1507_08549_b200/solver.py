@@ -1,0 +1,86 @@
+"""Convenience wrapper: torch tensors in, torch tensors out; pointer / stream marshalling only."""
+from __future__ import annotations
+
+from . import binding as B
+
+
+class PoissonSolver:
+    """Owns one sn_poisson handle.  ``rho`` / ``phi`` are float64 CUDA tensors of shape (nz, nr) or (nbatch, nz, nr)."""
+
+    def __init__(self, nr, nz, dr, dz, symmetry, lmax, omega=None):
+        self.nr, self.nz, self.dr, self.dz, self.symmetry, self.lmax = nr, nz, dr, dz, symmetry, lmax
+        self.h = B.sn_poisson_create(nr, nz, dr, dz, symmetry, lmax)
+        if omega is not None:
+            if B.sn_poisson_set_omega(self.h, omega) != 0:
+                raise B.SnPoissonError(B.sn_poisson_last_error())
+
+    @classmethod
+    def for_workload(cls, w):
+        return cls(w.nr, w.nz, w.dr, w.dz, w.symmetry, w.lmax, omega=w.omega)
+
+    def close(self):
+        if getattr(self, "h", None):
+            B.sn_poisson_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def _check(self, t):
+        import torch
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise ValueError("expected a contiguous float64 CUDA tensor")
+
+    def solve(self, rho, phi, tol, max_sweeps):
+        """In-place on ``phi``.  Returns sn_poisson_result (or a list for a 3-D batch)."""
+        import torch
+        self._check(rho)
+        self._check(phi)
+        stream = torch.cuda.current_stream().cuda_stream
+        if rho.dim() == 3:
+            if rho.shape != phi.shape or tuple(rho.shape[1:]) != (self.nz, self.nr):
+                raise ValueError("shape mismatch")
+            return B.sn_poisson_solve_batch(self.h, rho.shape[0], rho.data_ptr(), phi.data_ptr(), tol, max_sweeps,
+                                            stream)
+        if tuple(rho.shape) != (self.nz, self.nr) or rho.shape != phi.shape:
+            raise ValueError("shape mismatch")
+        r = B.sn_poisson_solve(self.h, rho.data_ptr(), phi.data_ptr(), tol, max_sweeps, stream)
+        if r.status < 0:
+            raise B.SnPoissonError(f"sn_poisson_solve status {r.status}: {B.sn_poisson_last_error()}")
+        return r
+
+    def solve_host(self, rho_np, phi_np, tol, max_sweeps):
+        """Host numpy arrays (C-contiguous float64); phi_np is updated in place.  H2D/D2H inside the call."""
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+        r = B.sn_poisson_solve_host(self.h, rho_np.ctypes.data, phi_np.ctypes.data, tol, max_sweeps, stream)
+        if r.status < 0:
+            raise B.SnPoissonError(f"sn_poisson_solve_host status {r.status}: {B.sn_poisson_last_error()}")
+        return r
+
+    def set_option(self, key, value):
+        return B.sn_poisson_set_option(self.h, key, value)
+
+    def stat(self, key):
+        return B.sn_poisson_get_stat(self.h, key)
+
+    def moments(self):
+        return B.sn_poisson_get_moments(self.h, self.lmax)
+
+    def boundary(self):
+        return B.sn_poisson_get_boundary(self.h, self.nr, self.nz, self.symmetry)
+
+    def set_boundary(self, bE, bN, bS=None):
+        return B.sn_poisson_set_boundary(self.h, bE, bN, bS)
+
+    def history(self, n):
+        return B.sn_poisson_get_history(self.h, n)
+
+    @property
+    def omega(self):
+        return B.sn_poisson_get_omega(self.h)

@@ -1,0 +1,295 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, same seeded inputs.
+
+Bars (BASELINE.json north_star): phi after an identical sweep count <= 1e-11 relative max-norm; converged sweep
+count within +-1.  With injected ghost arrays the pinned fp64 expression tree (R10) makes the two
+bit-identical, which is what most tests here assert; with the library's own moments only the reduction order of
+the moment sums differs (~1e-15).
+"""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+REL = 1e-11          # north_star tolerance, relative max-norm
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def P(torch_cuda):
+    import paper_1507_08549_b200 as pkg
+    from paper_1507_08549_b200 import build
+    build.build()
+    pkg.load()
+    return pkg
+
+
+def gpu_solve(P, torch, w, phi0=None, tol=None, max_sweeps=None, boundary=None, options=None, omega="w"):
+    tol = w.tol if tol is None else tol
+    max_sweeps = w.max_sweeps if max_sweeps is None else max_sweeps
+    s = P.PoissonSolver(w.nr, w.nz, w.dr, w.dz, w.symmetry, w.lmax, omega=(w.omega if omega == "w" else omega))
+    for k, v in (options or {}).items():
+        s.set_option(k, v)
+    if boundary is not None:
+        s.set_boundary(*boundary)
+    rho = torch.from_numpy(w.rho).cuda()
+    phi = torch.zeros_like(rho) if phi0 is None else torch.from_numpy(np.ascontiguousarray(phi0)).cuda()
+    r = s.solve(rho, phi, tol, max_sweeps)
+    torch.cuda.synchronize()
+    return s, phi.cpu().numpy(), r
+
+
+def relmax(a, b):
+    return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
+
+
+PATHS = [{"path": 1}, {"path": 1, "chunk": 3}]
+
+
+# ----------------------------------------------------------------------------------------------------------
+# bit-exact iteration history with injected ghosts (several tiles + ragged tails, both symmetries)
+# ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nr,nz,symmetry", [(37, 53, 1), (130, 70, 0), (64, 64, 1), (2, 2, 0), (3, 2, 1), (257, 33, 0)])
+@pytest.mark.parametrize("opts", PATHS)
+def test_sweeps_bit_exact_with_injected_ghosts(P, torch_cuda, oracle, nr, nz, symmetry, opts):
+    w = W.random_smooth(nr, nz, symmetry, seed=100 + nr, lmax=4)
+    M = oracle.moments(w.rho, w.dr, w.dz, symmetry, w.lmax)
+    bnd = oracle.boundary(nr, nz, w.dr, w.dz, symmetry, w.lmax, M)
+    omega = oracle.default_omega(nr, nz, w.dr, w.dz, symmetry)
+    phi0 = np.array([[W.uniform(3, nr, j * nr + i, -1, 1) for i in range(nr)] for j in range(nz)])
+    for k in (1, 2, 10, 100):
+        want, Rabs, Pk = oracle.sweeps(w.rho, phi0, w.dr, w.dz, symmetry, omega, *bnd, k)
+        s, got, r = gpu_solve(P, torch_cuda, w, phi0=phi0, tol=0.0, max_sweeps=k, boundary=bnd, options=opts)
+        assert r.sweeps == k and r.status == 0
+        assert s.omega == omega
+        assert np.array_equal(got, want), f"k={k}: max diff {np.max(np.abs(got - want))}"
+        maxf = np.max(np.abs(12.566370614359172 * w.rho))
+        hist = s.history(k)
+        want_hist = np.array([oracle.ratio(Rabs[q], Pk[q], maxf, w.dr, w.dz) for q in range(k)])
+        assert np.array_equal(hist, want_hist)
+        assert r.residual == want_hist[-1]
+
+
+# ----------------------------------------------------------------------------------------------------------
+# whole path with the library's own moments / boundary
+# ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nr,nz,symmetry,lmax", [(48, 40, 1, 8), (40, 72, 0, 7), (96, 96, 1, 16), (33, 65, 0, 32),
+                                                 (20, 20, 1, 64), (16, 16, 0, 0)])
+def test_moments_and_boundary_match_oracle(P, torch_cuda, oracle, nr, nz, symmetry, lmax):
+    w = W.random_smooth(nr, nz, symmetry, seed=200 + lmax, lmax=lmax)
+    s, _, _ = gpu_solve(P, torch_cuda, w, tol=0.0, max_sweeps=1)
+    M = oracle.moments(w.rho, w.dr, w.dz, symmetry, lmax)
+    got = s.moments()
+    scale = np.abs(M[0])
+    assert np.max(np.abs(got - M)) <= 1e-13 * scale
+    if symmetry == 1:
+        assert np.all(got[1::2] == 0.0)
+    bnd = oracle.boundary(nr, nz, w.dr, w.dz, symmetry, lmax, M)
+    gb = s.boundary()
+    for a, b in zip(gb, bnd):
+        if b is not None:
+            assert relmax(a, b) <= 1e-13
+
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2_128", "cfg3_64"])
+def test_config_parity_small(P, torch_cuda, oracle, name):
+    w = {"cfg0": W.cfg0, "cfg1": lambda: W.cfg1(128), "cfg2_128": lambda: W.cfg2(128),
+         "cfg3_64": lambda: W.cfg3(64).first}[name]()
+    ref = oracle.solve_workload(w, history=True)
+    s, got, r = gpu_solve(P, torch_cuda, w)
+    assert r.status == ref["status"] == 0
+    assert abs(r.sweeps - ref["sweeps"]) <= 1
+    if r.sweeps == ref["sweeps"]:
+        assert relmax(got, ref["phi"]) <= REL
+        assert r.residual == pytest.approx(ref["residual"], rel=1e-6)
+    # identical sweep count, fixed: k = 1, 10, 100 (the end state alone tests little once stagnated)
+    for k in (1, 10, 100):
+        refk = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, w.symmetry, w.lmax, 0.0, k, omega=w.omega)
+        _, gk, rk = gpu_solve(P, torch_cuda, w, tol=0.0, max_sweeps=k)
+        assert rk.sweeps == k
+        assert relmax(gk, refk["phi"]) <= REL
+
+
+def test_cfg1_full_size_parity_and_closed_form(P, torch_cuda, oracle):
+    """[CFG 1] 256x256 polytrope to 1e-10 -- the configuration bench.py times."""
+    w = W.cfg1()
+    ref = oracle.solve_workload(w)
+    s, got, r = gpu_solve(P, torch_cuda, w)
+    assert r.status == 0 and abs(r.sweeps - ref["sweeps"]) <= 1
+    if r.sweeps == ref["sweeps"]:
+        assert relmax(got, ref["phi"]) <= REL
+    rr, zz = W.cell_centres(w.nr, w.nz, w.dr, w.dz, 1)
+    sph = np.hypot(rr[None, :], zz[:, None])
+    R = 0.8
+    x = np.pi * sph / R
+    exact = np.where(sph < R, -4 * np.pi * (R / np.pi) ** 2 * (1 + np.sin(x) / x), -(4 * R ** 3 / np.pi) / sph)
+    assert np.max(np.abs(got - exact)) < 2.5e-5
+
+
+def test_cfg2_full_size_parity(P, torch_cuda, oracle):
+    """[CFG 2] 512x512 WD with 20 bubbles to 1e-10."""
+    w = W.cfg2()
+    ref = oracle.solve_workload(w)
+    s, got, r = gpu_solve(P, torch_cuda, w)
+    assert r.status == 0 and abs(r.sweeps - ref["sweeps"]) <= 1
+    if r.sweeps == ref["sweeps"]:
+        assert relmax(got, ref["phi"]) <= REL
+
+
+def test_cfg3_warm_started_sequence_reduced(P, torch_cuda, oracle):
+    """[CFG 3] at 128x256: cold solve then warm-started solves on the perturbed density, each vs the oracle."""
+    seq = W.cfg3(128, nsteps=3)
+    w = seq.first
+    s = P.PoissonSolver.for_workload(w)
+    rho = w.rho
+    phi_ref = np.zeros_like(rho)
+    phi_gpu = torch_cuda.zeros(rho.shape, dtype=torch_cuda.float64, device="cuda")
+    counts = []
+    for t in range(3):
+        if t > 0:
+            rho = seq.step(rho, t)
+        ref = oracle.solve(rho, phi_ref, w.dr, w.dz, 0, w.lmax, w.tol, w.max_sweeps)
+        r = s.solve(torch_cuda.from_numpy(rho).cuda(), phi_gpu, w.tol, w.max_sweeps)
+        assert r.status == 0 and abs(r.sweeps - ref["sweeps"]) <= 1
+        if r.sweeps == ref["sweeps"]:
+            assert relmax(phi_gpu.cpu().numpy(), ref["phi"]) <= REL
+        phi_ref = ref["phi"]
+        phi_gpu.copy_(torch_cuda.from_numpy(phi_ref))      # keep both on the same trajectory
+        counts.append(r.sweeps)
+    assert counts[1] < counts[0] and counts[2] < counts[0]      # warm start helps
+
+
+def test_cfg3_full_size_fixed_sweeps_and_converged_property(P, torch_cuda, oracle):
+    """[CFG 3] 1024x2048, lmax 32: 12 sweeps element by element (bit-exact ghosts aside), then the converged solve
+    is checked by a property that holds at any size: the oracle's plain-arithmetic operator residual is tiny."""
+    w = W.cfg3().first
+    ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, 0, w.lmax, 0.0, 12)
+    s, got, r = gpu_solve(P, torch_cuda, w, tol=0.0, max_sweeps=12)
+    assert r.sweeps == 12 and relmax(got, ref["phi"]) <= REL
+    s, got, r = gpu_solve(P, torch_cuda, w)
+    assert r.status == 0 and 3000 < r.sweeps < 8000
+    bE, bN, bS = s.boundary()
+    f = 12.566370614359172 * w.rho
+    res = oracle.apply_operator(got, w.dr, w.dz, 0, bE, bN, bS) - f
+    D = 2 / w.dr ** 2 + 2 / w.dz ** 2
+    assert np.max(np.abs(res)) / (np.max(np.abs(f)) + D * np.max(np.abs(got))) < 5e-10
+    # sampled rows re-derived by the oracle from the GPU field: one more oracle sweep barely moves it
+    nxt, Rabs, Pk = oracle.sweeps(w.rho, got, w.dr, w.dz, 0, s.omega, bE, bN, bS, 1)
+    assert oracle.ratio(Rabs[0], Pk[0], np.max(np.abs(f)), w.dr, w.dz) <= 1.05e-10
+
+
+def test_batch_matches_individual_oracle_solves(P, torch_cuda, oracle):
+    """[CFG 4a] reduced to 6 members of 128x128; members converge at different sweep counts."""
+    ws = [W.cfg4a_member(b, 128) for b in range(6)]
+    w0 = ws[0]
+    s = P.PoissonSolver.for_workload(w0)
+    rho = torch_cuda.from_numpy(np.stack([w.rho for w in ws])).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    res = s.solve(rho, phi, w0.tol, w0.max_sweeps)
+    got = phi.cpu().numpy()
+    sweeps = set()
+    for b, w in enumerate(ws):
+        ref = oracle.solve_workload(w)
+        assert res[b].status == 0 and abs(res[b].sweeps - ref["sweeps"]) <= 1
+        if res[b].sweeps == ref["sweeps"]:
+            assert relmax(got[b], ref["phi"]) <= REL
+        sweeps.add(res[b].sweeps)
+    assert len(sweeps) > 1
+
+
+def test_batch_full_size_sampled_members(P, torch_cuda, oracle):
+    """[CFG 4a] 64 x 512x512 in the launch configuration bench.py uses; 2 sampled members vs the oracle."""
+    ws = W.cfg4a(64)
+    s = P.PoissonSolver.for_workload(ws[0])
+    rho = torch_cuda.from_numpy(np.stack([w.rho for w in ws])).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    res = s.solve(rho, phi, ws[0].tol, ws[0].max_sweeps)
+    assert all(r.status == 0 for r in res)
+    for b in (5, 41):
+        ref = oracle.solve_workload(ws[b])
+        assert abs(res[b].sweeps - ref["sweeps"]) <= 1
+        if res[b].sweeps == ref["sweeps"]:
+            assert relmax(phi[b].cpu().numpy(), ref["phi"]) <= REL
+
+
+def test_size_sweep_points_fixed_sweeps(P, torch_cuda, oracle):
+    """[CFG 4b] fixed-sweep throughput points: 30 sweeps at 1024 and 2048 vs the oracle, element by element."""
+    for n in (1024, 2048):
+        w = W.cfg4b(n, max_sweeps=30)
+        ref = oracle.solve_workload(w)
+        _, got, r = gpu_solve(P, torch_cuda, w)
+        assert r.sweeps == 30 and relmax(got, ref["phi"]) <= REL
+
+
+# ----------------------------------------------------------------------------------------------------------
+# contract / edge cases
+# ----------------------------------------------------------------------------------------------------------
+def test_status_codes_and_degenerate_inputs(P, torch_cuda, oracle):
+    w = W.random_smooth(24, 24, 1, seed=15, lmax=6)
+    ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, 1, 6, 1e-9, 5000)
+    _, got, r = gpu_solve(P, torch_cuda, w, tol=1e-9, max_sweeps=5000)
+    assert (r.sweeps, r.status) == (ref["sweeps"], 0)
+    # max_sweeps hit
+    _, _, r = gpu_solve(P, torch_cuda, w, tol=1e-9, max_sweeps=ref["sweeps"] - 1)
+    assert r.status == 1 and r.sweeps == ref["sweeps"] - 1
+    # exactly at max_sweeps
+    _, _, r = gpu_solve(P, torch_cuda, w, tol=1e-9, max_sweeps=ref["sweeps"])
+    assert r.status == 0 and r.sweeps == ref["sweeps"]
+    # zero sweeps: phi untouched
+    phi0 = np.full_like(w.rho, 0.25)
+    _, got, r = gpu_solve(P, torch_cuda, w, phi0=phi0, tol=1e-9, max_sweeps=0)
+    assert r.sweeps == 0 and r.status == 1 and np.array_equal(got, phi0)
+    # warm start from the converged field stops after one sweep
+    _, _, r = gpu_solve(P, torch_cuda, w, phi0=oracle.solve(w.rho, phi0, w.dr, w.dz, 1, 6, 0.0, 3000)["phi"],
+                        tol=1e-9, max_sweeps=50)
+    assert r.sweeps == 1 and r.status == 0
+    # zero density: converged at once with residual 0
+    z = W.Workload("z", 16, 16, 0.1, 0.1, 1, 4, 1e-10, 50, np.zeros((16, 16)))
+    _, got, r = gpu_solve(P, torch_cuda, z)
+    assert r.sweeps == 1 and r.status == 0 and r.residual == 0.0 and np.all(got == 0)
+    # NaN density -> status -3 raised as an error by the wrapper
+    n = W.Workload("n", 16, 16, 0.1, 0.1, 1, 0, 1e-10, 50, np.full((16, 16), np.nan))
+    with pytest.raises(P.SnPoissonError):
+        gpu_solve(P, torch_cuda, n)
+
+
+def test_user_omega_and_default_restore(P, torch_cuda, oracle):
+    w = W.random_smooth(30, 30, 1, seed=31, lmax=4)
+    s = P.PoissonSolver.for_workload(w)
+    assert s.omega == oracle.default_omega(30, 30, w.dr, w.dz, 1)
+    assert P.sn_poisson_set_omega(s.h, 1.5) == 0 and s.omega == 1.5
+    assert P.sn_poisson_set_omega(s.h, 2.5) == -1
+    assert P.sn_poisson_set_omega(s.h, 0.0) == 0 and s.omega == oracle.default_omega(30, 30, w.dr, w.dz, 1)
+    _, got, r = gpu_solve(P, torch_cuda, w, tol=0.0, max_sweeps=40, omega=1.5)
+    ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, 1, 4, 0.0, 40, omega=1.5)
+    assert relmax(got, ref["phi"]) <= REL
+
+
+def test_solve_host_equals_device_solve(P, torch_cuda, oracle):
+    w = W.cfg1(64)
+    s, got, r = gpu_solve(P, torch_cuda, w)
+    phi_h = np.zeros_like(w.rho)
+    r2 = s.solve_host(w.rho, phi_h, w.tol, w.max_sweeps)
+    assert (r2.sweeps, r2.status, r2.residual) == (r.sweeps, r.status, r.residual)
+    assert np.array_equal(phi_h, got)
+    assert s.stat("launches") > 0 and s.stat("sweep_ms") > 0
+
+
+def test_rho_is_never_modified_and_stream_is_respected(P, torch_cuda):
+    w = W.cfg2(128)
+    s = P.PoissonSolver.for_workload(w)
+    rho = torch_cuda.from_numpy(w.rho).cuda()
+    keep = rho.clone()
+    st = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(st):
+        phi = torch_cuda.zeros_like(rho)
+        r = s.solve(rho, phi, w.tol, w.max_sweeps)
+    st.synchronize()
+    assert r.status == 0 and torch_cuda.equal(rho, keep)
