@@ -3,16 +3,20 @@
 // moments.cuh / sweep_stream.cuh / sweep_resident.cuh.  No CPU fallback.
 #include "../../include/sn_poisson.h"
 
+#include <type_traits>
+
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <string>
 #include <vector>
 
 #include "common.cuh"
 #include "moments.cuh"
 #include "sweep_stream.cuh"
+#include "sweep_resident.cuh"
 
 using namespace snp;
 
@@ -57,7 +61,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -68,12 +72,16 @@ struct sn_poisson {
     Ctl* d_ctl = nullptr;
     Ctl* h_ctl = nullptr;       // pinned, 2 * cap_batch (double-buffered polls)
     double *d_rho_stage = nullptr, *d_phi_stage = nullptr;   // solve_host staging
+    double* d_alt = nullptr;                                 // resident path: odd-epoch phi buffer
+    unsigned int* d_sync = nullptr;                          // resident path: flags | arrived | gbar
+    size_t sync_cap = 0;
     bool user_boundary = false;
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
     cudaEvent_t ev_t[3] = {nullptr, nullptr, nullptr};
 
     // stats of the last solve
     double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
+    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1;
     int last_sweeps0 = 0;
 };
 
@@ -203,6 +211,125 @@ int run_stream(sn_poisson* h, const Geom& g, int nbatch, const double* rho, doub
     return 0;
 }
 
+
+// ---- resident path: shapes, planner, launcher ------------------------------------------------------------------
+struct ShapeInfo {
+    int H, TXN, TYN;
+    size_t smem;
+    const void* fn;
+    int BW() const { return 4 * TXN; }
+    int BH() const { return H * TYN; }
+    int NT() const { return TXN * TYN; }
+};
+
+template <int H, int TXN, int TYN>
+ShapeInfo shape_of() {
+    return {H, TXN, TYN, ResShape<H, TXN, TYN>::smem_bytes, (const void*)k_sor_resident<H, TXN, TYN>};
+}
+
+const std::vector<ShapeInfo>& shapes() {
+    static const std::vector<ShapeInfo> v = {
+        shape_of<8, 32, 14>(),   // 0: box 128 x 112, 448 threads
+        shape_of<8, 32, 8>(),    // 1: box 128 x 64,  256 threads
+        shape_of<8, 16, 8>(),    // 2: box 64 x 64,   128 threads
+        shape_of<4, 16, 8>(),    // 3: box 64 x 32,   128 threads
+        shape_of<4, 8, 8>(),     // 4: box 32 x 32,    64 threads
+        shape_of<2, 8, 16>(),    // 5: box 32 x 32,   128 threads
+    };
+    return v;
+}
+
+struct ResPlan {
+    int shape = -1, m = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
+    double cost = 0;
+};
+
+int round_up(int v, int q) { return (v + q - 1) / q * q; }
+
+// Tiling of one axis: n cells, box extent B, margin h per interior side, alignment q.
+// Returns the number of tiles and the owned extent (multiple of q), or false if the box cannot hold a tile.
+bool plan_axis(int n, int B, int h, int q, int* nt, int* own) {
+    if (n % q || n < B) return false;
+    if (n == B) { *nt = 1; *own = n; return true; }
+    const int slack = h % q;                       // the box origin is rounded down to a multiple of q
+    int omax = (B - 2 * h - slack) / q * q;
+    if (omax < q) return false;
+    int t = (n + omax - 1) / omax;
+    int o = round_up((n + t - 1) / t, q);
+    if (o > omax) o = omax;
+    t = (n + o - 1) / o;
+    *nt = t;
+    *own = o;
+    return true;
+}
+
+// Pick (shape, m) minimising a simple per-sweep cost model; honours the "shape"/"tblock" overrides.
+ResPlan plan_resident(sn_poisson* h, const double* rho, const double* phi) {
+    ResPlan best;
+    if (((uintptr_t)rho | (uintptr_t)phi) & 15) return best;
+    const auto& sh = shapes();
+    for (int si = 0; si < (int)sh.size(); ++si) {
+        if (h->opt_shape >= 0 && si != h->opt_shape) continue;
+        const ShapeInfo& S = sh[si];
+        int occ = 0;
+        if (cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn, S.NT(), S.smem) != cudaSuccess || occ < 1) {
+            cudaGetLastError();
+            continue;
+        }
+        const int max_tiles = occ * h->num_sms;
+        for (int m = 1; m <= kMaxTB; ++m) {
+            if (h->opt_tblock > 0 && m != h->opt_tblock) continue;
+            ResPlan p;
+            if (!plan_axis(h->nr, S.BW(), 2 * m, 4, &p.ntx, &p.ow)) continue;
+            if (!plan_axis(h->nz, S.BH(), 2 * m, S.H, &p.nty, &p.oh)) continue;
+            p.ntiles = p.ntx * p.nty;
+            if (p.ntiles > max_tiles) continue;
+            p.shape = si;
+            p.m = m;
+            // cost model (SM clocks per sweep): CTAs sharing an SM serialise on the fp64 pipe; one exchange per m sweeps
+            const double per_sm = (double)((p.ntiles + h->num_sms - 1) / h->num_sms);
+            const double warps = per_sm * S.NT() / 32.0;
+            const double rate = std::min(3.2, 0.45 * warps);             // cell-updates per clock per SM
+            const double compute = per_sm * S.BW() * S.BH() / rate + 2.0 * 150.0;
+            const double exchange = 3500.0 + 8.0 * S.BW() * S.BH() / 48.0;
+            p.cost = compute + exchange / m;
+            if (best.shape < 0 || p.cost < best.cost) best = p;
+        }
+    }
+    return best;
+}
+
+int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, const double* rho, double* phi, int max_sweeps,
+                 cudaStream_t st) {
+    const ShapeInfo& S = shapes()[pl.shape];
+    const size_t ncell = (size_t)h->nr * h->nz;
+    if (!h->d_alt) CU_TRY(cudaMalloc((void**)&h->d_alt, sizeof(double) * ncell));
+    const size_t nep = (size_t)(max_sweeps + pl.m - 1) / pl.m + 2;
+    const size_t nsync = (size_t)pl.ntiles + nep + 1;
+    if (nsync > h->sync_cap) {
+        cudaFree(h->d_sync);
+        h->d_sync = nullptr;
+        CU_TRY(cudaMalloc((void**)&h->d_sync, sizeof(unsigned int) * nsync));
+        h->sync_cap = nsync;
+    }
+    CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * nsync, st));
+    ResParams P;
+    P.g = g;
+    P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.max_sweeps = max_sweeps;
+    P.rho = rho; P.buf0 = phi; P.buf1 = h->d_alt;
+    P.bE = h->d_bE; P.bN = h->d_bN; P.bS = h->d_bS;
+    P.slots = h->d_slots; P.ctl = h->d_ctl; P.hist = h->d_hist;
+    P.flags = h->d_sync; P.arrived = h->d_sync + pl.ntiles; P.gbar = h->d_sync + pl.ntiles + nep;
+    void* args[] = {&P};
+    CU_TRY(cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
+    CU_TRY(cudaLaunchCooperativeKernel(S.fn, dim3(pl.ntiles), dim3(S.NT()), args, S.smem, st));
+    h->st_launches += 1;
+    h->st_path = 2;
+    h->st_ctas = pl.ntiles; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.m; h->st_shape = pl.shape;
+    return 0;
+}
+
 int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double tol, int max_sweeps,
                cudaStream_t st, sn_poisson_result* out) {
     CU_TRY(cudaSetDevice(h->device));
@@ -226,7 +353,18 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     }
     CU_TRY(cudaEventRecord(h->ev_t[1], st));
     // a-2 + a-3
-    if (int rc = run_stream(h, g, nbatch, rho, phi, max_sweeps, st)) return rc;
+    ResPlan pl;
+    if (h->opt_path != 1 && nbatch == 1 && max_sweeps > 0) pl = plan_resident(h, rho, phi);
+    if (h->opt_path == 2 && pl.shape < 0 && max_sweeps > 0) {
+        set_err("resident path requested but not eligible (needs nbatch=1, nr%%4==0, nz%%H==0, grid >= one box, "
+                "16-byte aligned pointers, tiles <= co-resident CTAs)");
+        return -1;
+    }
+    if (pl.shape >= 0) {
+        if (int rc = run_resident(h, g, pl, rho, phi, max_sweeps, st)) return rc;
+    } else {
+        if (int rc = run_stream(h, g, nbatch, rho, phi, max_sweeps, st)) return rc;
+    }
     CU_TRY(cudaEventRecord(h->ev_t[2], st));
     CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl) * nbatch, cudaMemcpyDeviceToHost, st));
     CU_TRY(cudaStreamSynchronize(st));
@@ -315,6 +453,7 @@ void sn_poisson_destroy(sn_poisson* h) {
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
     cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage);
+    cudaFree(h->d_alt); cudaFree(h->d_sync);
     for (auto& e : h->ev_poll) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev_t) if (e) cudaEventDestroy(e);
     delete h;
@@ -430,7 +569,8 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!h || !key) { set_err("NULL argument"); return -1; }
     if (!strcmp(key, "path")) { if (value < 0 || value > 2) { set_err("path must be 0..2"); return -1; } h->opt_path = (int)value; return 0; }
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
-    if (!strcmp(key, "tblock")) { if (value < 0 || value > 16) { set_err("tblock must be 0..16"); return -1; } h->opt_tblock = (int)value; return 0; }
+    if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)shapes().size()) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
+    if (!strcmp(key, "tblock")) { if (value < 0 || value > kMaxTB) { set_err("tblock must be 0..%d", kMaxTB); return -1; } h->opt_tblock = (int)value; return 0; }
     set_err("unknown option '%s'", key);
     return -1;
 }
@@ -442,6 +582,11 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "sweep_ms")) { *out = h->st_sweep_ms; return 0; }
     if (!strcmp(key, "setup_ms")) { *out = h->st_setup_ms; return 0; }
     if (!strcmp(key, "path")) { *out = h->st_path; return 0; }
+    if (!strcmp(key, "ctas")) { *out = h->st_ctas; return 0; }
+    if (!strcmp(key, "tile_w")) { *out = h->st_tile_w; return 0; }
+    if (!strcmp(key, "tile_h")) { *out = h->st_tile_h; return 0; }
+    if (!strcmp(key, "tblock")) { *out = h->st_tblock; return 0; }
+    if (!strcmp(key, "shape")) { *out = h->st_shape; return 0; }
     set_err("unknown stat '%s'", key);
     return -1;
 }
