@@ -72,7 +72,7 @@ struct sn_poisson {
     Ctl* d_ctl = nullptr;
     Ctl* h_ctl = nullptr;       // pinned, 2 * cap_batch (double-buffered polls)
     double *d_rho_stage = nullptr, *d_phi_stage = nullptr;   // solve_host staging
-    double* d_alt = nullptr;                                 // resident path: odd-epoch phi buffer
+    double* d_alt = nullptr;                                 // resident path: 2 x nr*nz, states of epochs e%3 = 1,2
     unsigned int* d_sync = nullptr;                          // resident path: flags | arrived | gbar
     size_t sync_cap = 0;
     bool user_boundary = false;
@@ -244,25 +244,6 @@ struct ResPlan {
     double cost = 0;
 };
 
-int round_up(int v, int q) { return (v + q - 1) / q * q; }
-
-// Tiling of one axis: n cells, box extent B, margin h per interior side, alignment q.
-// Returns the number of tiles and the owned extent (multiple of q), or false if the box cannot hold a tile.
-bool plan_axis(int n, int B, int h, int q, int* nt, int* own) {
-    if (n % q || n < B) return false;
-    if (n == B) { *nt = 1; *own = n; return true; }
-    const int slack = h % q;                       // the box origin is rounded down to a multiple of q
-    int omax = (B - 2 * h - slack) / q * q;
-    if (omax < q) return false;
-    int t = (n + omax - 1) / omax;
-    int o = round_up((n + t - 1) / t, q);
-    if (o > omax) o = omax;
-    t = (n + o - 1) / o;
-    *nt = t;
-    *own = o;
-    return true;
-}
-
 // Pick (shape, m) minimising a simple per-sweep cost model; honours the "shape"/"tblock" overrides.
 ResPlan plan_resident(sn_poisson* h, const double* rho, const double* phi) {
     ResPlan best;
@@ -285,6 +266,10 @@ ResPlan plan_resident(sn_poisson* h, const double* rho, const double* phi) {
             if (!plan_axis(h->nz, S.BH(), 2 * m, S.H, &p.nty, &p.oh)) continue;
             p.ntiles = p.ntx * p.nty;
             if (p.ntiles > max_tiles) continue;
+            bool ok = true;                      // the property the kernel relies on, checked for every tile
+            for (int t = 0; t < p.ntx && ok; ++t) ok = box_covers(t, p.ow, 2 * m, 4, S.BW(), h->nr);
+            for (int t = 0; t < p.nty && ok; ++t) ok = box_covers(t, p.oh, 2 * m, S.H, S.BH(), h->nz);
+            if (!ok) continue;
             p.shape = si;
             p.m = m;
             // cost model (SM clocks per sweep): CTAs sharing an SM serialise on the fp64 pipe; one exchange per m sweeps
@@ -304,7 +289,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, const double* 
                  cudaStream_t st) {
     const ShapeInfo& S = shapes()[pl.shape];
     const size_t ncell = (size_t)h->nr * h->nz;
-    if (!h->d_alt) CU_TRY(cudaMalloc((void**)&h->d_alt, sizeof(double) * ncell));
+    if (!h->d_alt) CU_TRY(cudaMalloc((void**)&h->d_alt, sizeof(double) * 2 * ncell));
     const size_t nep = (size_t)(max_sweeps + pl.m - 1) / pl.m + 2;
     const size_t nsync = (size_t)pl.ntiles + nep + 1;
     if (nsync > h->sync_cap) {
@@ -317,7 +302,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, const double* 
     ResParams P;
     P.g = g;
     P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.max_sweeps = max_sweeps;
-    P.rho = rho; P.buf0 = phi; P.buf1 = h->d_alt;
+    P.rho = rho; P.buf[0] = phi; P.buf[1] = h->d_alt; P.buf[2] = h->d_alt + ncell;
     P.bE = h->d_bE; P.bN = h->d_bN; P.bS = h->d_bS;
     P.slots = h->d_slots; P.ctl = h->d_ctl; P.hist = h->d_hist;
     P.flags = h->d_sync; P.arrived = h->d_sync + pl.ntiles; P.gbar = h->d_sync + pl.ntiles + nep;

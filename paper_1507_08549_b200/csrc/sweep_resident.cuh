@@ -24,6 +24,7 @@
 //    exactly k* sweeps applied, like the oracle's.
 #pragma once
 #include "common.cuh"
+#include "tiling.h"
 
 namespace snp {
 
@@ -36,8 +37,8 @@ struct ResParams {
     int m;                     // sweeps per epoch
     int max_sweeps;
     const double* rho;
-    double* buf0;              // caller's phi_inout: state of even epochs, initial guess and final result
-    double* buf1;              // workspace: state of odd epochs
+    double* buf[3];            // state of epoch e lives in buf[e % 3]; buf[0] = caller's phi_inout (initial guess,
+                               // final result), buf[1..2] = workspace
     const double* bE;
     const double* bN;
     const double* bS;
@@ -56,6 +57,9 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
 }
 __device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void red_release_add_u32(unsigned* p, unsigned v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ void spin_until_ge(const unsigned* p, unsigned want) {
     while (ld_acquire_u32(p) < want) __nanosleep(20);
@@ -108,10 +112,8 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
     // owned tile [x0,x1) x [y0,y1) and box origin (bx,by), all aligned to (4,H)
     const int x0 = tx * p.ow, x1 = min(g.nr, x0 + p.ow);
     const int y0 = ty * p.oh, y1 = min(g.nz, y0 + p.oh);
-    int bx = max(x0 - h, 0) & ~3;
-    bx = min(bx, g.nr - BW);
-    int by = (max(y0 - h, 0) / H) * H;
-    by = min(by, g.nz - BH);
+    const int bx = box_origin(x0, h, 4, BW, g.nr);
+    const int by = box_origin(y0, h, H, BH, g.nz);
     const int gi0 = bx + 4 * a, gj0 = by + H * b;
     const bool own = gi0 >= x0 && gi0 < x1 && gj0 >= y0 && gj0 < y1;
     const int rowbase = H * b;
@@ -188,7 +190,7 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
         exB[c] = 0.0;
         exT[(size_t)(TYN + 1) * BW + c] = 0.0;
     }
-    load_patch(p.buf0);
+    load_patch(p.buf[0]);
     publish_all();
     __syncthreads();
 
@@ -274,6 +276,10 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
     };
 
     // ---- epoch loop ------------------------------------------------------------------------------------------
+    // End of epoch e:  store state e -> release flag  |  post maxima, arrive  |  acquire neighbour flags -> reload
+    // margins  |  decide epoch e-1 while those loads are in flight.  State e overwrites state e-3, which nobody can
+    // still be reading: the decision for epoch e-2 (taken during the end of epoch e-1) waited for every CTA to have
+    // finished epoch e-2.  The state before any epoch whose sweeps are still undecided therefore stays intact.
     int done = 0, e = 0, kstar = 0, e_cross = 0;
     while (done < p.max_sweeps) {
         ++e;
@@ -289,6 +295,9 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
                 smax[(2 * s + 1) * NW + warp] = wp;
             }
         }
+        const bool last = done + nsw >= p.max_sweeps;
+        double* cur = p.buf[e % 3];
+        if (!last && own) store_patch(cur);
         // any non-finite owned value persists (NaN/Inf never relax away): poison this epoch's maxima
         bool bad = false;
         if (own) {
@@ -297,7 +306,8 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
 #pragma unroll
                 for (int c = 0; c < 4; ++c) bad |= !(fabs(phi[q][c]) < INFINITY);
         }
-        const int anybad = __syncthreads_or(bad);
+        const int anybad = __syncthreads_or(bad);            // also: every thread's state stores are issued
+        if (!last && tid == 0) st_release_u32(p.flags + tile, (unsigned)e);
         if (warp == 0) {
             for (int idx = lane; idx < 2 * nsw; idx += 32) {
                 unsigned long long v = 0ull;
@@ -309,31 +319,19 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
                 atomicMax(p.slots + 2 * (size_t)(done + (idx >> 1)) + (idx & 1), v);
             }
             __syncwarp();
-            if (lane == 0) {
-                __threadfence();
-                atomicAdd(p.arrived + e, 1u);
-            }
+            if (lane == 0) red_release_add_u32(p.arrived + e, 1u);
         }
         done += nsw;
-        // decide epoch e-1 (one epoch late: its arrivals are long complete), then, at the very end, epoch e
-        if (e >= 2) {
-            kstar = check_epoch(e - 1);
-            if (kstar) { e_cross = e - 1; break; }
-        }
-        if (done >= p.max_sweeps) {
+        if (last) {
+            if (e >= 2) {
+                kstar = check_epoch(e - 1);
+                if (kstar) { e_cross = e - 1; break; }
+            }
             kstar = check_epoch(e);
             if (kstar) e_cross = e;
             break;
         }
-        // publish state e, then pull the margins of the box from the neighbours' state e
-        double* cur = (e & 1) ? p.buf1 : p.buf0;
-        if (own) store_patch(cur);
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            st_release_u32(p.flags + tile, (unsigned)e);
-        }
-        if (warp == 0) {
+        if (warp == NW - 1) {
             for (int n = lane; n < nnb; n += 32) {
                 const int nx = ntx0 + n % (ntx1 - ntx0 + 1), ny = nty0 + n / (ntx1 - ntx0 + 1);
                 spin_until_ge(p.flags + ny * p.ntx + nx, (unsigned)e);
@@ -341,20 +339,23 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
         }
         __syncthreads();
         if (!own) load_patch(cur);
+        if (e >= 2) {
+            kstar = check_epoch(e - 1);
+            if (kstar) { e_cross = e - 1; break; }
+        }
         publish_all();
         __syncthreads();
     }
 
     // ---- finish ----------------------------------------------------------------------------------------------
-    if (kstar) {
+    if (kstar && !(e_cross == e && kstar == done)) {
         // the rule fired at sweep kstar of epoch e_cross: replay it exactly from the state before that epoch
         const int es = e_cross - 1;
         const int r = kstar - es * m;
-        load_patch((es & 1) ? p.buf1 : p.buf0);
+        load_patch(p.buf[es % 3]);
         __syncthreads();
-        if (tid == 0) {                      // everyone has read its box before anyone overwrites buf0
-            __threadfence();
-            atomicAdd(p.gbar, 1u);
+        if (tid == 0) {                      // everyone has read its box before anyone overwrites buf[0]
+            red_release_add_u32(p.gbar, 1u);
             spin_until_ge(p.gbar, (unsigned)ntiles);
         }
         __syncthreads();
@@ -365,7 +366,7 @@ __global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p)
             half_sweep(C1{}, std::false_type{});
         }
     }
-    if (own) store_patch(p.buf0);
+    if (own) store_patch(p.buf[0]);
     if (tile == 0 && tid == 0) {
         Ctl* c = p.ctl;
         const double R = s_R;
