@@ -10,15 +10,29 @@ constexpr double kFourPi = 12.566370614359172;   // 4*pi rounded to fp64 (DESIGN
 constexpr double kPi = 3.141592653589793;
 constexpr int kMaxL = 64;
 
-// Per-member control block written by the device-side stopping decision (step a-3).
+// Per-member control block.  Result fields are written by the device-side stopping decision (step a-3); the
+// "director" fields drive the blocked path (sweep_blocked.cuh), where the last CTA of every launch decides what
+// the next launch does for this member.
 struct Ctl {
-    int done;          // 1 once the stopping rule fired (or a non-finite ratio was seen)
-    int sweeps;        // full sweeps applied when it fired
+    int done;          // 1 once the member is finished (result fields valid, phi_inout holds the result)
+    int sweeps;        // full sweeps applied to the returned phi
     int status;        // 0 / 1 / -3 as in sn_poisson_result
     int pad;
-    double residual;   // R_k of that sweep
+    double residual;   // R_k of the last applied sweep
     double maxf;       // max |4 pi rho| (written by the moments pass)
+    // ---- director state (blocked path) ----
+    int action;        // what the next launch does: kActSkip / kActAdvance / kActRedo / kActReplay / kActCopy
+    int src;           // buffer the action reads (0 = caller's phi_inout, 1 = workspace); it writes the other one
+    int k0;            // sweeps already applied in the state it reads
+    int n;             // sweeps it runs
+    int track;         // TrackMode of the run
+    int fin_sweeps;    // result to publish once a replay / copy has completed
+    int fin_status;
+    unsigned int arrived;   // CTAs of this member that have finished the current launch
+    double fin_R;
 };
+
+enum BlockedAction : int { kActSkip = 0, kActAdvance = 1, kActRedo = 2, kActReplay = 3, kActCopy = 4 };
 
 // Grid geometry + coefficient tables; passed by value to every kernel.
 struct Geom {

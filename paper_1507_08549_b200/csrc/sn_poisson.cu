@@ -16,6 +16,7 @@
 #include "common.cuh"
 #include "moments.cuh"
 #include "sweep_stream.cuh"
+#include "sweep_blocked.cuh"
 #include "sweep_resident.cuh"
 
 using namespace snp;
@@ -61,13 +62,16 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
     double *d_cE = nullptr, *d_cW = nullptr;
     double *d_bE = nullptr, *d_bN = nullptr, *d_bS = nullptr, *d_M = nullptr, *d_partial = nullptr;
     unsigned long long* d_slots = nullptr;
+    unsigned int* d_slots_f = nullptr;                       // blocked path: FAST maxima (upper words)
+    double* d_work = nullptr;                                // blocked path: second phi buffer, work_cap doubles
+    size_t work_cap = 0;
     double* d_hist = nullptr;
     Ctl* d_ctl = nullptr;
     Ctl* h_ctl = nullptr;       // pinned, 2 * cap_batch (double-buffered polls)
@@ -117,10 +121,10 @@ Geom make_geom(const sn_poisson* h, double tol) {
 
 void free_batch_ws(sn_poisson* h) {
     cudaFree(h->d_bE); cudaFree(h->d_bN); cudaFree(h->d_bS); cudaFree(h->d_M); cudaFree(h->d_partial);
-    cudaFree(h->d_slots); cudaFree(h->d_hist); cudaFree(h->d_ctl);
+    cudaFree(h->d_slots); cudaFree(h->d_slots_f); cudaFree(h->d_hist); cudaFree(h->d_ctl);
     if (h->h_ctl) cudaFreeHost(h->h_ctl);
     h->d_bE = h->d_bN = h->d_bS = h->d_M = h->d_partial = h->d_hist = nullptr;
-    h->d_slots = nullptr; h->d_ctl = nullptr; h->h_ctl = nullptr;
+    h->d_slots = nullptr; h->d_slots_f = nullptr; h->d_ctl = nullptr; h->h_ctl = nullptr;
     h->cap_batch = 0; h->cap_sweeps = 0;
 }
 
@@ -140,7 +144,7 @@ int ensure_ws(sn_poisson* h, int nbatch, int max_sweeps) {
     free_batch_ws(h);
     if (dev_alloc(&h->d_bE, (size_t)nb * h->nz) || dev_alloc(&h->d_bN, (size_t)nb * h->nr) ||
         dev_alloc(&h->d_bS, (size_t)nb * h->nr) || dev_alloc(&h->d_M, (size_t)nb * (kMaxL + 1)) ||
-        dev_alloc(&h->d_partial, (size_t)nb * h->mom_blocks * h->NL) || dev_alloc(&h->d_slots, (size_t)nb * 2 * ns) ||
+        dev_alloc(&h->d_partial, (size_t)nb * h->mom_blocks * h->NL) || dev_alloc(&h->d_slots, (size_t)nb * 2 * ns) || dev_alloc(&h->d_slots_f, (size_t)nb * 2 * ns) ||
         dev_alloc(&h->d_hist, (size_t)nb * ns) || dev_alloc(&h->d_ctl, (size_t)nb))
         return -2;
     CU_TRY(cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl) * 2 * nb));
@@ -208,6 +212,141 @@ int run_stream(sn_poisson* h, const Geom& g, int nbatch, const double* rho, doub
     k_decide_last<<<nbatch, 32, 0, st>>>(g, k - 1, slot_stride, hist_stride, h->d_slots, h->d_ctl, h->d_hist);
     h->st_launches += 1;
     CU_TRY(cudaGetLastError());
+    return 0;
+}
+
+
+// ---- blocked path: shapes, planner, launcher -------------------------------------------------------------------
+struct BlkShapeInfo {
+    int H, TXN, TYN, minb;
+    size_t smem;
+    const void* fn;
+    double hs_clk;             // measured clocks per half-sweep of one box with `minb` CTAs sharing an SM (cost model)
+    int BW() const { return 4 * TXN; }
+    int BH() const { return H * TYN; }
+    int NT() const { return TXN * TYN; }
+};
+
+template <int H, int TXN, int TYN, int MINB>
+BlkShapeInfo blk_shape_of(double hs_clk) {
+    return {H, TXN, TYN, MINB, BlkShape<H, TXN, TYN>::smem_bytes, (const void*)k_sor_blocked<H, TXN, TYN, MINB>, hs_clk};
+}
+
+const std::vector<BlkShapeInfo>& blk_shapes() {
+    static const std::vector<BlkShapeInfo> v = {
+        blk_shape_of<8, 32, 8, 2>(1853.0),    // 0: box 128 x 64,  256 threads, 2 CTAs / SM
+        blk_shape_of<8, 32, 14, 1>(1516.0),   // 1: box 128 x 112, 448 threads
+        blk_shape_of<16, 32, 8, 1>(1562.0),   // 2: box 128 x 128, 256 threads
+        blk_shape_of<8, 16, 8, 3>(1400.0),    // 3: box 64 x 64,   128 threads, 3 CTAs / SM
+        blk_shape_of<4, 16, 8, 4>(1200.0),    // 4: box 64 x 32,   128 threads, 4 CTAs / SM
+    };
+    return v;
+}
+
+struct BlkPlan {
+    int shape = -1, m = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0, occ = 0;
+    double cost = 0;
+};
+
+// Pick (shape, m) minimising modelled clocks per sweep; honours the "shape"/"tblock" overrides.
+BlkPlan plan_blocked(sn_poisson* h, int nbatch, const double* rho, const double* phi) {
+    BlkPlan best;
+    if (((uintptr_t)rho | (uintptr_t)phi) & 15) return best;
+    const auto& sh = blk_shapes();
+    for (int si = 0; si < (int)sh.size(); ++si) {
+        if (h->opt_shape >= 0 && si != h->opt_shape) continue;
+        const BlkShapeInfo& S = sh[si];
+        int occ = 0;
+        if (cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn, S.NT(), S.smem) != cudaSuccess || occ < 1) {
+            cudaGetLastError();
+            continue;
+        }
+        if (occ > S.minb) occ = S.minb;
+        for (int m = 1; m <= kMaxTB; ++m) {
+            if (h->opt_tblock > 0 && m != h->opt_tblock) continue;
+            BlkPlan p;
+            if (!plan_axis(h->nr, S.BW(), 2 * m, 4, &p.ntx, &p.ow)) continue;
+            if (!plan_axis(h->nz, S.BH(), 2 * m, S.H, &p.nty, &p.oh)) continue;
+            bool ok = true;                      // the property the kernel relies on, checked for every tile
+            for (int t = 0; t < p.ntx && ok; ++t) ok = box_covers(t, p.ow, 2 * m, 4, S.BW(), h->nr);
+            for (int t = 0; t < p.nty && ok; ++t) ok = box_covers(t, p.oh, 2 * m, S.H, S.BH(), h->nz);
+            if (!ok) continue;
+            p.ntiles = p.ntx * p.nty;
+            p.shape = si;
+            p.m = m;
+            p.occ = occ;
+            // cost model (SM clocks per sweep): waves of CTAs; each CTA loads its box (16 B / cell at a share of the
+            // L2 / HBM bandwidth), runs 2m half-sweeps and stores its tile; plus the launch gap.
+            const double ctas = (double)p.ntiles * nbatch;
+            const double slots = (double)h->num_sms * occ;
+            const double waves = std::ceil(ctas / slots);
+            const double bytes = 16.0 * S.BW() * S.BH() + 8.0 * p.ow * p.oh;
+            const bool in_l2 = 16.0 * h->nr * h->nz * nbatch < 100e6;
+            const double bw_per_sm = (in_l2 ? 40.0 : 18.0) / occ;          // bytes per clock per CTA
+            const double t_cta = bytes / bw_per_sm * (occ > 1 ? 0.5 : 1.0) + 2.0 * m * S.hs_clk + 1500.0;
+            p.cost = (waves * t_cta + 4000.0) / m;
+            if (best.shape < 0 || p.cost < best.cost) best = p;
+        }
+    }
+    return best;
+}
+
+int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, const double* rho, double* phi,
+                int max_sweeps, cudaStream_t st) {
+    const BlkShapeInfo& S = blk_shapes()[pl.shape];
+    const size_t ncell = (size_t)h->nr * h->nz;
+    if (h->work_cap < ncell * nbatch) {
+        cudaFree(h->d_work);
+        h->d_work = nullptr;
+        h->work_cap = 0;
+        CU_TRY(cudaMalloc((void**)&h->d_work, sizeof(double) * ncell * nbatch));
+        h->work_cap = ncell * nbatch;
+    }
+    CU_TRY(cudaMemsetAsync(h->d_slots_f, 0, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
+    BlkParams P;
+    P.g = g;
+    P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.max_sweeps = max_sweeps;
+    P.force_exact = h->opt_exact;
+    P.nbatch = nbatch;
+    P.rho = rho; P.buf[0] = phi; P.buf[1] = h->d_work;
+    P.bE = h->d_bE; P.bN = h->d_bN; P.bS = h->d_bS;
+    P.slots_f = h->d_slots_f; P.slots_x = h->d_slots;
+    P.slot_stride = 2 * h->cap_sweeps; P.hist_stride = h->cap_sweeps;
+    P.ctl = h->d_ctl; P.hist = h->d_hist;
+    k_blocked_init<<<nbatch, 32, 0, st>>>(h->d_ctl, pl.m, max_sweeps, h->opt_exact);
+    h->st_launches += 1;
+    CU_TRY(cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
+    void* args[] = {&P};
+    const dim3 grid(pl.ntiles, nbatch), block(S.NT());
+    // every advance may be followed by one exact re-run; plus replay and copy
+    const long long bound = 2ll * ((max_sweeps + pl.m - 1) / pl.m) + 4;
+    const int chunk = h->opt_chunk < 1 ? 1 : h->opt_chunk;
+    long long launched = 0;
+    int poll = 0;
+    bool have_poll[2] = {false, false};
+    bool all_done = false;
+    while (launched < bound && !all_done) {
+        for (int i = 0; i < chunk && launched < bound; ++i, ++launched) {
+            CU_TRY(cudaLaunchKernel(S.fn, grid, block, args, S.smem, st));
+            h->st_launches += 1;
+        }
+        // poll the device-side decision one chunk behind, so the queue never drains
+        CU_TRY(cudaMemcpyAsync(h->h_ctl + (size_t)poll * h->cap_batch, h->d_ctl, sizeof(Ctl) * nbatch,
+                               cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaEventRecord(h->ev_poll[poll], st));
+        have_poll[poll] = true;
+        const int prev = poll ^ 1;
+        if (have_poll[prev]) {
+            CU_TRY(cudaEventSynchronize(h->ev_poll[prev]));
+            all_done = true;
+            for (int b = 0; b < nbatch; ++b) all_done = all_done && h->h_ctl[(size_t)prev * h->cap_batch + b].done;
+        }
+        poll ^= 1;
+    }
+    h->st_path = 3;
+    h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.m;
+    h->st_shape = pl.shape;
     return 0;
 }
 
@@ -339,14 +478,23 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     CU_TRY(cudaEventRecord(h->ev_t[1], st));
     // a-2 + a-3
     ResPlan pl;
-    if (h->opt_path != 1 && nbatch == 1 && max_sweeps > 0) pl = plan_resident(h, rho, phi);
+    BlkPlan bp;
+    if ((h->opt_path == 0 || h->opt_path == 2) && nbatch == 1 && max_sweeps > 0) pl = plan_resident(h, rho, phi);
     if (h->opt_path == 2 && pl.shape < 0 && max_sweeps > 0) {
         set_err("resident path requested but not eligible (needs nbatch=1, nr%%4==0, nz%%H==0, grid >= one box, "
                 "16-byte aligned pointers, tiles <= co-resident CTAs)");
         return -1;
     }
+    if ((h->opt_path == 0 || h->opt_path == 3) && pl.shape < 0 && max_sweeps > 0) bp = plan_blocked(h, nbatch, rho, phi);
+    if (h->opt_path == 3 && bp.shape < 0 && max_sweeps > 0) {
+        set_err("blocked path requested but not eligible (needs nr%%4==0, nz%%H==0, grid >= one box, 16-byte aligned "
+                "pointers)");
+        return -1;
+    }
     if (pl.shape >= 0) {
         if (int rc = run_resident(h, g, pl, rho, phi, max_sweeps, st)) return rc;
+    } else if (bp.shape >= 0) {
+        if (int rc = run_blocked(h, g, bp, nbatch, rho, phi, max_sweeps, st)) return rc;
     } else {
         if (int rc = run_stream(h, g, nbatch, rho, phi, max_sweeps, st)) return rc;
     }
@@ -359,6 +507,10 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     CU_TRY(cudaEventElapsedTime(&ms, h->ev_t[1], h->ev_t[2]));
     h->st_sweep_ms = ms;
     for (int b = 0; b < nbatch; ++b) {
+        if (!h->h_ctl[b].done) {
+            set_err("internal error: member %d not finished after the enqueued launches", b);
+            return -2;
+        }
         out[b].sweeps = h->h_ctl[b].sweeps;
         out[b].status = h->h_ctl[b].status;
         out[b].residual = h->h_ctl[b].residual;
@@ -438,7 +590,7 @@ void sn_poisson_destroy(sn_poisson* h) {
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
     cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage);
-    cudaFree(h->d_alt); cudaFree(h->d_sync);
+    cudaFree(h->d_alt); cudaFree(h->d_sync); cudaFree(h->d_work);
     for (auto& e : h->ev_poll) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev_t) if (e) cudaEventDestroy(e);
     delete h;
@@ -552,9 +704,10 @@ int sn_poisson_get_history(sn_poisson* h, double* R, int n) {
 int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     g_err.clear();
     if (!h || !key) { set_err("NULL argument"); return -1; }
-    if (!strcmp(key, "path")) { if (value < 0 || value > 2) { set_err("path must be 0..2"); return -1; } h->opt_path = (int)value; return 0; }
+    if (!strcmp(key, "path")) { if (value < 0 || value > 3) { set_err("path must be 0..3"); return -1; } h->opt_path = (int)value; return 0; }
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
-    if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)shapes().size()) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
+    if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)std::max(shapes().size(), blk_shapes().size())) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
     if (!strcmp(key, "tblock")) { if (value < 0 || value > kMaxTB) { set_err("tblock must be 0..%d", kMaxTB); return -1; } h->opt_tblock = (int)value; return 0; }
     set_err("unknown option '%s'", key);
     return -1;

@@ -23,12 +23,12 @@
 //    phi buffer, so the crossing sweep k* is then REPLAYED exactly from it (<= m sweeps): the returned phi has
 //    exactly k* sweeps applied, like the oracle's.
 #pragma once
-#include "common.cuh"
+#include "box_engine.cuh"
+#include "sweep_blocked.cuh"
 #include "tiling.h"
 
 namespace snp {
 
-constexpr int kMaxTB = 8;      // max sweeps per exchange (m)
 
 struct ResParams {
     Geom g;
@@ -63,14 +63,6 @@ __device__ __forceinline__ void red_release_add_u32(unsigned* p, unsigned v) {
 }
 __device__ __forceinline__ void spin_until_ge(const unsigned* p, unsigned want) {
     while (ld_acquire_u32(p) < want) __nanosleep(20);
-}
-
-// Exact max of order-preserving u64 keys across a warp with two 32-bit REDUX steps.
-__device__ __forceinline__ unsigned long long warp_max_key(unsigned long long k) {
-    const unsigned hi = (unsigned)(k >> 32), lo = (unsigned)k;
-    const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
-    const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
-    return ((unsigned long long)mh << 32) | ml;
 }
 
 template <int H, int TXN, int TYN>

@@ -135,6 +135,92 @@ def test_resident_kernel_stops_at_the_oracle_sweep(P, torch_cuda, oracle, nr, nz
             assert np.array_equal(got2, ref2["phi"])
 
 
+BLOCKED_CASES = [
+    # nr, nz, symmetry, shape, tblock     (shape table: sn_poisson.cu blk_shapes())
+    (128, 64, 1, 0, 1),       # one tile, box == grid
+    (256, 192, 0, 0, 4),      # 128x64 boxes, 2 CTAs / SM
+    (384, 128, 1, 0, 3),      # odd m (box origin rounding)
+    (256, 224, 0, 1, 8),      # 128x112 boxes
+    (256, 256, 1, 2, 6),      # 128x128 boxes, 64-cell patches
+    (128, 128, 0, 3, 2),      # 64x64 boxes
+    (192, 160, 1, 3, 5),
+    (128, 96, 1, 4, 3),       # 64x32 boxes
+    (320, 32, 0, 4, 12),      # deepest temporal blocking, one tile row
+]
+
+
+@pytest.mark.parametrize("nr,nz,symmetry,shape,tb", BLOCKED_CASES)
+@pytest.mark.parametrize("exact", [0, 1])
+def test_blocked_kernel_bit_exact_fixed_sweeps(P, torch_cuda, oracle, nr, nz, symmetry, shape, tb, exact):
+    """Blocked path (one launch per m sweeps, double-buffered tiles + margins): not a bit may change.
+    History: exact with the "exact" option; otherwise the launches before the last one report the lower bound R_lo
+    from the upper words of the maxima (within 2^-19 below R_k), the last launch is always exact."""
+    w = W.random_smooth(nr, nz, symmetry, seed=500 + nr + shape, lmax=4)
+    M = oracle.moments(w.rho, w.dr, w.dz, symmetry, w.lmax)
+    bnd = oracle.boundary(nr, nz, w.dr, w.dz, symmetry, w.lmax, M)
+    omega = oracle.default_omega(nr, nz, w.dr, w.dz, symmetry)
+    rng = np.random.default_rng(nr * 11 + nz)
+    phi0 = rng.uniform(-1, 1, size=(nz, nr))
+    opts = {"path": 3, "shape": shape, "tblock": tb, "exact": exact}
+    maxf = np.max(np.abs(12.566370614359172 * w.rho))
+    for k in (1, 2, 5, 17, 64):
+        want, Rabs, Pk = oracle.sweeps(w.rho, phi0, w.dr, w.dz, symmetry, omega, *bnd, k)
+        s, got, r = gpu_solve(P, torch_cuda, w, phi0=phi0, tol=0.0, max_sweeps=k, boundary=bnd, options=opts)
+        assert s.stat("path") == 3 and s.stat("tblock") == tb and s.stat("shape") == shape
+        assert r.sweeps == k and r.status == 0
+        assert np.array_equal(got, want), f"k={k}: max diff {np.max(np.abs(got - want))}"
+        want_hist = np.array([oracle.ratio(Rabs[q], Pk[q], maxf, w.dr, w.dz) for q in range(k)])
+        hist = s.history(k)
+        assert r.residual == want_hist[-1] == hist[-1]
+        if exact:
+            assert np.array_equal(hist, want_hist)
+        else:
+            assert np.all(hist <= want_hist) and np.all(hist >= want_hist * (1 - 2.0 ** -19))
+
+
+@pytest.mark.parametrize("nr,nz,symmetry,shape,tb", BLOCKED_CASES)
+def test_blocked_kernel_stops_at_the_oracle_sweep(P, torch_cuda, oracle, nr, nz, symmetry, shape, tb):
+    """Upper-word maxima -> exact re-run of the candidate launch -> replay to the crossing sweep: same sweep count,
+    same residual, same bits as the oracle at every tolerance."""
+    w = W.random_smooth(nr, nz, symmetry, seed=600 + nr + shape, lmax=4)
+    M = oracle.moments(w.rho, w.dr, w.dz, symmetry, w.lmax)
+    bnd = oracle.boundary(nr, nz, w.dr, w.dz, symmetry, w.lmax, M)
+    opts = {"path": 3, "shape": shape, "tblock": tb}
+    for tol in (1e-2, 1e-3, 3e-5, 1e-7):
+        ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, symmetry, w.lmax, tol, 3000, boundary_arrays=bnd)
+        s, got, r = gpu_solve(P, torch_cuda, w, tol=tol, max_sweeps=3000, boundary=bnd, options=opts)
+        assert (r.sweeps, r.status) == (ref["sweeps"], ref["status"])
+        assert r.residual == ref["residual"]
+        assert np.array_equal(got, ref["phi"])
+        for ms in (ref["sweeps"] - 1, ref["sweeps"]):
+            if ms < 1:
+                continue
+            ref2 = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, symmetry, w.lmax, tol, ms, boundary_arrays=bnd)
+            s, got2, r2 = gpu_solve(P, torch_cuda, w, tol=tol, max_sweeps=ms, boundary=bnd, options=opts)
+            assert (r2.sweeps, r2.status) == (ref2["sweeps"], ref2["status"])
+            assert r2.residual == ref2["residual"]
+            assert np.array_equal(got2, ref2["phi"])
+
+
+def test_blocked_batch_members_finish_independently(P, torch_cuda, oracle):
+    """Blocked path with a batch: every member has its own director state and stops at its own sweep."""
+    ws = [W.cfg4a_member(b, 128) for b in range(5)]
+    w0 = ws[0]
+    s = P.PoissonSolver.for_workload(w0)
+    s.set_option("path", 3)
+    rho = torch_cuda.from_numpy(np.stack([w.rho for w in ws])).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    res = s.solve(rho, phi, w0.tol, w0.max_sweeps)
+    assert s.stat("path") == 3
+    got = phi.cpu().numpy()
+    for b, w in enumerate(ws):
+        ref = oracle.solve_workload(w)
+        assert (res[b].sweeps, res[b].status) == (ref["sweeps"], 0)
+        assert relmax(got[b], ref["phi"]) <= REL
+        assert res[b].residual == pytest.approx(ref["residual"], rel=1e-6)
+    assert len({r.sweeps for r in res}) > 1
+
+
 # ----------------------------------------------------------------------------------------------------------
 # whole path with the library's own moments / boundary
 # ----------------------------------------------------------------------------------------------------------
