@@ -195,7 +195,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg1")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 streaming kernels, 2 resident kernel")
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 streaming kernels, 2 resident kernel, 3 blocked kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -323,7 +323,7 @@ def main():
     path = int(solver.stat("path"))
     sw_ms = float(np.mean(sweep_ms))
     sweeps_per_step = sum(r.sweeps for r in results)
-    sweep_launches = max(1, int(solver.stat("launches")) - 2 - (1 if path == 1 else 0))
+    sweep_launches = max(1, int(solver.stat("sweep_launches")))
     alg_bytes_per_launch = BYTES_PER_UPDATE * sweeps_per_step * cells / sweep_launches
     achieved = alg_bytes_per_launch / (sw_ms * 1e-3 / sweep_launches) / 1e9
     hbm_peak, hbm_src = measured_peaks()
@@ -334,7 +334,7 @@ def main():
         bound, peak = "l2", l2_copy_peak_gbs(torch)
         src = "L2-resident torch copy (2 x 24 MiB, read+write bytes), measured live in this run (of measured)"
     roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "k_halfsweep" if path == 1 else "k_sor_resident",
+                "traffic": None, "kernel": {1: "k_halfsweep", 2: "k_sor_resident", 3: "k_sor_blocked"}[path],
                 "alg_bytes_per_launch": alg_bytes_per_launch, "launch_ms": sw_ms / sweep_launches,
                 "sweep_launches_per_step": sweep_launches, "peak_source": src,
                 "frac_of_hbm_peak": achieved / hbm_peak}
@@ -345,7 +345,9 @@ def main():
         "scaling": scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": label, "grid": [w0.nr, w0.nz], "batch_per_gpu": nb, "lmax": w0.lmax,
                    "tol": w0.tol, "l2": "flushed between timed solves (256 MiB write)",
-                   "path": {1: "streaming", 2: "resident"}.get(path, str(path)),
+                   "path": {1: "streaming", 2: "resident", 3: "blocked"}.get(path, str(path)),
+                   "tblock": int(solver.stat("tblock")), "ctas": int(solver.stat("ctas")),
+                   "tile": [int(solver.stat("tile_w")), int(solver.stat("tile_h"))],
                    "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"},
         "time_to_residual_ms": total_ms / args.steps, "sweeps_per_solve": [r.sweeps for r in results][:8],
         "final_residual": results[0].residual,

@@ -99,14 +99,19 @@ int sn_poisson_get_boundary(sn_poisson* h, double* bE, double* bN, double* bS);
 int sn_poisson_get_history(sn_poisson* h, double* R, int n);
 
 /* Tuning knobs; unknown keys return -1.
- *   "path"        0 auto, 1 streaming kernels (phi in L2/HBM), 2 resident persistent kernel (phi on chip)
- *   "chunk"       sweeps enqueued between host polls of the device-side decision (streaming path)
- *   "tblock"      sweeps per halo exchange of the resident kernel (temporal blocking depth m)           */
+ *   "path"        0 auto, 1 streaming kernels (one launch per colour), 2 resident persistent cooperative kernel
+ *                 (phi on chip for the whole solve; single solve whose tiles are all co-resident), 3 blocked kernel
+ *                 (one launch per m sweeps; any size, batches)
+ *   "chunk"       launches enqueued between host polls of the device-side decision (paths 1 and 3)
+ *   "tblock"      sweeps per halo exchange / per launch (temporal blocking depth m); 0 = planner's choice
+ *   "shape"       box shape index of path 2 / 3; -1 = planner's choice
+ *   "exact"       1: path 3 tracks the per-sweep maxima exactly in every launch (exact R_k history)         */
 int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value);
 
-/* Counters of the last solve / batch: "launches" (kernels launched), "sweep_ms" (device time of the relaxation
- * phase, CUDA events on the caller's stream), "setup_ms" (moments + boundary), "path" (1 or 2 as above),
- * "ctas", "tile_w", "tile_h", "tblock".  Returns 0 or -1. */
+/* Counters of the last solve / batch: "launches" (kernels launched), "sweep_launches" (those that ran relaxation
+ * sweeps), "sweep_ms" (device time of the relaxation phase, CUDA events on the caller's stream), "setup_ms"
+ * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape".
+ * Returns 0 or -1. */
 int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out);
 
 /* Message of the last failure on this thread ("" if none). */

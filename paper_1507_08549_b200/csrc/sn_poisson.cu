@@ -84,6 +84,7 @@ struct sn_poisson {
     cudaEvent_t ev_t[3] = {nullptr, nullptr, nullptr};
 
     // stats of the last solve
+    double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
     double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
     double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1;
     int last_sweeps0 = 0;
@@ -211,6 +212,7 @@ int run_stream(sn_poisson* h, const Geom& g, int nbatch, const double* rho, doub
     }
     k_decide_last<<<nbatch, 32, 0, st>>>(g, k - 1, slot_stride, hist_stride, h->d_slots, h->d_ctl, h->d_hist);
     h->st_launches += 1;
+    h->st_aux_launches += 1;
     CU_TRY(cudaGetLastError());
     return 0;
 }
@@ -316,6 +318,7 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
     P.ctl = h->d_ctl; P.hist = h->d_hist;
     k_blocked_init<<<nbatch, 32, 0, st>>>(h->d_ctl, pl.m, max_sweeps, h->opt_exact);
     h->st_launches += 1;
+    h->st_aux_launches += 1;
     CU_TRY(cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
     void* args[] = {&P};
     const dim3 grid(pl.ntiles, nbatch), block(S.NT());
@@ -461,6 +464,7 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     if (!h->omega_user) h->omega = default_omega(h->nr, h->nz, h->dr, h->dz, h->symmetry);
     const Geom g = make_geom(h, tol);
     h->st_launches = 0;
+    h->st_aux_launches = 0;
     h->st_path = 1;
 
     CU_TRY(cudaEventRecord(h->ev_t[0], st));
@@ -469,11 +473,13 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     // a-1: moments (+ max|4 pi rho|), a-1b: boundary fill (skipped when ghosts were injected by the test hook)
     if (int rc = launch_moments(h, g, nbatch, rho, st)) return rc;
     h->st_launches += 1;
+    h->st_aux_launches += 1;
     if (!h->user_boundary) {
         k_boundary<<<nbatch, 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN,
                                            h->d_bS, 0);
         CU_TRY(cudaGetLastError());
         h->st_launches += 1;
+        h->st_aux_launches += 1;
     }
     CU_TRY(cudaEventRecord(h->ev_t[1], st));
     // a-2 + a-3
@@ -717,6 +723,7 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     g_err.clear();
     if (!h || !key || !out) { set_err("NULL argument"); return -1; }
     if (!strcmp(key, "launches")) { *out = h->st_launches; return 0; }
+    if (!strcmp(key, "sweep_launches")) { *out = h->st_launches - h->st_aux_launches; return 0; }
     if (!strcmp(key, "sweep_ms")) { *out = h->st_sweep_ms; return 0; }
     if (!strcmp(key, "setup_ms")) { *out = h->st_setup_ms; return 0; }
     if (!strcmp(key, "path")) { *out = h->st_path; return 0; }
