@@ -210,6 +210,7 @@ def main():
 
     import paper_1507_08549_b200 as P
     from paper_1507_08549_b200 import build as pbuild
+    from paper_1507_08549_b200.sharding import reduce_timing, shard_members
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -226,12 +227,8 @@ def main():
     P.load()
 
     # multi-GPU: batch members are sharded across ranks with no collective; a single solve runs as replicas
-    if len(members) >= world and len(members) > 1:
-        mine = members[rank::world]
-        scaling = "strong"
-    else:
-        mine = members
-        scaling = "weak"
+    idx, scaling = shard_members(len(members), rank, world)
+    mine = [members[i] for i in idx]
     w0 = mine[0]
     nb = len(mine)
     solver = P.PoissonSolver.for_workload(w0)
@@ -300,18 +297,12 @@ def main():
         e2e_time = sum(e2e_ms) * 1e-3
 
     total_ms = float(sum(step_ms))
-    t = torch.tensor([total_ms, float(updates), float(launches), e2e_time if nb == 1 else 0.0,
-                      float(e2e_upd) if nb == 1 else 0.0], dtype=torch.float64, device="cuda")
-    if world > 1:
-        tmax = t.clone()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone()
-        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        total_ms, updates_all, launches_all = float(tmax[0]), float(tsum[1]), int(tsum[2])
-        e2e_time_all, e2e_upd_all = float(tmax[3]), float(tsum[4])
-    else:
-        updates_all, launches_all = float(updates), launches
-        e2e_time_all, e2e_upd_all = float(t[3]), float(t[4])
+    counters = [float(updates), float(launches), float(e2e_upd) if nb == 1 else 0.0]
+    dev = torch.device("cuda", local_rank)
+    total_ms, (updates_all, launches_all, e2e_upd_all) = reduce_timing(total_ms, counters, world, dev)
+    e2e_time_all, _ = reduce_timing(e2e_time * 1e3 if nb == 1 else 0.0, [], world, dev)
+    e2e_time_all *= 1e-3
+    launches_all = int(launches_all)
 
     if rank != 0:
         if world > 1:
