@@ -17,6 +17,8 @@
 
 namespace snp {
 
+constexpr int kMaxTB = 12;     // max sweeps per launch (blocked path) / per interval and exchange (resident path)
+
 enum TrackMode : int {
     kTrackNone = 0,    // replay: no maxima
     kTrackExact = 1,   // exact max|res|, max|phi_new| as order-preserving u64 keys
@@ -36,10 +38,65 @@ struct BoxShape {
     static_assert(NT % 32 == 0 && H % 2 == 0, "shape");
 };
 
-template <int H, int TXN, int TYN>
+// A double with a 32-bit tag in each 8-byte half: {lo, tag, hi, tag}.  Aligned 8-byte words are never torn, so a
+// reader that sees the expected tag in both halves has the whole value; no fence and no separate flag are needed
+// (the producer's tag is the step number, unique within a solve phase).
+__device__ __forceinline__ void ll_store(uint4* p, double v, unsigned tag) {
+    const unsigned lo = (unsigned)__double2loint(v), hi = (unsigned)__double2hiint(v);
+    asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag)
+                 : "memory");
+}
+__device__ __forceinline__ uint4 ll_load(const uint4* p) {
+    uint4 v;
+    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "l"(p)
+                 : "memory");
+    return v;
+}
+__device__ __forceinline__ bool ll_ready(const uint4& v, unsigned tag) { return v.y == tag && v.w == tag; }
+__device__ __forceinline__ double ll_value(const uint4& v) { return __hiloint2double((int)v.z, (int)v.x); }
+
+// Every wait on another CTA is bounded: a poll gives up when *quit becomes non-zero (the solve is leaving the phase)
+// or when the watchdog trips (budget exceeded here, or tripped elsewhere: *g_panic non-zero).  A tripped watchdog
+// makes every later wait fall through, so the kernel always terminates; the host then reports status -2.
+struct PollCtx {
+    const volatile int* quit;    // shared memory
+    volatile int* s_panic;       // shared memory
+    int* g_panic;                // Ctl::panic of this member
+    int* g_info;                 // Ctl::panic_tile, panic_arg
+    int tile;
+};
+constexpr unsigned kPollBudget = 1u << 21;      // polls (each an L2 round trip or a nanosleep): ~1 s
+
+__device__ __forceinline__ void trip_watchdog(const PollCtx& c, int code, int arg) {
+    if (atomicCAS(c.g_panic, 0, code) == 0) {
+        c.g_info[0] = c.tile;
+        c.g_info[1] = arg;
+    }
+    *c.s_panic = 1;
+}
+// true: stop waiting
+__device__ __forceinline__ bool poll_giveup(const PollCtx& c, unsigned& n, int code, int arg) {
+    if (*c.quit || *c.s_panic) return true;
+    if ((++n & 63u) == 0u) {
+        if (*(volatile int*)c.g_panic) { *c.s_panic = 1; return true; }
+        if (n > kPollBudget) { trip_watchdog(c, code, arg); return true; }
+    }
+    return false;
+}
+
+// BAR = 0: the engine's barrier is __syncthreads(); BAR > 0: named barrier BAR over the first NT threads of the CTA
+// (the resident kernel runs an extra service warp that must not take part in it).
+template <int H, int TXN, int TYN, int BAR = 0>
 struct BoxEngine {
     using S = BoxShape<H, TXN, TYN>;
     static constexpr int BW = S::BW, BH = S::BH, LS = S::LS, PW = S::PW;
+
+    static __device__ __forceinline__ void sync() {
+        if (BAR == 0) __syncthreads();
+        else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(S::NT) : "memory");
+    }
 
     // shared memory
     double* fs;     // [BH][2][PW]     f; plane p holds the columns with (c & 1) == p, thread a's pair at [2a, 2a+1]
@@ -50,6 +107,8 @@ struct BoxEngine {
 
     // per-thread state
     int a, b, rowbase;
+    bool active = true;         // false: the patch lies outside the grid (ragged last tile row of the halo mode);
+                                // such a thread never updates and keeps publishing the north ghosts as its bottom row
     double phi[H][4];
     double cEr[4], cWr[4];
     double iz2, D, wD;          // interior rows
@@ -167,9 +226,14 @@ struct BoxEngine {
         }
     }
 
-    // One half-sweep of colour COL over the patch, then publish the updated edge cells and __syncthreads().
-    template <int COL, int TRACK>
+    // One half-sweep of colour COL over the patch, then publish the updated edge cells and (SYNC) the barrier.
+    template <int COL, int TRACK, bool SYNC = true>
     __device__ __forceinline__ void half_sweep() {
+        if (active) half_sweep_body<COL, TRACK>();
+        if (SYNC) sync();
+    }
+    template <int COL, int TRACK>
+    __device__ __forceinline__ void half_sweep_body() {
         // vertical outer neighbours of the bottom (q=0) and top (q=H-1) rows: other-colour cells of the rows outside
         constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;                 // column parity updated in those rows
         const double2 So = *reinterpret_cast<const double2*>(exT + (size_t)b * BW + pb * PW + 2 * a);
@@ -206,13 +270,153 @@ struct BoxEngine {
         *reinterpret_cast<double2*>(exB + (size_t)(b + 1) * BW + pb * PW + 2 * a) = make_double2(phi[0][pb], phi[0][pb + 2]);
         *reinterpret_cast<double2*>(exT + (size_t)(b + 1) * BW + pt * PW + 2 * a) =
             make_double2(phi[H - 1][pt], phi[H - 1][pt + 2]);
-        __syncthreads();
     }
 
     template <int TRACK>
     __device__ __forceinline__ void sweep() {
         half_sweep<0, TRACK>();
         half_sweep<1, TRACK>();
+    }
+
+    // ---- halo mode (box == owned tile; the neighbours' edge cells arrive every half-sweep) ------------------------
+    // Fill the border slots on the box edges that have a neighbouring tile from a full state array (both colours);
+    // called after set_borders() whenever the box is (re)loaded.
+    __device__ __forceinline__ void load_halo_borders(const double* __restrict__ src, int nr, int nz, int bx, int by) {
+        const int gi0 = bx + 4 * a, gj0 = by + rowbase;
+        if (!active) return;
+        if (a == TXN - 1 && bx + BW < nr) {
+#pragma unroll
+            for (int q = 0; q < H; ++q) exL[(rowbase + q) * LS + TXN + 1] = __ldcg(src + (size_t)(gj0 + q) * nr + bx + BW);
+        }
+        if (a == 0 && bx > 0) {
+#pragma unroll
+            for (int q = 0; q < H; ++q) exR[(rowbase + q) * LS + 0] = __ldcg(src + (size_t)(gj0 + q) * nr + bx - 1);
+        }
+        if (b == TYN - 1 && by + BH < nz) {
+            const double* row = src + (size_t)(gj0 + H) * nr + gi0;
+            double* dst = exB + (size_t)(TYN + 1) * BW + 2 * a;
+            *reinterpret_cast<double2*>(dst) = make_double2(__ldcg(row), __ldcg(row + 2));
+            *reinterpret_cast<double2*>(dst + PW) = make_double2(__ldcg(row + 1), __ldcg(row + 3));
+        }
+        if (b == 0 && by > 0) {
+            const double* row = src + (size_t)(gj0 - 1) * nr + gi0;
+            double* dst = exT + 2 * a;
+            *reinterpret_cast<double2*>(dst) = make_double2(__ldcg(row), __ldcg(row + 2));
+            *reinterpret_cast<double2*>(dst + PW) = make_double2(__ldcg(row + 1), __ldcg(row + 3));
+        }
+    }
+
+    // After the half-sweep of colour COL: send this box's updated edge cells to the neighbouring tiles and receive
+    // theirs into the border slots.  `mail` is indexed like the grid (one tagged packet per cell; only box-edge
+    // cells are ever used); a cell of colour COL is written once per sweep with a strictly increasing tag and its
+    // reader consumes tag t before the writer can produce t + 2, so one buffer is enough.  The poll gives up when
+    // *stop becomes non-zero (the solve is leaving this phase; the box is reloaded afterwards).
+    template <int COL>
+    __device__ __forceinline__ void halo_exchange(uint4* __restrict__ mail, unsigned tag, int nr, int nz, int bx,
+                                                  int by, const PollCtx& pc) {
+        unsigned spins = 0;
+        if (!active) return;
+        constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;
+        const int gi0 = bx + 4 * a, gj0 = by + rowbase;
+        const bool west = a == 0 && bx > 0, east = a == TXN - 1 && bx + BW < nr;
+        const bool south = b == 0 && by > 0, north = b == TYN - 1 && by + BH < nz;
+        if (!(west || east || south || north)) return;
+        // send
+        if (west) {
+#pragma unroll
+            for (int q = 0; q < H; ++q)
+                if (((q + COL) & 1) == 0) ll_store(mail + (size_t)(gj0 + q) * nr + gi0, phi[q][0], tag);
+        }
+        if (east) {
+#pragma unroll
+            for (int q = 0; q < H; ++q)
+                if (((q + COL) & 1) == 1) ll_store(mail + (size_t)(gj0 + q) * nr + gi0 + 3, phi[q][3], tag);
+        }
+        if (south) {
+            ll_store(mail + (size_t)gj0 * nr + gi0 + pb, phi[0][pb], tag);
+            ll_store(mail + (size_t)gj0 * nr + gi0 + pb + 2, phi[0][pb + 2], tag);
+        }
+        if (north) {
+            ll_store(mail + (size_t)(gj0 + H - 1) * nr + gi0 + pt, phi[H - 1][pt], tag);
+            ll_store(mail + (size_t)(gj0 + H - 1) * nr + gi0 + pt + 2, phi[H - 1][pt + 2], tag);
+        }
+        // receive: the cells of colour COL just outside the box
+        if (east) {          // the east tile's column 0, updated in the rows with (q + COL) even
+            const uint4* col = mail + (size_t)gj0 * nr + bx + BW;
+            bool done;
+            do {
+                done = true;
+#pragma unroll
+                for (int q = 0; q < H; ++q)
+                    if (((q + COL) & 1) == 0) {
+                        const uint4 v = ll_load(col + (size_t)q * nr);
+                        if (ll_ready(v, tag)) exL[(rowbase + q) * LS + TXN + 1] = ll_value(v);
+                        else done = false;
+                    }
+            } while (!done && !poll_giveup(pc, spins, 1, (int)tag));
+        }
+        if (west) {          // the west tile's column 3, updated in the rows with (q + COL) odd
+            const uint4* col = mail + (size_t)gj0 * nr + bx - 1;
+            bool done;
+            do {
+                done = true;
+#pragma unroll
+                for (int q = 0; q < H; ++q)
+                    if (((q + COL) & 1) == 1) {
+                        const uint4 v = ll_load(col + (size_t)q * nr);
+                        if (ll_ready(v, tag)) exR[(rowbase + q) * LS + 0] = ll_value(v);
+                        else done = false;
+                    }
+            } while (!done && !poll_giveup(pc, spins, 2, (int)tag));
+        }
+        if (north) {         // the north tile's bottom row: columns of parity pb
+            const uint4* row = mail + (size_t)(gj0 + H) * nr + gi0 + pb;
+            double* dst = exB + (size_t)(TYN + 1) * BW + pb * PW + 2 * a;
+            bool done;
+            do {
+                const uint4 v0 = ll_load(row), v1 = ll_load(row + 2);
+                done = ll_ready(v0, tag) && ll_ready(v1, tag);
+                if (done) *reinterpret_cast<double2*>(dst) = make_double2(ll_value(v0), ll_value(v1));
+            } while (!done && !poll_giveup(pc, spins, 3, (int)tag));
+        }
+        if (south) {         // the south tile's top row: columns of parity pt
+            const uint4* row = mail + (size_t)(gj0 - 1) * nr + gi0 + pt;
+            double* dst = exT + pt * PW + 2 * a;
+            bool done;
+            do {
+                const uint4 v0 = ll_load(row), v1 = ll_load(row + 2);
+                done = ll_ready(v0, tag) && ll_ready(v1, tag);
+                if (done) *reinterpret_cast<double2*>(dst) = make_double2(ll_value(v0), ll_value(v1));
+            } while (!done && !poll_giveup(pc, spins, 4, (int)tag));
+        }
+    }
+
+    // ---- block mode (temporal blocking): the whole owned patch travels as tagged packets once per interval -------
+    __device__ __forceinline__ void ll_store_patch(uint4* __restrict__ mail, unsigned tag, int nr, int gi0, int gj0) const {
+#pragma unroll
+        for (int q = 0; q < H; ++q) {
+            uint4* row = mail + (size_t)(gj0 + q) * nr + gi0;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) ll_store(row + c, phi[q][c], tag);
+        }
+    }
+    __device__ __forceinline__ void ll_wait_patch(const uint4* __restrict__ mail, unsigned tag, int nr, int gi0, int gj0,
+                                                  const PollCtx& pc) {
+        unsigned spins = 0;
+        bool done;
+        do {
+            done = true;
+#pragma unroll
+            for (int q = 0; q < H; ++q) {
+                const uint4* row = mail + (size_t)(gj0 + q) * nr + gi0;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const uint4 v = ll_load(row + c);
+                    if (ll_ready(v, tag)) phi[q][c] = ll_value(v);
+                    else done = false;
+                }
+            }
+        } while (!done && !poll_giveup(pc, spins, 5, (int)tag));
     }
 
     // any non-finite value in the patch (NaN/Inf never relax away)

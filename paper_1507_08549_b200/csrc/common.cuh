@@ -17,7 +17,7 @@ struct Ctl {
     int done;          // 1 once the member is finished (result fields valid, phi_inout holds the result)
     int sweeps;        // full sweeps applied to the returned phi
     int status;        // 0 / 1 / -3 as in sn_poisson_result
-    int pad;
+    int panic;         // resident path watchdog: non-zero = a wait exceeded its budget (code of the first one)
     double residual;   // R_k of the last applied sweep
     double maxf;       // max |4 pi rho| (written by the moments pass)
     // ---- director state (blocked path) ----
@@ -30,6 +30,7 @@ struct Ctl {
     int fin_status;
     unsigned int arrived;   // CTAs of this member that have finished the current launch
     double fin_R;
+    int panic_tile, panic_arg;   // where the watchdog tripped (diagnostics)
 };
 
 enum BlockedAction : int { kActSkip = 0, kActAdvance = 1, kActRedo = 2, kActReplay = 3, kActCopy = 4 };

@@ -62,7 +62,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -76,9 +76,10 @@ struct sn_poisson {
     Ctl* d_ctl = nullptr;
     Ctl* h_ctl = nullptr;       // pinned, 2 * cap_batch (double-buffered polls)
     double *d_rho_stage = nullptr, *d_phi_stage = nullptr;   // solve_host staging
-    double* d_alt = nullptr;                                 // resident path: 2 x nr*nz, states of epochs e%3 = 1,2
-    unsigned int* d_sync = nullptr;                          // resident path: flags | arrived | gbar
-    size_t sync_cap = 0;
+    double* d_ring = nullptr;                                // resident path: checkpoint ring, nb x kResRing x nr*nz
+    void* d_mail = nullptr;                                  // resident path: tagged packets, nb x 2 x nr*nz x 16 B
+    unsigned int* d_sync = nullptr;                          // resident path: arrived counters | grid barriers
+    size_t ring_cap = 0, mail_cap = 0, sync_cap = 0;
     bool user_boundary = false;
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
     cudaEvent_t ev_t[3] = {nullptr, nullptr, nullptr};
@@ -86,7 +87,7 @@ struct sn_poisson {
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
     double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
-    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1;
+    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0;
     int last_sweeps0 = 0;
 };
 
@@ -356,38 +357,51 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
 
 // ---- resident path: shapes, planner, launcher ------------------------------------------------------------------
 struct ShapeInfo {
-    int H, TXN, TYN;
+    int H, TXN, TYN, minb;
     size_t smem;
     const void* fn;
     int BW() const { return 4 * TXN; }
     int BH() const { return H * TYN; }
     int NT() const { return TXN * TYN; }
+    int threads() const { return TXN * TYN + 32; }     // + the service warp
 };
 
-template <int H, int TXN, int TYN>
+template <int H, int TXN, int TYN, int MINB>
 ShapeInfo shape_of() {
-    return {H, TXN, TYN, ResShape<H, TXN, TYN>::smem_bytes, (const void*)k_sor_resident<H, TXN, TYN>};
+    return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes, (const void*)k_sor_resident<H, TXN, TYN, MINB>};
 }
 
 const std::vector<ShapeInfo>& shapes() {
     static const std::vector<ShapeInfo> v = {
-        shape_of<8, 32, 14>(),   // 0: box 128 x 112, 448 threads
-        shape_of<8, 32, 8>(),    // 1: box 128 x 64,  256 threads
-        shape_of<8, 16, 8>(),    // 2: box 64 x 64,   128 threads
-        shape_of<4, 16, 8>(),    // 3: box 64 x 32,   128 threads
-        shape_of<4, 8, 8>(),     // 4: box 32 x 32,    64 threads
-        shape_of<2, 8, 16>(),    // 5: box 32 x 32,   128 threads
+        shape_of<8, 32, 14, 1>(),   // 0: box 128 x 112, 448 threads
+        shape_of<8, 32, 8, 1>(),    // 1: box 128 x 64,  256 threads
+        shape_of<8, 16, 8, 2>(),    // 2: box 64 x 64,   128 threads
+        shape_of<4, 16, 8, 2>(),    // 3: box 64 x 32,   128 threads
+        shape_of<4, 8, 8, 2>(),     // 4: box 32 x 32,    64 threads
+        shape_of<2, 8, 16, 2>(),    // 5: box 32 x 32,   128 threads
+        shape_of<8, 32, 7, 2>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
+        shape_of<4, 16, 16, 1>(),   // 7: box 64 x 64,   256 threads
+        shape_of<6, 12, 8, 2>(),    // 8: box 48 x 48,    96 threads
+        shape_of<4, 12, 16, 1>(),   // 9: box 48 x 64,   192 threads
     };
     return v;
 }
 
 struct ResPlan {
-    int shape = -1, m = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
+    int shape = -1, halo = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
     double cost = 0;
 };
 
-// Pick (shape, m) minimising a simple per-sweep cost model; honours the "shape"/"tblock" overrides.
-ResPlan plan_resident(sn_poisson* h, const double* rho, const double* phi) {
+// Modelled SM clocks of one half-sweep of a box when `k` CTAs of that shape share an SM: the fp64 pipe issues one
+// warp instruction per 2 clocks per SM sub-partition, 7 per cell update; measured efficiency ~0.55 plus a fixed
+// exchange / barrier latency per half-sweep.
+double model_half_sweep(const ShapeInfo& S, int k) {
+    const double warps_per_smsp = std::ceil(k * (S.NT() / 32.0) / 4.0);
+    return warps_per_smsp * (2.0 * S.H) * 7.0 * 2.0 / 0.55 + 130.0;
+}
+
+// Pick (shape, mode, m) minimising modelled clocks per sweep; honours the "shape" / "tblock" / "halo" overrides.
+ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double* phi) {
     ResPlan best;
     if (((uintptr_t)rho | (uintptr_t)phi) & 15) return best;
     const auto& sh = shapes();
@@ -396,64 +410,99 @@ ResPlan plan_resident(sn_poisson* h, const double* rho, const double* phi) {
         const ShapeInfo& S = sh[si];
         int occ = 0;
         if (cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn, S.NT(), S.smem) != cudaSuccess || occ < 1) {
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn, S.threads(), S.smem) != cudaSuccess || occ < 1) {
             cudaGetLastError();
             continue;
         }
-        const int max_tiles = occ * h->num_sms;
+        const long long max_ctas = (long long)occ * h->num_sms;
+        // halo mode: box == tile on a regular lattice, ragged last tile row allowed
+        if (h->opt_halo != 0 && h->nr % S.BW() == 0 && h->nz % S.H == 0) {
+            ResPlan p;
+            p.shape = si; p.halo = 1;
+            p.ntx = h->nr / S.BW(); p.nty = (h->nz + S.BH() - 1) / S.BH();
+            p.ow = S.BW(); p.oh = S.BH();
+            p.ntiles = p.ntx * p.nty;
+            p.Q = h->opt_tblock > 0 ? h->opt_tblock : 8;
+            p.m = p.Q;
+            if ((long long)p.ntiles * nbatch <= max_ctas && (p.ntiles > 1 || h->opt_halo == 1)) {
+                const int k = (int)((p.ntiles * (long long)nbatch + h->num_sms - 1) / h->num_sms);
+                const double t1 = model_half_sweep(S, 1), tk = model_half_sweep(S, k);
+                p.cost = 2.0 * std::max(tk, t1 + 1300.0);
+                if (best.shape < 0 || p.cost < best.cost) best = p;
+            }
+        }
+        if (h->opt_halo == 1) continue;
+        // block mode: temporal blocking with margins of 2m cells
         for (int m = 1; m <= kMaxTB; ++m) {
             if (h->opt_tblock > 0 && m != h->opt_tblock) continue;
             ResPlan p;
             if (!plan_axis(h->nr, S.BW(), 2 * m, 4, &p.ntx, &p.ow)) continue;
             if (!plan_axis(h->nz, S.BH(), 2 * m, S.H, &p.nty, &p.oh)) continue;
             p.ntiles = p.ntx * p.nty;
-            if (p.ntiles > max_tiles) continue;
+            if ((long long)p.ntiles * nbatch > max_ctas) continue;
             bool ok = true;                      // the property the kernel relies on, checked for every tile
             for (int t = 0; t < p.ntx && ok; ++t) ok = box_covers(t, p.ow, 2 * m, 4, S.BW(), h->nr);
             for (int t = 0; t < p.nty && ok; ++t) ok = box_covers(t, p.oh, 2 * m, S.H, S.BH(), h->nz);
             if (!ok) continue;
-            p.shape = si;
-            p.m = m;
-            // cost model (SM clocks per sweep): CTAs sharing an SM serialise on the fp64 pipe; one exchange per m sweeps
-            const double per_sm = (double)((p.ntiles + h->num_sms - 1) / h->num_sms);
-            const double warps = per_sm * S.NT() / 32.0;
-            const double rate = std::min(3.2, 0.45 * warps);             // cell-updates per clock per SM
-            const double compute = per_sm * S.BW() * S.BH() / rate + 2.0 * 150.0;
-            const double exchange = 3500.0 + 8.0 * S.BW() * S.BH() / 48.0;
-            p.cost = compute + exchange / m;
+            p.shape = si; p.halo = 0; p.m = m; p.Q = m;
+            const int k = (int)((p.ntiles * (long long)nbatch + h->num_sms - 1) / h->num_sms);
+            const double exchange = p.ntiles > 1 ? 1600.0 + 16.0 * S.BW() * S.BH() / 32.0 : 300.0;
+            p.cost = 2.0 * model_half_sweep(S, k) + (k * exchange) / m;
             if (best.shape < 0 || p.cost < best.cost) best = p;
         }
     }
     return best;
 }
 
-int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, const double* rho, double* phi, int max_sweeps,
-                 cudaStream_t st) {
+int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, const double* rho, double* phi,
+                 int max_sweeps, cudaStream_t st) {
     const ShapeInfo& S = shapes()[pl.shape];
     const size_t ncell = (size_t)h->nr * h->nz;
-    if (!h->d_alt) CU_TRY(cudaMalloc((void**)&h->d_alt, sizeof(double) * 2 * ncell));
-    const size_t nep = (size_t)(max_sweeps + pl.m - 1) / pl.m + 2;
-    const size_t nsync = (size_t)pl.ntiles + nep + 1;
-    if (nsync > h->sync_cap) {
-        cudaFree(h->d_sync);
-        h->d_sync = nullptr;
-        CU_TRY(cudaMalloc((void**)&h->d_sync, sizeof(unsigned int) * nsync));
-        h->sync_cap = nsync;
+    const size_t nint = (size_t)(max_sweeps + pl.Q - 1) / pl.Q;
+    const size_t need_ring = (size_t)nbatch * kResRing * ncell;
+    const size_t need_mail = (size_t)nbatch * 2 * ncell;
+    const size_t need_sync = (size_t)nbatch * (2 * (nint + 2) + 1);
+    if (h->ring_cap < need_ring) {
+        cudaFree(h->d_ring); h->d_ring = nullptr; h->ring_cap = 0;
+        CU_TRY(cudaMalloc((void**)&h->d_ring, sizeof(double) * need_ring));
+        h->ring_cap = need_ring;
     }
-    CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * nsync, st));
+    if (h->mail_cap < need_mail) {
+        cudaFree(h->d_mail); h->d_mail = nullptr; h->mail_cap = 0;
+        CU_TRY(cudaMalloc((void**)&h->d_mail, 16 * need_mail));
+        h->mail_cap = need_mail;
+    }
+    if (h->sync_cap < need_sync) {
+        cudaFree(h->d_sync); h->d_sync = nullptr; h->sync_cap = 0;
+        CU_TRY(cudaMalloc((void**)&h->d_sync, sizeof(unsigned int) * need_sync));
+        h->sync_cap = need_sync;
+    }
+    CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * need_sync, st));
+    CU_TRY(cudaMemsetAsync(h->d_slots_f, 0, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
+    if (pl.ntiles > 1) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
     ResParams P;
     P.g = g;
-    P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.max_sweeps = max_sweeps;
-    P.rho = rho; P.buf[0] = phi; P.buf[1] = h->d_alt; P.buf[2] = h->d_alt + ncell;
+    P.halo = pl.halo;
+    P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.Q = pl.Q;
+    P.max_sweeps = max_sweeps;
+    P.force_exact = h->opt_exact;
+    P.rho = rho; P.phi = phi;
+    P.ring = h->d_ring;
+    P.mail = reinterpret_cast<uint4*>(h->d_mail);
     P.bE = h->d_bE; P.bN = h->d_bN; P.bS = h->d_bS;
-    P.slots = h->d_slots; P.ctl = h->d_ctl; P.hist = h->d_hist;
-    P.flags = h->d_sync; P.arrived = h->d_sync + pl.ntiles; P.gbar = h->d_sync + pl.ntiles + nep;
+    P.slots_f = h->d_slots_f; P.slots_x = h->d_slots;
+    P.slot_stride = 2 * h->cap_sweeps; P.hist_stride = h->cap_sweeps;
+    P.arrived = h->d_sync;
+    P.arr_stride = (int)(nint + 2);
+    P.gbar = h->d_sync + (size_t)nbatch * 2 * (nint + 2);
+    P.ctl = h->d_ctl; P.hist = h->d_hist;
     void* args[] = {&P};
     CU_TRY(cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
-    CU_TRY(cudaLaunchCooperativeKernel(S.fn, dim3(pl.ntiles), dim3(S.NT()), args, S.smem, st));
+    CU_TRY(cudaLaunchCooperativeKernel(S.fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, S.smem, st));
     h->st_launches += 1;
     h->st_path = 2;
-    h->st_ctas = pl.ntiles; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.m; h->st_shape = pl.shape;
+    h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.Q;
+    h->st_shape = pl.shape; h->st_halo = pl.halo;
     return 0;
 }
 
@@ -466,6 +515,7 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     h->st_launches = 0;
     h->st_aux_launches = 0;
     h->st_path = 1;
+    h->st_halo = 0;
 
     CU_TRY(cudaEventRecord(h->ev_t[0], st));
     CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl) * nbatch, st));
@@ -485,10 +535,10 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     // a-2 + a-3
     ResPlan pl;
     BlkPlan bp;
-    if ((h->opt_path == 0 || h->opt_path == 2) && nbatch == 1 && max_sweeps > 0) pl = plan_resident(h, rho, phi);
+    if ((h->opt_path == 0 || h->opt_path == 2) && max_sweeps > 0) pl = plan_resident(h, nbatch, rho, phi);
     if (h->opt_path == 2 && pl.shape < 0 && max_sweeps > 0) {
-        set_err("resident path requested but not eligible (needs nbatch=1, nr%%4==0, nz%%H==0, grid >= one box, "
-                "16-byte aligned pointers, tiles <= co-resident CTAs)");
+        set_err("resident path requested but not eligible (needs nr%%4==0, nz%%H==0, grid >= one box, 16-byte aligned "
+                "pointers, tiles x batch <= co-resident CTAs)");
         return -1;
     }
     if ((h->opt_path == 0 || h->opt_path == 3) && pl.shape < 0 && max_sweeps > 0) bp = plan_blocked(h, nbatch, rho, phi);
@@ -498,7 +548,7 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
         return -1;
     }
     if (pl.shape >= 0) {
-        if (int rc = run_resident(h, g, pl, rho, phi, max_sweeps, st)) return rc;
+        if (int rc = run_resident(h, g, pl, nbatch, rho, phi, max_sweeps, st)) return rc;
     } else if (bp.shape >= 0) {
         if (int rc = run_blocked(h, g, bp, nbatch, rho, phi, max_sweeps, st)) return rc;
     } else {
@@ -513,6 +563,11 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     CU_TRY(cudaEventElapsedTime(&ms, h->ev_t[1], h->ev_t[2]));
     h->st_sweep_ms = ms;
     for (int b = 0; b < nbatch; ++b) {
+        if (h->h_ctl[b].panic) {
+            set_err("resident kernel watchdog: a wait exceeded its budget (member %d, code %d, tile %d, arg %d)", b,
+                    h->h_ctl[b].panic, h->h_ctl[b].panic_tile, h->h_ctl[b].panic_arg);
+            return -2;
+        }
         if (!h->h_ctl[b].done) {
             set_err("internal error: member %d not finished after the enqueued launches", b);
             return -2;
@@ -596,7 +651,7 @@ void sn_poisson_destroy(sn_poisson* h) {
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
     cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage);
-    cudaFree(h->d_alt); cudaFree(h->d_sync); cudaFree(h->d_work);
+    cudaFree(h->d_ring); cudaFree(h->d_mail); cudaFree(h->d_sync); cudaFree(h->d_work);
     for (auto& e : h->ev_poll) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev_t) if (e) cudaEventDestroy(e);
     delete h;
@@ -713,6 +768,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "path")) { if (value < 0 || value > 3) { set_err("path must be 0..3"); return -1; } h->opt_path = (int)value; return 0; }
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "halo")) { if (value < -1 || value > 1) { set_err("halo must be -1, 0 or 1"); return -1; } h->opt_halo = (int)value; return 0; }
     if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)std::max(shapes().size(), blk_shapes().size())) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
     if (!strcmp(key, "tblock")) { if (value < 0 || value > kMaxTB) { set_err("tblock must be 0..%d", kMaxTB); return -1; } h->opt_tblock = (int)value; return 0; }
     set_err("unknown option '%s'", key);
@@ -732,6 +788,7 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "tile_h")) { *out = h->st_tile_h; return 0; }
     if (!strcmp(key, "tblock")) { *out = h->st_tblock; return 0; }
     if (!strcmp(key, "shape")) { *out = h->st_shape; return 0; }
+    if (!strcmp(key, "halo")) { *out = h->st_halo; return 0; }
     set_err("unknown stat '%s'", key);
     return -1;
 }

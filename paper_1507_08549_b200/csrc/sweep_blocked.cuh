@@ -23,8 +23,6 @@
 
 namespace snp {
 
-constexpr int kMaxTB = 12;     // max sweeps per launch / per exchange (m)
-
 struct BlkParams {
     Geom g;
     int ntx, nty;              // tiles in r and z

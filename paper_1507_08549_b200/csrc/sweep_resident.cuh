@@ -2,52 +2,64 @@
 //
 // PAPER.md:99 "successive overrelaxation method with the Gauss-Seidel method"; PAPER.md:149 names the cost this
 // design removes ("data migration, if not handled carefully, can take up even more time than using CPU solely").
-// Discretisation / ordering / pinned arithmetic: DESIGN.md R1, R3, R7, R10.  Design: DESIGN.md §6.
+// Discretisation / ordering / pinned arithmetic: DESIGN.md R1, R3, R7, R10.  Design: DESIGN.md section 6.
 //
-//  * The grid is cut into tiles, one CTA per tile, all co-resident (cooperative launch).  A CTA works on a fixed
-//    BW x BH "box" of cells = its owned tile plus a margin of 2m cells towards every neighbour.
-//  * Thread (a,b) keeps a 4 x H patch of phi in REGISTERS for the whole solve; f = 4 pi rho sits in shared memory.
-//    A red (black) update needs the 4 black (red) neighbours: inside the patch they are registers; across patch
-//    edges they come from small shared-memory exchange arrays the owning thread publishes after each half-sweep.
-//  * Temporal blocking: m full sweeps run between two inter-CTA exchanges.  Every box cell is updated every
-//    half-sweep; cells closer than t to an interior box edge are stale after t half-sweeps, so after 2m
-//    half-sweeps exactly the owned tile (distance >= 2m) is still exact -- no trapezoid bookkeeping, and a
-//    colour's updates are mutually independent, so tiling cannot change a bit of the result.
-//  * Exchange: owners store their patches to the global phi buffer of parity (epoch & 1), release a per-tile
-//    epoch flag, acquire the flags of the tiles their box overlaps and reload the non-owned patches (L2 traffic,
-//    ld.global.cg).  No grid-wide barrier on the critical path.
-//  * a-3: every owned cell's pre-update |res| and post-update |phi| feed per-sweep maxima (DSETP/FSEL on |x|),
-//    reduced warp -> CTA -> global atomicMax on order-preserving u64 keys in slot k.  The stopping decision for
-//    the sweeps of epoch e-1 is taken by every CTA (identically) at the end of epoch e, one epoch late, so the
-//    wait for the slowest CTA is off the critical path; the state two epochs back is still intact in the other
-//    phi buffer, so the crossing sweep k* is then REPLAYED exactly from it (<= m sweeps): the returned phi has
-//    exactly k* sweeps applied, like the oracle's.
+//  * The grid (of every batch member) is cut into tiles, one CTA per tile, all co-resident (cooperative launch).
+//    Thread (a,b) of a CTA keeps a 4 x H patch of phi in REGISTERS for the whole solve, f = 4 pi rho sits in shared
+//    memory (BoxEngine, box_engine.cuh).  Two ways of coupling the tiles:
+//      - halo mode: box == owned tile.  After every half-sweep the edge cells of the colour just updated go to the
+//        four neighbouring tiles and theirs come back into the border slots of the engine.  No redundant work;
+//        the latency of the exchange is hidden by the other CTA(s) sharing the SM.  For grids that fill the chip.
+//      - block mode (temporal blocking): box = owned tile + a margin of 2m cells towards every neighbour; m full
+//        sweeps run between two exchanges.  Every box cell is updated every half-sweep, cells closer than t to an
+//        interior box edge are stale after t half-sweeps, so after 2m half-sweeps exactly the owned tile is still
+//        exact; then the margins are refilled from the neighbours' tiles.  For grids that leave the chip idle.
+//    In both modes a colour's updates are mutually independent, so tiling cannot change a bit of the result (R10).
+//  * Exchange without fences or flags: every value travels as a 16-byte packet carrying the step number in both
+//    8-byte halves (ll_store / ll_load); the consumer polls the packet itself.  One L2 round trip per exchange.
+//  * a-3: per-sweep maxima of |res| and |phi_new| over the owned cells go warp -> CTA -> (service warp) atomicMax
+//    into per-sweep global slots.  An extra SERVICE WARP per CTA does all of that and the stopping decision, so the
+//    fences and L2 round trips of the reduction never stall the sweeps: the compute warps only hand it their maxima
+//    at the end of every interval (Q sweeps) and run at most one interval ahead of its decisions.
+//  * Main phase: FAST maxima (upper 32 bits of the doubles; one FMNMX per value).  They bound R_k from below within
+//    2^-20, enough to know that the rule has NOT fired.  When it may have (interval r_c), every CTA stops, the
+//    state at the start of r_c is reloaded from the checkpoint ring (each CTA stores its tile once per interval)
+//    and the ENDGAME runs interval by interval with EXACT maxima until the first sweep k* with R_k <= tol; if k* is
+//    inside an interval, its first sweeps are REPLAYED from the checkpoint.  The returned phi has exactly k* sweeps
+//    applied and `residual` is the exact R_k*, like the oracle's (R_k is not monotone, so nothing may be skipped).
 #pragma once
 #include "box_engine.cuh"
-#include "sweep_blocked.cuh"
 #include "tiling.h"
 
 namespace snp {
 
+constexpr int kResRing = 3;          // checkpoint ring depth (main phase runs <= 1 interval ahead of the decision)
+constexpr unsigned kTagEndgame = 1u << 28, kTagReplay = 2u << 28;
 
 struct ResParams {
     Geom g;
+    int halo;                  // 1: halo mode, 0: block mode
     int ntx, nty;              // tiles in r and z
-    int ow, oh;                // nominal owned tile size (multiples of 4 and H)
-    int m;                     // sweeps per epoch
+    int ow, oh;                // nominal owned tile size (halo mode: the box size)
+    int m;                     // block mode: sweeps per exchange (== Q)
+    int Q;                     // sweeps per interval (report / checkpoint / decision granularity)
     int max_sweeps;
-    const double* rho;
-    double* buf[3];            // state of epoch e lives in buf[e % 3]; buf[0] = caller's phi_inout (initial guess,
-                               // final result), buf[1..2] = workspace
-    const double* bE;
-    const double* bN;
-    const double* bS;
-    unsigned long long* slots; // [2*max_sweeps] per-sweep (max|res|, max|phi|) keys
-    Ctl* ctl;
-    double* hist;
-    unsigned int* flags;       // [ntiles] last epoch whose state this tile has published
-    unsigned int* arrived;     // [nepochs+2] CTAs that have posted the maxima of epoch e
-    unsigned int* gbar;        // single-use grid barrier counter
+    int force_exact;           // 1: exact maxima in every interval (exact history; every interval decided before the next)
+    const double* rho;         // [nb][ncell]
+    double* phi;               // [nb][ncell]  initial guess in, result out
+    double* ring;              // [nb][kResRing][ncell]  checkpoints: state after interval r in ring[r % kResRing]
+    uint4* mail;               // [nb][2][ncell]  tagged packets (halo mode uses buffer 0 only)
+    const double* bE;          // [nb][nz]
+    const double* bN;          // [nb][nr]
+    const double* bS;          // [nb][nr]
+    unsigned int* slots_f;     // [nb][2*cap]  FAST maxima (upper words) per sweep
+    unsigned long long* slots_x;   // [nb][2*cap]  EXACT maxima keys per sweep
+    int slot_stride, hist_stride;
+    unsigned int* arrived;     // [nb][2][nint+2]  CTAs that have reported interval r (main / endgame)
+    int arr_stride;            // nint + 2
+    unsigned int* gbar;        // [nb]  monotone grid-barrier counter
+    Ctl* ctl;                  // [nb]
+    double* hist;              // [nb][cap]
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -55,323 +67,399 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
 __device__ __forceinline__ void red_release_add_u32(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-__device__ __forceinline__ void spin_until_ge(const unsigned* p, unsigned want) {
-    while (ld_acquire_u32(p) < want) __nanosleep(20);
-}
+
+// One report of the compute warps to the service warp (shared memory, double-buffered by sequence parity).
+struct ResReport {
+    int r;          // interval (1-based)
+    int k0;         // sweeps applied before it
+    int n;          // sweeps in it
+    int exact;      // 1: exact maxima (endgame), 0: FAST
+    int bad;        // a non-finite owned value was seen
+    int quit;       // 1: no more reports
+};
+
+// What the service warp hands back (shared memory).
+struct ResDecision {
+    volatile int seq;        // last report sequence number fully processed
+    volatile int stop;       // main phase: a FAST candidate (or a non-finite value) was found in interval stop_r
+    volatile int stop_r;
+    volatile int stop_seq;   // ... by the decision of the report with this sequence number
+    volatile int fire_k;     // endgame: first sweep whose exact ratio fires in the last decided interval (0: none)
+    volatile int fire_bad;   // ... and whether it is non-finite
+    volatile double R;       // exact ratio at fire_k, else of the last sweep of the interval
+};
 
 template <int H, int TXN, int TYN>
 struct ResShape {
-    static constexpr int BW = 4 * TXN, BH = H * TYN, NT = TXN * TYN, NW = NT / 32;
-    static constexpr int LS = TXN + 2;                         // row stride of the lateral exchange arrays
-    static constexpr size_t smem_bytes =
-        sizeof(double) * ((size_t)BH * BW + 2 * (size_t)BH * LS + 2 * (size_t)(TYN + 2) * BW) +
-        sizeof(unsigned long long) * 2 * kMaxTB * NW;
+    using S = BoxShape<H, TXN, TYN>;
+    static constexpr int NT = S::NT, NW = S::NW, NTHREADS = S::NT + 32;
+    static constexpr size_t smax_entries = (size_t)2 * 2 * kMaxTB * NW;       // [parity][2Q][NW]
+    static constexpr size_t smem_bytes = sizeof(double) * S::engine_doubles + sizeof(unsigned long long) * smax_entries;
 };
 
-// Position of column c of a 4-group in the colour-permuted layout [c0, c2, c1, c3].
-__device__ __forceinline__ constexpr int perm4(int c) { return (c & 1) * 2 + (c >> 1); }
-
-template <int H, int TXN, int TYN>
-__global__ void __launch_bounds__(TXN* TYN, 1) k_sor_resident(const ResParams p) {
-    using S = ResShape<H, TXN, TYN>;
-    constexpr int BW = S::BW, BH = S::BH, NT = S::NT, NW = S::NW, LS = S::LS;
-    static_assert(NT % 32 == 0 && H % 2 == 0 && H <= 8, "shape");
+// grid = (ntx*nty, nbatch), block = TXN*TYN + 32 threads (the last warp is the service warp), cooperative launch.
+template <int H, int TXN, int TYN, int MINB>
+__global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResParams p) {
+    using S = BoxShape<H, TXN, TYN>;
+    using RS = ResShape<H, TXN, TYN>;
+    constexpr int BW = S::BW, BH = S::BH, NT = S::NT, NW = S::NW;
+    using Engine = BoxEngine<H, TXN, TYN, 1>;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* fs = reinterpret_cast<double*>(smem_raw);          // [BH][BW]   f, colour-permuted per 4-group
-    double* exL = fs + (size_t)BH * BW;                        // [BH][LS]   column 0 of thread a at [row][a+1]
-    double* exR = exL + (size_t)BH * LS;                       // [BH][LS]   column 3 of thread a at [row][a+1]
-    double* exB = exR + (size_t)BH * LS;                       // [TYN+2][BW] bottom row of thread-row b at [b+1]
-    double* exT = exB + (size_t)(TYN + 2) * BW;                // [TYN+2][BW] top row of thread-row b at [b+1]
-    unsigned long long* smax = reinterpret_cast<unsigned long long*>(exT + (size_t)(TYN + 2) * BW);  // [2*kMaxTB][NW]
-    __shared__ int s_k;            // decision broadcast: crossing sweep (0 = none)
-    __shared__ double s_R;
+    __shared__ ResReport s_rep[2];
+    __shared__ ResDecision s_dec;
+    __shared__ int s_bad;
+    __shared__ int s_panic;        // watchdog tripped (here or in another CTA): every wait falls through
+    __shared__ int s_zero;         // a quit word that never fires (endgame / replay polls)
 
     const Geom& g = p.g;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int a = tid % TXN, b = tid / TXN;
+    const int member = blockIdx.y;
+    const size_t ncell = (size_t)g.nr * g.nz;
     const int ntiles = p.ntx * p.nty;
     const int tile = blockIdx.x;
-    const int tx = tile % p.ntx, ty = tile / p.ntx;
-    const int m = p.m, h = 2 * m;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int Q = p.Q;
+    const int R_last = (p.max_sweeps + Q - 1) / Q;          // number of intervals
+    unsigned long long* smax =
+        reinterpret_cast<unsigned long long*>(smem_raw + sizeof(double) * S::engine_doubles);   // [2][2*kMaxTB][NW]
+    Ctl* ctl = p.ctl + member;
+    unsigned int* arrived = p.arrived + (size_t)member * 2 * p.arr_stride;
 
-    // owned tile [x0,x1) x [y0,y1) and box origin (bx,by), all aligned to (4,H)
-    const int x0 = tx * p.ow, x1 = min(g.nr, x0 + p.ow);
-    const int y0 = ty * p.oh, y1 = min(g.nz, y0 + p.oh);
-    const int bx = box_origin(x0, h, 4, BW, g.nr);
-    const int by = box_origin(y0, h, H, BH, g.nz);
-    const int gi0 = bx + 4 * a, gj0 = by + H * b;
-    const bool own = gi0 >= x0 && gi0 < x1 && gj0 >= y0 && gj0 < y1;
-    const int rowbase = H * b;
-
-    // tiles whose owned cells this box overlaps (their flags gate the halo reload)
-    const int ntx0 = bx / p.ow, ntx1 = (bx + BW - 1) / p.ow;
-    const int nty0 = by / p.oh, nty1 = (by + BH - 1) / p.oh;
-    const int nnb = (ntx1 - ntx0 + 1) * (nty1 - nty0 + 1);
-
-    // per-thread constants
-    double cEr[4], cWr[4];
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        cEr[c] = g.cE[gi0 + c];
-        cWr[c] = g.cW[gi0 + c];
+    if (tid == 0) {
+        s_dec.seq = 0; s_dec.stop = 0; s_dec.stop_r = 0; s_dec.stop_seq = 0; s_dec.fire_k = 0; s_dec.fire_bad = 0; s_dec.R = 0.0;
+        s_bad = 0; s_panic = 0; s_zero = 0;
     }
-    const bool mirror0 = (g.symmetry == 1 && gj0 == 0);
-    const double cS0 = mirror0 ? 0.0 : g.iz2;
-    const double diag0 = mirror0 ? g.D0 : g.D;
-    const double w0 = mirror0 ? g.wD0 : g.wD;
-
-    double phi[H][4];
-
-    auto load_patch = [&](const double* src) {
-#pragma unroll
-        for (int q = 0; q < H; ++q) {
-            const double2* s2 = reinterpret_cast<const double2*>(src + (size_t)(gj0 + q) * g.nr + gi0);
-            const double2 v0 = __ldcg(s2), v1 = __ldcg(s2 + 1);
-            phi[q][0] = v0.x; phi[q][1] = v0.y; phi[q][2] = v1.x; phi[q][3] = v1.y;
-        }
-    };
-    auto store_patch = [&](double* dst) {
-#pragma unroll
-        for (int q = 0; q < H; ++q) {
-            double2* d2 = reinterpret_cast<double2*>(dst + (size_t)(gj0 + q) * g.nr + gi0);
-            __stcg(d2, make_double2(phi[q][0], phi[q][1]));
-            __stcg(d2 + 1, make_double2(phi[q][2], phi[q][3]));
-        }
-    };
-    // publish every edge value of the patch (both colours) to the exchange arrays
-    auto publish_all = [&]() {
-#pragma unroll
-        for (int q = 0; q < H; ++q) {
-            exL[(rowbase + q) * LS + a + 1] = phi[q][0];
-            exR[(rowbase + q) * LS + a + 1] = phi[q][3];
-        }
-        double* bb = exB + (size_t)(b + 1) * BW + 4 * a;
-        double* tt = exT + (size_t)(b + 1) * BW + 4 * a;
-        *reinterpret_cast<double2*>(bb) = make_double2(phi[0][0], phi[0][2]);
-        *reinterpret_cast<double2*>(bb + 2) = make_double2(phi[0][1], phi[0][3]);
-        *reinterpret_cast<double2*>(tt) = make_double2(phi[H - 1][0], phi[H - 1][2]);
-        *reinterpret_cast<double2*>(tt + 2) = make_double2(phi[H - 1][1], phi[H - 1][3]);
-    };
-
-    // ---- one-time set-up: f into shared memory, constant borders of the exchange arrays, initial phi ----------
-#pragma unroll
-    for (int q = 0; q < H; ++q) {
-        const double2* r2 = reinterpret_cast<const double2*>(p.rho + (size_t)(gj0 + q) * g.nr + gi0);
-        const double2 v0 = __ldg(r2), v1 = __ldg(r2 + 1);
-        double* fr = fs + (size_t)(rowbase + q) * BW + 4 * a;
-        *reinterpret_cast<double2*>(fr) = make_double2(__dmul_rn(kFourPi, v0.x), __dmul_rn(kFourPi, v1.x));
-        *reinterpret_cast<double2*>(fr + 2) = make_double2(__dmul_rn(kFourPi, v0.y), __dmul_rn(kFourPi, v1.y));
-    }
-    for (int r = tid; r < BH; r += NT) {
-        exR[r * LS + 0] = 0.0;                                              // west of the box (cW = 0 on the axis)
-        exL[r * LS + TXN + 1] = (bx + BW == g.nr) ? p.bE[by + r] : 0.0;     // east: Dirichlet ghost or stale margin
-        exL[r * LS + 0] = 0.0;
-        exR[r * LS + TXN + 1] = 0.0;
-    }
-    for (int c = tid; c < BW; c += NT) {
-        const int gi = bx + (c & ~3) + ((c & 3) == 0 ? 0 : (c & 3) == 1 ? 2 : (c & 3) == 2 ? 1 : 3);  // inverse of perm4
-        exT[c] = (by == 0 && g.symmetry == 0) ? p.bS[gi] : 0.0;             // south ghost (unused when mirrored)
-        exB[(size_t)(TYN + 1) * BW + c] = (by + BH == g.nz) ? p.bN[gi] : 0.0;  // north ghost or stale margin
-        exB[c] = 0.0;
-        exT[(size_t)(TYN + 1) * BW + c] = 0.0;
-    }
-    load_patch(p.buf[0]);
-    publish_all();
     __syncthreads();
 
-    // ---- one half-sweep of colour COL over the thread's patch ------------------------------------------------
-    double mres = 0.0, mphi = 0.0;
-    auto half_sweep = [&](auto colTag, auto trackTag) {
-        constexpr int COL = decltype(colTag)::value;
-        constexpr bool TRACK = decltype(trackTag)::value;
-        // vertical outer neighbours of the bottom (q=0) and top (q=H-1) rows: other-colour cells of the rows outside
-        constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;                 // first updated column in those rows
-        const double2 So = *reinterpret_cast<const double2*>(exT + (size_t)b * BW + 4 * a + 2 * pb);
-        const double2 No = *reinterpret_cast<const double2*>(exB + (size_t)(b + 2) * BW + 4 * a + 2 * pt);
-#pragma unroll
-        for (int q = 0; q < H; ++q) {
-            constexpr int dummy = 0;
-            (void)dummy;
-            const int pq = (q + COL) & 1;                                   // compile-time after unrolling
-            const double outer = pq == 0 ? exR[(rowbase + q) * LS + a] : exL[(rowbase + q) * LS + a + 2];
-            const double2 fv = *reinterpret_cast<const double2*>(fs + (size_t)(rowbase + q) * BW + 4 * a + 2 * pq);
-            const double cS = q == 0 ? cS0 : g.iz2;
-            const double dg = q == 0 ? diag0 : g.D;
-            const double ww = q == 0 ? w0 : g.wD;
-#pragma unroll
-            for (int cc = 0; cc < 2; ++cc) {
-                const int c = pq + 2 * cc;
-                const double pW = c == 0 ? outer : phi[q][c == 0 ? 0 : c - 1];
-                const double pE = c == 3 ? outer : phi[q][c == 3 ? 3 : c + 1];
-                const double pN = q == H - 1 ? (cc == 0 ? No.x : No.y) : phi[q == H - 1 ? q : q + 1][c];
-                const double pS = q == 0 ? (cc == 0 ? So.x : So.y) : phi[q == 0 ? 0 : q - 1][c];
-                double res;
-                const double pn = sor_update(cEr[c], cWr[c], g.iz2, cS, dg, ww, pE, pW, pN, pS, phi[q][c],
-                                             cc == 0 ? fv.x : fv.y, res);
-                phi[q][c] = pn;
-                if (TRACK) {
-                    const bool ur = own & (fabs(res) > mres);
-                    mres = ur ? fabs(res) : mres;
-                    const bool up = own & (fabs(pn) > mphi);
-                    mphi = up ? fabs(pn) : mphi;
+    // =============================================================================================================
+    // service warp
+    // =============================================================================================================
+    if (warp == NW) {
+        unsigned int* slots_f = p.slots_f + (size_t)member * p.slot_stride;
+        unsigned long long* slots_x = p.slots_x + (size_t)member * p.slot_stride;
+        double* hist = p.hist + (size_t)member * p.hist_stride;
+        bool stopped = false;
+        const PollCtx pc_svc = {&s_zero, &s_panic, &ctl->panic, &ctl->panic_tile, tile};
+        for (int seq = 1;; ++seq) {
+            const int par = seq & 1;
+            if (par) asm volatile("bar.sync 3, %0;" ::"n"(RS::NTHREADS) : "memory");
+            else asm volatile("bar.sync 2, %0;" ::"n"(RS::NTHREADS) : "memory");
+            const ResReport rep = s_rep[par];
+            if (rep.quit) break;
+            // ---- report: this CTA's maxima of the interval -> global slots, then arrive
+            for (int idx = lane; idx < 2 * rep.n; idx += 32) {
+                unsigned long long v = 0ull;
+                for (int w = 0; w < NW; ++w) {
+                    const unsigned long long t = smax[((size_t)par * 2 * kMaxTB + idx) * NW + w];
+                    v = t > v ? t : v;
+                }
+                const size_t slot = 2 * (size_t)rep.k0 + idx;
+                if (rep.exact) atomicMax(slots_x + slot, rep.bad ? 0x7ff8000000000000ull : v);
+                else atomicMax(slots_f + slot, rep.bad ? 0x7ff80000u : (unsigned)v);
+            }
+            __syncwarp();
+            unsigned int* arr = arrived + (size_t)rep.exact * p.arr_stride + rep.r;
+            if (lane == 0) {
+                __threadfence();
+                red_release_add_u32(arr, 1u);
+            }
+            // ---- decide the interval (every CTA reads the same final slots -> the same answer)
+            if (rep.exact || !stopped) {
+                if (lane == 0) {
+                    unsigned spins = 0;
+                    while (ld_acquire_u32(arr) < (unsigned)ntiles && !poll_giveup(pc_svc, spins, 10 + rep.exact, rep.r))
+                        __nanosleep(64);
+                }
+                __syncwarp();
+                bool fire = false, bad = false;
+                double R = 0.0;
+                if (lane < rep.n) {
+                    const size_t slot = 2 * (size_t)(rep.k0 + lane);
+                    if (rep.exact) {
+                        R = stop_ratio(__ldcg(slots_x + slot), __ldcg(slots_x + slot + 1), ctl->maxf, g.D);
+                        bad = is_nonfinite(R);
+                        fire = bad || (g.tol > 0.0 && R <= g.tol);
+                    } else {
+                        // upper words only: R_lo <= R_k (up to rounding, covered by the factor)
+                        const unsigned long long kr = (unsigned long long)__ldcg(slots_f + slot) << 32;
+                        const unsigned long long kp = ((unsigned long long)__ldcg(slots_f + slot + 1) << 32) | 0xffffffffull;
+                        R = stop_ratio(kr, kp, ctl->maxf, g.D);
+                        bad = is_nonfinite(R);
+                        fire = bad || (g.tol > 0.0 && R <= g.tol * 1.000000001);
+                    }
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, fire);
+                const int first = bal ? __ffs(bal) - 1 : -1;
+                if (tile == 0 && lane < rep.n && (first < 0 || lane <= first || !rep.exact)) hist[rep.k0 + lane] = R;
+                if (rep.exact) {
+                    const int src = first < 0 ? rep.n - 1 : first;
+                    const double Rsel = __shfl_sync(0xffffffffu, R, src);
+                    const int badsel = __shfl_sync(0xffffffffu, (int)bad, src);
+                    if (lane == 0) {
+                        s_dec.fire_k = first < 0 ? 0 : rep.k0 + first + 1;
+                        s_dec.fire_bad = badsel;
+                        s_dec.R = Rsel;
+                    }
+                } else if (first >= 0) {
+                    stopped = true;
+                    if (lane == 0) {
+                        s_dec.stop_r = rep.r;
+                        s_dec.stop_seq = seq;
+                        __threadfence_block();
+                        s_dec.stop = 1;
+                    }
                 }
             }
-        }
-        // publish the updated edge cells of this colour
-#pragma unroll
-        for (int q = 0; q < H; ++q) {
-            const int pq = (q + COL) & 1;
-            if (pq == 0) exL[(rowbase + q) * LS + a + 1] = phi[q][0];
-            else exR[(rowbase + q) * LS + a + 1] = phi[q][3];
-        }
-        *reinterpret_cast<double2*>(exB + (size_t)(b + 1) * BW + 4 * a + 2 * pb) = make_double2(phi[0][pb], phi[0][pb + 2]);
-        *reinterpret_cast<double2*>(exT + (size_t)(b + 1) * BW + 4 * a + 2 * pt) =
-            make_double2(phi[H - 1][pt], phi[H - 1][pt + 2]);
-        __syncthreads();
-    };
-    using C0 = std::integral_constant<int, 0>;
-    using C1 = std::integral_constant<int, 1>;
-
-    // Decision for the sweeps of epoch ee (all CTAs evaluate the same final slot values -> same answer).
-    // Returns the first sweep k of that epoch whose ratio fires (non-finite, or <= tol when tol > 0), else 0.
-    auto check_epoch = [&](int ee) -> int {
-        const int kfirst = (ee - 1) * m + 1;
-        const int nsw = min(m, p.max_sweeps - (ee - 1) * m);
-        if (tid == 0) spin_until_ge(p.arrived + ee, (unsigned)ntiles);
-        __syncthreads();
-        if (warp == 0) {
-            bool fire = false;
-            double R = 0.0;
-            if (lane < nsw) {
-                const unsigned long long kr = __ldcg(p.slots + 2 * (size_t)(kfirst + lane - 1));
-                const unsigned long long kp = __ldcg(p.slots + 2 * (size_t)(kfirst + lane - 1) + 1);
-                R = stop_ratio(kr, kp, p.ctl->maxf, g.D);
-                fire = is_nonfinite(R) || (g.tol > 0.0 && R <= g.tol);
-            }
-            const unsigned bal = __ballot_sync(0xffffffffu, fire);
-            const int first = bal ? __ffs(bal) - 1 : -1;
-            if (tile == 0 && lane < nsw && (first < 0 || lane <= first)) p.hist[kfirst + lane - 1] = R;
-            if (lane == (first < 0 ? nsw - 1 : first)) {
-                s_k = first < 0 ? 0 : kfirst + first;
-                s_R = R;
-            }
-        }
-        __syncthreads();
-        return s_k;
-    };
-
-    // ---- epoch loop ------------------------------------------------------------------------------------------
-    // End of epoch e:  store state e -> release flag  |  post maxima, arrive  |  acquire neighbour flags -> reload
-    // margins  |  decide epoch e-1 while those loads are in flight.  State e overwrites state e-3, which nobody can
-    // still be reading: the decision for epoch e-2 (taken during the end of epoch e-1) waited for every CTA to have
-    // finished epoch e-2.  The state before any epoch whose sweeps are still undecided therefore stays intact.
-    int done = 0, e = 0, kstar = 0, e_cross = 0;
-    while (done < p.max_sweeps) {
-        ++e;
-        const int nsw = min(m, p.max_sweeps - done);
-        for (int s = 0; s < nsw; ++s) {
-            mres = 0.0;
-            mphi = 0.0;
-            half_sweep(C0{}, std::true_type{});
-            half_sweep(C1{}, std::true_type{});
-            const unsigned long long wr = warp_max_key(dbits(mres)), wp = warp_max_key(dbits(mphi));
+            __syncwarp();
             if (lane == 0) {
-                smax[(2 * s) * NW + warp] = wr;
-                smax[(2 * s + 1) * NW + warp] = wp;
+                __threadfence_block();
+                s_dec.seq = seq;
             }
         }
-        const bool last = done + nsw >= p.max_sweeps;
-        double* cur = p.buf[e % 3];
-        if (!last && own) store_patch(cur);
-        // any non-finite owned value persists (NaN/Inf never relax away): poison this epoch's maxima
-        bool bad = false;
-        if (own) {
+        return;
+    }
+
+    // =============================================================================================================
+    // compute warps
+    // =============================================================================================================
+    Engine E;
+    E.carve(reinterpret_cast<double*>(smem_raw));
+    E.bind_thread(tid);
+
+    const int tx = tile % p.ntx, ty = tile / p.ntx;
+    int x0, x1, y0, y1, bx, by;
+    if (p.halo) {
+        x0 = bx = tx * BW; x1 = x0 + BW;
+        y0 = by = ty * BH; y1 = min(g.nz, y0 + BH);
+    } else {
+        const int h = 2 * p.m;
+        x0 = tx * p.ow; x1 = min(g.nr, x0 + p.ow);
+        y0 = ty * p.oh; y1 = min(g.nz, y0 + p.oh);
+        bx = box_origin(x0, h, 4, BW, g.nr);
+        by = box_origin(y0, h, H, BH, g.nz);
+    }
+    const int gi0 = bx + 4 * E.a, gj0 = by + H * E.b;
+    E.active = gj0 < g.nz;                                      // false only in the ragged last tile row (halo mode)
+    const bool own = gi0 >= x0 && gi0 < x1 && gj0 >= y0 && gj0 < y1;
+
+    const double* rho = p.rho + (size_t)member * ncell;
+    double* phi_io = p.phi + (size_t)member * ncell;
+    double* ring = p.ring + (size_t)member * kResRing * ncell;
+    uint4* mail = p.mail + (size_t)member * 2 * ncell;
+    const double* bE = p.bE + (size_t)member * g.nz;
+    const double* bN = p.bN + (size_t)member * g.nr;
+    const double* bS = p.bS + (size_t)member * g.nr;
+    unsigned int* gbar = p.gbar + member;
+    const volatile int* stop = &s_dec.stop;
+    const PollCtx pc_main = {&s_dec.stop, &s_panic, &ctl->panic, &ctl->panic_tile, tile};   // main phase: polls end at a stop
+    const PollCtx pc_end = {&s_zero, &s_panic, &ctl->panic, &ctl->panic_tile, tile};        // endgame / replay
+
+    // state after interval r (r = 0: the caller's initial guess, untouched until the very end)
+    auto state_of = [&](int r) -> double* { return r == 0 ? phi_io : ring + (size_t)(r % kResRing) * ncell; };
+
+    // (re)load the whole box from a full state array
+    auto load_box = [&](const double* src) {
+        if (E.active) {
+            E.load_patch(src, g.nr, gi0, gj0);
+        } else {
 #pragma unroll
             for (int q = 0; q < H; ++q)
 #pragma unroll
-                for (int c = 0; c < 4; ++c) bad |= !(fabs(phi[q][c]) < INFINITY);
+                for (int c = 0; c < 4; ++c) E.phi[q][c] = bN[gi0 + c];   // published as the north ghost row below
         }
-        const int anybad = __syncthreads_or(bad);            // also: every thread's state stores are issued
-        if (!last && tid == 0) st_release_u32(p.flags + tile, (unsigned)e);
-        if (warp == 0) {
-            for (int idx = lane; idx < 2 * nsw; idx += 32) {
-                unsigned long long v = 0ull;
-                for (int w = 0; w < NW; ++w) {
-                    const unsigned long long t = smax[idx * NW + w];
-                    v = t > v ? t : v;
+        E.set_borders(g, bx, by, bE, bN, bS, tid, NT);
+        Engine::sync();                                          // borders first: halo loads overwrite some of them
+        if (p.halo) E.load_halo_borders(src, g.nr, g.nz, bx, by);
+        E.publish_all();
+        Engine::sync();
+    };
+
+    auto panicked = [&]() -> bool { return *(volatile int*)&s_panic != 0; };
+    // The service warp (and the watchdog) write their words at any time, so two compute threads may read different
+    // values; every branch that leads to a different sequence of barriers is taken on the OR over the compute warps.
+    auto uniform_or = [&](bool v) -> bool {
+        int out;
+        asm volatile(
+            "{\n\t.reg .pred p, q;\n\tsetp.ne.s32 q, %1, 0;\n\tbar.red.or.pred p, 1, %2, q;\n\tselp.s32 %0, 1, 0, p;\n\t}"
+            : "=r"(out)
+            : "r"((int)v), "n"(NT)
+            : "memory");
+        return out != 0;
+    };
+    unsigned gbar_gen = 0;
+    auto grid_barrier = [&]() {
+        ++gbar_gen;
+        Engine::sync();
+        if (tid == 0) {
+            __threadfence();
+            red_release_add_u32(gbar, 1u);
+            unsigned spins = 0;
+            while (ld_acquire_u32(gbar) < gbar_gen * (unsigned)ntiles && !poll_giveup(pc_end, spins, 20, (int)gbar_gen))
+                __nanosleep(64);
+        }
+        Engine::sync();
+    };
+
+    // hand a report to the service warp: named barriers 2 / 3 alternate with the report's sequence parity
+    auto report_arrive = [&](int par) {
+        if (par) asm volatile("bar.arrive 3, %0;" ::"n"(RS::NTHREADS) : "memory");
+        else asm volatile("bar.arrive 2, %0;" ::"n"(RS::NTHREADS) : "memory");
+    };
+    int seq = 0;                                                 // reports handed to the service warp so far
+    auto wait_decided = [&](int want) {
+        unsigned spins = 0;
+        while (s_dec.seq < want && !poll_giveup(pc_end, spins, 30, want)) __nanosleep(32);
+    };
+
+    // n sweeps starting after k0 applied sweeps; maxima of sweep s of the interval go to smax[par][2s..2s+1][warp]
+    auto run_sweeps = [&](auto trackTag, int k0, int n, unsigned tagbase, int par, const PollCtx& pc) {
+        constexpr int TRACK = decltype(trackTag)::value;
+        for (int s = 0; s < n; ++s) {
+            E.reset_maxima();
+            E.template half_sweep<0, TRACK, false>();
+            if (p.halo) E.template halo_exchange<0>(mail, tagbase + 2u * (unsigned)(k0 + s) + 1u, g.nr, g.nz, bx, by, pc);
+            Engine::sync();
+            E.template half_sweep<1, TRACK, false>();
+            if (p.halo) E.template halo_exchange<1>(mail, tagbase + 2u * (unsigned)(k0 + s) + 2u, g.nr, g.nz, bx, by, pc);
+            Engine::sync();
+            if (TRACK == kTrackFast) {
+                const unsigned wr = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres_f) : 0u);
+                const unsigned wp = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mphi_f) : 0u);
+                if (lane == 0) {
+                    smax[((size_t)par * 2 * kMaxTB + 2 * s) * NW + warp] = wr;
+                    smax[((size_t)par * 2 * kMaxTB + 2 * s + 1) * NW + warp] = wp;
                 }
-                if (anybad) v = 0x7ff8000000000000ull;
-                atomicMax(p.slots + 2 * (size_t)(done + (idx >> 1)) + (idx & 1), v);
-            }
-            __syncwarp();
-            if (lane == 0) red_release_add_u32(p.arrived + e, 1u);
-        }
-        done += nsw;
-        if (last) {
-            if (e >= 2) {
-                kstar = check_epoch(e - 1);
-                if (kstar) { e_cross = e - 1; break; }
-            }
-            kstar = check_epoch(e);
-            if (kstar) e_cross = e;
-            break;
-        }
-        if (warp == NW - 1) {
-            for (int n = lane; n < nnb; n += 32) {
-                const int nx = ntx0 + n % (ntx1 - ntx0 + 1), ny = nty0 + n / (ntx1 - ntx0 + 1);
-                spin_until_ge(p.flags + ny * p.ntx + nx, (unsigned)e);
+            } else if (TRACK == kTrackExact) {
+                const unsigned long long wr = warp_max_key(own ? E.mres_k : 0ull);
+                const unsigned long long wp = warp_max_key(own ? E.mphi_k : 0ull);
+                if (lane == 0) {
+                    smax[((size_t)par * 2 * kMaxTB + 2 * s) * NW + warp] = wr;
+                    smax[((size_t)par * 2 * kMaxTB + 2 * s + 1) * NW + warp] = wp;
+                }
             }
         }
-        __syncthreads();
-        if (!own) load_patch(cur);
-        if (e >= 2) {
-            kstar = check_epoch(e - 1);
-            if (kstar) { e_cross = e - 1; break; }
+    };
+
+    // end of interval r (n sweeps after k0): checkpoint, block-mode exchange, report.  Returns the report's sequence
+    // number.  The margins are NOT yet valid in block mode when this returns (see finish_exchange).
+    auto end_interval = [&](int r, int k0, int n, int exact, unsigned tagbase) -> int {
+        if (own) E.store_patch(state_of(r), g.nr, gi0, gj0);
+        uint4* mb = mail + (size_t)(r & 1) * ncell;
+        if (!p.halo && own && ntiles > 1) E.ll_store_patch(mb, tagbase + (unsigned)r, g.nr, gi0, gj0);
+        // FAST maxima drop NaN (FMNMX); any non-finite owned value persists (NaN/Inf never relax away), so one
+        // check per interval is enough to poison its maxima and send the solve to the exact endgame
+        if (!exact && own && E.any_nonfinite()) s_bad = 1;
+        ++seq;
+        const int par = seq & 1;
+        Engine::sync();                                          // smax + s_bad complete
+        if (tid == 0) {
+            ResReport& rp = s_rep[par];
+            rp.r = r; rp.k0 = k0; rp.n = n; rp.exact = exact; rp.quit = 0;
+            rp.bad = exact ? 0 : s_bad;      // exact keys carry NaN/Inf themselves (abs_key sorts them highest)
         }
-        publish_all();
-        __syncthreads();
+        __threadfence_block();
+        report_arrive(par);
+        return seq;
+    };
+    // block mode: refill the margins from the neighbours' tiles of interval r and republish the patch edges
+    auto finish_exchange = [&](int r, unsigned tagbase, const PollCtx& pc) {
+        if (p.halo || ntiles == 1) return;
+        const uint4* mb = mail + (size_t)(r & 1) * ncell;
+        if (!own) E.ll_wait_patch(mb, tagbase + (unsigned)r, g.nr, gi0, gj0, pc);
+        E.publish_all();
+        Engine::sync();
+    };
+
+    // one-time set-up: f, coefficients, initial phi
+    if (E.active) E.load_f(rho, g.nr, gi0, gj0);
+    E.load_coeffs(g, gi0, E.active ? gj0 : 0);
+    load_box(phi_io);
+
+    // ---- main phase: FAST maxima, decisions one interval late -------------------------------------------------
+    int r_c = 1;                 // interval the endgame starts with
+    bool reload = false;         // endgame must reload the state before r_c (CTAs stopped at different intervals)
+    if (!p.force_exact) {
+        int r = 1;
+        for (; r < R_last; ++r) {
+            const int k0 = (r - 1) * Q;
+            run_sweeps(std::integral_constant<int, kTrackFast>{}, k0, Q, 0u, (seq + 1) & 1, pc_main);
+            const int sq = end_interval(r, k0, Q, 0, 0u);
+            finish_exchange(r, 0u, pc_main);
+            wait_decided(sq - 1);
+            // a stop decided by report sq (being processed right now) must not be seen by some threads only
+            const bool stopped_now = *stop && s_dec.stop_seq <= sq - 1;
+            if (uniform_or(stopped_now || panicked())) break;
+        }
+        if (r == R_last) {       // ran to the last interval: wait for every earlier decision
+            wait_decided(seq);
+        }
+        if (uniform_or(*stop != 0)) {
+            r_c = s_dec.stop_r;
+            reload = true;
+        } else {
+            r_c = R_last;
+        }
     }
 
-    // ---- finish ----------------------------------------------------------------------------------------------
-    if (kstar && !(e_cross == e && kstar == done)) {
-        // the rule fired at sweep kstar of epoch e_cross: replay it exactly from the state before that epoch
-        const int es = e_cross - 1;
-        const int r = kstar - es * m;
-        load_patch(p.buf[es % 3]);
-        __syncthreads();
-        if (tid == 0) {                      // everyone has read its box before anyone overwrites buf[0]
-            red_release_add_u32(p.gbar, 1u);
-            spin_until_ge(p.gbar, (unsigned)ntiles);
+    // ---- endgame: EXACT maxima, every interval decided before the next ------------------------------------------
+    int sweeps = 0, status = 0;
+    double Rfinal = 0.0;
+    {
+        unsigned tagbase = 0u;
+        if (reload) {
+            grid_barrier();
+            load_box(state_of(r_c - 1));
+            tagbase = kTagEndgame;
         }
-        __syncthreads();
-        publish_all();
-        __syncthreads();
-        for (int s = 0; s < r; ++s) {
-            half_sweep(C0{}, std::false_type{});
-            half_sweep(C1{}, std::false_type{});
+        int r = r_c;
+        for (;; ++r) {
+            const int k0 = (r - 1) * Q;
+            const int n = min(Q, p.max_sweeps - k0);
+            if (n <= 0) {        // max_sweeps == 0
+                sweeps = 0; status = g.tol > 0.0 ? 1 : 0; Rfinal = 0.0;
+                break;
+            }
+            run_sweeps(std::integral_constant<int, kTrackExact>{}, k0, n, tagbase, (seq + 1) & 1, pc_end);
+            const int sq = end_interval(r, k0, n, 1, tagbase);
+            wait_decided(sq);
+            if (uniform_or(panicked())) { sweeps = k0 + n; status = -2; break; }
+            const int fk = s_dec.fire_k;
+            if (fk) {
+                sweeps = fk; status = s_dec.fire_bad ? -3 : 0; Rfinal = s_dec.R;
+                if (fk != k0 + n) {                              // crossing inside the interval: replay from its start
+                    grid_barrier();
+                    load_box(state_of(r - 1));
+                    run_sweeps(std::integral_constant<int, kTrackNone>{}, k0, fk - k0, kTagReplay, 0, pc_end);
+                }
+                break;
+            }
+            if (k0 + n >= p.max_sweeps) {
+                sweeps = p.max_sweeps; status = g.tol > 0.0 ? 1 : 0; Rfinal = s_dec.R;
+                break;
+            }
+            finish_exchange(r, tagbase, pc_end);
         }
     }
-    if (own) store_patch(p.buf[0]);
+
+    // ---- finish ---------------------------------------------------------------------------------------------------
+    // Nobody may still be reading phi_io as "state 0": a reload from it is followed by a grid barrier-free run, so
+    // make every CTA pass one more barrier before the result overwrites it.
+    grid_barrier();
+    if (own) E.store_patch(phi_io, g.nr, gi0, gj0);
+    ++seq;
+    Engine::sync();
+    if (tid == 0) s_rep[seq & 1].quit = 1;
+    __threadfence_block();
+    report_arrive(seq & 1);
     if (tile == 0 && tid == 0) {
-        Ctl* c = p.ctl;
-        const double R = s_R;
-        if (kstar) {
-            c->sweeps = kstar;
-            c->residual = R;
-            c->status = is_nonfinite(R) ? -3 : 0;
-        } else {
-            c->sweeps = p.max_sweeps;
-            c->residual = R;
-            c->status = g.tol > 0.0 ? 1 : 0;
-        }
-        c->done = 1;
+        ctl->sweeps = sweeps;
+        ctl->status = status;
+        ctl->residual = Rfinal;
+        __threadfence();
+        ctl->done = 1;
     }
 }
 
