@@ -62,7 +62,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -80,6 +80,9 @@ struct sn_poisson {
     void* d_mail = nullptr;                                  // resident path: tagged packets, nb x 2 x nr*nz x 16 B
     unsigned int* d_sync = nullptr;                          // resident path: arrived counters | grid barriers
     size_t ring_cap = 0, mail_cap = 0, sync_cap = 0;
+    long long* d_prof = nullptr;                             // resident path: optional in-kernel profile, ctas x 8
+    size_t prof_cap = 0, prof_ctas = 0;
+    double prof_mean[8] = {0}, prof_max[8] = {0};
     bool user_boundary = false;
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
     cudaEvent_t ev_t[3] = {nullptr, nullptr, nullptr};
@@ -496,6 +499,19 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     P.arr_stride = (int)(nint + 2);
     P.gbar = h->d_sync + (size_t)nbatch * 2 * (nint + 2);
     P.ctl = h->d_ctl; P.hist = h->d_hist;
+    P.prof = nullptr;
+    h->prof_ctas = 0;
+    if (h->opt_prof) {
+        const size_t need = (size_t)pl.ntiles * nbatch * 8;
+        if (h->prof_cap < need) {
+            cudaFree(h->d_prof); h->d_prof = nullptr; h->prof_cap = 0;
+            CU_TRY(cudaMalloc((void**)&h->d_prof, sizeof(long long) * need));
+            h->prof_cap = need;
+        }
+        CU_TRY(cudaMemsetAsync(h->d_prof, 0, sizeof(long long) * need, st));
+        P.prof = h->d_prof;
+        h->prof_ctas = (size_t)pl.ntiles * nbatch;
+    }
     void* args[] = {&P};
     CU_TRY(cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
     CU_TRY(cudaLaunchCooperativeKernel(S.fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, S.smem, st));
@@ -577,6 +593,19 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
         out[b].residual = h->h_ctl[b].residual;
     }
     h->last_sweeps0 = out[0].sweeps;
+    if (h->prof_ctas) {                         // in-kernel profile of the resident kernel: mean / max over its CTAs
+        std::vector<long long> pf(h->prof_ctas * 8);
+        CU_TRY(cudaMemcpy(pf.data(), h->d_prof, sizeof(long long) * pf.size(), cudaMemcpyDeviceToHost));
+        for (int i = 0; i < 8; ++i) {
+            double sum = 0, mx = 0;
+            for (size_t c = 0; c < h->prof_ctas; ++c) {
+                sum += (double)pf[c * 8 + i];
+                mx = std::max(mx, (double)pf[c * 8 + i]);
+            }
+            h->prof_mean[i] = sum / h->prof_ctas;
+            h->prof_max[i] = mx;
+        }
+    }
     return 0;
 }
 
@@ -651,7 +680,7 @@ void sn_poisson_destroy(sn_poisson* h) {
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
     cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage);
-    cudaFree(h->d_ring); cudaFree(h->d_mail); cudaFree(h->d_sync); cudaFree(h->d_work);
+    cudaFree(h->d_prof); cudaFree(h->d_ring); cudaFree(h->d_mail); cudaFree(h->d_sync); cudaFree(h->d_work);
     for (auto& e : h->ev_poll) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev_t) if (e) cudaEventDestroy(e);
     delete h;
@@ -768,6 +797,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "path")) { if (value < 0 || value > 3) { set_err("path must be 0..3"); return -1; } h->opt_path = (int)value; return 0; }
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "prof")) { h->opt_prof = value ? 1 : 0; return 0; }
     if (!strcmp(key, "halo")) { if (value < -1 || value > 1) { set_err("halo must be -1, 0 or 1"); return -1; } h->opt_halo = (int)value; return 0; }
     if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)std::max(shapes().size(), blk_shapes().size())) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
     if (!strcmp(key, "tblock")) { if (value < 0 || value > kMaxTB) { set_err("tblock must be 0..%d", kMaxTB); return -1; } h->opt_tblock = (int)value; return 0; }
@@ -789,6 +819,8 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "tblock")) { *out = h->st_tblock; return 0; }
     if (!strcmp(key, "shape")) { *out = h->st_shape; return 0; }
     if (!strcmp(key, "halo")) { *out = h->st_halo; return 0; }
+    if (!strncmp(key, "prof_mean", 9) && key[9] >= '0' && key[9] <= '7' && !key[10]) { *out = h->prof_mean[key[9] - '0']; return 0; }
+    if (!strncmp(key, "prof_max", 8) && key[8] >= '0' && key[8] <= '7' && !key[9]) { *out = h->prof_max[key[8] - '0']; return 0; }
     set_err("unknown stat '%s'", key);
     return -1;
 }

@@ -60,6 +60,7 @@ struct ResParams {
     unsigned int* gbar;        // [nb]  monotone grid-barrier counter
     Ctl* ctl;                  // [nb]
     double* hist;              // [nb][cap]
+    long long* prof;           // optional [ctas][8] SM-clock counters of thread 0 of every CTA ("prof" option), else NULL
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -289,6 +290,12 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             : "memory");
         return out != 0;
     };
+    // optional in-kernel profile (thread 0 of the CTA): 0 total, 1 half-sweep compute, 2 halo exchange, 3 barrier,
+    // 4 end of interval, 5 margin refill, 6 wait for the decision, 7 half-sweeps
+    const bool prof_on = p.prof != nullptr && tid == 0;
+    long long pf[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    auto tick = [&]() -> long long { return prof_on ? clock64() : 0ll; };
+    const long long t_begin = tick();
     unsigned gbar_gen = 0;
     auto grid_barrier = [&]() {
         ++gbar_gen;
@@ -319,12 +326,20 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         constexpr int TRACK = decltype(trackTag)::value;
         for (int s = 0; s < n; ++s) {
             E.reset_maxima();
+            const long long t0 = tick();
             E.template half_sweep<0, TRACK, false>();
+            const long long t1 = tick();
             if (p.halo) E.template halo_exchange<0>(mail, tagbase + 2u * (unsigned)(k0 + s) + 1u, g.nr, g.nz, bx, by, pc);
+            const long long t2 = tick();
             Engine::sync();
+            const long long t3 = tick();
             E.template half_sweep<1, TRACK, false>();
+            const long long t4 = tick();
             if (p.halo) E.template halo_exchange<1>(mail, tagbase + 2u * (unsigned)(k0 + s) + 2u, g.nr, g.nz, bx, by, pc);
+            const long long t5 = tick();
             Engine::sync();
+            const long long t6 = tick();
+            pf[1] += (t1 - t0) + (t4 - t3); pf[2] += (t2 - t1) + (t5 - t4); pf[3] += (t3 - t2) + (t6 - t5); pf[7] += 2;
             if (TRACK == kTrackFast) {
                 const unsigned wr = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres_f) : 0u);
                 const unsigned wp = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mphi_f) : 0u);
@@ -386,9 +401,13 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         for (; r < R_last; ++r) {
             const int k0 = (r - 1) * Q;
             run_sweeps(std::integral_constant<int, kTrackFast>{}, k0, Q, 0u, (seq + 1) & 1, pc_main);
+            const long long ta = tick();
             const int sq = end_interval(r, k0, Q, 0, 0u);
+            const long long tb = tick();
             finish_exchange(r, 0u, pc_main);
+            const long long tc = tick();
             wait_decided(sq - 1);
+            pf[4] += tb - ta; pf[5] += tc - tb; pf[6] += tick() - tc;
             // a stop decided by report sq (being processed right now) must not be seen by some threads only
             const bool stopped_now = *stop && s_dec.stop_seq <= sq - 1;
             if (uniform_or(stopped_now || panicked())) break;
@@ -454,6 +473,11 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     if (tid == 0) s_rep[seq & 1].quit = 1;
     __threadfence_block();
     report_arrive(seq & 1);
+    if (prof_on) {
+        pf[0] = clock64() - t_begin;
+        long long* dst = p.prof + ((size_t)member * ntiles + tile) * 8;
+        for (int i = 0; i < 8; ++i) dst[i] = pf[i];
+    }
     if (tile == 0 && tid == 0) {
         ctl->sweeps = sweeps;
         ctl->status = status;
