@@ -306,117 +306,104 @@ struct BoxEngine {
         }
     }
 
-    // After the half-sweep of colour COL: send this box's updated edge cells to the neighbouring tiles and receive
-    // theirs into the border slots.  `mail` is indexed like the grid (one tagged packet per cell; only box-edge
-    // cells are ever used); a cell of colour COL is written once per sweep with a strictly increasing tag and its
-    // reader consumes tag t before the writer can produce t + 2, so one buffer is enough.  The poll gives up when
-    // *stop becomes non-zero (the solve is leaving this phase; the box is reloaded afterwards).
-    template <int COL>
-    __device__ __forceinline__ void halo_exchange(uint4* __restrict__ mail, unsigned tag, int nr, int nz, int bx,
-                                                  int by, const PollCtx& pc) {
-        unsigned spins = 0;
-        if (!active) return;
-        constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;
-        const int gi0 = bx + 4 * a, gj0 = by + rowbase;
-        const bool west = a == 0 && bx > 0, east = a == TXN - 1 && bx + BW < nr;
-        const bool south = b == 0 && by > 0, north = b == TYN - 1 && by + BH < nz;
-        if (!(west || east || south || north)) return;
-        // send
-        if (west) {
-#pragma unroll
-            for (int q = 0; q < H; ++q)
-                if (((q + COL) & 1) == 0) ll_store(mail + (size_t)(gj0 + q) * nr + gi0, phi[q][0], tag);
+    // Inbox of one tile: tagged packets it receives from its four neighbours, [E: BH][W: BH][N: BW][S: BW], each edge
+    // split by colour so that the packets of one half-sweep are contiguous: slot(i) = (i & 1) * n/2 + (i >> 1).
+    // A slot is written once per sweep with a strictly increasing tag, and its reader consumes tag t before the
+    // writer can produce t + 2, so one buffer is enough.
+    static constexpr int kInboxE = 0, kInboxW = BH, kInboxN = 2 * BH, kInboxS = 2 * BH + BW, kInboxPackets = 2 * (BH + BW);
+
+    // Which neighbours exist and where their inboxes are.
+    struct HaloLinks {
+        uint4* own;                  // this tile's inbox
+        uint4 *w, *e, *s, *n;        // neighbours' inboxes (NULL: no neighbour on that side)
+        int rows;                    // box rows inside the grid (== BH except in the ragged last tile row), even
+    };
+
+    // Per-thread halo state, computed once (halo_bind) so that the per-half-sweep exchange is a handful of
+    // instructions.  Receive: thread tid < BH + BW fetches ONE packet per half-sweep; for colour 0 it reads h_src
+    // and writes h_dst, for colour 1 both move by the deltas.  Send: a box-edge thread keeps the base of its slots
+    // in the neighbour's inbox (a thread sits on at most one column edge and one row edge: TXN, TYN >= 2).
+    const uint4* h_src = nullptr;
+    double* h_dst = nullptr;
+    int h_dsrc = 0, h_ddst = 0;
+    uint4* h_scol = nullptr;         // column edge: west (h_west) or east
+    uint4* h_srow = nullptr;         // row edge: south (h_south) or north
+    bool h_west = false, h_south = false;
+
+    __device__ __forceinline__ void halo_bind(const HaloLinks& L, int tid) {
+        static_assert(BH + BW <= S::NT && TXN >= 2 && TYN >= 2, "halo mode: one packet per thread, one edge per axis");
+        if (tid < BH / 2) {                                  // east tile's column 0
+            const int j = tid;
+            if (L.e && 2 * j < L.rows) {
+                h_src = L.own + kInboxE + j; h_dsrc = BH / 2;
+                h_dst = exL + 2 * j * LS + TXN + 1; h_ddst = LS;
+            }
+        } else if (tid < BH) {                               // west tile's column 3
+            const int j = tid - BH / 2;
+            if (L.w && 2 * j < L.rows) {
+                h_src = L.own + kInboxW + BH / 2 + j; h_dsrc = -(BH / 2);
+                h_dst = exR + (2 * j + 1) * LS; h_ddst = -LS;
+            }
+        } else if (tid < BH + BW / 2) {                      // north tile's bottom row
+            const int j = tid - BH;
+            if (L.n) {
+                h_src = L.own + kInboxN + j; h_dsrc = BW / 2;
+                h_dst = exB + (size_t)(TYN + 1) * BW + j; h_ddst = PW;
+            }
+        } else if (tid < BH + BW) {                          // south tile's top row
+            const int j = tid - BH - BW / 2;
+            if (L.s) {
+                h_src = L.own + kInboxS + BW / 2 + j; h_dsrc = -(BW / 2);
+                h_dst = exT + PW + j; h_ddst = -PW;
+            }
         }
-        if (east) {
-#pragma unroll
-            for (int q = 0; q < H; ++q)
-                if (((q + COL) & 1) == 1) ll_store(mail + (size_t)(gj0 + q) * nr + gi0 + 3, phi[q][3], tag);
-        }
-        if (south) {
-            ll_store(mail + (size_t)gj0 * nr + gi0 + pb, phi[0][pb], tag);
-            ll_store(mail + (size_t)gj0 * nr + gi0 + pb + 2, phi[0][pb + 2], tag);
-        }
-        if (north) {
-            ll_store(mail + (size_t)(gj0 + H - 1) * nr + gi0 + pt, phi[H - 1][pt], tag);
-            ll_store(mail + (size_t)(gj0 + H - 1) * nr + gi0 + pt + 2, phi[H - 1][pt + 2], tag);
-        }
-        // receive: the cells of colour COL just outside the box
-        if (east) {          // the east tile's column 0, updated in the rows with (q + COL) even
-            const uint4* col = mail + (size_t)gj0 * nr + bx + BW;
-            bool done;
-            do {
-                done = true;
-#pragma unroll
-                for (int q = 0; q < H; ++q)
-                    if (((q + COL) & 1) == 0) {
-                        const uint4 v = ll_load(col + (size_t)q * nr);
-                        if (ll_ready(v, tag)) exL[(rowbase + q) * LS + TXN + 1] = ll_value(v);
-                        else done = false;
-                    }
-            } while (!done && !poll_giveup(pc, spins, 1, (int)tag));
-        }
-        if (west) {          // the west tile's column 3, updated in the rows with (q + COL) odd
-            const uint4* col = mail + (size_t)gj0 * nr + bx - 1;
-            bool done;
-            do {
-                done = true;
-#pragma unroll
-                for (int q = 0; q < H; ++q)
-                    if (((q + COL) & 1) == 1) {
-                        const uint4 v = ll_load(col + (size_t)q * nr);
-                        if (ll_ready(v, tag)) exR[(rowbase + q) * LS + 0] = ll_value(v);
-                        else done = false;
-                    }
-            } while (!done && !poll_giveup(pc, spins, 2, (int)tag));
-        }
-        if (north) {         // the north tile's bottom row: columns of parity pb
-            const uint4* row = mail + (size_t)(gj0 + H) * nr + gi0 + pb;
-            double* dst = exB + (size_t)(TYN + 1) * BW + pb * PW + 2 * a;
-            bool done;
-            do {
-                const uint4 v0 = ll_load(row), v1 = ll_load(row + 2);
-                done = ll_ready(v0, tag) && ll_ready(v1, tag);
-                if (done) *reinterpret_cast<double2*>(dst) = make_double2(ll_value(v0), ll_value(v1));
-            } while (!done && !poll_giveup(pc, spins, 3, (int)tag));
-        }
-        if (south) {         // the south tile's top row: columns of parity pt
-            const uint4* row = mail + (size_t)(gj0 - 1) * nr + gi0 + pt;
-            double* dst = exT + pt * PW + 2 * a;
-            bool done;
-            do {
-                const uint4 v0 = ll_load(row), v1 = ll_load(row + 2);
-                done = ll_ready(v0, tag) && ll_ready(v1, tag);
-                if (done) *reinterpret_cast<double2*>(dst) = make_double2(ll_value(v0), ll_value(v1));
-            } while (!done && !poll_giveup(pc, spins, 4, (int)tag));
+        if (active) {
+            if (a == 0 && L.w) { h_scol = L.w + kInboxE + rowbase / 2; h_west = true; }
+            else if (a == TXN - 1 && L.e) { h_scol = L.e + kInboxW + rowbase / 2; }
+            if (b == 0 && L.s) { h_srow = L.s + kInboxN + 2 * a; h_south = true; }
+            else if (b == TYN - 1 && L.n) { h_srow = L.n + kInboxS + 2 * a; }
         }
     }
 
-    // ---- block mode (temporal blocking): the whole owned patch travels as tagged packets once per interval -------
-    __device__ __forceinline__ void ll_store_patch(uint4* __restrict__ mail, unsigned tag, int nr, int gi0, int gj0) const {
+    // After the half-sweep of colour COL: the owners of this box's edge cells send the values just updated ...
+    template <int COL>
+    __device__ __forceinline__ void halo_send(unsigned tag) const {
+        constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;
+        if (h_scol) {
+            if (h_west) {                    // my column 0 (rows with (q + COL) even) -> the west tile's E edge
 #pragma unroll
-        for (int q = 0; q < H; ++q) {
-            uint4* row = mail + (size_t)(gj0 + q) * nr + gi0;
+                for (int q = 0; q < H; ++q)
+                    if (((q + COL) & 1) == 0) ll_store(h_scol + (q & 1) * (BH / 2) + (q >> 1), phi[q][0], tag);
+            } else {                         // my column 3 (rows with (q + COL) odd) -> the east tile's W edge
 #pragma unroll
-            for (int c = 0; c < 4; ++c) ll_store(row + c, phi[q][c], tag);
+                for (int q = 0; q < H; ++q)
+                    if (((q + COL) & 1) == 1) ll_store(h_scol + (q & 1) * (BH / 2) + (q >> 1), phi[q][3], tag);
+            }
+        }
+        if (h_srow) {
+            if (h_south) {                   // my bottom row -> the south tile's N edge
+                ll_store(h_srow + pb * (BW / 2), phi[0][pb], tag);
+                ll_store(h_srow + pb * (BW / 2) + 1, phi[0][pb + 2], tag);
+            } else {                         // my top row -> the north tile's S edge
+                ll_store(h_srow + pt * (BW / 2), phi[H - 1][pt], tag);
+                ll_store(h_srow + pt * (BW / 2) + 1, phi[H - 1][pt + 2], tag);
+            }
         }
     }
-    __device__ __forceinline__ void ll_wait_patch(const uint4* __restrict__ mail, unsigned tag, int nr, int gi0, int gj0,
-                                                  const PollCtx& pc) {
+
+    // ... and every receiving thread fetches its ONE packet (coalesced, all four sides in flight at once) into the
+    // border slot.  The poll gives up when the context says so.
+    template <int COL>
+    __device__ __forceinline__ void halo_recv(unsigned tag, const PollCtx& pc) {
+        if (!h_src) return;
+        const uint4* src = h_src + (COL ? h_dsrc : 0);
+        double* dst = h_dst + (COL ? h_ddst : 0);
         unsigned spins = 0;
-        bool done;
-        do {
-            done = true;
-#pragma unroll
-            for (int q = 0; q < H; ++q) {
-                const uint4* row = mail + (size_t)(gj0 + q) * nr + gi0;
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const uint4 v = ll_load(row + c);
-                    if (ll_ready(v, tag)) phi[q][c] = ll_value(v);
-                    else done = false;
-                }
-            }
-        } while (!done && !poll_giveup(pc, spins, 5, (int)tag));
+        for (;;) {
+            const uint4 v = ll_load(src);
+            if (ll_ready(v, tag)) { *dst = ll_value(v); break; }
+            if (poll_giveup(pc, spins, 1, (int)tag)) break;
+        }
     }
 
     // any non-finite value in the patch (NaN/Inf never relax away)

@@ -77,8 +77,8 @@ struct sn_poisson {
     Ctl* h_ctl = nullptr;       // pinned, 2 * cap_batch (double-buffered polls)
     double *d_rho_stage = nullptr, *d_phi_stage = nullptr;   // solve_host staging
     double* d_ring = nullptr;                                // resident path: checkpoint ring, nb x kResRing x nr*nz
-    void* d_mail = nullptr;                                  // resident path: tagged packets, nb x 2 x nr*nz x 16 B
-    unsigned int* d_sync = nullptr;                          // resident path: arrived counters | grid barriers
+    void* d_mail = nullptr;                                  // resident path, halo mode: per-tile inboxes of 16-byte tagged packets
+    unsigned int* d_sync = nullptr;                          // resident path: arrived counters | grid barriers | tile flags
     size_t ring_cap = 0, mail_cap = 0, sync_cap = 0;
     long long* d_prof = nullptr;                             // resident path: optional in-kernel profile, ctas x 8
     size_t prof_cap = 0, prof_ctas = 0;
@@ -463,8 +463,8 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     const size_t ncell = (size_t)h->nr * h->nz;
     const size_t nint = (size_t)(max_sweeps + pl.Q - 1) / pl.Q;
     const size_t need_ring = (size_t)nbatch * kResRing * ncell;
-    const size_t need_mail = (size_t)nbatch * 2 * ncell;
-    const size_t need_sync = (size_t)nbatch * (2 * (nint + 2) + 1);
+    const size_t need_mail = pl.halo ? (size_t)nbatch * pl.ntiles * 2 * (S.BW() + S.BH()) : 1;      // 16-byte packets
+    const size_t need_sync = (size_t)nbatch * (2 * (nint + 2) + 1 + pl.ntiles);
     if (h->ring_cap < need_ring) {
         cudaFree(h->d_ring); h->d_ring = nullptr; h->ring_cap = 0;
         CU_TRY(cudaMalloc((void**)&h->d_ring, sizeof(double) * need_ring));
@@ -482,7 +482,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     }
     CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * need_sync, st));
     CU_TRY(cudaMemsetAsync(h->d_slots_f, 0, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
-    if (pl.ntiles > 1) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
+    if (pl.halo) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
     ResParams P;
     P.g = g;
     P.halo = pl.halo;
@@ -498,6 +498,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     P.arrived = h->d_sync;
     P.arr_stride = (int)(nint + 2);
     P.gbar = h->d_sync + (size_t)nbatch * 2 * (nint + 2);
+    P.flags = P.gbar + nbatch;
     P.ctl = h->d_ctl; P.hist = h->d_hist;
     P.prof = nullptr;
     h->prof_ctas = 0;

@@ -48,7 +48,8 @@ struct ResParams {
     const double* rho;         // [nb][ncell]
     double* phi;               // [nb][ncell]  initial guess in, result out
     double* ring;              // [nb][kResRing][ncell]  checkpoints: state after interval r in ring[r % kResRing]
-    uint4* mail;               // [nb][2][ncell]  tagged packets (halo mode uses buffer 0 only)
+    uint4* mail;               // halo mode: [nb][ntiles][2(BH+BW)] inboxes of tagged packets
+    unsigned int* flags;       // block mode: [nb][ntiles] last interval (phase tag + r) whose state the tile has published
     const double* bE;          // [nb][nz]
     const double* bN;          // [nb][nr]
     const double* bS;          // [nb][nr]
@@ -67,6 +68,9 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
     unsigned v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ void red_release_add_u32(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
@@ -115,6 +119,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     __shared__ int s_bad;
     __shared__ int s_panic;        // watchdog tripped (here or in another CTA): every wait falls through
     __shared__ int s_zero;         // a quit word that never fires (endgame / replay polls)
+    __shared__ long long s_pf[8];  // in-kernel profile of thread 0 ("prof" option)
 
     const Geom& g = p.g;
     const int member = blockIdx.y;
@@ -132,6 +137,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     if (tid == 0) {
         s_dec.seq = 0; s_dec.stop = 0; s_dec.stop_r = 0; s_dec.stop_seq = 0; s_dec.fire_k = 0; s_dec.fire_bad = 0; s_dec.R = 0.0;
         s_bad = 0; s_panic = 0; s_zero = 0;
+        for (int i = 0; i < 8; ++i) s_pf[i] = 0;
     }
     __syncthreads();
 
@@ -249,7 +255,24 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     const double* rho = p.rho + (size_t)member * ncell;
     double* phi_io = p.phi + (size_t)member * ncell;
     double* ring = p.ring + (size_t)member * kResRing * ncell;
-    uint4* mail = p.mail + (size_t)member * 2 * ncell;
+    // halo mode: inboxes of this tile and of its four neighbours
+    if (p.halo) {
+        typename Engine::HaloLinks links;
+        uint4* mb = p.mail + (size_t)member * ntiles * Engine::kInboxPackets;
+        auto inbox = [&](int t) { return mb + (size_t)t * Engine::kInboxPackets; };
+        links.own = inbox(tile);
+        links.w = (tx > 0) ? inbox(tile - 1) : nullptr;
+        links.e = (tx + 1 < p.ntx) ? inbox(tile + 1) : nullptr;
+        links.s = (ty > 0) ? inbox(tile - p.ntx) : nullptr;
+        links.n = (ty + 1 < p.nty) ? inbox(tile + p.ntx) : nullptr;
+        links.rows = min(BH, g.nz - by);
+        E.halo_bind(links, tid);
+    }
+    // block mode: the tiles whose owned cells this box overlaps (their flags gate the margin refill)
+    unsigned int* flags = p.flags + (size_t)member * ntiles;
+    const int nbx0 = bx / p.ow, nbx1 = (bx + BW - 1) / p.ow;
+    const int nby0 = by / p.oh, nby1 = min(p.nty - 1, (by + BH - 1) / p.oh);
+    const int nnb = (nbx1 - nbx0 + 1) * (nby1 - nby0 + 1);
     const double* bE = p.bE + (size_t)member * g.nz;
     const double* bN = p.bN + (size_t)member * g.nr;
     const double* bS = p.bS + (size_t)member * g.nr;
@@ -293,7 +316,6 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     // optional in-kernel profile (thread 0 of the CTA): 0 total, 1 half-sweep compute, 2 halo exchange, 3 barrier,
     // 4 end of interval, 5 margin refill, 6 wait for the decision, 7 half-sweeps
     const bool prof_on = p.prof != nullptr && tid == 0;
-    long long pf[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     auto tick = [&]() -> long long { return prof_on ? clock64() : 0ll; };
     const long long t_begin = tick();
     unsigned gbar_gen = 0;
@@ -329,17 +351,28 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             const long long t0 = tick();
             E.template half_sweep<0, TRACK, false>();
             const long long t1 = tick();
-            if (p.halo) E.template halo_exchange<0>(mail, tagbase + 2u * (unsigned)(k0 + s) + 1u, g.nr, g.nz, bx, by, pc);
+            if (p.halo) {
+                const unsigned tag = tagbase + 2u * (unsigned)(k0 + s) + 1u;
+                E.template halo_send<0>(tag);
+                E.template halo_recv<0>(tag, pc);
+            }
             const long long t2 = tick();
             Engine::sync();
             const long long t3 = tick();
             E.template half_sweep<1, TRACK, false>();
             const long long t4 = tick();
-            if (p.halo) E.template halo_exchange<1>(mail, tagbase + 2u * (unsigned)(k0 + s) + 2u, g.nr, g.nz, bx, by, pc);
+            if (p.halo) {
+                const unsigned tag = tagbase + 2u * (unsigned)(k0 + s) + 2u;
+                E.template halo_send<1>(tag);
+                E.template halo_recv<1>(tag, pc);
+            }
             const long long t5 = tick();
             Engine::sync();
             const long long t6 = tick();
-            pf[1] += (t1 - t0) + (t4 - t3); pf[2] += (t2 - t1) + (t5 - t4); pf[3] += (t3 - t2) + (t6 - t5); pf[7] += 2;
+            if (prof_on) {
+                s_pf[1] += (t1 - t0) + (t4 - t3); s_pf[2] += (t2 - t1) + (t5 - t4); s_pf[3] += (t3 - t2) + (t6 - t5);
+                s_pf[7] += 2;
+            }
             if (TRACK == kTrackFast) {
                 const unsigned wr = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres_f) : 0u);
                 const unsigned wp = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mphi_f) : 0u);
@@ -362,8 +395,6 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     // number.  The margins are NOT yet valid in block mode when this returns (see finish_exchange).
     auto end_interval = [&](int r, int k0, int n, int exact, unsigned tagbase) -> int {
         if (own) E.store_patch(state_of(r), g.nr, gi0, gj0);
-        uint4* mb = mail + (size_t)(r & 1) * ncell;
-        if (!p.halo && own && ntiles > 1) E.ll_store_patch(mb, tagbase + (unsigned)r, g.nr, gi0, gj0);
         // FAST maxima drop NaN (FMNMX); any non-finite owned value persists (NaN/Inf never relax away), so one
         // check per interval is enough to poison its maxima and send the solve to the exact endgame
         if (!exact && own && E.any_nonfinite()) s_bad = 1;
@@ -377,13 +408,27 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         }
         __threadfence_block();
         report_arrive(par);
+        // block mode: publish "state r of this tile is in the ring" (the barrier above ordered every thread's stores
+        // before this thread's fence)
+        if (!p.halo && ntiles > 1 && tid == 0) {
+            st_release_u32(flags + tile, tagbase + (unsigned)r);
+        }
         return seq;
     };
     // block mode: refill the margins from the neighbours' tiles of interval r and republish the patch edges
     auto finish_exchange = [&](int r, unsigned tagbase, const PollCtx& pc) {
         if (p.halo || ntiles == 1) return;
-        const uint4* mb = mail + (size_t)(r & 1) * ncell;
-        if (!own) E.ll_wait_patch(mb, tagbase + (unsigned)r, g.nr, gi0, gj0, pc);
+        if (warp == NW - 1) {
+            const unsigned want = tagbase + (unsigned)r;
+            for (int i = lane; i < nnb; i += 32) {
+                const int t = (nby0 + i / (nbx1 - nbx0 + 1)) * p.ntx + nbx0 + i % (nbx1 - nbx0 + 1);
+                if (t == tile) continue;
+                unsigned spins = 0;
+                while (ld_acquire_u32(flags + t) < want && !poll_giveup(pc, spins, 5, (int)want)) {}
+            }
+        }
+        Engine::sync();
+        if (!own) E.load_patch(state_of(r), g.nr, gi0, gj0);
         E.publish_all();
         Engine::sync();
     };
@@ -407,7 +452,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             finish_exchange(r, 0u, pc_main);
             const long long tc = tick();
             wait_decided(sq - 1);
-            pf[4] += tb - ta; pf[5] += tc - tb; pf[6] += tick() - tc;
+            if (prof_on) { s_pf[4] += tb - ta; s_pf[5] += tc - tb; s_pf[6] += tick() - tc; }
             // a stop decided by report sq (being processed right now) must not be seen by some threads only
             const bool stopped_now = *stop && s_dec.stop_seq <= sq - 1;
             if (uniform_or(stopped_now || panicked())) break;
@@ -474,9 +519,9 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     __threadfence_block();
     report_arrive(seq & 1);
     if (prof_on) {
-        pf[0] = clock64() - t_begin;
+        s_pf[0] = clock64() - t_begin;
         long long* dst = p.prof + ((size_t)member * ntiles + tile) * 8;
-        for (int i = 0; i < 8; ++i) dst[i] = pf[i];
+        for (int i = 0; i < 8; ++i) dst[i] = s_pf[i];
     }
     if (tile == 0 && tid == 0) {
         ctl->sweeps = sweeps;
