@@ -111,8 +111,9 @@ struct BoxEngine {
                                 // such a thread never updates and keeps publishing the north ghosts as its bottom row
     double phi[H][4];
     double cEr[4], cWr[4];
-    double iz2, D, wD;          // interior rows
-    double cS0, diag0, w0;      // row q = 0 of this patch (differs on the reflecting equator)
+    double iz2, D, wD;          // interior rows (uniform: the compiler keeps them in the constant bank / uniform registers)
+    double D0, wD0;             // reflecting-equator row (uniform)
+    bool mirror0;               // row q = 0 of this patch is the reflecting equator row
     // running maxima of the current sweep
     unsigned long long mres_k, mphi_k;     // exact keys
     float mres_f, mphi_f;                  // fast: |upper word| compared as fp32 (same order for finite values)
@@ -139,11 +140,8 @@ struct BoxEngine {
             cEr[c] = g.cE[gi0 + c];
             cWr[c] = g.cW[gi0 + c];
         }
-        iz2 = g.iz2; D = g.D; wD = g.wD;
-        const bool mirror0 = (g.symmetry == 1 && gj0 == 0);
-        cS0 = mirror0 ? 0.0 : g.iz2;
-        diag0 = mirror0 ? g.D0 : g.D;
-        w0 = mirror0 ? g.wD0 : g.wD;
+        iz2 = g.iz2; D = g.D; wD = g.wD; D0 = g.D0; wD0 = g.wD0;
+        mirror0 = (g.symmetry == 1 && gj0 == 0);
     }
 
     // f = 4 pi rho of this thread's patch into shared memory (rho row pitch nr, 16-byte aligned rows)
@@ -229,25 +227,49 @@ struct BoxEngine {
     // One half-sweep of colour COL over the patch, then publish the updated edge cells and (SYNC) the barrier.
     template <int COL, int TRACK, bool SYNC = true>
     __device__ __forceinline__ void half_sweep() {
-        if (active) half_sweep_body<COL, TRACK>();
+        if (active) {
+            update_cells<COL, TRACK, 0>();
+            publish_colour<COL>();
+        }
         if (SYNC) sync();
     }
+    // Halo mode: the cells a neighbouring TILE may need (first and last patch row, first / last patch column) are
+    // updated first and sent at once, so that the packets travel while the rest of the patch is updated.  The order
+    // of a colour's updates is free (they are mutually independent, R10).  No barrier here.
     template <int COL, int TRACK>
-    __device__ __forceinline__ void half_sweep_body() {
+    __device__ __forceinline__ void half_sweep_halo(unsigned tag) {
+        if (!active) return;
+        update_cells<COL, TRACK, 1>();
+        halo_send<COL>(tag);
+        update_cells<COL, TRACK, 2>();
+        publish_colour<COL>();
+    }
+    // WHICH: 0 all cells of colour COL, 1 only the patch-edge cells (rows 0 and H-1, column 0 / 3), 2 the others
+    template <int COL, int TRACK, int WHICH>
+    __device__ __forceinline__ void update_cells() {
         // vertical outer neighbours of the bottom (q=0) and top (q=H-1) rows: other-colour cells of the rows outside
         constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;                 // column parity updated in those rows
-        const double2 So = *reinterpret_cast<const double2*>(exT + (size_t)b * BW + pb * PW + 2 * a);
-        const double2 No = *reinterpret_cast<const double2*>(exB + (size_t)(b + 2) * BW + pt * PW + 2 * a);
+        double2 So = make_double2(0.0, 0.0), No = make_double2(0.0, 0.0);
+        if (WHICH != 2) {
+            So = *reinterpret_cast<const double2*>(exT + (size_t)b * BW + pb * PW + 2 * a);
+            No = *reinterpret_cast<const double2*>(exB + (size_t)(b + 2) * BW + pt * PW + 2 * a);
+        }
 #pragma unroll
         for (int q = 0; q < H; ++q) {
             const int pq = (q + COL) & 1;                                   // compile-time after unrolling
-            const double outer = pq == 0 ? exR[(rowbase + q) * LS + a] : exL[(rowbase + q) * LS + a + 2];
+            const bool edge_row = q == 0 || q == H - 1;
+            const bool any0 = WHICH == 0 || (WHICH == 1 ? (edge_row || pq == 0) : (!edge_row && pq != 0));   // cc = 0
+            const bool any1 = WHICH == 0 || (WHICH == 1 ? (edge_row || pq == 1) : (!edge_row && pq != 1));   // cc = 1
+            if (!any0 && !any1) continue;
+            const bool need_outer = (pq == 0 && any0) || (pq == 1 && any1);
+            const double outer = !need_outer ? 0.0 : pq == 0 ? exR[(rowbase + q) * LS + a] : exL[(rowbase + q) * LS + a + 2];
             const double2 fv = *reinterpret_cast<const double2*>(fs + (size_t)(rowbase + q) * BW + pq * PW + 2 * a);
-            const double cS = q == 0 ? cS0 : iz2;
-            const double dg = q == 0 ? diag0 : D;
-            const double ww = q == 0 ? w0 : wD;
+            const double cS = (q == 0 && mirror0) ? 0.0 : iz2;
+            const double dg = (q == 0 && mirror0) ? D0 : D;
+            const double ww = (q == 0 && mirror0) ? wD0 : wD;
 #pragma unroll
             for (int cc = 0; cc < 2; ++cc) {
+                if (!(cc == 0 ? any0 : any1)) continue;
                 const int c = pq + 2 * cc;
                 const double pW = c == 0 ? outer : phi[q][c == 0 ? 0 : c - 1];
                 const double pE = c == 3 ? outer : phi[q][c == 3 ? 3 : c + 1];
@@ -260,7 +282,11 @@ struct BoxEngine {
                 track<TRACK>(res, pn);
             }
         }
-        // publish the updated edge cells of this colour
+    }
+    // publish the updated patch-edge cells of colour COL to the exchange arrays of the CTA
+    template <int COL>
+    __device__ __forceinline__ void publish_colour() {
+        constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;
 #pragma unroll
         for (int q = 0; q < H; ++q) {
             const int pq = (q + COL) & 1;
@@ -325,7 +351,7 @@ struct BoxEngine {
     // in the neighbour's inbox (a thread sits on at most one column edge and one row edge: TXN, TYN >= 2).
     const uint4* h_src = nullptr;
     double* h_dst = nullptr;
-    int h_dsrc = 0, h_ddst = 0;
+    int h_edge = 0;                  // 0 E, 1 W, 2 N, 3 S: fixes the two deltas
     uint4* h_scol = nullptr;         // column edge: west (h_west) or east
     uint4* h_srow = nullptr;         // row edge: south (h_south) or north
     bool h_west = false, h_south = false;
@@ -335,26 +361,26 @@ struct BoxEngine {
         if (tid < BH / 2) {                                  // east tile's column 0
             const int j = tid;
             if (L.e && 2 * j < L.rows) {
-                h_src = L.own + kInboxE + j; h_dsrc = BH / 2;
-                h_dst = exL + 2 * j * LS + TXN + 1; h_ddst = LS;
+                h_src = L.own + kInboxE + j; h_edge = 0;
+                h_dst = exL + 2 * j * LS + TXN + 1;
             }
         } else if (tid < BH) {                               // west tile's column 3
             const int j = tid - BH / 2;
             if (L.w && 2 * j < L.rows) {
-                h_src = L.own + kInboxW + BH / 2 + j; h_dsrc = -(BH / 2);
-                h_dst = exR + (2 * j + 1) * LS; h_ddst = -LS;
+                h_src = L.own + kInboxW + BH / 2 + j; h_edge = 1;
+                h_dst = exR + (2 * j + 1) * LS;
             }
         } else if (tid < BH + BW / 2) {                      // north tile's bottom row
             const int j = tid - BH;
             if (L.n) {
-                h_src = L.own + kInboxN + j; h_dsrc = BW / 2;
-                h_dst = exB + (size_t)(TYN + 1) * BW + j; h_ddst = PW;
+                h_src = L.own + kInboxN + j; h_edge = 2;
+                h_dst = exB + (size_t)(TYN + 1) * BW + j;
             }
         } else if (tid < BH + BW) {                          // south tile's top row
             const int j = tid - BH - BW / 2;
             if (L.s) {
-                h_src = L.own + kInboxS + BW / 2 + j; h_dsrc = -(BW / 2);
-                h_dst = exT + PW + j; h_ddst = -PW;
+                h_src = L.own + kInboxS + BW / 2 + j; h_edge = 3;
+                h_dst = exT + PW + j;
             }
         }
         if (active) {
@@ -396,14 +422,49 @@ struct BoxEngine {
     template <int COL>
     __device__ __forceinline__ void halo_recv(unsigned tag, const PollCtx& pc) {
         if (!h_src) return;
-        const uint4* src = h_src + (COL ? h_dsrc : 0);
-        double* dst = h_dst + (COL ? h_ddst : 0);
+        const uint4* src = h_src;
+        double* dst = h_dst;
+        if (COL) {                           // deltas of the colour-1 slot / border element (see halo_bind)
+            const int dsrc = h_edge == 0 ? BH / 2 : h_edge == 1 ? -(BH / 2) : h_edge == 2 ? BW / 2 : -(BW / 2);
+            const int ddst = h_edge == 0 ? LS : h_edge == 1 ? -LS : h_edge == 2 ? PW : -PW;
+            src += dsrc;
+            dst += ddst;
+        }
         unsigned spins = 0;
         for (;;) {
             const uint4 v = ll_load(src);
             if (ll_ready(v, tag)) { *dst = ll_value(v); break; }
             if (poll_giveup(pc, spins, 1, (int)tag)) break;
         }
+    }
+
+    // ---- block mode, small tiles: the whole owned patch travels as tagged packets once per interval ---------------
+    // (two buffers by interval parity: an owner writes interval r + 2 only after every neighbour has consumed r)
+    __device__ __forceinline__ void ll_store_patch(uint4* __restrict__ mail, unsigned tag, int nr, int gi0, int gj0) const {
+#pragma unroll
+        for (int q = 0; q < H; ++q) {
+            uint4* row = mail + (size_t)(gj0 + q) * nr + gi0;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) ll_store(row + c, phi[q][c], tag);
+        }
+    }
+    __device__ __forceinline__ void ll_wait_patch(const uint4* __restrict__ mail, unsigned tag, int nr, int gi0, int gj0,
+                                                  const PollCtx& pc) {
+        unsigned spins = 0;
+        bool done;
+        do {
+            done = true;
+#pragma unroll
+            for (int q = 0; q < H; ++q) {
+                const uint4* row = mail + (size_t)(gj0 + q) * nr + gi0;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const uint4 v = ll_load(row + c);
+                    if (ll_ready(v, tag)) phi[q][c] = ll_value(v);
+                    else done = false;
+                }
+            }
+        } while (!done && !poll_giveup(pc, spins, 5, (int)tag));
     }
 
     // any non-finite value in the patch (NaN/Inf never relax away)

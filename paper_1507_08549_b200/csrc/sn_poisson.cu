@@ -62,7 +62,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -362,27 +362,29 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
 struct ShapeInfo {
     int H, TXN, TYN, minb;
     size_t smem;
-    const void* fn;
+    const void* fn[2];          // [0] block mode, [1] halo mode
     int BW() const { return 4 * TXN; }
     int BH() const { return H * TYN; }
     int NT() const { return TXN * TYN; }
     int threads() const { return TXN * TYN + 32; }     // + the service warp
 };
 
-template <int H, int TXN, int TYN, int MINB>
+template <int H, int TXN, int TYN, int MINB, bool EF = true>
 ShapeInfo shape_of() {
-    return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes, (const void*)k_sor_resident<H, TXN, TYN, MINB>};
+    return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes,
+            {(const void*)k_sor_resident<H, TXN, TYN, MINB, false, false>,
+             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, EF>}};
 }
 
 const std::vector<ShapeInfo>& shapes() {
     static const std::vector<ShapeInfo> v = {
-        shape_of<8, 32, 14, 1>(),   // 0: box 128 x 112, 448 threads
+        shape_of<8, 32, 14, 1, false>(),   // 0: box 128 x 112, 448 threads (128-register cap: no edge-first)
         shape_of<8, 32, 8, 1>(),    // 1: box 128 x 64,  256 threads
         shape_of<8, 16, 8, 2>(),    // 2: box 64 x 64,   128 threads
         shape_of<4, 16, 8, 2>(),    // 3: box 64 x 32,   128 threads
         shape_of<4, 8, 8, 2>(),     // 4: box 32 x 32,    64 threads
         shape_of<2, 8, 16, 2>(),    // 5: box 32 x 32,   128 threads
-        shape_of<8, 32, 7, 2>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
+        shape_of<8, 32, 7, 2, false>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
         shape_of<4, 16, 16, 1>(),   // 7: box 64 x 64,   256 threads
         shape_of<6, 12, 8, 2>(),    // 8: box 48 x 48,    96 threads
         shape_of<4, 12, 16, 1>(),   // 9: box 48 x 64,   192 threads
@@ -391,16 +393,22 @@ const std::vector<ShapeInfo>& shapes() {
 }
 
 struct ResPlan {
-    int shape = -1, halo = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
+    int shape = -1, halo = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
     double cost = 0;
 };
 
-// Modelled SM clocks of one half-sweep of a box when `k` CTAs of that shape share an SM: the fp64 pipe issues one
-// warp instruction per 2 clocks per SM sub-partition, 7 per cell update; measured efficiency ~0.55 plus a fixed
-// exchange / barrier latency per half-sweep.
+// Modelled SM clocks of one half-sweep of a box when `k` CTAs of that shape share an SM, calibrated with the
+// in-kernel profile ("prof" option; profiles/r01c_resident_inkernel.md): a warp needs `lat` clocks for its 2H cell
+// updates (7 dependent fp64 instructions each, little ILP left once 4 x H values of phi live in registers), and the
+// fp64 pipe issues one warp instruction per 2 clocks per SM sub-partition at ~62 % efficiency.
 double model_half_sweep(const ShapeInfo& S, int k) {
+    const double dpw = 2.0 * S.H * 7.0;                          // fp64 instructions per warp and half-sweep
+    const double lat = S.H <= 2 ? 215.0 : S.H <= 4 ? 420.0 : S.H <= 6 ? 480.0 : 545.0;
     const double warps_per_smsp = std::ceil(k * (S.NT() / 32.0) / 4.0);
-    return warps_per_smsp * (2.0 * S.H) * 7.0 * 2.0 / 0.55 + 130.0;
+    // CTAs sharing an SM also share its latency-bound phases (measured: ~ +50 % per extra CTA)
+    double t = std::max(lat * (1.0 + 0.5 * (k - 1)), warps_per_smsp * dpw * 2.0 / 0.62 + 100.0);
+    if (S.threads() * S.minb > 448 && k == 1 && S.H == 8 && S.NT() < 448) t = std::max(t, 1400.0);   // 128-register cap
+    return t;
 }
 
 // Pick (shape, mode, m) minimising modelled clocks per sweep; honours the "shape" / "tblock" / "halo" overrides.
@@ -411,13 +419,16 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
     for (int si = 0; si < (int)sh.size(); ++si) {
         if (h->opt_shape >= 0 && si != h->opt_shape) continue;
         const ShapeInfo& S = sh[si];
-        int occ = 0;
-        if (cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn, S.threads(), S.smem) != cudaSuccess || occ < 1) {
-            cudaGetLastError();
-            continue;
+        long long max_ctas_mode[2] = {0, 0};
+        for (int md = 0; md < 2; ++md) {
+            int occ = 0;
+            if (cudaFuncSetAttribute(S.fn[md], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn[md], S.threads(), S.smem) != cudaSuccess) {
+                cudaGetLastError();
+                occ = 0;
+            }
+            max_ctas_mode[md] = (long long)occ * h->num_sms;
         }
-        const long long max_ctas = (long long)occ * h->num_sms;
         // halo mode: box == tile on a regular lattice, ragged last tile row allowed
         if (h->opt_halo != 0 && h->nr % S.BW() == 0 && h->nz % S.H == 0) {
             ResPlan p;
@@ -425,12 +436,13 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
             p.ntx = h->nr / S.BW(); p.nty = (h->nz + S.BH() - 1) / S.BH();
             p.ow = S.BW(); p.oh = S.BH();
             p.ntiles = p.ntx * p.nty;
-            p.Q = h->opt_tblock > 0 ? h->opt_tblock : 8;
+            p.Q = h->opt_tblock > 0 ? h->opt_tblock : kMaxTB;
             p.m = p.Q;
-            if ((long long)p.ntiles * nbatch <= max_ctas && (p.ntiles > 1 || h->opt_halo == 1)) {
+            if ((long long)p.ntiles * nbatch <= max_ctas_mode[1] && (p.ntiles > 1 || h->opt_halo == 1)) {
                 const int k = (int)((p.ntiles * (long long)nbatch + h->num_sms - 1) / h->num_sms);
-                const double t1 = model_half_sweep(S, 1), tk = model_half_sweep(S, k);
-                p.cost = 2.0 * std::max(tk, t1 + 1300.0);
+                // per half-sweep: compute + the exposed part of the edge exchange (poll round trips, barrier, the
+                // neighbour's slowest warp) + the checkpoint / report of the interval
+                p.cost = 2.0 * (model_half_sweep(S, k) + 1500.0 + 0.1 * S.BW() * S.BH());
                 if (best.shape < 0 || p.cost < best.cost) best = p;
             }
         }
@@ -442,15 +454,17 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
             if (!plan_axis(h->nr, S.BW(), 2 * m, 4, &p.ntx, &p.ow)) continue;
             if (!plan_axis(h->nz, S.BH(), 2 * m, S.H, &p.nty, &p.oh)) continue;
             p.ntiles = p.ntx * p.nty;
-            if ((long long)p.ntiles * nbatch > max_ctas) continue;
+            if ((long long)p.ntiles * nbatch > max_ctas_mode[0]) continue;
             bool ok = true;                      // the property the kernel relies on, checked for every tile
             for (int t = 0; t < p.ntx && ok; ++t) ok = box_covers(t, p.ow, 2 * m, 4, S.BW(), h->nr);
             for (int t = 0; t < p.nty && ok; ++t) ok = box_covers(t, p.oh, 2 * m, S.H, S.BH(), h->nz);
             if (!ok) continue;
             p.shape = si; p.halo = 0; p.m = m; p.Q = m;
+            p.ll = h->opt_ll >= 0 ? h->opt_ll : (S.H == 2 && p.ow * p.oh <= 256 ? 1 : 0);   // tiny tiles: packets beat flags
             const int k = (int)((p.ntiles * (long long)nbatch + h->num_sms - 1) / h->num_sms);
-            const double exchange = p.ntiles > 1 ? 1600.0 + 16.0 * S.BW() * S.BH() / 32.0 : 300.0;
-            p.cost = 2.0 * model_half_sweep(S, k) + (k * exchange) / m;
+            // per exchange: checkpoint store, release of the tile flag, the neighbours' acquire, margin refill
+            const double exchange = p.ntiles == 1 ? 2000.0 : p.ll ? 3800.0 : 4200.0 + 0.7 * S.BW() * S.BH();
+            p.cost = 2.0 * model_half_sweep(S, k) + exchange * (1.0 + 0.5 * (k - 1)) / m;
             if (best.shape < 0 || p.cost < best.cost) best = p;
         }
     }
@@ -463,7 +477,8 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     const size_t ncell = (size_t)h->nr * h->nz;
     const size_t nint = (size_t)(max_sweeps + pl.Q - 1) / pl.Q;
     const size_t need_ring = (size_t)nbatch * kResRing * ncell;
-    const size_t need_mail = pl.halo ? (size_t)nbatch * pl.ntiles * 2 * (S.BW() + S.BH()) : 1;      // 16-byte packets
+    const size_t need_mail = pl.halo ? (size_t)nbatch * pl.ntiles * 2 * (S.BW() + S.BH())
+                                     : pl.ll ? (size_t)nbatch * 2 * ncell : 1;                       // 16-byte packets
     const size_t need_sync = (size_t)nbatch * (2 * (nint + 2) + 1 + pl.ntiles);
     if (h->ring_cap < need_ring) {
         cudaFree(h->d_ring); h->d_ring = nullptr; h->ring_cap = 0;
@@ -482,10 +497,11 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     }
     CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * need_sync, st));
     CU_TRY(cudaMemsetAsync(h->d_slots_f, 0, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
-    if (pl.halo) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
+    if (pl.halo || pl.ll) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
     ResParams P;
     P.g = g;
     P.halo = pl.halo;
+    P.ll = pl.ll;
     P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.Q = pl.Q;
     P.max_sweeps = max_sweeps;
     P.force_exact = h->opt_exact;
@@ -514,8 +530,9 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         h->prof_ctas = (size_t)pl.ntiles * nbatch;
     }
     void* args[] = {&P};
-    CU_TRY(cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
-    CU_TRY(cudaLaunchCooperativeKernel(S.fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, S.smem, st));
+    const void* fn = S.fn[pl.halo ? 1 : 0];
+    CU_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
+    CU_TRY(cudaLaunchCooperativeKernel(fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, S.smem, st));
     h->st_launches += 1;
     h->st_path = 2;
     h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.Q;
@@ -799,6 +816,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
     if (!strcmp(key, "prof")) { h->opt_prof = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "ll")) { if (value < -1 || value > 1) { set_err("ll must be -1, 0 or 1"); return -1; } h->opt_ll = (int)value; return 0; }
     if (!strcmp(key, "halo")) { if (value < -1 || value > 1) { set_err("halo must be -1, 0 or 1"); return -1; } h->opt_halo = (int)value; return 0; }
     if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)std::max(shapes().size(), blk_shapes().size())) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
     if (!strcmp(key, "tblock")) { if (value < 0 || value > kMaxTB) { set_err("tblock must be 0..%d", kMaxTB); return -1; } h->opt_tblock = (int)value; return 0; }

@@ -38,7 +38,8 @@ constexpr unsigned kTagEndgame = 1u << 28, kTagReplay = 2u << 28;
 
 struct ResParams {
     Geom g;
-    int halo;                  // 1: halo mode, 0: block mode
+    int halo;                  // 1: halo mode, 0: block mode (the kernel's HALO template argument)
+    int ll;                    // block mode: 1 = margins travel as tagged packets (small tiles), 0 = tile flags + ring loads
     int ntx, nty;              // tiles in r and z
     int ow, oh;                // nominal owned tile size (halo mode: the box size)
     int m;                     // block mode: sweeps per exchange (== Q)
@@ -48,7 +49,7 @@ struct ResParams {
     const double* rho;         // [nb][ncell]
     double* phi;               // [nb][ncell]  initial guess in, result out
     double* ring;              // [nb][kResRing][ncell]  checkpoints: state after interval r in ring[r % kResRing]
-    uint4* mail;               // halo mode: [nb][ntiles][2(BH+BW)] inboxes of tagged packets
+    uint4* mail;               // halo mode: [nb][ntiles][2(BH+BW)] inboxes of tagged packets; block mode with ll: [nb][2][ncell]
     unsigned int* flags;       // block mode: [nb][ntiles] last interval (phase tag + r) whose state the tile has published
     const double* bE;          // [nb][nz]
     const double* bN;          // [nb][nr]
@@ -106,7 +107,8 @@ struct ResShape {
 };
 
 // grid = (ntx*nty, nbatch), block = TXN*TYN + 32 threads (the last warp is the service warp), cooperative launch.
-template <int H, int TXN, int TYN, int MINB>
+// EF (halo mode): update and send the patch-edge cells first (half_sweep_halo); only where registers allow it.
+template <int H, int TXN, int TYN, int MINB, bool HALO, bool EF>
 __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResParams p) {
     using S = BoxShape<H, TXN, TYN>;
     using RS = ResShape<H, TXN, TYN>;
@@ -238,7 +240,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
 
     const int tx = tile % p.ntx, ty = tile / p.ntx;
     int x0, x1, y0, y1, bx, by;
-    if (p.halo) {
+    if (HALO) {
         x0 = bx = tx * BW; x1 = x0 + BW;
         y0 = by = ty * BH; y1 = min(g.nz, y0 + BH);
     } else {
@@ -256,7 +258,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     double* phi_io = p.phi + (size_t)member * ncell;
     double* ring = p.ring + (size_t)member * kResRing * ncell;
     // halo mode: inboxes of this tile and of its four neighbours
-    if (p.halo) {
+    if (HALO) {
         typename Engine::HaloLinks links;
         uint4* mb = p.mail + (size_t)member * ntiles * Engine::kInboxPackets;
         auto inbox = [&](int t) { return mb + (size_t)t * Engine::kInboxPackets; };
@@ -296,7 +298,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         }
         E.set_borders(g, bx, by, bE, bN, bS, tid, NT);
         Engine::sync();                                          // borders first: halo loads overwrite some of them
-        if (p.halo) E.load_halo_borders(src, g.nr, g.nz, bx, by);
+        if (HALO) E.load_halo_borders(src, g.nr, g.nz, bx, by);
         E.publish_all();
         Engine::sync();
     };
@@ -349,23 +351,26 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         for (int s = 0; s < n; ++s) {
             E.reset_maxima();
             const long long t0 = tick();
-            E.template half_sweep<0, TRACK, false>();
-            const long long t1 = tick();
-            if (p.halo) {
-                const unsigned tag = tagbase + 2u * (unsigned)(k0 + s) + 1u;
-                E.template halo_send<0>(tag);
-                E.template halo_recv<0>(tag, pc);
+            const unsigned tag0 = tagbase + 2u * (unsigned)(k0 + s) + 1u;
+            if (HALO && EF) {
+                E.template half_sweep_halo<0, TRACK>(tag0);
+            } else {
+                E.template half_sweep<0, TRACK, false>();
+                if (HALO) E.template halo_send<0>(tag0);
             }
+            const long long t1 = tick();
+            if (HALO) E.template halo_recv<0>(tag0, pc);
             const long long t2 = tick();
             Engine::sync();
             const long long t3 = tick();
-            E.template half_sweep<1, TRACK, false>();
-            const long long t4 = tick();
-            if (p.halo) {
-                const unsigned tag = tagbase + 2u * (unsigned)(k0 + s) + 2u;
-                E.template halo_send<1>(tag);
-                E.template halo_recv<1>(tag, pc);
+            if (HALO && EF) {
+                E.template half_sweep_halo<1, TRACK>(tag0 + 1u);
+            } else {
+                E.template half_sweep<1, TRACK, false>();
+                if (HALO) E.template halo_send<1>(tag0 + 1u);
             }
+            const long long t4 = tick();
+            if (HALO) E.template halo_recv<1>(tag0 + 1u, pc);
             const long long t5 = tick();
             Engine::sync();
             const long long t6 = tick();
@@ -410,14 +415,24 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         report_arrive(par);
         // block mode: publish "state r of this tile is in the ring" (the barrier above ordered every thread's stores
         // before this thread's fence)
-        if (!p.halo && ntiles > 1 && tid == 0) {
-            st_release_u32(flags + tile, tagbase + (unsigned)r);
+        if (!HALO && ntiles > 1) {
+            if (p.ll) {
+                if (own) E.ll_store_patch(p.mail + ((size_t)member * 2 + (r & 1)) * ncell, tagbase + (unsigned)r, g.nr, gi0, gj0);
+            } else if (tid == 0) {
+                st_release_u32(flags + tile, tagbase + (unsigned)r);
+            }
         }
         return seq;
     };
     // block mode: refill the margins from the neighbours' tiles of interval r and republish the patch edges
     auto finish_exchange = [&](int r, unsigned tagbase, const PollCtx& pc) {
-        if (p.halo || ntiles == 1) return;
+        if (HALO || ntiles == 1) return;
+        if (p.ll) {
+            if (!own) E.ll_wait_patch(p.mail + ((size_t)member * 2 + (r & 1)) * ncell, tagbase + (unsigned)r, g.nr, gi0, gj0, pc);
+            E.publish_all();
+            Engine::sync();
+            return;
+        }
         if (warp == NW - 1) {
             const unsigned want = tagbase + (unsigned)r;
             for (int i = lane; i < nnb; i += 32) {
