@@ -40,7 +40,8 @@ typedef struct sn_poisson sn_poisson; /* opaque handle; owns all device workspac
  *   sweeps   : full sweeps (red half-sweep + black half-sweep) applied to the returned phi
  *   status   : 0 converged (tol > 0) or fixed-sweep run completed (tol <= 0);
  *              1 hit max_sweeps without reaching tol (not an error);
- *             -1 bad argument / NULL (phi untouched); -2 CUDA error; -3 non-finite residual
+ *             -1 bad argument / NULL (phi untouched); -2 CUDA error, or the resident kernel's watchdog tripped (a
+ *                wait on another CTA exceeded its budget; phi unspecified); -3 non-finite residual
  *   residual : R_k of the last applied sweep k,
  *              R_k = max|res| / (max|4 pi rho| + (2/dr^2+2/dz^2) max|phi_new|)   (R9)            */
 typedef struct {
@@ -92,7 +93,10 @@ double sn_poisson_get_omega(const sn_poisson* h);
  * set_boundary: inject ghost values bE[nz], bN[nr], bS[nr] (bS ignored when symmetry = 1) and skip the moment and
  *               boundary kernels in later solves; (NULL, NULL, NULL) restores the multipole boundary.
  * get_boundary: the ghost arrays used by batch member 0 of the last solve.
- * get_history : R_k for k = 1..min(n, sweeps) of batch member 0 of the last solve; returns the count copied. */
+ * get_history : R_k for k = 1..min(n, sweeps) of batch member 0 of the last solve; returns the count copied.
+ *               Paths 2 / 3 without the "exact" option track only the upper 32 bits of the maxima until the rule
+ *               may have fired: entries before the last (exactly tracked) interval are lower bounds within 2^-19
+ *               of R_k; the returned `residual` and the last entry are always exact. */
 int sn_poisson_get_moments(sn_poisson* h, double* M);
 int sn_poisson_set_boundary(sn_poisson* h, const double* bE, const double* bN, const double* bS);
 int sn_poisson_get_boundary(sn_poisson* h, double* bE, double* bN, double* bS);
@@ -100,17 +104,24 @@ int sn_poisson_get_history(sn_poisson* h, double* R, int n);
 
 /* Tuning knobs; unknown keys return -1.
  *   "path"        0 auto, 1 streaming kernels (one launch per colour), 2 resident persistent cooperative kernel
- *                 (phi on chip for the whole solve; single solve whose tiles are all co-resident), 3 blocked kernel
+ *                 (phi on chip for the whole solve; every tile of every batch member co-resident), 3 blocked kernel
  *                 (one launch per m sweeps; any size, batches)
  *   "chunk"       launches enqueued between host polls of the device-side decision (paths 1 and 3)
- *   "tblock"      sweeps per halo exchange / per launch (temporal blocking depth m); 0 = planner's choice
+ *   "tblock"      path 2 block mode / path 3: sweeps per halo exchange / per launch (temporal blocking depth m);
+ *                 path 2 halo mode: sweeps per report / checkpoint interval; 0 = planner's choice
  *   "shape"       box shape index of path 2 / 3; -1 = planner's choice
- *   "exact"       1: path 3 tracks the per-sweep maxima exactly in every launch (exact R_k history)         */
+ *   "halo"        path 2: 1 = halo mode (box == tile, edge exchange every half-sweep), 0 = block mode (margins of
+ *                 2m cells, exchange every m sweeps), -1 = planner's choice
+ *   "ll"          path 2 block mode: 1 = margins travel as tagged packets, 0 = tile flags + ring loads, -1 = auto
+ *   "exact"       1: paths 2 / 3 track the per-sweep maxima exactly in every interval / launch (exact R_k history)
+ *   "prof"        1: path 2 records an in-kernel SM-clock profile (stats "prof_mean0..7", "prof_max0..7": total,
+ *                 half-sweep compute, halo exchange, barrier, end of interval, margin refill, wait for the
+ *                 decision, half-sweeps; mean / max over the CTAs, thread 0 of each)                         */
 int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value);
 
 /* Counters of the last solve / batch: "launches" (kernels launched), "sweep_launches" (those that ran relaxation
  * sweeps), "sweep_ms" (device time of the relaxation phase, CUDA events on the caller's stream), "setup_ms"
- * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape".
+ * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo".
  * Returns 0 or -1. */
 int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out);
 

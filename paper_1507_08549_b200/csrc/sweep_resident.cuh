@@ -9,14 +9,20 @@
 //    memory (BoxEngine, box_engine.cuh).  Two ways of coupling the tiles:
 //      - halo mode: box == owned tile.  After every half-sweep the edge cells of the colour just updated go to the
 //        four neighbouring tiles and theirs come back into the border slots of the engine.  No redundant work;
-//        the latency of the exchange is hidden by the other CTA(s) sharing the SM.  For grids that fill the chip.
+//        where registers allow, the patch-edge cells are updated and sent first so that the packets travel while
+//        the rest of the patch is updated.  For grids that fill the chip.
 //      - block mode (temporal blocking): box = owned tile + a margin of 2m cells towards every neighbour; m full
 //        sweeps run between two exchanges.  Every box cell is updated every half-sweep, cells closer than t to an
 //        interior box edge are stale after t half-sweeps, so after 2m half-sweeps exactly the owned tile is still
 //        exact; then the margins are refilled from the neighbours' tiles.  For grids that leave the chip idle.
 //    In both modes a colour's updates are mutually independent, so tiling cannot change a bit of the result (R10).
-//  * Exchange without fences or flags: every value travels as a 16-byte packet carrying the step number in both
-//    8-byte halves (ll_store / ll_load); the consumer polls the packet itself.  One L2 round trip per exchange.
+//  * Exchange.  Halo mode: every edge value travels as a 16-byte packet carrying the half-sweep number in both
+//    8-byte halves (ll_store / ll_load) into the neighbour's per-tile inbox; every receiving thread polls exactly
+//    ONE packet (strong loads of one thread do not pipeline: measured ~+75 clocks per extra packet, profiles/
+//    r01_microbench_b200.txt), so an exchange costs one L2 round trip and needs no fence and no flag.  Block mode:
+//    the tile is stored to the checkpoint ring anyway; one release-store of a per-tile flag publishes it and the
+//    neighbours refill their margins with ordinary (pipelined) loads after an acquire-poll of the flags of the tiles
+//    their box overlaps.  Tiny tiles (H = 2, <= 256 cells) send their patches as tagged packets instead.
 //  * a-3: per-sweep maxima of |res| and |phi_new| over the owned cells go warp -> CTA -> (service warp) atomicMax
 //    into per-sweep global slots.  An extra SERVICE WARP per CTA does all of that and the stopping decision, so the
 //    fences and L2 round trips of the reduction never stall the sweeps: the compute warps only hand it their maxima
@@ -318,7 +324,11 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     // optional in-kernel profile (thread 0 of the CTA): 0 total, 1 half-sweep compute, 2 halo exchange, 3 barrier,
     // 4 end of interval, 5 margin refill, 6 wait for the decision, 7 half-sweeps
     const bool prof_on = p.prof != nullptr && tid == 0;
-    auto tick = [&]() -> long long { return prof_on ? clock64() : 0ll; };
+    auto tick = [&]() -> long long {          // asm volatile under the branch: never executed speculatively
+        long long t = 0;
+        if (prof_on) asm volatile("mov.u64 %0, %%clock64;" : "=l"(t));
+        return t;
+    };
     const long long t_begin = tick();
     unsigned gbar_gen = 0;
     auto grid_barrier = [&]() {
