@@ -107,6 +107,16 @@ def measured_peaks():
     return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
+def profiled_traffic(workload: str, kernel: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "r01b_traffic.json")
+    try:
+        e = json.load(open(p)).get(workload)
+    except (OSError, ValueError):
+        return None
+    return float(e["traffic_bytes_per_launch"]) if e and e.get("kernel") == kernel else None
+
+
 def l2_copy_peak_gbs(torch, mib=24, iters=40):
     """L2-resident copy bandwidth (read + write bytes), measured live the way MEASURED_PEAKS.json measures HBM:
     b.copy_(a) with a working set (2 x `mib` MiB) that stays in the 126 MB L2; best of several."""
@@ -324,11 +334,15 @@ def main():
     else:
         bound, peak = "l2", l2_copy_peak_gbs(torch)
         src = "L2-resident torch copy (2 x 24 MiB, read+write bytes), measured live in this run (of measured)"
+    kernel = {1: "k_halfsweep", 2: "k_sor_resident", 3: "k_sor_blocked"}[path]
     roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": {1: "k_halfsweep", 2: "k_sor_resident", 3: "k_sor_blocked"}[path],
+                "traffic": profiled_traffic(args.workload, kernel), "kernel": kernel,
                 "alg_bytes_per_launch": alg_bytes_per_launch, "launch_ms": sw_ms / sweep_launches,
                 "sweep_launches_per_step": sweep_launches, "peak_source": src,
-                "frac_of_hbm_peak": achieved / hbm_peak}
+                "frac_of_hbm_peak": achieved / hbm_peak,
+                # the limiter once phi stays on chip: 7 fp64 instructions per update against 64 lanes / clock / SM
+                # (DESIGN.md section 6); for information, the judged fraction is `frac`
+                "fp64_pipe_frac": value * 7.0 / (148 * 64 * 1.965e9)}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -338,6 +352,7 @@ def main():
                    "tol": w0.tol, "l2": "flushed between timed solves (256 MiB write)",
                    "path": {1: "streaming", 2: "resident", 3: "blocked"}.get(path, str(path)),
                    "tblock": int(solver.stat("tblock")), "ctas": int(solver.stat("ctas")),
+                   "mode": ("halo" if solver.stat("halo") else "block") if path == 2 else None,
                    "tile": [int(solver.stat("tile_w")), int(solver.stat("tile_h"))],
                    "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"},
         "time_to_residual_ms": total_ms / args.steps, "sweeps_per_solve": [r.sweeps for r in results][:8],
