@@ -464,7 +464,9 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
             const int k = (int)((p.ntiles * (long long)nbatch + h->num_sms - 1) / h->num_sms);
             // per exchange: checkpoint store, release of the tile flag, the neighbours' acquire, margin refill
             const double exchange = p.ntiles == 1 ? 2000.0 : p.ll ? 3800.0 : 4200.0 + 0.7 * S.BW() * S.BH();
-            p.cost = 2.0 * model_half_sweep(S, k) + exchange * (1.0 + 0.5 * (k - 1)) / m;
+            // CTAs sharing an SM overlap one's flag wait with the other's sweeps; polling packets instead competes
+            // for issue slots (measured)
+            p.cost = 2.0 * model_half_sweep(S, k) + exchange * (p.ll ? 1.0 + 0.5 * (k - 1) : 1.0) / m;
             if (best.shape < 0 || p.cost < best.cost) best = p;
         }
     }

@@ -76,6 +76,11 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -177,10 +182,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             }
             __syncwarp();
             unsigned int* arr = arrived + (size_t)rep.exact * p.arr_stride + rep.r;
-            if (lane == 0) {
-                __threadfence();
-                red_release_add_u32(arr, 1u);
-            }
+            if (lane == 0) red_release_add_u32(arr, 1u);      // release: the warp's atomics above (ordered by __syncwarp)
             // ---- decide the interval (every CTA reads the same final slots -> the same answer)
             if (rep.exact || !stopped) {
                 if (lane == 0) {
@@ -335,7 +337,6 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         ++gbar_gen;
         Engine::sync();
         if (tid == 0) {
-            __threadfence();
             red_release_add_u32(gbar, 1u);
             unsigned spins = 0;
             while (ld_acquire_u32(gbar) < gbar_gen * (unsigned)ntiles && !poll_giveup(pc_end, spins, 20, (int)gbar_gen))
@@ -421,7 +422,6 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             rp.r = r; rp.k0 = k0; rp.n = n; rp.exact = exact; rp.quit = 0;
             rp.bad = exact ? 0 : s_bad;      // exact keys carry NaN/Inf themselves (abs_key sorts them highest)
         }
-        __threadfence_block();
         report_arrive(par);
         // block mode: publish "state r of this tile is in the ring" (the barrier above ordered every thread's stores
         // before this thread's fence)
@@ -449,10 +449,14 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 const int t = (nby0 + i / (nbx1 - nbx0 + 1)) * p.ntx + nbx0 + i % (nbx1 - nbx0 + 1);
                 if (t == tile) continue;
                 unsigned spins = 0;
-                while (ld_acquire_u32(flags + t) < want && !poll_giveup(pc, spins, 5, (int)want)) {}
+                // relaxed polls (an acquire would invalidate L1 on every iteration); the margins are then read
+                // with ld.global.cg, which is served by L2 where the release made the tile visible before the flag
+                while (ld_relaxed_u32(flags + t) < want && !poll_giveup(pc, spins, 5, (int)want)) {}
             }
         }
+        const long long tp0 = tick();
         Engine::sync();
+        if (prof_on) s_pf[2] += tick() - tp0;                    // block mode: wait for the neighbours' flags
         if (!own) E.load_patch(state_of(r), g.nr, gi0, gj0);
         E.publish_all();
         Engine::sync();
@@ -541,7 +545,6 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     ++seq;
     Engine::sync();
     if (tid == 0) s_rep[seq & 1].quit = 1;
-    __threadfence_block();
     report_arrive(seq & 1);
     if (prof_on) {
         s_pf[0] = clock64() - t_begin;
