@@ -47,6 +47,10 @@ def make_workload(name: str):
     if name == "cfg3":
         return "cfg3: 1024x2048 full-plane offset WD, lmax=32, tol=1e-10, cold solve (first of the sequence)", \
             [W.cfg3().first]
+    if name.startswith("cfg3seq"):
+        n = int(name[7:] or 100)
+        return (f"cfg3 sequence: {n} warm-started solves on 1024x2048 (rho evolves by seeded 0.1 % perturbations), "
+                f"lmax=32, tol=1e-10"), [W.cfg3(nsteps=n)]
     if name == "cfg4a":
         return "cfg4a: batch of 64 x 512x512 half-plane WDs, lmax=16, tol=1e-10, cold start", W.cfg4a(64)
     if name.startswith("sweep"):
@@ -239,6 +243,10 @@ def main():
     # multi-GPU: batch members are sharded across ranks with no collective; a single solve runs as replicas
     idx, scaling = shard_members(len(members), rank, world)
     mine = [members[i] for i in idx]
+    seq = None
+    if hasattr(mine[0], "first"):                     # cfg3 sequence: rho_t precomputed on the host, solves in order
+        seq = mine[0]
+        mine = [seq.first]
     w0 = mine[0]
     nb = len(mine)
     solver = P.PoissonSolver.for_workload(w0)
@@ -250,9 +258,27 @@ def main():
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     cells = w0.cells
 
+    rho_seq = None
+    if seq is not None:
+        rhos, r_t = [w0.rho], w0.rho
+        for t in range(1, seq.nsteps):
+            r_t = seq.step(r_t, t)
+            rhos.append(r_t)
+        rho_seq = [torch.from_numpy(r).cuda() for r in rhos]
+
+    acc = {"sweep_ms": 0.0, "setup_ms": 0.0, "launches": 0, "sweep_launches": 0}
+
     def solve_dev():
-        res = solver.solve(rho, phi, w0.tol, w0.max_sweeps)
-        return res if isinstance(res, list) else [res]
+        """One step: one solve (or batch), or the whole warm-started sequence; accumulates the library's counters."""
+        for k in acc:
+            acc[k] = 0
+        out = []
+        for rt in (rho_seq if rho_seq is not None else [rho]):
+            res = solver.solve(rt, phi, w0.tol, w0.max_sweeps)        # phi carries over inside a sequence
+            out += res if isinstance(res, list) else [res]
+            for k in acc:
+                acc[k] += solver.stat(k)
+        return out
 
     def barrier():
         if world > 1:
@@ -278,22 +304,25 @@ def main():
         e1.record()
         torch.cuda.synchronize()
         step_ms.append(e0.elapsed_time(e1))
-        sweep_ms.append(solver.stat("sweep_ms"))
-        setup_ms.append(solver.stat("setup_ms"))
-        launches += int(solver.stat("launches"))
+        sweep_ms.append(acc["sweep_ms"])
+        setup_ms.append(acc["setup_ms"])
+        launches += int(acc["launches"])
         updates += sum(r.sweeps for r in results) * cells
     barrier()
     region_s = time.perf_counter() - t_region
     clocks = sampler.stop()
     assert all(r.status == 0 for r in results), results
 
-    # end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
-    e2e = None
-    if nb == 1:
+    # end to end with HOST buffers (pinned), H2D + D2H inside the timed region.  Single solve: through the C ABI
+    # (sn_poisson_solve_host).  Batch / sequence: every solve's rho goes host -> device and its phi device -> host
+    # around the device call (what a hydro step that lives on the host does).
+    has_e2e = True
+    e2e_ms, e2e_upd, h2d_bytes, d2h_bytes = [], 0, 0, 0
+    if nb == 1 and seq is None:
         rho_pin = torch.from_numpy(w0.rho).pin_memory()
         phi_pin = torch.zeros(w0.rho.shape, dtype=torch.float64).pin_memory()
         rho_np, phi_np = rho_pin.numpy(), phi_pin.numpy()
-        e2e_ms, e2e_upd = [], 0
+        h2d_bytes, d2h_bytes = 2 * cells * 8, cells * 8
         for i in range(args.warmup + args.steps):
             phi_np[...] = 0.0
             flush.fill_(1)
@@ -304,13 +333,39 @@ def main():
             if i >= args.warmup:
                 e2e_ms.append(dt * 1e3)
                 e2e_upd += r.sweeps * cells
-        e2e_time = sum(e2e_ms) * 1e-3
+    else:
+        host_rhos = ([torch.from_numpy(r).pin_memory() for r in rhos] if seq is not None
+                     else [torch.from_numpy(rho_h).pin_memory()])
+        phi_host = torch.zeros(rho.shape, dtype=torch.float64).pin_memory()
+        rho_dev = torch.empty_like(rho)
+        n_e2e = min(args.steps, 3)                        # these steps are long; a few suffice
+        h2d_bytes = sum(t.numel() * 8 for t in host_rhos) + phi_host.numel() * 8
+        d2h_bytes = len(host_rhos) * phi_host.numel() * 8
+        for i in range(1 + n_e2e):
+            phi_host.zero_()
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            phi.copy_(phi_host, non_blocking=True)
+            sw = 0
+            for hr in host_rhos:
+                rho_dev.copy_(hr, non_blocking=True)
+                res = solver.solve(rho_dev, phi, w0.tol, w0.max_sweeps)
+                sw += sum(x.sweeps for x in res) if isinstance(res, list) else res.sweeps
+                phi_host.copy_(phi, non_blocking=True)
+                torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            if i >= 1:
+                e2e_ms.append(dt * 1e3)
+                e2e_upd += sw * cells
+    e2e_time = sum(e2e_ms) * 1e-3
+    e2e_steps = len(e2e_ms)
 
     total_ms = float(sum(step_ms))
-    counters = [float(updates), float(launches), float(e2e_upd) if nb == 1 else 0.0]
+    counters = [float(updates), float(launches), float(e2e_upd)]
     dev = torch.device("cuda", local_rank)
     total_ms, (updates_all, launches_all, e2e_upd_all) = reduce_timing(total_ms, counters, world, dev)
-    e2e_time_all, _ = reduce_timing(e2e_time * 1e3 if nb == 1 else 0.0, [], world, dev)
+    e2e_time_all, _ = reduce_timing(e2e_time * 1e3, [], world, dev)
     e2e_time_all *= 1e-3
     launches_all = int(launches_all)
 
@@ -324,7 +379,7 @@ def main():
     path = int(solver.stat("path"))
     sw_ms = float(np.mean(sweep_ms))
     sweeps_per_step = sum(r.sweeps for r in results)
-    sweep_launches = max(1, int(solver.stat("sweep_launches")))
+    sweep_launches = max(1, int(acc["sweep_launches"]))
     alg_bytes_per_launch = BYTES_PER_UPDATE * sweeps_per_step * cells / sweep_launches
     achieved = alg_bytes_per_launch / (sw_ms * 1e-3 / sweep_launches) / 1e9
     hbm_peak, hbm_src = measured_peaks()
@@ -356,17 +411,17 @@ def main():
                    "tile": [int(solver.stat("tile_w")), int(solver.stat("tile_h"))],
                    "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"},
         "time_to_residual_ms": total_ms / args.steps, "sweeps_per_solve": [r.sweeps for r in results][:8],
+        "solves_per_step": len(results), "sweeps_per_step": sum(r.sweeps for r in results),
         "final_residual": results[0].residual,
         "setup_ms": float(np.mean(setup_ms)), "sweep_ms": sw_ms,
         "gpu_launches": launches_all, "clocks": clocks, "roofline": roofline,
         "region_wall_s": region_s,
     }
-    if nb == 1:
-        out["e2e"] = {"value": e2e_upd_all / e2e_time_all, "unit": UNIT,
-                      "h2d_bytes_per_step": 2 * cells * 8, "d2h_bytes_per_step": cells * 8,
-                      "ms_per_step": e2e_time_all / args.steps * 1e3}
-    else:
-        out["e2e"] = None
+    out["e2e"] = {"value": e2e_upd_all / e2e_time_all, "unit": UNIT,
+                  "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
+                  "ms_per_step": e2e_time_all / e2e_steps * 1e3, "steps": e2e_steps,
+                  "api": "sn_poisson_solve_host" if (nb == 1 and seq is None) else
+                         "pinned tensor.copy_ + sn_poisson_solve / _solve_batch + copy back, per solve"}
     if not args.no_cpu_baseline and world == 1:
         v, sample = oracle_rate(mine)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
