@@ -182,6 +182,54 @@ def test_resident_batch_members_finish_independently(P, torch_cuda, oracle, halo
     assert len({r.sweeps for r in res}) > 1
 
 
+def test_planner_choice_random_grids_bit_exact(P, torch_cuda, oracle):
+    """Whatever (path, shape, mode, m) the planner picks for a grid, the result has the oracle's bits: seeded random
+    grid sizes (multiples of 4 x 8 so that the on-chip paths are eligible, plus odd ones that fall back to the
+    streaming path), fixed sweeps and a tolerance run each."""
+    rng = np.random.default_rng(2024)
+    seen = set()
+    for case in range(14):
+        if case < 10:
+            nr, nz = 4 * int(rng.integers(8, 100)), 8 * int(rng.integers(4, 50))
+        else:
+            nr, nz = int(rng.integers(30, 200)), int(rng.integers(30, 200))
+        symmetry = int(rng.integers(0, 2))
+        w = W.random_smooth(nr, nz, symmetry, seed=900 + case, lmax=4)
+        M = oracle.moments(w.rho, w.dr, w.dz, symmetry, w.lmax)
+        bnd = oracle.boundary(nr, nz, w.dr, w.dz, symmetry, w.lmax, M)
+        omega = oracle.default_omega(nr, nz, w.dr, w.dz, symmetry)
+        phi0 = rng.uniform(-1, 1, size=(nz, nr))
+        want, _, _ = oracle.sweeps(w.rho, phi0, w.dr, w.dz, symmetry, omega, *bnd, 37)
+        s, got, r = gpu_solve(P, torch_cuda, w, phi0=phi0, tol=0.0, max_sweeps=37, boundary=bnd)
+        seen.add((int(s.stat("path")), int(s.stat("halo"))))
+        assert r.sweeps == 37 and np.array_equal(got, want), (nr, nz, symmetry, s.stat("path"), s.stat("shape"))
+        ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, symmetry, w.lmax, 1e-6, 5000, boundary_arrays=bnd)
+        s, got, r = gpu_solve(P, torch_cuda, w, tol=1e-6, max_sweeps=5000, boundary=bnd)
+        assert (r.sweeps, r.status, r.residual) == (ref["sweeps"], ref["status"], ref["residual"])
+        assert np.array_equal(got, ref["phi"])
+    assert len(seen) >= 2                                     # on-chip and streaming paths were both exercised
+
+
+def test_resident_kernel_is_repeatable(P, torch_cuda):
+    """The inter-CTA protocols (packets, flags, late decision, endgame) are timing dependent; the result must not be:
+    the same solve repeated gives the same bits, sweeps and residual every time (block mode and halo mode)."""
+    for w, opts in ((W.cfg2(256), {"path": 2}), (W.cfg3(128).first, {"path": 2, "halo": 1, "shape": 3})):
+        s = P.PoissonSolver.for_workload(w)
+        for k, v in opts.items():
+            s.set_option(k, v)
+        rho = torch_cuda.from_numpy(w.rho).cuda()
+        first = None
+        for it in range(12):
+            phi = torch_cuda.zeros_like(rho)
+            r = s.solve(rho, phi, w.tol, w.max_sweeps)
+            assert s.stat("path") == 2 and r.status == 0
+            cur = (r.sweeps, r.residual, phi.clone())
+            if first is None:
+                first = cur
+            else:
+                assert cur[0] == first[0] and cur[1] == first[1] and torch_cuda.equal(cur[2], first[2])
+
+
 BLOCKED_CASES = [
     # nr, nz, symmetry, shape, tblock     (shape table: sn_poisson.cu blk_shapes())
     (128, 64, 1, 0, 1),       # one tile, box == grid
