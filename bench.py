@@ -1,16 +1,22 @@
 #!/usr/bin/env python
 """bench.py -- Poisson relaxation throughput (fp64 cell-updates/s) and time-to-residual per solve.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg3|cfg4a|sweep<N>] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+                    [--workload cfg0|cfg1|cfg2|cfg3|cfg3seq<N>|cfg4a|sweep<N>]
 
 One "step" = one pass of the whole hot path over one synthetic input: multipole moments -> boundary fill ->
 red-black SOR sweeps with the fused residual reduction until the device-side stopping rule fires (cold start,
 phi = 0), through the C ABI (sn_poisson_solve / _solve_batch).  Default workload: BASELINE.json configs[1]
-(256x256 n=1 polytrope, lmax 16, tol 1e-10).  Prints ONE JSON line (rank 0).
+(256x256 n=1 polytrope, lmax 16, tol 1e-10).  cfg3seq<N>: one step = the warm-started sequence of N solves of
+[CFG 3].  Prints ONE JSON line (rank 0).
 
-Timing: W warm-up solves, then K solves each bracketed by CUDA events on the launching stream (the call
-synchronises that stream itself); L2 is flushed (a 256 MiB write) and phi re-zeroed between solves, outside the
-events; the K-step region is bracketed by barrier + torch.cuda.synchronize(); max over ranks.
+Timing: W warm-up steps, then K steps each bracketed by CUDA events on the launching stream (the call
+synchronises that stream itself); L2 is flushed (a 256 MiB write) and phi re-zeroed between steps, outside the
+events; the K-step region is bracketed by barrier + torch.cuda.synchronize(); max over ranks.  `value` = all
+cell-updates of the K steps / that device time (inputs resident in HBM); `e2e` = the same with pinned HOST buffers,
+H2D / D2H inside the timed wall-clock region; `roofline` = 24 B x cell-updates of the relaxation kernel's launches /
+their device time (the library's own CUDA events) against the measured L2 / HBM peak; `cpu_baseline` = the oracle
+as it stands on one host core on a bounded sample.
 `--impl reference` times the CPU oracle (oracle/, single thread) on the same workload -- a deliberately slow
 program; parity and the roofline fraction are the headline, not that ratio.
 """
