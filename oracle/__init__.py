@@ -44,6 +44,7 @@ def lib():
                                     _dp, _dp, C.c_int, _dp, _dp]
         _lib.sno_solve.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, _dp,
                                    _dp, C.c_double, C.c_int, C.POINTER(C.c_int), _dp, _dp, _dp, _dp, _dp]
+        _lib.sno_gravity.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib.sno_apply_operator.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp,
                                             _dp, _dp]
     return _lib
@@ -137,6 +138,16 @@ def apply_operator(phi, dr, dz, symmetry, bE, bN, bS):
     out = np.zeros_like(phi)
     lib().sno_apply_operator(nr, nz, dr, dz, symmetry, _p(phi), _p(_f64(bE)), _p(_f64(bN)), _p(bS), _p(out))
     return out
+
+
+def gravity(phi, dr, dz, symmetry, bE, bN, bS):
+    """(g_r, g_z) = -grad phi at the cell centres (R15)."""
+    phi = _f64(phi)
+    nz, nr = phi.shape
+    bS = _f64(bS) if bS is not None else np.zeros(nr)
+    gr, gz = np.zeros_like(phi), np.zeros_like(phi)
+    lib().sno_gravity(nr, nz, dr, dz, symmetry, _p(phi), _p(_f64(bE)), _p(_f64(bN)), _p(bS), _p(gr), _p(gz))
+    return gr, gz
 
 
 def solve_workload(w, phi0=None, history=False):

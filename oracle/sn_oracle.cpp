@@ -22,6 +22,7 @@
 //                                      point-mass ring potential via elliptic K; Legendre closed forms
 //   * reflecting boundary           <- mirrored full-plane solve == half-plane solve
 //   * discrete Gauss law, linearity, omega formula vs Jacobi spectral radius, omega=1 == Gauss-Seidel
+//   * gravity epilogue (sno_gravity) <- exact on quadratic potentials, closed-form polytrope field at O(h^2)
 //   * iteration history (the per-sweep iterate): defined by this file; nothing external can pin it
 //     beyond the above -- stated in DESIGN.md §5.
 #include <cmath>
@@ -275,6 +276,26 @@ int sno_apply_operator(int nr, int nz, double dr, double dz, int symmetry, const
             const bool mirror_row = (symmetry == 1 && j == 0);
             const double pS = (j > 0) ? phi[c - nr] : (mirror_row ? phi[c] : bS[i]);
             out[c] = cE * (pE - phi[c]) - cW * (phi[c] - pW) + iz2 * (pN - phi[c]) - iz2 * (phi[c] - pS);
+        }
+    return 0;
+}
+
+// NEXT-1: the gravity field the momentum and energy equations use as source terms,
+// PAPER.md:83-89, eqs. (2)-(4): -rho dPhi/dr, -rho dPhi/dz.  [R15] centred differences at the cell centres with the
+// solver's own boundary handling: reflecting axis (phi_{-1,j} = phi_{0,j}), reflecting equator when symmetry = 1
+// (phi_{i,-1} = phi_{i,0}), the Dirichlet ghosts bE / bN / bS elsewhere.  Pinned arithmetic: (lo - hi) * (0.5/d).
+int sno_gravity(int nr, int nz, double dr, double dz, int symmetry, const double* phi, const double* bE,
+                const double* bN, const double* bS, double* gr, double* gz) {
+    const double hr = 0.5 / dr, hz = 0.5 / dz;
+    for (int j = 0; j < nz; ++j)
+        for (int i = 0; i < nr; ++i) {
+            const size_t c = (size_t)j * nr + i;
+            const double pE = (i + 1 < nr) ? phi[c + 1] : bE[j];
+            const double pW = (i > 0) ? phi[c - 1] : phi[c];
+            const double pN = (j + 1 < nz) ? phi[c + nr] : bN[i];
+            const double pS = (j > 0) ? phi[c - nr] : (symmetry == 1 ? phi[c] : bS[i]);
+            gr[c] = (pW - pE) * hr;
+            gz[c] = (pS - pN) * hz;
         }
     return 0;
 }

@@ -438,3 +438,80 @@ def test_wd_config_quadrupole_is_small(oracle):
     # mass of the bubble-free synthetic star == Table 5's 1.377 Msun in code units, to quadrature error
     w0 = W.cfg4b(128)
     assert oracle.moments(w0.rho, w0.dr, w0.dz, 1, 0)[0] == pytest.approx(W.M_WD_CODE, rel=0.01)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# NEXT-1: gravity epilogue g = -grad phi (eqs. 2-4; R15)
+# ----------------------------------------------------------------------------------------------------------
+def _ghost_samples(fun, nr, nz, dr, dz, symmetry):
+    """fun(r, z) sampled at the east / north / south ghost-cell centres (R4)."""
+    r, z = W.cell_centres(nr, nz, dr, dz, symmetry)
+    bE = fun((nr + 0.5) * dr, z)
+    bN = fun(r, z[-1] + dz)
+    bS = fun(r, z[0] - dz)
+    return r, z, bE, bN, bS
+
+
+@pytest.mark.parametrize("symmetry", [0, 1])
+def test_gravity_is_exact_on_quadratic_potentials(oracle, symmetry):
+    """Centred differences are exact for a + b r^2 + c z^2 (+ d z when there is no equatorial mirror), including the
+    reflecting axis (phi is even in r) and equator rows and the rows / columns next to the Dirichlet ghosts."""
+    nr, nz, dr, dz = 11, 9, 0.07, 0.11
+    a, b, c, d = 1.5, -3.0, 0.7, (0.0 if symmetry == 1 else 2.5)
+    fun = lambda r, z: a + b * r ** 2 + c * z ** 2 + d * z
+    r, z, bE, bN, bS = _ghost_samples(fun, nr, nz, dr, dz, symmetry)
+    phi = fun(r[None, :], z[:, None])
+    gr, gz = oracle.gravity(phi, dr, dz, symmetry, bE, bN, bS)
+    assert np.allclose(gr, -2 * b * r[None, :] * np.ones((nz, 1)), rtol=0, atol=1e-13)
+    assert np.allclose(gz, -(2 * c * z[:, None] + d) * np.ones((1, nr)), rtol=0, atol=1e-13)
+
+
+def test_gravity_second_order_on_the_polytrope_field(oracle):
+    """The analytic n=1 polytrope potential (R13) sampled on the grid: the differenced field converges to the closed
+    form g = -dphi/ds s_hat at second order (error x1/4 per refinement), inside and outside the star."""
+    R = 0.8
+    k = np.pi / R
+
+    def phi_fun(r, z):
+        s = np.hypot(r, z)
+        x = k * s
+        return np.where(s < R, -4 * np.pi / k ** 2 * (1 + np.sin(x) / x), -(4 * R ** 3 / np.pi) / s)
+
+    def g_mag(s):        # -dphi/ds
+        x = k * s
+        inside = 4 * np.pi / k * (x * np.cos(x) - np.sin(x)) / x ** 2
+        return np.where(s < R, inside, -(4 * R ** 3 / np.pi) / s ** 2)
+
+    errs = []
+    for n in (32, 64, 128):
+        dr = dz = 1.0 / n
+        r, z, bE, bN, bS = _ghost_samples(phi_fun, n, n, dr, dz, 1)
+        phi = phi_fun(r[None, :], z[:, None])
+        gr, gz = oracle.gravity(phi, dr, dz, 1, bE, bN, bS)
+        s = np.hypot(r[None, :], z[:, None])
+        g = g_mag(s)
+        errs.append(max(np.max(np.abs(gr - g * r[None, :] / s)), np.max(np.abs(gz - g * z[:, None] / s))))
+    assert errs[0] < 2e-2 and 3.0 < errs[0] / errs[1] < 5.0 and 3.0 < errs[1] / errs[2] < 5.0
+
+
+def test_gravity_of_the_solved_polytrope_and_mirror_antisymmetry(oracle):
+    """End to end: the solved cfg-1 potential differenced by the oracle matches the closed-form field; on a full
+    plane with a z-symmetric density g_z is odd and g_r even in z."""
+    w = W.cfg1(64)
+    ref = oracle.solve_workload(w)
+    M = oracle.moments(w.rho, w.dr, w.dz, 1, w.lmax)
+    bnd = oracle.boundary(w.nr, w.nz, w.dr, w.dz, 1, w.lmax, M)
+    gr, gz = oracle.gravity(ref["phi"], w.dr, w.dz, 1, *bnd)
+    r, z = W.cell_centres(w.nr, w.nz, w.dr, w.dz, 1)
+    s = np.hypot(r[None, :], z[:, None])
+    R, k = 0.8, np.pi / 0.8
+    x = k * s
+    g = np.where(s < R, 4 * np.pi / k * (x * np.cos(x) - np.sin(x)) / x ** 2, -(4 * R ** 3 / np.pi) / s ** 2)
+    assert np.max(np.abs(gr - g * r[None, :] / s)) < 5e-3 and np.max(np.abs(gz - g * z[:, None] / s)) < 5e-3
+    # mirrored full plane
+    rho_full = np.concatenate([w.rho[::-1], w.rho])
+    full = oracle.solve(rho_full, np.zeros_like(rho_full), w.dr, w.dz, 0, w.lmax, 0.0, 3000)
+    Mf = oracle.moments(rho_full, w.dr, w.dz, 0, w.lmax)
+    bf = oracle.boundary(w.nr, 2 * w.nz, w.dr, w.dz, 0, w.lmax, Mf)
+    grf, gzf = oracle.gravity(full["phi"], w.dr, w.dz, 0, *bf)
+    assert np.max(np.abs(gzf + gzf[::-1])) < 1e-9 and np.max(np.abs(grf - grf[::-1])) < 1e-9
