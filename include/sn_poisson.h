@@ -88,6 +88,14 @@ void sn_poisson_destroy(sn_poisson* h);
 int sn_poisson_set_omega(sn_poisson* h, double omega);
 double sn_poisson_get_omega(const sn_poisson* h);
 
+/* NEXT-1: the gravity field g = -grad phi at the cell centres, the source term of the paper's
+ * momentum and energy equations (eqs. 2-4).  Centred differences with the solver's boundary handling
+ * (R15): reflecting axis, reflecting equator when symmetry = 1, elsewhere the ghost values of the LAST solve
+ * / batch on this handle (or the injected ones).  phi, gr, gz: DEVICE pointers to nbatch consecutive grids (layout of
+ * sn_poisson_solve_batch); gr, gz must not alias phi.  The kernel is enqueued on `stream` and NOT synchronised.
+ * Returns 0, -1 (bad argument, or no ghost values for nbatch members yet), -2 (CUDA error). */
+int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr, double* gz, void* stream);
+
 /* Test hooks.  All pointers are HOST pointers.
  * get_moments : M[0..lmax] of batch member 0 of the last solve (odd entries 0 when symmetry = 1).
  * set_boundary: inject ghost values bE[nz], bN[nr], bS[nr] (bS ignored when symmetry = 1) and skip the moment and

@@ -4,7 +4,8 @@ The product is the C-ABI library ``libsn_poisson.so`` (include/sn_poisson.h); th
 """
 from .binding import (EXPORTS, LIB_PATH, SnPoissonError, load, sn_poisson_create, sn_poisson_destroy,
                       sn_poisson_get_boundary, sn_poisson_get_history, sn_poisson_get_moments,
-                      sn_poisson_get_omega, sn_poisson_get_stat, sn_poisson_last_error, sn_poisson_result,
+                      sn_poisson_get_omega, sn_poisson_get_stat, sn_poisson_gravity, sn_poisson_last_error,
+                      sn_poisson_result,
                       sn_poisson_set_boundary, sn_poisson_set_omega, sn_poisson_set_option, sn_poisson_solve,
                       sn_poisson_solve_batch, sn_poisson_solve_host, sn_poisson_version)
 from .solver import PoissonSolver

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libsn_poisson.so")
 # every symbol include/sn_poisson.h declares
 EXPORTS = (
     "sn_poisson_create", "sn_poisson_solve", "sn_poisson_solve_host", "sn_poisson_solve_batch",
-    "sn_poisson_destroy", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
+    "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
     "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
 )
@@ -57,6 +57,8 @@ def load():
                                            C.POINTER(sn_poisson_result)]
     lib.sn_poisson_destroy.restype = None
     lib.sn_poisson_destroy.argtypes = [_vp]
+    lib.sn_poisson_gravity.restype = C.c_int
+    lib.sn_poisson_gravity.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp]
     lib.sn_poisson_set_omega.restype = C.c_int
     lib.sn_poisson_set_omega.argtypes = [_vp, C.c_double]
     lib.sn_poisson_get_omega.restype = C.c_double
@@ -118,6 +120,13 @@ def sn_poisson_solve_batch(h, nbatch, rho_ptr, phi_ptr, tol, max_sweeps, stream=
     if rc != 0:
         raise SnPoissonError(f"sn_poisson_solve_batch failed ({rc}): " + sn_poisson_last_error())
     return list(out)
+
+
+def sn_poisson_gravity(h, nbatch, phi_ptr, gr_ptr, gz_ptr, stream=0):
+    rc = load().sn_poisson_gravity(h, int(nbatch), phi_ptr, gr_ptr, gz_ptr, stream or None)
+    if rc != 0:
+        raise SnPoissonError(f"sn_poisson_gravity failed ({rc}): " + sn_poisson_last_error())
+    return rc
 
 
 def sn_poisson_set_omega(h, omega) -> int:

@@ -15,6 +15,7 @@
 
 #include "common.cuh"
 #include "moments.cuh"
+#include "gravity.cuh"
 #include "sweep_stream.cuh"
 #include "sweep_blocked.cuh"
 #include "sweep_resident.cuh"
@@ -750,6 +751,29 @@ sn_poisson_result sn_poisson_solve_host(sn_poisson* h, const double* rho_host, d
     if ((e = cudaMemcpyAsync(phi_inout_host, h->d_phi_stage, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e, "D2H phi");
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return fail(e, "cudaStreamSynchronize");
     return r;
+}
+
+int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr, double* gz, void* stream) {
+    g_err.clear();
+    if (!h || !phi || !gr || !gz) { set_err("NULL argument"); return -1; }
+    if (nbatch < 1 || nbatch > 65535) { set_err("nbatch must be in [1, 65535]"); return -1; }
+    if (!h->d_bE || nbatch > h->cap_batch) {
+        set_err("no ghost values for %d member(s): solve (or set_boundary) on this handle first", nbatch);
+        return -1;
+    }
+    CU_TRY(cudaSetDevice(h->device));
+    const Geom g = make_geom(h, 0.0);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool vec = h->nr % 4 == 0 && ((((uintptr_t)phi | (uintptr_t)gr | (uintptr_t)gz) & 15) == 0);
+    if (vec) {
+        const dim3 grid((h->nr / 4 + 127) / 128, h->nz, nbatch);
+        k_gravity4<<<grid, 128, 0, st>>>(g, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
+    } else {
+        const dim3 grid((h->nr + 127) / 128, h->nz, nbatch);
+        k_gravity1<<<grid, 128, 0, st>>>(g, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
+    }
+    CU_TRY(cudaGetLastError());
+    return 0;
 }
 
 int sn_poisson_set_omega(sn_poisson* h, double omega) {

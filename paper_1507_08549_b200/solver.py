@@ -19,7 +19,7 @@ class PoissonSolver:
         return cls(w.nr, w.nz, w.dr, w.dz, w.symmetry, w.lmax, omega=w.omega)
 
     def close(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and getattr(B, "sn_poisson_destroy", None):     # B is torn down at interpreter exit
             B.sn_poisson_destroy(self.h)
             self.h = None
 
@@ -62,6 +62,21 @@ class PoissonSolver:
         if r.status < 0:
             raise B.SnPoissonError(f"sn_poisson_solve_host status {r.status}: {B.sn_poisson_last_error()}")
         return r
+
+    def gravity(self, phi, gr=None, gz=None):
+        """(g_r, g_z) = -grad phi with the ghost values of the last solve; enqueued on the current stream."""
+        import torch
+        self._check(phi)
+        gr = torch.empty_like(phi) if gr is None else gr
+        gz = torch.empty_like(phi) if gz is None else gz
+        self._check(gr)
+        self._check(gz)
+        nb = phi.shape[0] if phi.dim() == 3 else 1
+        if tuple(phi.shape[-2:]) != (self.nz, self.nr) or gr.shape != phi.shape or gz.shape != phi.shape:
+            raise ValueError("shape mismatch")
+        B.sn_poisson_gravity(self.h, nb, phi.data_ptr(), gr.data_ptr(), gz.data_ptr(),
+                             torch.cuda.current_stream().cuda_stream)
+        return gr, gz
 
     def set_option(self, key, value):
         return B.sn_poisson_set_option(self.h, key, value)

@@ -542,3 +542,54 @@ def test_rho_is_never_modified_and_stream_is_respected(P, torch_cuda):
         r = s.solve(rho, phi, w.tol, w.max_sweeps)
     st.synchronize()
     assert r.status == 0 and torch_cuda.equal(rho, keep)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# NEXT-1: gravity epilogue g = -grad phi (R15)
+# ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nr,nz,symmetry", [(64, 48, 1), (128, 72, 0), (37, 53, 1), (130, 70, 0), (4, 2, 0), (2, 2, 1)])
+def test_gravity_bit_exact(P, torch_cuda, oracle, nr, nz, symmetry):
+    """Vector kernel (nr % 4 == 0) and scalar fallback, both symmetries, edges next to every kind of boundary:
+    bit-identical to the oracle for an arbitrary field with injected ghosts; phi is not modified."""
+    w = W.random_smooth(nr, nz, symmetry, seed=700 + nr, lmax=4)
+    rng = np.random.default_rng(nr * 13 + nz)
+    phi = rng.uniform(-1, 1, size=(nz, nr))
+    bE, bN, bS = rng.uniform(-1, 1, nz), rng.uniform(-1, 1, nr), rng.uniform(-1, 1, nr)
+    want_r, want_z = oracle.gravity(phi, w.dr, w.dz, symmetry, bE, bN, bS)
+    s = P.PoissonSolver(w.nr, w.nz, w.dr, w.dz, symmetry, w.lmax)
+    s.set_boundary(bE, bN, bS)
+    p = torch_cuda.from_numpy(phi).cuda()
+    keep = p.clone()
+    gr, gz = s.gravity(p)
+    torch_cuda.cuda.synchronize()
+    assert np.array_equal(gr.cpu().numpy(), want_r) and np.array_equal(gz.cpu().numpy(), want_z)
+    assert torch_cuda.equal(p, keep)
+
+
+def test_gravity_after_solve_and_batch(P, torch_cuda, oracle):
+    """After a solve the epilogue uses that solve's ghost values; after a batch, every member's own."""
+    w = W.cfg1(128)
+    s, got, r = gpu_solve(P, torch_cuda, w)
+    gr, gz = s.gravity(torch_cuda.from_numpy(got).cuda())
+    want_r, want_z = oracle.gravity(got, w.dr, w.dz, 1, *s.boundary())
+    assert np.array_equal(gr.cpu().numpy(), want_r) and np.array_equal(gz.cpu().numpy(), want_z)
+    # physical check: the field points inwards and matches the closed form of the polytrope
+    rr, zz = W.cell_centres(w.nr, w.nz, w.dr, w.dz, 1)
+    sph = np.hypot(rr[None, :], zz[:, None])
+    R, k = 0.8, np.pi / 0.8
+    x = k * sph
+    g = np.where(sph < R, 4 * np.pi / k * (x * np.cos(x) - np.sin(x)) / x ** 2, -(4 * R ** 3 / np.pi) / sph ** 2)
+    assert np.max(np.abs(gr.cpu().numpy() - g * rr[None, :] / sph)) < 2e-3
+    ws = [W.cfg4a_member(b, 128) for b in range(3)]
+    sb = P.PoissonSolver.for_workload(ws[0])
+    rho = torch_cuda.from_numpy(np.stack([m.rho for m in ws])).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    sb.solve(rho, phi, ws[0].tol, ws[0].max_sweeps)
+    gr, gz = sb.gravity(phi)
+    for b, m in enumerate(ws):
+        M = oracle.moments(m.rho, m.dr, m.dz, 1, m.lmax)
+        bnd = oracle.boundary(m.nr, m.nz, m.dr, m.dz, 1, m.lmax, M)
+        want_r, want_z = oracle.gravity(phi[b].cpu().numpy(), m.dr, m.dz, 1, *bnd)
+        assert relmax(gr[b].cpu().numpy(), want_r) <= REL and relmax(gz[b].cpu().numpy(), want_z) <= REL
+    with pytest.raises(P.SnPoissonError):
+        P.PoissonSolver.for_workload(w).gravity(torch_cuda.zeros((w.nz, w.nr), dtype=torch_cuda.float64, device="cuda"))
