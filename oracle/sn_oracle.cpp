@@ -6,7 +6,7 @@
 // coordinates ... inner boundaries are assumed to be reflecting and the outer boundaries are fixed by
 // using the Roche approximation Phi(r,z) = -GM/sqrt(r^2+z^2) ... in general higher multipole terms are
 // needed").  The paper gives no stencil, relaxation factor, ordering or stopping arithmetic; every such
-// choice is a reading listed in DESIGN.md §3 (R1..R14), cited below as [R#].
+// choice is a reading listed in DESIGN.md §3 (R1..R15), cited below as [R#].
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load this
 // file's library.  It shares no code with paper_1507_08549_b200/csrc and is never called by the product.
