@@ -121,6 +121,9 @@ int sn_poisson_get_history(sn_poisson* h, double* R, int n);
  *   "halo"        path 2: 1 = halo mode (box == tile, edge exchange every half-sweep), 0 = block mode (margins of
  *                 2m cells, exchange every m sweeps), -1 = planner's choice
  *   "ll"          path 2 block mode: 1 = margins travel as tagged packets, 0 = tile flags + ring loads, -1 = auto
+ *   "group"       batches on path 2: G > 0 = solve the batch in groups of G members, one resident launch after the
+ *                 other; 0 = never group (all members co-resident or another path); -1 = group when the whole batch
+ *                 cannot be co-resident and a group fills the chip in halo mode
  *   "exact"       1: paths 2 / 3 track the per-sweep maxima exactly in every interval / launch (exact R_k history)
  *   "prof"        1: path 2 records an in-kernel SM-clock profile (stats "prof_mean0..7", "prof_max0..7": total,
  *                 half-sweep compute, halo exchange, barrier, end of interval, margin refill, wait for the
@@ -129,7 +132,8 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value);
 
 /* Counters of the last solve / batch: "launches" (kernels launched), "sweep_launches" (those that ran relaxation
  * sweeps), "sweep_ms" (device time of the relaxation phase, CUDA events on the caller's stream), "setup_ms"
- * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo".
+ * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo",
+ * "group" (members per resident launch).
  * Returns 0 or -1. */
 int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out);
 

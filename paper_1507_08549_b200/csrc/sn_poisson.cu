@@ -63,7 +63,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -91,7 +91,7 @@ struct sn_poisson {
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
     double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
-    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0;
+    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0, st_group = 0;
     int last_sweeps0 = 0;
 };
 
@@ -474,8 +474,9 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
     return best;
 }
 
+// Members member0 .. member0 + nbatch - 1 of the caller's batch (rho, phi point at member 0 of the batch).
 int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, const double* rho, double* phi,
-                 int max_sweeps, cudaStream_t st) {
+                 int max_sweeps, cudaStream_t st, int member0 = 0) {
     const ShapeInfo& S = shapes()[pl.shape];
     const size_t ncell = (size_t)h->nr * h->nz;
     const size_t nint = (size_t)(max_sweeps + pl.Q - 1) / pl.Q;
@@ -499,7 +500,8 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         h->sync_cap = need_sync;
     }
     CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * need_sync, st));
-    CU_TRY(cudaMemsetAsync(h->d_slots_f, 0, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
+    CU_TRY(cudaMemsetAsync(h->d_slots_f + (size_t)member0 * 2 * h->cap_sweeps, 0,
+                           sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
     if (pl.halo || pl.ll) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
     ResParams P;
     P.g = g;
@@ -508,17 +510,19 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.Q = pl.Q;
     P.max_sweeps = max_sweeps;
     P.force_exact = h->opt_exact;
-    P.rho = rho; P.phi = phi;
+    P.rho = rho + (size_t)member0 * ncell; P.phi = phi + (size_t)member0 * ncell;
     P.ring = h->d_ring;
     P.mail = reinterpret_cast<uint4*>(h->d_mail);
-    P.bE = h->d_bE; P.bN = h->d_bN; P.bS = h->d_bS;
-    P.slots_f = h->d_slots_f; P.slots_x = h->d_slots;
+    P.bE = h->d_bE + (size_t)member0 * h->nz; P.bN = h->d_bN + (size_t)member0 * h->nr;
+    P.bS = h->d_bS + (size_t)member0 * h->nr;
+    P.slots_f = h->d_slots_f + (size_t)member0 * 2 * h->cap_sweeps;
+    P.slots_x = h->d_slots + (size_t)member0 * 2 * h->cap_sweeps;
     P.slot_stride = 2 * h->cap_sweeps; P.hist_stride = h->cap_sweeps;
     P.arrived = h->d_sync;
     P.arr_stride = (int)(nint + 2);
     P.gbar = h->d_sync + (size_t)nbatch * 2 * (nint + 2);
     P.flags = P.gbar + nbatch;
-    P.ctl = h->d_ctl; P.hist = h->d_hist;
+    P.ctl = h->d_ctl + member0; P.hist = h->d_hist + (size_t)member0 * h->cap_sweeps;
     P.prof = nullptr;
     h->prof_ctas = 0;
     if (h->opt_prof) {
@@ -539,7 +543,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     h->st_launches += 1;
     h->st_path = 2;
     h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.Q;
-    h->st_shape = pl.shape; h->st_halo = pl.halo;
+    h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch;
     return 0;
 }
 
@@ -572,7 +576,28 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     // a-2 + a-3
     ResPlan pl;
     BlkPlan bp;
-    if ((h->opt_path == 0 || h->opt_path == 2) && max_sweeps > 0) pl = plan_resident(h, nbatch, rho, phi);
+    int group = nbatch;          // members per resident launch
+    if ((h->opt_path == 0 || h->opt_path == 2) && max_sweeps > 0) {
+        pl = plan_resident(h, nbatch, rho, phi);
+        // A batch whose tiles cannot all be co-resident: solve it in groups of G members, one resident launch after
+        // the other, if a group fills the chip (otherwise the blocked path streams the whole batch).  "group"
+        // option: 0 never, G > 0 exactly G, -1 this rule.
+        const bool forced = h->opt_group > 0 && h->opt_group < nbatch;
+        if (forced) pl = ResPlan();
+        if (pl.shape < 0 && nbatch > 1 && h->opt_group != 0) {
+            double best_total = 0;
+            for (int G = std::min(nbatch - 1, h->opt_group > 0 ? h->opt_group : nbatch - 1); G >= 1; --G) {
+                if (h->opt_group > 0 && G != h->opt_group) break;
+                const ResPlan cand = plan_resident(h, G, rho, phi);
+                if (cand.shape < 0) continue;
+                const double total = cand.cost * ((nbatch + G - 1) / G);
+                if (pl.shape < 0 || total < best_total) { pl = cand; best_total = total; group = G; }
+            }
+            const int occ_ctas = pl.shape >= 0 ? pl.ntiles * group : 0;
+            if (pl.shape >= 0 && !forced && (occ_ctas < 1.7 * h->num_sms || !pl.halo)) pl = ResPlan();
+            if (pl.shape < 0) group = nbatch;
+        }
+    }
     if (h->opt_path == 2 && pl.shape < 0 && max_sweeps > 0) {
         set_err("resident path requested but not eligible (needs nr%%4==0, nz%%H==0, grid >= one box, 16-byte aligned "
                 "pointers, tiles x batch <= co-resident CTAs)");
@@ -585,7 +610,10 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
         return -1;
     }
     if (pl.shape >= 0) {
-        if (int rc = run_resident(h, g, pl, nbatch, rho, phi, max_sweeps, st)) return rc;
+        for (int m0 = 0; m0 < nbatch; m0 += group)
+            if (int rc = run_resident(h, g, pl, std::min(group, nbatch - m0), rho, phi, max_sweeps, st, m0)) return rc;
+        h->st_group = group;
+        h->st_ctas = (double)pl.ntiles * group;
     } else if (bp.shape >= 0) {
         if (int rc = run_blocked(h, g, bp, nbatch, rho, phi, max_sweeps, st)) return rc;
     } else {
@@ -842,6 +870,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
     if (!strcmp(key, "prof")) { h->opt_prof = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "group")) { if (value < -1 || value > 65535) { set_err("group must be -1, 0 or a member count"); return -1; } h->opt_group = (int)value; return 0; }
     if (!strcmp(key, "ll")) { if (value < -1 || value > 1) { set_err("ll must be -1, 0 or 1"); return -1; } h->opt_ll = (int)value; return 0; }
     if (!strcmp(key, "halo")) { if (value < -1 || value > 1) { set_err("halo must be -1, 0 or 1"); return -1; } h->opt_halo = (int)value; return 0; }
     if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)std::max(shapes().size(), blk_shapes().size())) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
@@ -864,6 +893,7 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "tblock")) { *out = h->st_tblock; return 0; }
     if (!strcmp(key, "shape")) { *out = h->st_shape; return 0; }
     if (!strcmp(key, "halo")) { *out = h->st_halo; return 0; }
+    if (!strcmp(key, "group")) { *out = h->st_group; return 0; }
     if (!strncmp(key, "prof_mean", 9) && key[9] >= '0' && key[9] <= '7' && !key[10]) { *out = h->prof_mean[key[9] - '0']; return 0; }
     if (!strncmp(key, "prof_max", 8) && key[8] >= '0' && key[8] <= '7' && !key[9]) { *out = h->prof_max[key[8] - '0']; return 0; }
     set_err("unknown stat '%s'", key);

@@ -160,15 +160,18 @@ def test_resident_kernel_stops_at_the_oracle_sweep(P, torch_cuda, oracle, nr, nz
             assert np.array_equal(got2, ref2["phi"])
 
 
-@pytest.mark.parametrize("halo,shape,tb", [(0, 4, 3), (1, 3, 4)])
-def test_resident_batch_members_finish_independently(P, torch_cuda, oracle, halo, shape, tb):
+@pytest.mark.parametrize("halo,shape,tb,group", [(0, 4, 3, 0), (1, 3, 4, 0), (1, 3, 4, 3), (0, 2, 2, 1)])
+def test_resident_batch_members_finish_independently(P, torch_cuda, oracle, halo, shape, tb, group):
     """Resident kernel with a batch: the tiles of all members are co-resident, every member has its own slots,
-    arrival counters and grid barrier, and stops at its own sweep."""
+    arrival counters and grid barrier, and stops at its own sweep.  With the "group" option the batch is solved in
+    groups of that many members, one resident launch after the other (ragged last group)."""
     ws = [W.cfg4a_member(b, 128) for b in range(4)]
     w0 = ws[0]
     s = P.PoissonSolver.for_workload(w0)
     for k, v in res_opts(shape, tb, halo).items():
         s.set_option(k, v)
+    if group:
+        s.set_option("group", group)
     rho = torch_cuda.from_numpy(np.stack([w.rho for w in ws])).cuda()
     phi = torch_cuda.zeros_like(rho)
     res = s.solve(rho, phi, w0.tol, w0.max_sweeps)
