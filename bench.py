@@ -176,6 +176,8 @@ def run_reference(args, label, members):
         return
     import oracle as O
     O.build()
+    if hasattr(members[0], "first"):                  # the cfg3 sequence: its first (cold) solve is the sample
+        members = [members[0].first]
     w = members[0]
     per_step_sweeps = None
     if w.cells * 2000.0 / 1.0e8 > 8.0:               # too slow for full solves: fixed-sweep sample per step
