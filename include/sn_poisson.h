@@ -120,6 +120,8 @@ int sn_poisson_get_history(sn_poisson* h, double* R, int n);
  *   "shape"       box shape index of path 2 / 3; -1 = planner's choice
  *   "halo"        path 2: 1 = halo mode (box == tile, edge exchange every half-sweep), 0 = block mode (margins of
  *                 2m cells, exchange every m sweeps), -1 = planner's choice
+ *   "ds"          path 2 halo mode: 1 = all tiles of a member in one thread-block cluster (<= 16 tiles), edges through
+ *                 distributed shared memory (st.async + mbarrier); 0 = never; -1 = planner's choice
  *   "ll"          path 2 block mode: 1 = margins travel as tagged packets, 0 = tile flags + ring loads, -1 = auto
  *   "group"       batches on path 2: G > 0 = solve the batch in groups of G members, one resident launch after the
  *                 other; 0 = never group (all members co-resident or another path); -1 = group when the whole batch
@@ -132,7 +134,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value);
 
 /* Counters of the last solve / batch: "launches" (kernels launched), "sweep_launches" (those that ran relaxation
  * sweeps), "sweep_ms" (device time of the relaxation phase, CUDA events on the caller's stream), "setup_ms"
- * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo",
+ * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo", "ds",
  * "group" (members per resident launch).
  * Returns 0 or -1. */
 int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out);

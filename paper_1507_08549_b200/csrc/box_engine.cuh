@@ -236,11 +236,12 @@ struct BoxEngine {
     // Halo mode: the cells a neighbouring TILE may need (first and last patch row, first / last patch column) are
     // updated first and sent at once, so that the packets travel while the rest of the patch is updated.  The order
     // of a colour's updates is free (they are mutually independent, R10).  No barrier here.
-    template <int COL, int TRACK>
+    template <int COL, int TRACK, bool DS = false>
     __device__ __forceinline__ void half_sweep_halo(unsigned tag) {
         if (!active) return;
         update_cells<COL, TRACK, 1>();
-        halo_send<COL>(tag);
+        if (DS) ds_send<COL>();
+        else halo_send<COL>(tag);
         update_cells<COL, TRACK, 2>();
         publish_colour<COL>();
     }
@@ -436,6 +437,90 @@ struct BoxEngine {
             if (ll_ready(v, tag)) { *dst = ll_value(v); break; }
             if (poll_giveup(pc, spins, 1, (int)tag)) break;
         }
+    }
+
+    // ---- halo mode inside ONE thread-block cluster: distributed shared memory instead of L2 packets ----------------
+    // When all tiles of a member fit in one cluster (<= 16 CTAs), an edge value is written straight into the
+    // neighbour's border slot with st.async, which also credits its bytes to an mbarrier in the neighbour's shared
+    // memory; the neighbour waits on that mbarrier (one per colour; the bytes it expects per half-sweep are fixed).
+    // One hop of ~250 clocks instead of an L2 round trip, no polling of memory.  Every CTA runs the same number of
+    // half-sweeps and consumes every message right after its own half-sweep, so no message is ever left over.
+    unsigned ds_col = 0, ds_row = 0;     // shared-window address of my first target slot in the (identical) layout
+    unsigned ds_col_rank = 0, ds_row_rank = 0;
+    unsigned ds_bar = 0;                 // shared-window address of mbar[0]; mbar[1] follows
+    unsigned ds_phase = 0;               // bit c: parity of the phase of mbar[c] to wait for next
+
+    static __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+    static __device__ __forceinline__ unsigned ds_mapa(unsigned addr, unsigned rank) {
+        unsigned r;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+        return r;
+    }
+    static __device__ __forceinline__ void ds_store(unsigned raddr, double v, unsigned rbar) {
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(raddr),
+                     "l"(__double_as_longlong(v)), "r"(rbar)
+                     : "memory");
+    }
+    static __device__ __forceinline__ void ds_arm(unsigned bar, unsigned bytes) {
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    }
+    static __device__ __forceinline__ bool ds_test(unsigned bar, unsigned parity) {
+        unsigned ok;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+        return ok != 0u;
+    }
+    // bytes this tile receives per half-sweep (both colours alike: rows and BW are even)
+    static __device__ __forceinline__ unsigned ds_expected_bytes(const HaloLinks& L) {
+        return 8u * (unsigned)((L.e ? L.rows / 2 : 0) + (L.w ? L.rows / 2 : 0) + (L.n ? BW / 2 : 0) + (L.s ? BW / 2 : 0));
+    }
+    // mbar: two 8-byte mbarriers in shared memory, initialised (count 1) and armed by thread 0 before the cluster sync
+    __device__ __forceinline__ void ds_bind(const HaloLinks& L, const unsigned long long* mbar, int tile, int ntx) {
+        static_assert(TXN >= 2 && TYN >= 2, "halo mode: one edge per axis");
+        ds_bar = smem_u32(mbar);
+        if (!active) return;
+        if (a == 0 && L.w) { ds_col = smem_u32(exL + rowbase * LS + TXN + 1); ds_col_rank = tile - 1; h_west = true; h_scol = L.own; }
+        else if (a == TXN - 1 && L.e) { ds_col = smem_u32(exR + rowbase * LS); ds_col_rank = tile + 1; h_scol = L.own; }
+        if (b == 0 && L.s) { ds_row = smem_u32(exB + (size_t)(TYN + 1) * BW + 2 * a); ds_row_rank = tile - ntx; h_south = true; h_srow = L.own; }
+        else if (b == TYN - 1 && L.n) { ds_row = smem_u32(exT + 2 * a); ds_row_rank = tile + ntx; h_srow = L.own; }
+    }
+    template <int COL>
+    __device__ __forceinline__ void ds_send() const {
+        constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;
+        if (h_scol) {
+            const unsigned base = ds_mapa(ds_col, ds_col_rank), bar = ds_mapa(ds_bar + 8u * COL, ds_col_rank);
+#pragma unroll
+            for (int q = 0; q < H; ++q) {
+                const int pq = (q + COL) & 1;
+                if (h_west ? pq == 0 : pq == 1) ds_store(base + (unsigned)(q * LS * 8), h_west ? phi[q][0] : phi[q][3], bar);
+            }
+        }
+        if (h_srow) {
+            const unsigned bar = ds_mapa(ds_bar + 8u * COL, ds_row_rank);
+            if (h_south) {                   // my bottom row -> the south tile's north border
+                const unsigned base = ds_mapa(ds_row + (unsigned)(pb * PW * 8), ds_row_rank);
+                ds_store(base, phi[0][pb], bar);
+                ds_store(base + 8u, phi[0][pb + 2], bar);
+            } else {                         // my top row -> the north tile's south border
+                const unsigned base = ds_mapa(ds_row + (unsigned)(pt * PW * 8), ds_row_rank);
+                ds_store(base, phi[H - 1][pt], bar);
+                ds_store(base + 8u, phi[H - 1][pt + 2], bar);
+            }
+        }
+    }
+    // wait for the neighbours' edge cells of colour COL; thread `arm` re-arms the mbarrier for its next phase
+    template <int COL>
+    __device__ __forceinline__ void ds_recv(unsigned expect_bytes, bool arm, const PollCtx& pc) {
+        const unsigned bar = ds_bar + 8u * COL, parity = (ds_phase >> COL) & 1u;
+        unsigned spins = 0;
+        while (!ds_test(bar, parity)) {
+            if (poll_giveup(pc, spins, 6, (int)parity)) break;
+        }
+        ds_phase ^= 1u << COL;
+        if (arm) ds_arm(bar, expect_bytes);
     }
 
     // ---- block mode, small tiles: the whole owned patch travels as tagged packets once per interval ---------------

@@ -63,7 +63,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -91,7 +91,7 @@ struct sn_poisson {
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
     double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
-    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0, st_group = 0;
+    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0, st_group = 0, st_ds = 0;
     int last_sweeps0 = 0;
 };
 
@@ -363,29 +363,32 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
 struct ShapeInfo {
     int H, TXN, TYN, minb;
     size_t smem;
-    const void* fn[2];          // [0] block mode, [1] halo mode
+    const void* fn[3];          // [0] block mode, [1] halo mode, [2] halo mode inside one cluster (DSMEM) or NULL
     int BW() const { return 4 * TXN; }
     int BH() const { return H * TYN; }
     int NT() const { return TXN * TYN; }
     int threads() const { return TXN * TYN + 32; }     // + the service warp
 };
 
-template <int H, int TXN, int TYN, int MINB, bool EF = true>
+template <int H, int TXN, int TYN, int MINB, bool EF = true, bool DS = EF>
 ShapeInfo shape_of() {
+    const void* ds = nullptr;
+    if constexpr (DS) ds = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false, true>;   // no edge-first: one
+    // DSMEM hop is shorter than the extra pass costs (measured)
     return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes,
             {(const void*)k_sor_resident<H, TXN, TYN, MINB, false, false>,
-             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, EF>}};
+             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, EF>, ds}};
 }
 
 const std::vector<ShapeInfo>& shapes() {
     static const std::vector<ShapeInfo> v = {
-        shape_of<8, 32, 14, 1, false>(),   // 0: box 128 x 112, 448 threads (128-register cap: no edge-first)
-        shape_of<8, 32, 8, 1>(),    // 1: box 128 x 64,  256 threads
+        shape_of<8, 32, 14, 1, false, false>(),   // 0: box 128 x 112, 448 threads (128-register cap: no edge-first)
+        shape_of<8, 32, 8, 1, true, false>(),    // 1: box 128 x 64,  256 threads
         shape_of<8, 16, 8, 2>(),    // 2: box 64 x 64,   128 threads
         shape_of<4, 16, 8, 2>(),    // 3: box 64 x 32,   128 threads
         shape_of<4, 8, 8, 2>(),     // 4: box 32 x 32,    64 threads
         shape_of<2, 8, 16, 2>(),    // 5: box 32 x 32,   128 threads
-        shape_of<8, 32, 7, 2, false>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
+        shape_of<8, 32, 7, 2, false, false>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
         shape_of<4, 16, 16, 1>(),   // 7: box 64 x 64,   256 threads
         shape_of<6, 12, 8, 2>(),    // 8: box 48 x 48,    96 threads
         shape_of<4, 12, 16, 1>(),   // 9: box 48 x 64,   192 threads
@@ -394,7 +397,7 @@ const std::vector<ShapeInfo>& shapes() {
 }
 
 struct ResPlan {
-    int shape = -1, halo = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
+    int shape = -1, halo = 0, ds = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
     double cost = 0;
 };
 
@@ -410,6 +413,28 @@ double model_half_sweep(const ShapeInfo& S, int k) {
     double t = std::max(lat * (1.0 + 0.5 * (k - 1)), warps_per_smsp * dpw * 2.0 / 0.62 + 100.0);
     if (S.threads() * S.minb > 448 && k == 1 && S.H == 8 && S.NT() < 448) t = std::max(t, 1400.0);   // 128-register cap
     return t;
+}
+
+// Can `nclusters` clusters of `csize` CTAs of this shape be resident at once?
+bool cluster_fits(sn_poisson* h, const ShapeInfo& S, int csize, int nclusters) {
+    const void* fn = S.fn[2];
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
+        (csize > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
+        cudaGetLastError();
+        return false;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(csize, nclusters);
+    cfg.blockDim = dim3(S.threads());
+    cfg.dynamicSmemBytes = S.smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, fn, &cfg) != cudaSuccess) { cudaGetLastError(); return false; }
+    (void)h;
+    return n >= nclusters;
 }
 
 // Pick (shape, mode, m) minimising modelled clocks per sweep; honours the "shape" / "tblock" / "halo" overrides.
@@ -447,6 +472,23 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
                 if (best.shape < 0 || p.cost < best.cost) best = p;
             }
         }
+        // halo mode with all tiles of a member in ONE thread-block cluster: edges through distributed shared memory
+        if (h->opt_halo != 0 && h->opt_ds != 0 && S.fn[2] && h->nr % S.BW() == 0 && h->nz % S.H == 0) {
+            ResPlan p;
+            p.shape = si; p.halo = 1; p.ds = 1;
+            p.ntx = h->nr / S.BW(); p.nty = (h->nz + S.BH() - 1) / S.BH();
+            p.ow = S.BW(); p.oh = S.BH();
+            p.ntiles = p.ntx * p.nty;
+            p.Q = h->opt_tblock > 0 ? h->opt_tblock : kMaxTB;
+            p.m = p.Q;
+            if (p.ntiles > 1 && p.ntiles <= 16 && cluster_fits(h, S, p.ntiles, nbatch)) {
+                // per half-sweep: compute + the edge threads' st.async (~250 clocks) + one DSMEM hop and the mbarrier
+                // wake-up (~300); 420 puts the model where the measurements are (128^2: wins; 64^2, 256^2: block mode)
+                p.cost = 2.0 * (model_half_sweep(S, 1) + 420.0);
+                if (best.shape < 0 || p.cost < best.cost || h->opt_ds == 1) best = p;
+            }
+        }
+        if (h->opt_ds == 1 && best.ds) continue;
         if (h->opt_halo == 1) continue;
         // block mode: temporal blocking with margins of 2m cells
         for (int m = 1; m <= kMaxTB; ++m) {
@@ -502,7 +544,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * need_sync, st));
     CU_TRY(cudaMemsetAsync(h->d_slots_f + (size_t)member0 * 2 * h->cap_sweeps, 0,
                            sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
-    if (pl.halo || pl.ll) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
+    if ((pl.halo && !pl.ds) || pl.ll) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
     ResParams P;
     P.g = g;
     P.halo = pl.halo;
@@ -537,13 +579,29 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         h->prof_ctas = (size_t)pl.ntiles * nbatch;
     }
     void* args[] = {&P};
-    const void* fn = S.fn[pl.halo ? 1 : 0];
+    const void* fn = S.fn[pl.ds ? 2 : pl.halo ? 1 : 0];
     CU_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
-    CU_TRY(cudaLaunchCooperativeKernel(fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, S.smem, st));
+    if (pl.ds) {
+        // one cluster per member (gang-scheduled, so its CTAs are co-resident by construction; the clusters of a batch
+        // were checked against cudaOccupancyMaxActiveClusters by the planner)
+        if (pl.ntiles > 8) CU_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(pl.ntiles, nbatch);
+        cfg.blockDim = dim3(S.threads());
+        cfg.dynamicSmemBytes = S.smem;
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = pl.ntiles; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        CU_TRY(cudaLaunchKernelExC(&cfg, fn, args));
+    } else {
+        CU_TRY(cudaLaunchCooperativeKernel(fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, S.smem, st));
+    }
     h->st_launches += 1;
     h->st_path = 2;
     h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.Q;
-    h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch;
+    h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch; h->st_ds = pl.ds;
     return 0;
 }
 
@@ -557,6 +615,7 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     h->st_aux_launches = 0;
     h->st_path = 1;
     h->st_halo = 0;
+    h->st_ds = 0;
 
     CU_TRY(cudaEventRecord(h->ev_t[0], st));
     CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl) * nbatch, st));
@@ -870,6 +929,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
     if (!strcmp(key, "prof")) { h->opt_prof = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "ds")) { if (value < -1 || value > 1) { set_err("ds must be -1, 0 or 1"); return -1; } h->opt_ds = (int)value; return 0; }
     if (!strcmp(key, "group")) { if (value < -1 || value > 65535) { set_err("group must be -1, 0 or a member count"); return -1; } h->opt_group = (int)value; return 0; }
     if (!strcmp(key, "ll")) { if (value < -1 || value > 1) { set_err("ll must be -1, 0 or 1"); return -1; } h->opt_ll = (int)value; return 0; }
     if (!strcmp(key, "halo")) { if (value < -1 || value > 1) { set_err("halo must be -1, 0 or 1"); return -1; } h->opt_halo = (int)value; return 0; }
@@ -893,6 +953,7 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "tblock")) { *out = h->st_tblock; return 0; }
     if (!strcmp(key, "shape")) { *out = h->st_shape; return 0; }
     if (!strcmp(key, "halo")) { *out = h->st_halo; return 0; }
+    if (!strcmp(key, "ds")) { *out = h->st_ds; return 0; }
     if (!strcmp(key, "group")) { *out = h->st_group; return 0; }
     if (!strncmp(key, "prof_mean", 9) && key[9] >= '0' && key[9] <= '7' && !key[10]) { *out = h->prof_mean[key[9] - '0']; return 0; }
     if (!strncmp(key, "prof_max", 8) && key[8] >= '0' && key[8] <= '7' && !key[9]) { *out = h->prof_max[key[8] - '0']; return 0; }

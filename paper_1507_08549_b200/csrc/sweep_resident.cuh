@@ -119,7 +119,8 @@ struct ResShape {
 
 // grid = (ntx*nty, nbatch), block = TXN*TYN + 32 threads (the last warp is the service warp), cooperative launch.
 // EF (halo mode): update and send the patch-edge cells first (half_sweep_halo); only where registers allow it.
-template <int H, int TXN, int TYN, int MINB, bool HALO, bool EF>
+// DS (halo mode, all tiles of a member in one thread-block cluster): edges travel through distributed shared memory.
+template <int H, int TXN, int TYN, int MINB, bool HALO, bool EF, bool DS = false>
 __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResParams p) {
     using S = BoxShape<H, TXN, TYN>;
     using RS = ResShape<H, TXN, TYN>;
@@ -132,6 +133,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     __shared__ int s_bad;
     __shared__ int s_panic;        // watchdog tripped (here or in another CTA): every wait falls through
     __shared__ int s_zero;         // a quit word that never fires (endgame / replay polls)
+    __shared__ __align__(8) unsigned long long s_mbar[2];   // DS: one mbarrier per colour, credited by the neighbours' st.async
     __shared__ long long s_pf[8];  // in-kernel profile of thread 0 ("prof" option)
 
     const Geom& g = p.g;
@@ -152,7 +154,25 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         s_bad = 0; s_panic = 0; s_zero = 0;
         for (int i = 0; i < 8; ++i) s_pf[i] = 0;
     }
+    // DS: bytes this tile receives per half-sweep; thread 0 initialises and arms both mbarriers, and the whole cluster
+    // (service warps included, once) synchronises before anybody sends
+    unsigned ds_expect = 0;
+    if (DS) {
+        const int tx_ = tile % p.ntx, ty_ = tile / p.ntx;
+        const int rows_ = min(BH, g.nz - ty_ * BH);
+        ds_expect = 8u * (unsigned)((tx_ + 1 < p.ntx ? rows_ / 2 : 0) + (tx_ > 0 ? rows_ / 2 : 0) +
+                                    (ty_ + 1 < p.nty ? BW / 2 : 0) + (ty_ > 0 ? BW / 2 : 0));
+        if (tid == 0) {
+            for (int c = 0; c < 2; ++c) {
+                const unsigned bar = (unsigned)__cvta_generic_to_shared(&s_mbar[c]);
+                asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1u) : "memory");
+            }
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            for (int c = 0; c < 2; ++c) Engine::ds_arm((unsigned)__cvta_generic_to_shared(&s_mbar[c]), ds_expect);
+        }
+    }
     __syncthreads();
+    if (DS) asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 
     // =============================================================================================================
     // service warp
@@ -276,7 +296,8 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         links.s = (ty > 0) ? inbox(tile - p.ntx) : nullptr;
         links.n = (ty + 1 < p.nty) ? inbox(tile + p.ntx) : nullptr;
         links.rows = min(BH, g.nz - by);
-        E.halo_bind(links, tid);
+        if (DS) E.ds_bind(links, s_mbar, tile, p.ntx);
+        else E.halo_bind(links, tid);
     }
     // block mode: the tiles whose owned cells this box overlaps (their flags gate the margin refill)
     unsigned int* flags = p.flags + (size_t)member * ntiles;
@@ -364,24 +385,28 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             const long long t0 = tick();
             const unsigned tag0 = tagbase + 2u * (unsigned)(k0 + s) + 1u;
             if (HALO && EF) {
-                E.template half_sweep_halo<0, TRACK>(tag0);
+                E.template half_sweep_halo<0, TRACK, DS>(tag0);
             } else {
                 E.template half_sweep<0, TRACK, false>();
-                if (HALO) E.template halo_send<0>(tag0);
+                if (HALO && DS) E.template ds_send<0>();
+                else if (HALO) E.template halo_send<0>(tag0);
             }
             const long long t1 = tick();
-            if (HALO) E.template halo_recv<0>(tag0, pc);
+            if (HALO && DS) E.template ds_recv<0>(ds_expect, tid == 0, pc_end);      // never abandoned: see box_engine.cuh
+            else if (HALO) E.template halo_recv<0>(tag0, pc);
             const long long t2 = tick();
             Engine::sync();
             const long long t3 = tick();
             if (HALO && EF) {
-                E.template half_sweep_halo<1, TRACK>(tag0 + 1u);
+                E.template half_sweep_halo<1, TRACK, DS>(tag0 + 1u);
             } else {
                 E.template half_sweep<1, TRACK, false>();
-                if (HALO) E.template halo_send<1>(tag0 + 1u);
+                if (HALO && DS) E.template ds_send<1>();
+                else if (HALO) E.template halo_send<1>(tag0 + 1u);
             }
             const long long t4 = tick();
-            if (HALO) E.template halo_recv<1>(tag0 + 1u, pc);
+            if (HALO && DS) E.template ds_recv<1>(ds_expect, tid == 0, pc_end);
+            else if (HALO) E.template halo_recv<1>(tag0 + 1u, pc);
             const long long t5 = tick();
             Engine::sync();
             const long long t6 = tick();
@@ -466,6 +491,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     if (E.active) E.load_f(rho, g.nr, gi0, gj0);
     E.load_coeffs(g, gi0, E.active ? gj0 : 0);
     load_box(phi_io);
+    if (DS) grid_barrier();      // DS: neighbours write straight into my border slots -- not before they are loaded
 
     // ---- main phase: FAST maxima, decisions one interval late -------------------------------------------------
     int r_c = 1;                 // interval the endgame starts with
@@ -505,6 +531,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         if (reload) {
             grid_barrier();
             load_box(state_of(r_c - 1));
+            if (DS) grid_barrier();
             tagbase = kTagEndgame;
         }
         int r = r_c;
@@ -525,6 +552,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 if (fk != k0 + n) {                              // crossing inside the interval: replay from its start
                     grid_barrier();
                     load_box(state_of(r - 1));
+                    if (DS) grid_barrier();
                     run_sweeps(std::integral_constant<int, kTrackNone>{}, k0, fk - k0, kTagReplay, 0, pc_end);
                 }
                 break;
