@@ -224,8 +224,10 @@ def test_planner_choice_random_grids_bit_exact(P, torch_cuda, oracle):
 
 def test_resident_kernel_is_repeatable(P, torch_cuda):
     """The inter-CTA protocols (packets, flags, late decision, endgame) are timing dependent; the result must not be:
-    the same solve repeated gives the same bits, sweeps and residual every time (block mode and halo mode)."""
-    for w, opts in ((W.cfg2(256), {"path": 2}), (W.cfg3(128).first, {"path": 2, "halo": 1, "shape": 3})):
+    the same solve repeated gives the same bits, sweeps and residual every time (block mode, halo mode through L2
+    packets, halo mode through distributed shared memory)."""
+    for w, opts in ((W.cfg2(256), {"path": 2}), (W.cfg3(128).first, {"path": 2, "halo": 1, "shape": 3, "ds": 0}),
+                    (W.cfg1(128), {"path": 2, "halo": 1, "ds": 1})):
         s = P.PoissonSolver.for_workload(w)
         for k, v in opts.items():
             s.set_option(k, v)
