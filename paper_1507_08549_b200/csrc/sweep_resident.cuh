@@ -23,6 +23,9 @@
 //    the tile is stored to the checkpoint ring anyway; one release-store of a per-tile flag publishes it and the
 //    neighbours refill their margins with ordinary (pipelined) loads after an acquire-poll of the flags of the tiles
 //    their box overlaps.  Tiny tiles (H = 2, <= 256 cells) send their patches as tagged packets instead.
+//    Halo mode with all tiles of a member in ONE thread-block cluster (DS): the edge values go straight into the
+//    neighbour's border slots in distributed shared memory with st.async, which credits their bytes to an mbarrier
+//    (one per colour) the neighbour waits on -- ~580 clocks per exchange instead of ~2300 through L2.
 //  * a-3: per-sweep maxima of |res| and |phi_new| over the owned cells go warp -> CTA -> (service warp) atomicMax
 //    into per-sweep global slots.  An extra SERVICE WARP per CTA does all of that and the stopping decision, so the
 //    fences and L2 round trips of the reduction never stall the sweeps: the compute warps only hand it their maxima

@@ -607,3 +607,25 @@ def test_gravity_after_solve_and_batch(P, torch_cuda, oracle):
         assert relmax(gr[b].cpu().numpy(), want_r) <= REL and relmax(gz[b].cpu().numpy(), want_z) <= REL
     with pytest.raises(P.SnPoissonError):
         P.PoissonSolver.for_workload(w).gravity(torch_cuda.zeros((w.nz, w.nr), dtype=torch_cuda.float64, device="cuda"))
+
+
+@pytest.mark.parametrize("opts", [{"path": 2, "halo": 0}, {"path": 2, "halo": 1, "ds": 0, "shape": 4},
+                                  {"path": 2, "halo": 1, "ds": 1, "shape": 4}, {"path": 3}])
+def test_non_finite_input_stops_the_on_chip_paths(P, torch_cuda, oracle, opts):
+    """A NaN (or Inf) in rho poisons the upper-word maxima of the main phase; the exact endgame then finds the first
+    sweep with a non-finite ratio, like the oracle: status -3 at the same sweep, and the kernel terminates."""
+    w = W.random_smooth(128, 96, 1, seed=77, lmax=4)
+    for bad in (np.nan, np.inf):
+        rho = w.rho.copy()
+        rho[40, 70] = bad
+        ref = oracle.solve(rho, np.zeros_like(rho), w.dr, w.dz, 1, w.lmax, 1e-8, 500)
+        assert ref["status"] == -3
+        s = P.PoissonSolver(w.nr, w.nz, w.dr, w.dz, 1, w.lmax)
+        for k, v in opts.items():
+            s.set_option(k, v)
+        d_rho = torch_cuda.from_numpy(rho).cuda()
+        phi = torch_cuda.zeros_like(d_rho)
+        r = P.sn_poisson_solve(s.h, d_rho.data_ptr(), phi.data_ptr(), 1e-8, 500,
+                               torch_cuda.cuda.current_stream().cuda_stream)
+        assert s.stat("path") == opts["path"]
+        assert (r.status, r.sweeps) == (-3, ref["sweeps"])
