@@ -121,7 +121,8 @@ int sn_poisson_get_history(sn_poisson* h, double* R, int n);
  *   "halo"        path 2: 1 = halo mode (box == tile, edge exchange every half-sweep), 0 = block mode (margins of
  *                 2m cells, exchange every m sweeps), -1 = planner's choice
  *   "ds"          path 2 halo mode: 1 = all tiles of a member in one thread-block cluster (<= 16 tiles), edges through
- *                 distributed shared memory (st.async + mbarrier); 0 = never; -1 = planner's choice
+ *                 distributed shared memory (st.async + mbarrier), one cluster per batch member (any batch size: the
+ *                 clusters are independent); 0 = never; -1 = planner's choice
  *   "ll"          path 2 block mode: 1 = margins travel as tagged packets, 0 = tile flags + ring loads, -1 = auto
  *   "group"       batches on path 2: G > 0 = solve the batch in groups of G members, one resident launch after the
  *                 other; 0 = never group (all members co-resident or another path); -1 = group when the whole batch

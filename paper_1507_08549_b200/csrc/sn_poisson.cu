@@ -481,7 +481,9 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
             p.ntiles = p.ntx * p.nty;
             p.Q = h->opt_tblock > 0 ? h->opt_tblock : kMaxTB;
             p.m = p.Q;
-            if (p.ntiles > 1 && p.ntiles <= 16 && cluster_fits(h, S, p.ntiles, nbatch)) {
+            // members are independent and a cluster is gang-scheduled, so the clusters of a batch need not be
+            // co-resident with each other: any batch size runs, in waves of clusters if it has to
+            if (p.ntiles > 1 && p.ntiles <= 16 && cluster_fits(h, S, p.ntiles, 1)) {
                 // per half-sweep: compute + the edge threads' st.async (~250 clocks) + one DSMEM hop and the mbarrier
                 // wake-up (~300); 420 puts the model where the measurements are (128^2: wins; 64^2, 256^2: block mode)
                 p.cost = 2.0 * (model_half_sweep(S, 1) + 420.0);

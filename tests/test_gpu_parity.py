@@ -629,3 +629,20 @@ def test_non_finite_input_stops_the_on_chip_paths(P, torch_cuda, oracle, opts):
                                torch_cuda.cuda.current_stream().cuda_stream)
         assert s.stat("path") == opts["path"]
         assert (r.status, r.sweeps) == (-3, ref["sweeps"])
+
+
+def test_cluster_mode_batch_runs_in_waves(P, torch_cuda, oracle):
+    """A batch of small grids in the DSMEM halo mode: one cluster of 16 CTAs per member, more clusters than the chip
+    holds at once (members are independent, clusters are gang-scheduled).  Sampled members against the oracle."""
+    ws = [W.cfg4a_member(b, 128) for b in range(24)]
+    s = P.PoissonSolver.for_workload(ws[0])
+    for k, v in {"path": 2, "halo": 1, "ds": 1, "shape": 5}.items():
+        s.set_option(k, v)
+    rho = torch_cuda.from_numpy(np.stack([w.rho for w in ws])).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    res = s.solve(rho, phi, ws[0].tol, ws[0].max_sweeps)
+    assert s.stat("path") == 2 and s.stat("ds") == 1 and s.stat("ctas") == 16 * 24
+    assert all(r.status == 0 for r in res)
+    for b in (0, 11, 23):
+        ref = oracle.solve_workload(ws[b])
+        assert res[b].sweeps == ref["sweeps"] and relmax(phi[b].cpu().numpy(), ref["phi"]) <= REL
