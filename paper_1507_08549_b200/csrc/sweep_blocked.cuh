@@ -196,24 +196,29 @@ __global__ void __launch_bounds__(TXN* TYN, MINB) k_sor_blocked(const BlkParams 
         if (track == kTrackFast) {
             for (int s = 0; s < n; ++s) {
                 E.reset_maxima();
-                E.template sweep<kTrackFast>();
+                E.template half_sweep<0, kTrackFast>();
+                E.template half_sweep<1, kTrackFast, false>();
+                // warp reduction BEFORE the sweep's last barrier: its latency hides in the barrier wait
                 const unsigned wr = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres_f) : 0u);
                 const unsigned wp = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mphi_f) : 0u);
                 if (lane == 0) {
                     smax[(2 * s) * NW + warp] = wr;
                     smax[(2 * s + 1) * NW + warp] = wp;
                 }
+                E.sync();
             }
         } else if (track == kTrackExact) {
             for (int s = 0; s < n; ++s) {
                 E.reset_maxima();
-                E.template sweep<kTrackExact>();
+                E.template half_sweep<0, kTrackExact>();
+                E.template half_sweep<1, kTrackExact, false>();
                 const unsigned long long wr = warp_max_key(own ? E.mres_k : 0ull);
                 const unsigned long long wp = warp_max_key(own ? E.mphi_k : 0ull);
                 if (lane == 0) {
                     smax[(2 * s) * NW + warp] = wr;
                     smax[(2 * s + 1) * NW + warp] = wp;
                 }
+                E.sync();
             }
         } else {
             for (int s = 0; s < n; ++s) E.template sweep<kTrackNone>();

@@ -408,15 +408,8 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 else if (HALO) E.template halo_send<1>(tag0 + 1u);
             }
             const long long t4 = tick();
-            if (HALO && DS) E.template ds_recv<1>(ds_expect, tid == 0, pc_end);
-            else if (HALO) E.template halo_recv<1>(tag0 + 1u, pc);
-            const long long t5 = tick();
-            Engine::sync();
-            const long long t6 = tick();
-            if (prof_on) {
-                s_pf[1] += (t1 - t0) + (t4 - t3); s_pf[2] += (t2 - t1) + (t5 - t4); s_pf[3] += (t3 - t2) + (t6 - t5);
-                s_pf[7] += 2;
-            }
+            // the sweep's maxima are complete: reduce them across the warp BEFORE the last wait / barrier of the sweep,
+            // so that the REDUX latency (measured ~135 clocks per half-sweep when done after the barrier) hides in it
             if (TRACK == kTrackFast) {
                 const unsigned wr = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres_f) : 0u);
                 const unsigned wp = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mphi_f) : 0u);
@@ -431,6 +424,15 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                     smax[((size_t)par * 2 * kMaxTB + 2 * s) * NW + warp] = wr;
                     smax[((size_t)par * 2 * kMaxTB + 2 * s + 1) * NW + warp] = wp;
                 }
+            }
+            if (HALO && DS) E.template ds_recv<1>(ds_expect, tid == 0, pc_end);
+            else if (HALO) E.template halo_recv<1>(tag0 + 1u, pc);
+            const long long t5 = tick();
+            Engine::sync();
+            const long long t6 = tick();
+            if (prof_on) {
+                s_pf[1] += (t1 - t0) + (t4 - t3); s_pf[2] += (t2 - t1) + (t5 - t4); s_pf[3] += (t3 - t2) + (t6 - t5);
+                s_pf[7] += 2;
             }
         }
     };
