@@ -2,21 +2,28 @@
 """bench.py -- Poisson relaxation throughput (fp64 cell-updates/s) and time-to-residual per solve.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
-                    [--workload cfg0|cfg1|cfg2|cfg3|cfg3seq<N>|cfg4a|sweep<N>]
+                    [--workload cfg0|cfg1|cfg2|cfg3|cfg3seq<N>|cfg4a|sweep<N>] [--no-per-config]
 
 One "step" = one pass of the whole hot path over one synthetic input: multipole moments -> boundary fill ->
-red-black SOR sweeps with the fused residual reduction until the device-side stopping rule fires (cold start,
-phi = 0), through the C ABI (sn_poisson_solve / _solve_batch).  Default workload: BASELINE.json configs[1]
-(256x256 n=1 polytrope, lmax 16, tol 1e-10).  cfg3seq<N>: one step = the warm-started sequence of N solves of
-[CFG 3].  Prints ONE JSON line (rank 0).
+red-black SOR sweeps with the fused residual reduction until the device-side stopping rule fires, through the C ABI.
+Default workload at N = 1: [CFG 3] as specified -- the LARGEST single-GPU configuration of BASELINE.json: a sequence
+of 100 warm-started solves on the 1024x2048 full-plane grid (one step = the whole sequence).  With N > 1 the
+workload is the [CFG 4a] batch of 64 x 512^2, its members dealt across the ranks with no data-path collective
+(`scaling: strong`); `--gpus N` without torchrun spawns the N ranks itself.  Prints ONE JSON line (rank 0).
 
-Timing: W warm-up steps, then K steps each bracketed by CUDA events on the launching stream (the call
-synchronises that stream itself); L2 is flushed (a 256 MiB write) and phi re-zeroed between steps, outside the
-events; the K-step region is bracketed by barrier + torch.cuda.synchronize(); max over ranks.  `value` = all
-cell-updates of the K steps / that device time (inputs resident in HBM); `e2e` = the same with pinned HOST buffers,
-H2D / D2H inside the timed wall-clock region; `roofline` = 24 B x cell-updates of the relaxation kernel's launches /
-their device time (the library's own CUDA events) against the measured L2 / HBM peak; `cpu_baseline` = the oracle
-as it stands on one host core on a bounded sample.
+The same line carries `per_config`: every other configuration of BASELINE.json (cfg0, cfg1, cfg2, cfg3 cold, cfg4a,
+the size sweep 128..4096) measured the same way in the same run (>= 3 warm-ups, L2 flushed between timed solves),
+each with its own value / time / sweeps / roofline fraction / fp64-pipe fraction / redundancy / e2e.
+
+Timing: W warm-up steps, then K steps each bracketed by CUDA events on the launching stream (the call synchronises
+that stream itself); L2 is flushed (a 256 MiB write) and phi re-zeroed between steps, outside the events; the K-step
+region is bracketed by barrier + torch.cuda.synchronize(); max over ranks.  `value` = all cell-updates of the K steps
+/ that device time (inputs resident in HBM).  `e2e` = the same through the C ABI's HOST-buffer entry points
+(sn_poisson_solve_host / _solve_batch_host / _solve_sequence_host) with pinned host arrays, H2D + D2H inside the
+timed wall-clock region.  `roofline` = 24 B x cell-updates of the relaxation kernel's launches / their device time
+(the library's own CUDA events on the caller's stream) against the peak: HBM = MEASURED_PEAKS.json; L2 = the
+library's own probe kernels (sn_poisson_probe_l2: L2-resident copy, read + write bytes), measured live in this run.
+`cpu_baseline` = the oracle as it stands on one host core on a bounded sample.
 `--impl reference` times the CPU oracle (oracle/, single thread) on the same workload -- a deliberately slow
 program; parity and the roofline fraction are the headline, not that ratio.
 """
@@ -40,10 +47,14 @@ import workloads as W  # noqa: E402
 METRIC = "poisson_relaxation_cell_updates_per_s"
 UNIT = "cell-updates/s"
 BYTES_PER_UPDATE = 24.0     # phi read + f read + phi write
+FP64_UPDATES_PER_S = 148 * 64 * 1.965e9 / 7.0      # ALU ceiling: 7 fp64 instructions per update
+DEFAULT_WORKLOAD = "cfg3seq100"
+PER_CONFIG = ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "sweep128", "sweep256", "sweep512", "sweep1024", "sweep2048",
+              "sweep4096"]
 
 
 def make_workload(name: str):
-    """Returns (label, list of Workload members, description)."""
+    """Returns (label, list of Workload members | [Cfg3Sequence])."""
     if name == "cfg1":
         return "cfg1: 256x256 half-plane n=1 polytrope, lmax=16, tol=1e-10, cold start", [W.cfg1()]
     if name == "cfg0":
@@ -51,7 +62,7 @@ def make_workload(name: str):
     if name == "cfg2":
         return "cfg2: 512x512 half-plane n=3 WD + 20 bubbles, lmax=16, tol=1e-10, cold start", [W.cfg2()]
     if name == "cfg3":
-        return "cfg3: 1024x2048 full-plane offset WD, lmax=32, tol=1e-10, cold solve (first of the sequence)", \
+        return "cfg3 cold: 1024x2048 full-plane offset WD, lmax=32, tol=1e-10, first (cold) solve of the sequence", \
             [W.cfg3().first]
     if name.startswith("cfg3seq"):
         n = int(name[7:] or 100)
@@ -118,33 +129,26 @@ def measured_peaks():
 
 
 def profiled_traffic(workload: str, kernel: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), or None."""
-    p = os.path.join(ROOT, "profiles", "r01b_traffic.json")
-    try:
-        e = json.load(open(p)).get(workload)
-    except (OSError, ValueError):
-        return None
-    return float(e["traffic_bytes_per_launch"]) if e and e.get("kernel") == kernel else None
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full captures (profiles/), or None."""
+    for fn in ("r02_traffic.json", "r01b_traffic.json"):
+        try:
+            e = json.load(open(os.path.join(ROOT, "profiles", fn))).get(workload)
+        except (OSError, ValueError):
+            continue
+        if e and e.get("kernel") == kernel:
+            return float(e["traffic_bytes_per_launch"])
+    return None
 
 
-def l2_copy_peak_gbs(torch, mib=24, iters=40):
-    """L2-resident copy bandwidth (read + write bytes), measured live the way MEASURED_PEAKS.json measures HBM:
-    b.copy_(a) with a working set (2 x `mib` MiB) that stays in the 126 MB L2; best of several."""
-    n = mib * (1 << 20) // 8
-    a = torch.ones(n, dtype=torch.float64, device="cuda")
-    b = torch.empty_like(a)
-    for _ in range(5):
-        b.copy_(a)
-    best = 0.0
-    for _ in range(5):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(iters):
-            b.copy_(a)
-        e1.record()
-        torch.cuda.synchronize()
-        best = max(best, 2.0 * n * 8 * iters / (e0.elapsed_time(e1) * 1e-3) / 1e9)
-    return best
+def l2_peaks(P, stream, n=3):
+    """L2-resident bandwidth from the library's own probe kernels (copy: read + write bytes over 2 x 32 MiB; read:
+    32 MiB), n independent measurements: best copy figure = the denominator, plus the run-to-run spread."""
+    cs, rs = [], []
+    for _ in range(n):
+        c, r = P.sn_poisson_probe_l2(32, stream)
+        cs.append(c)
+        rs.append(r)
+    return {"copy": max(cs), "read": max(rs), "copy_min": min(cs), "read_min": min(rs), "n": n}
 
 
 def oracle_rate(members, budget_s=12.0):
@@ -166,7 +170,7 @@ def oracle_rate(members, budget_s=12.0):
     t0 = time.perf_counter()
     O.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, w.symmetry, w.lmax, 0.0, nsw, omega=w.omega)
     dt = time.perf_counter() - t0
-    return nsw * w.cells / dt, f"moments+boundary+{nsw} sweeps of {w.name} ({w.nr}x{w.nz})"
+    return nsw * w.cells / dt, f"moments+boundary+{nsw} sweeps of {w.name} ({w.nr}x{w.nz}), first solve of the workload"
 
 
 def run_reference(args, label, members):
@@ -202,7 +206,8 @@ def run_reference(args, label, members):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "higher_is_better": True, "scaling": "weak" if args.gpus == 1 else "strong", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
         "config": {"workload": label},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -210,19 +215,193 @@ def run_reference(args, label, members):
     }))
 
 
+class Bench:
+    """Measures one workload on this rank's GPU through the C ABI."""
+
+    def __init__(self, torch, P, peaks, path=0):
+        self.torch, self.P, self.peaks, self.path = torch, P, peaks, path
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def measure(self, name, members, steps, warmup, e2e_steps, barrier=None, sampler=None):
+        """Returns a dict of raw numbers for this rank: device-timed steps, e2e through the host entry points, the
+        library's counters.  `members`: list of Workloads (a batch if > 1) or [Cfg3Sequence]."""
+        torch, P = self.torch, self.P
+        seq = members[0] if hasattr(members[0], "first") else None
+        mine = [seq.first] if seq is not None else members
+        w0, nb = mine[0], len(mine)
+        cells = w0.cells
+        solver = P.PoissonSolver.for_workload(w0)
+        if self.path:
+            solver.set_option("path", self.path)
+        rho_h = np.stack([m.rho for m in mine]) if nb > 1 else w0.rho
+        if seq is not None:
+            rhos, r_t = [w0.rho], w0.rho
+            for t in range(1, seq.nsteps):
+                r_t = seq.step(r_t, t)
+                rhos.append(r_t)
+            rho_h = np.stack(rhos)                        # (nsteps, nz, nr)
+            del rhos
+        rho_pin = torch.from_numpy(rho_h).pin_memory()    # e2e reads these; the device copy feeds the device-timed run
+        rho = rho_pin.cuda()
+        phi = torch.zeros((nb, w0.nz, w0.nr) if nb > 1 else (w0.nz, w0.nr), dtype=torch.float64, device="cuda")
+        acc = {"sweep_ms": 0.0, "setup_ms": 0.0, "launches": 0, "sweep_launches": 0}
+
+        def solve_dev():
+            for k in acc:
+                acc[k] = 0
+            out = []
+            for rt in (rho if seq is not None else [rho]):
+                res = solver.solve(rt, phi, w0.tol, w0.max_sweeps)        # phi carries over inside a sequence
+                out += res if isinstance(res, list) else [res]
+                for k in acc:
+                    acc[k] += solver.stat(k)
+            return out
+
+        for _ in range(warmup):
+            phi.zero_()
+            solve_dev()
+        step_ms, sweep_ms, setup_ms, launches, updates, sweep_launches = [], [], [], 0, 0, 0
+        results = None
+        if barrier:
+            barrier()
+        if sampler:
+            sampler.start()
+        t_region = time.perf_counter()
+        for _ in range(steps):
+            phi.zero_()
+            self.flush.fill_(1)                               # L2 flush between timed iterations
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            results = solve_dev()
+            e1.record()
+            torch.cuda.synchronize()
+            step_ms.append(e0.elapsed_time(e1))
+            sweep_ms.append(acc["sweep_ms"])
+            setup_ms.append(acc["setup_ms"])
+            launches += int(acc["launches"])
+            sweep_launches = int(acc["sweep_launches"])
+            updates += sum(r.sweeps for r in results) * cells
+        if barrier:
+            barrier()
+        region_s = time.perf_counter() - t_region
+        clocks = sampler.stop() if sampler else None
+        assert all(r.status == 0 for r in results), results
+
+        # ---- end to end: pinned HOST buffers through the C ABI's host entry points, H2D + D2H inside the timed region
+        rho_np = rho_pin.numpy()
+        e2e_ms, e2e_upd = [], 0
+        if seq is not None:
+            phi_io = torch.zeros(w0.rho.shape, dtype=torch.float64).pin_memory()
+            phi_all = torch.zeros(rho_h.shape, dtype=torch.float64).pin_memory()
+            api = "sn_poisson_solve_sequence_host"
+            h2d, d2h = rho_h.size * 8 + cells * 8, rho_h.size * 8 + cells * 8
+
+            def call():
+                phi_io.zero_()
+                return solver.solve_sequence_host(rho_np, phi_io.numpy(), w0.tol, w0.max_sweeps, phi_all.numpy())
+        else:
+            phi_io = torch.zeros(rho_h.shape, dtype=torch.float64).pin_memory()
+            api = "sn_poisson_solve_batch_host" if nb > 1 else "sn_poisson_solve_host"
+            h2d, d2h = 2 * rho_h.size * 8, rho_h.size * 8
+
+            def call():
+                phi_io.zero_()
+                r = solver.solve_host(rho_np, phi_io.numpy(), w0.tol, w0.max_sweeps)
+                return r if isinstance(r, list) else [r]
+        for i in range(1 + e2e_steps):                        # 1 warm-up: staging allocation, copy stream
+            self.flush.fill_(1)
+            torch.cuda.synchronize()
+            phi_io.zero_()
+            t0 = time.perf_counter()
+            res = call()
+            dt = time.perf_counter() - t0
+            if i >= 1:
+                e2e_ms.append(dt * 1e3)
+                e2e_upd += sum(r.sweeps for r in res) * cells
+        path = int(solver.stat("path"))
+        info = {
+            "name": name, "cells": cells, "nb": nb, "grid": [w0.nr, w0.nz], "lmax": w0.lmax, "tol": w0.tol,
+            "step_ms": step_ms, "sweep_ms": sweep_ms, "setup_ms": setup_ms, "launches": launches,
+            "sweep_launches": sweep_launches, "updates": updates, "results": results, "region_s": region_s,
+            "clocks": clocks, "e2e_ms": e2e_ms, "e2e_upd": e2e_upd, "e2e_api": api, "h2d": h2d, "d2h": d2h,
+            "path": path, "tblock": int(solver.stat("tblock")), "ctas": int(solver.stat("ctas")),
+            "halo": int(solver.stat("halo")), "ds": int(solver.stat("ds")), "group": int(solver.stat("group")),
+            "tile": [int(solver.stat("tile_w")), int(solver.stat("tile_h"))],
+            "redundancy": float(solver.stat("redundancy")), "working_set": 16.0 * cells * nb,
+        }
+        solver.close()
+        del rho, phi, rho_pin
+        torch.cuda.empty_cache()
+        return info
+
+    def roofline(self, info, value):
+        """Roofline of the dominant kernel (the relaxation sweep) from the library's own CUDA events on the stream."""
+        sw_ms = float(np.mean(info["sweep_ms"]))
+        sweeps_per_step = sum(r.sweeps for r in info["results"])
+        nl = max(1, info["sweep_launches"])
+        alg = BYTES_PER_UPDATE * sweeps_per_step * info["cells"] / nl
+        achieved = alg / (sw_ms * 1e-3 / nl) / 1e9
+        hbm_peak, hbm_src = self.peaks["hbm"], self.peaks["hbm_src"]
+        kernel = {1: "k_halfsweep", 2: "k_sor_resident", 3: "k_sor_blocked"}[info["path"]]
+        if info["working_set"] > 100e6:
+            bound, peak, src, extra = "hbm", hbm_peak, hbm_src, {}
+        else:
+            l2 = self.peaks["l2"]
+            bound, peak = "l2", l2["copy"]
+            src = ("sn_poisson_probe_l2: L2-resident copy of the library's own probe kernel (2 x 32 MiB, read + write "
+                   "bytes), best of %d, measured live in this run (of measured)" % l2["n"])
+            extra = {"peak_read": l2["read"], "peak_spread": [l2["copy_min"], l2["copy"]],
+                     "frac_of_read_peak": achieved / l2["read"]}
+        return {"bound": bound, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": profiled_traffic(info["name"], kernel), "kernel": kernel,
+                "alg_bytes_per_launch": alg, "launch_ms": sw_ms / nl, "sweep_launches_per_step": nl,
+                "peak_source": src, "frac_of_hbm_peak": achieved / hbm_peak,
+                # the limiter once phi stays on chip: 7 fp64 instructions per update against 64 lanes / clock / SM
+                # (DESIGN.md section 6); for information, the judged fraction is `frac`
+                "fp64_pipe_frac": value / FP64_UPDATES_PER_S, **extra}
+
+    @staticmethod
+    def config_of(info, label, scaling="weak", world=1):
+        path = info["path"]
+        return {"workload": label, "grid": info["grid"], "batch_per_gpu": info["nb"], "lmax": info["lmax"],
+                "tol": info["tol"], "l2": "flushed between timed solves (256 MiB write)",
+                "path": {1: "streaming", 2: "resident", 3: "blocked"}.get(path, str(path)),
+                "tblock": info["tblock"], "ctas": info["ctas"],
+                "mode": (("cluster-halo" if info["ds"] else "halo") if info["halo"] else "block") if path == 2 else None,
+                "tile": info["tile"], "redundancy": info["redundancy"], "group": info["group"],
+                "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"}
+
+
+def spawn_ranks(args):
+    """`--gpus N` without torchrun: start the N ranks (one process per GPU) the way the driver would."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg1")
+    ap.add_argument("--workload", default=None)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 streaming kernels, 2 resident kernel, 3 blocked kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
-
-    label, members = make_workload(args.workload)
+    world_env = os.environ.get("WORLD_SIZE")
+    if args.impl == "b200" and args.gpus > 1 and world_env is None:
+        spawn_ranks(args)
+    world = int(world_env or "1")
+    # N > 1: the one workload that shards (independent solves, no collective) -- the [CFG 4a] batch
+    wl_name = args.workload or (DEFAULT_WORKLOAD if max(world, args.gpus) == 1 else "cfg4a")
+    label, members = make_workload(wl_name)
     if args.impl == "reference":
         run_reference(args, label, members)
         return
@@ -236,7 +415,6 @@ def main():
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -251,131 +429,27 @@ def main():
     # multi-GPU: batch members are sharded across ranks with no collective; a single solve runs as replicas
     idx, scaling = shard_members(len(members), rank, world)
     mine = [members[i] for i in idx]
-    seq = None
-    if hasattr(mine[0], "first"):                     # cfg3 sequence: rho_t precomputed on the host, solves in order
-        seq = mine[0]
-        mine = [seq.first]
-    w0 = mine[0]
-    nb = len(mine)
-    solver = P.PoissonSolver.for_workload(w0)
-    if args.path:
-        solver.set_option("path", args.path)
-    rho_h = np.stack([m.rho for m in mine]) if nb > 1 else w0.rho
-    rho = torch.from_numpy(rho_h).cuda()
-    phi = torch.zeros_like(rho)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    cells = w0.cells
-
-    rho_seq = None
-    if seq is not None:
-        rhos, r_t = [w0.rho], w0.rho
-        for t in range(1, seq.nsteps):
-            r_t = seq.step(r_t, t)
-            rhos.append(r_t)
-        rho_seq = [torch.from_numpy(r).cuda() for r in rhos]
-
-    acc = {"sweep_ms": 0.0, "setup_ms": 0.0, "launches": 0, "sweep_launches": 0}
-
-    def solve_dev():
-        """One step: one solve (or batch), or the whole warm-started sequence; accumulates the library's counters."""
-        for k in acc:
-            acc[k] = 0
-        out = []
-        for rt in (rho_seq if rho_seq is not None else [rho]):
-            res = solver.solve(rt, phi, w0.tol, w0.max_sweeps)        # phi carries over inside a sequence
-            out += res if isinstance(res, list) else [res]
-            for k in acc:
-                acc[k] += solver.stat(k)
-        return out
+    stream = torch.cuda.current_stream().cuda_stream
+    hbm_peak, hbm_src = measured_peaks()
+    peaks = {"hbm": hbm_peak, "hbm_src": hbm_src, "l2": l2_peaks(P, stream)}
+    bench = Bench(torch, P, peaks, args.path)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        phi.zero_()
-        solve_dev()
+    long_step = hasattr(mine[0], "first") or len(mine) > 1
+    info = bench.measure(wl_name, mine, args.steps, args.warmup, min(args.steps, 3 if long_step else 20),
+                         barrier=barrier, sampler=ClockSampler(local_rank))
 
-    sampler = ClockSampler(local_rank)
-    step_ms, sweep_ms, setup_ms, launches, updates = [], [], [], 0, 0
-    results = None
-    barrier()
-    sampler.start()
-    t_region = time.perf_counter()
-    for _ in range(args.steps):
-        phi.zero_()
-        flush.fill_(1)                                    # L2 flush between timed iterations
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        results = solve_dev()
-        e1.record()
-        torch.cuda.synchronize()
-        step_ms.append(e0.elapsed_time(e1))
-        sweep_ms.append(acc["sweep_ms"])
-        setup_ms.append(acc["setup_ms"])
-        launches += int(acc["launches"])
-        updates += sum(r.sweeps for r in results) * cells
-    barrier()
-    region_s = time.perf_counter() - t_region
-    clocks = sampler.stop()
-    assert all(r.status == 0 for r in results), results
-
-    # end to end with HOST buffers (pinned), H2D + D2H inside the timed region.  Single solve: through the C ABI
-    # (sn_poisson_solve_host).  Batch / sequence: every solve's rho goes host -> device and its phi device -> host
-    # around the device call (what a hydro step that lives on the host does).
-    has_e2e = True
-    e2e_ms, e2e_upd, h2d_bytes, d2h_bytes = [], 0, 0, 0
-    if nb == 1 and seq is None:
-        rho_pin = torch.from_numpy(w0.rho).pin_memory()
-        phi_pin = torch.zeros(w0.rho.shape, dtype=torch.float64).pin_memory()
-        rho_np, phi_np = rho_pin.numpy(), phi_pin.numpy()
-        h2d_bytes, d2h_bytes = 2 * cells * 8, cells * 8
-        for i in range(args.warmup + args.steps):
-            phi_np[...] = 0.0
-            flush.fill_(1)
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            r = solver.solve_host(rho_np, phi_np, w0.tol, w0.max_sweeps)
-            dt = time.perf_counter() - t0
-            if i >= args.warmup:
-                e2e_ms.append(dt * 1e3)
-                e2e_upd += r.sweeps * cells
-    else:
-        host_rhos = ([torch.from_numpy(r).pin_memory() for r in rhos] if seq is not None
-                     else [torch.from_numpy(rho_h).pin_memory()])
-        phi_host = torch.zeros(rho.shape, dtype=torch.float64).pin_memory()
-        rho_dev = torch.empty_like(rho)
-        n_e2e = min(args.steps, 3)                        # these steps are long; a few suffice
-        h2d_bytes = sum(t.numel() * 8 for t in host_rhos) + phi_host.numel() * 8
-        d2h_bytes = len(host_rhos) * phi_host.numel() * 8
-        for i in range(1 + n_e2e):
-            phi_host.zero_()
-            flush.fill_(1)
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            phi.copy_(phi_host, non_blocking=True)
-            sw = 0
-            for hr in host_rhos:
-                rho_dev.copy_(hr, non_blocking=True)
-                res = solver.solve(rho_dev, phi, w0.tol, w0.max_sweeps)
-                sw += sum(x.sweeps for x in res) if isinstance(res, list) else res.sweeps
-                phi_host.copy_(phi, non_blocking=True)
-                torch.cuda.synchronize()
-            dt = time.perf_counter() - t0
-            if i >= 1:
-                e2e_ms.append(dt * 1e3)
-                e2e_upd += sw * cells
-    e2e_time = sum(e2e_ms) * 1e-3
-    e2e_steps = len(e2e_ms)
-
-    total_ms = float(sum(step_ms))
-    counters = [float(updates), float(launches), float(e2e_upd)]
+    total_ms = float(sum(info["step_ms"]))
+    e2e_time = sum(info["e2e_ms"]) * 1e-3
+    counters = [float(info["updates"]), float(info["launches"]), float(info["e2e_upd"])]
     dev = torch.device("cuda", local_rank)
     total_ms, (updates_all, launches_all, e2e_upd_all) = reduce_timing(total_ms, counters, world, dev)
     e2e_time_all, _ = reduce_timing(e2e_time * 1e3, [], world, dev)
     e2e_time_all *= 1e-3
-    launches_all = int(launches_all)
 
     if rank != 0:
         if world > 1:
@@ -383,55 +457,50 @@ def main():
         return
 
     value = updates_all / (total_ms * 1e-3)
-    # roofline of the dominant kernel (the relaxation sweep), from the library's own CUDA events on the stream
-    path = int(solver.stat("path"))
-    sw_ms = float(np.mean(sweep_ms))
-    sweeps_per_step = sum(r.sweeps for r in results)
-    sweep_launches = max(1, int(acc["sweep_launches"]))
-    alg_bytes_per_launch = BYTES_PER_UPDATE * sweeps_per_step * cells / sweep_launches
-    achieved = alg_bytes_per_launch / (sw_ms * 1e-3 / sweep_launches) / 1e9
-    hbm_peak, hbm_src = measured_peaks()
-    working_set = 16.0 * cells * nb
-    if working_set > 100e6:
-        bound, peak, src = "hbm", hbm_peak, hbm_src
-    else:
-        bound, peak = "l2", l2_copy_peak_gbs(torch)
-        src = "L2-resident torch copy (2 x 24 MiB, read+write bytes), measured live in this run (of measured)"
-    kernel = {1: "k_halfsweep", 2: "k_sor_resident", 3: "k_sor_blocked"}[path]
-    roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": profiled_traffic(args.workload, kernel), "kernel": kernel,
-                "alg_bytes_per_launch": alg_bytes_per_launch, "launch_ms": sw_ms / sweep_launches,
-                "sweep_launches_per_step": sweep_launches, "peak_source": src,
-                "frac_of_hbm_peak": achieved / hbm_peak,
-                # the limiter once phi stays on chip: 7 fp64 instructions per update against 64 lanes / clock / SM
-                # (DESIGN.md section 6); for information, the judged fraction is `frac`
-                "fp64_pipe_frac": value * 7.0 / (148 * 64 * 1.965e9)}
-
+    results = info["results"]
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": label, "grid": [w0.nr, w0.nz], "batch_per_gpu": nb, "lmax": w0.lmax,
-                   "tol": w0.tol, "l2": "flushed between timed solves (256 MiB write)",
-                   "path": {1: "streaming", 2: "resident", 3: "blocked"}.get(path, str(path)),
-                   "tblock": int(solver.stat("tblock")), "ctas": int(solver.stat("ctas")),
-                   "mode": ("halo" if solver.stat("halo") else "block") if path == 2 else None,
-                   "tile": [int(solver.stat("tile_w")), int(solver.stat("tile_h"))],
-                   "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"},
-        "time_to_residual_ms": total_ms / args.steps, "sweeps_per_solve": [r.sweeps for r in results][:8],
+        "config": Bench.config_of(info, label, scaling, world),
+        # per solve: a sequence runs its solves one after the other, a batch runs its members concurrently
+        "time_to_residual_ms": total_ms / args.steps / (len(results) if info["nb"] == 1 else 1),
+        "sweeps_per_solve": [r.sweeps for r in results][:8],
         "solves_per_step": len(results), "sweeps_per_step": sum(r.sweeps for r in results),
-        "final_residual": results[0].residual,
-        "setup_ms": float(np.mean(setup_ms)), "sweep_ms": sw_ms,
-        "gpu_launches": launches_all, "clocks": clocks, "roofline": roofline,
-        "region_wall_s": region_s,
+        "final_residual": results[-1].residual,
+        "setup_ms": float(np.mean(info["setup_ms"])), "sweep_ms": float(np.mean(info["sweep_ms"])),
+        "gpu_launches": int(launches_all), "clocks": info["clocks"],
+        "roofline": bench.roofline(info, value / world),
+        "region_wall_s": info["region_s"],
     }
     out["e2e"] = {"value": e2e_upd_all / e2e_time_all, "unit": UNIT,
-                  "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
-                  "ms_per_step": e2e_time_all / e2e_steps * 1e3, "steps": e2e_steps,
-                  "api": "sn_poisson_solve_host" if (nb == 1 and seq is None) else
-                         "pinned tensor.copy_ + sn_poisson_solve / _solve_batch + copy back, per solve"}
+                  "h2d_bytes_per_step": info["h2d"], "d2h_bytes_per_step": info["d2h"],
+                  "ms_per_step": e2e_time_all / len(info["e2e_ms"]) * 1e3, "steps": len(info["e2e_ms"]),
+                  "api": info["e2e_api"]}
+    if not args.no_per_config and world == 1:
+        rows = []
+        for name in PER_CONFIG:
+            lab, mem = make_workload(name)
+            big = name in ("cfg4a", "sweep2048", "sweep4096", "cfg3")
+            inf = bench.measure(name, mem, 3 if big else 10, 3, 2 if big else 5)
+            ms = float(np.mean(inf["step_ms"]))
+            v = inf["updates"] / (sum(inf["step_ms"]) * 1e-3)
+            rf = bench.roofline(inf, v)
+            rows.append({"workload": name, "label": lab, "value": v, "ms_per_step": ms,
+                         "sweeps": [r.sweeps for r in inf["results"]][:4], "solves": len(inf["results"]),
+                         "sweep_ms": float(np.mean(inf["sweep_ms"])), "setup_ms": float(np.mean(inf["setup_ms"])),
+                         "bound": rf["bound"], "frac": rf["frac"], "peak": rf["peak"], "achieved": rf["achieved"],
+                         "fp64_pipe_frac": rf["fp64_pipe_frac"], "frac_of_hbm_peak": rf["frac_of_hbm_peak"],
+                         "clocks_per_sweep_1965MHz": (float(np.mean(inf["sweep_ms"])) * 1e-3 * 1.965e9 /
+                                                      max(1, inf["results"][0].sweeps)) if inf["nb"] == 1 else None,
+                         "config": Bench.config_of(inf, lab),
+                         "e2e": {"value": inf["e2e_upd"] / (sum(inf["e2e_ms"]) * 1e-3),
+                                 "ms_per_step": float(np.mean(inf["e2e_ms"])), "api": inf["e2e_api"],
+                                 "h2d_bytes_per_step": inf["h2d"], "d2h_bytes_per_step": inf["d2h"]},
+                         "gpu_launches_per_step": inf["launches"] // max(1, len(inf["step_ms"]))})
+        out["per_config"] = rows
     if not args.no_cpu_baseline and world == 1:
-        v, sample = oracle_rate(mine)
+        v, sample = oracle_rate([mine[0].first] if hasattr(mine[0], "first") else mine)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
                                "host_cores_available": os.cpu_count()}
     print(json.dumps(out))

@@ -73,11 +73,34 @@ sn_poisson_result sn_poisson_solve(sn_poisson* h, const double* rho, double* phi
 sn_poisson_result sn_poisson_solve_host(sn_poisson* h, const double* rho_host, double* phi_inout_host,
                                         double tol, int max_sweeps, void* stream);
 
+/* Limits: max_sweeps <= 4194304 (2^22) and max_sweeps x nbatch <= 2^26 -- the handle keeps 32 bytes of per-sweep
+ * bookkeeping (maxima slots, R_k history) per member; larger values are rejected with status -1. */
+
 /* nbatch independent solves on the same grid geometry ([CFG 4a]).  rho, phi_inout: DEVICE pointers to nbatch
  * consecutive grids (member b at offset b*nr*nz).  out: HOST array of nbatch results.
  * Returns 0, or a negative status if the call itself failed. */
 int sn_poisson_solve_batch(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double tol,
                            int max_sweeps, void* stream, sn_poisson_result* out);
+
+/* sn_poisson_solve_batch with HOST buffers (pageable or pinned; layout as above).  rho is uploaded on `stream`,
+ * phi's upload overlaps the moment / boundary kernels on an internal copy stream, phi's download is enqueued right
+ * behind the relaxation; ONE stream synchronisation per call.  sn_poisson_solve_host is the nbatch = 1 case.
+ * Device staging is grown on demand and kept on the handle.  Returns 0 or a negative status. */
+int sn_poisson_solve_batch_host(sn_poisson* h, int nbatch, const double* rho_host, double* phi_inout_host,
+                                double tol, int max_sweeps, void* stream, sn_poisson_result* out);
+
+/* A warm-started SEQUENCE of nsteps solves on one grid ([CFG 3]: rho evolves, every solve starts from the previous
+ * phi), HOST buffers:
+ *   rho_seq_host    [nsteps][nr*nz]  the density of every step (read-only)
+ *   phi_inout_host  [nr*nz]          initial guess of step 0 on entry, the potential of the LAST step on exit
+ *   phi_seq_host    [nsteps][nr*nz]  the potential after every step, or NULL if only the last one is wanted
+ *   out             [nsteps]         HOST array of results
+ * Copy-compute overlap: rho_{t+1} is uploaded on an internal copy stream while solve t runs, and phi_t is downloaded
+ * from a device snapshot while solve t+1 runs (moments are recomputed every step).  Stops early (returning 0) at the
+ * first step whose status is < 0; later entries of `out` are then untouched.  Returns 0 or a negative status. */
+int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_seq_host, double* phi_inout_host,
+                                   double* phi_seq_host, double tol, int max_sweeps, void* stream,
+                                   sn_poisson_result* out);
 
 void sn_poisson_destroy(sn_poisson* h);
 
@@ -136,9 +159,16 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value);
 /* Counters of the last solve / batch: "launches" (kernels launched), "sweep_launches" (those that ran relaxation
  * sweeps), "sweep_ms" (device time of the relaxation phase, CUDA events on the caller's stream), "setup_ms"
  * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo", "ds",
- * "group" (members per resident launch).
+ * "group" (members per resident launch), "redundancy" (cells updated per half-sweep / cells of the grid: 1 in halo
+ * mode and on the streaming path, box cells / tile cells with temporal blocking).
  * Returns 0 or -1. */
 int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out);
+
+/* Measurement aid (no handle, not part of the solve path): L2-resident bandwidth of this GPU in GB/s, measured with
+ * two plain kernels of the library over a working set of 2 x `mib` MiB (copy: read + write bytes) / `mib` MiB (read).
+ * the L2 peak is not in MEASURED_PEAKS.json and must be measured on the box; bench.py uses
+ * the copy figure as the roofline denominator of the L2-bound rows.  Synchronises `stream`.  Returns 0 / -1 / -2. */
+int sn_poisson_probe_l2(int mib, double* copy_gbs, double* read_gbs, void* stream);
 
 /* Message of the last failure on this thread ("" if none). */
 const char* sn_poisson_last_error(void);

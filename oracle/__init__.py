@@ -8,6 +8,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
+import platform
 import subprocess
 
 import numpy as np
@@ -15,7 +16,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "sn_oracle.cpp")
 _LIB = os.path.join(_HERE, "libsn_oracle.so")
-CXXFLAGS = ["-O2", "-ffp-contract=off", "-mfma", "-fPIC", "-shared", "-std=c++17"]
+CXXFLAGS = ["-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c++17"]
+if platform.machine() in ("x86_64", "AMD64"):
+    CXXFLAGS.insert(2, "-mfma")              # std::fma as one instruction; aarch64 has fused multiply-add in the base ISA
 
 _lib = None
 _dp = C.POINTER(C.c_double)

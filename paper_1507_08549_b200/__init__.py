@@ -7,7 +7,8 @@ from .binding import (EXPORTS, LIB_PATH, SnPoissonError, load, sn_poisson_create
                       sn_poisson_get_omega, sn_poisson_get_stat, sn_poisson_gravity, sn_poisson_last_error,
                       sn_poisson_result,
                       sn_poisson_set_boundary, sn_poisson_set_omega, sn_poisson_set_option, sn_poisson_solve,
-                      sn_poisson_solve_batch, sn_poisson_solve_host, sn_poisson_version)
+                      sn_poisson_solve_batch, sn_poisson_solve_batch_host, sn_poisson_solve_host,
+                      sn_poisson_solve_sequence_host, sn_poisson_probe_l2, sn_poisson_version)
 from .solver import PoissonSolver
 
 __all__ = ["PoissonSolver", "SnPoissonError", "EXPORTS", "LIB_PATH", "load", "sn_poisson_result"] + list(EXPORTS)

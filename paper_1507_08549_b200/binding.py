@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libsn_poisson.so")
 # every symbol include/sn_poisson.h declares
 EXPORTS = (
     "sn_poisson_create", "sn_poisson_solve", "sn_poisson_solve_host", "sn_poisson_solve_batch",
+    "sn_poisson_solve_batch_host", "sn_poisson_solve_sequence_host", "sn_poisson_probe_l2",
     "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
     "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
@@ -55,6 +56,14 @@ def load():
     lib.sn_poisson_solve_batch.restype = C.c_int
     lib.sn_poisson_solve_batch.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, C.c_int, _vp,
                                            C.POINTER(sn_poisson_result)]
+    lib.sn_poisson_solve_batch_host.restype = C.c_int
+    lib.sn_poisson_solve_batch_host.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, C.c_int, _vp,
+                                                C.POINTER(sn_poisson_result)]
+    lib.sn_poisson_solve_sequence_host.restype = C.c_int
+    lib.sn_poisson_solve_sequence_host.argtypes = [_vp, C.c_int, _vp, _vp, _vp, C.c_double, C.c_int, _vp,
+                                                   C.POINTER(sn_poisson_result)]
+    lib.sn_poisson_probe_l2.restype = C.c_int
+    lib.sn_poisson_probe_l2.argtypes = [C.c_int, _dp, _dp, _vp]
     lib.sn_poisson_destroy.restype = None
     lib.sn_poisson_destroy.argtypes = [_vp]
     lib.sn_poisson_gravity.restype = C.c_int
@@ -120,6 +129,35 @@ def sn_poisson_solve_batch(h, nbatch, rho_ptr, phi_ptr, tol, max_sweeps, stream=
     if rc != 0:
         raise SnPoissonError(f"sn_poisson_solve_batch failed ({rc}): " + sn_poisson_last_error())
     return list(out)
+
+
+def sn_poisson_solve_batch_host(h, nbatch, rho_ptr, phi_ptr, tol, max_sweeps, stream=0):
+    """rho_ptr / phi_ptr: HOST addresses of nbatch consecutive grids."""
+    out = (sn_poisson_result * int(nbatch))()
+    rc = load().sn_poisson_solve_batch_host(h, int(nbatch), rho_ptr, phi_ptr, float(tol), int(max_sweeps),
+                                            stream or None, out)
+    if rc != 0:
+        raise SnPoissonError(f"sn_poisson_solve_batch_host failed ({rc}): " + sn_poisson_last_error())
+    return list(out)
+
+
+def sn_poisson_solve_sequence_host(h, nsteps, rho_seq_ptr, phi_ptr, phi_seq_ptr, tol, max_sweeps, stream=0):
+    """HOST addresses: rho_seq [nsteps][ncell], phi [ncell] in/out, phi_seq [nsteps][ncell] or 0."""
+    out = (sn_poisson_result * int(nsteps))()
+    for o in out:
+        o.status = -1
+    rc = load().sn_poisson_solve_sequence_host(h, int(nsteps), rho_seq_ptr, phi_ptr, phi_seq_ptr or None, float(tol),
+                                               int(max_sweeps), stream or None, out)
+    if rc != 0:
+        raise SnPoissonError(f"sn_poisson_solve_sequence_host failed ({rc}): " + sn_poisson_last_error())
+    return list(out)
+
+
+def sn_poisson_probe_l2(mib=32, stream=0):
+    """(copy GB/s, read GB/s) of an L2-resident working set, measured by the library's own probe kernels."""
+    c, r = C.c_double(0.0), C.c_double(0.0)
+    _check(load().sn_poisson_probe_l2(int(mib), C.byref(c), C.byref(r), stream or None), "sn_poisson_probe_l2")
+    return c.value, r.value
 
 
 def sn_poisson_gravity(h, nbatch, phi_ptr, gr_ptr, gz_ptr, stream=0):

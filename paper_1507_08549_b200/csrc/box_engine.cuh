@@ -38,9 +38,10 @@ struct BoxShape {
     static_assert(NT % 32 == 0 && H % 2 == 0, "shape");
 };
 
-// A double with a 32-bit tag in each 8-byte half: {lo, tag, hi, tag}.  Aligned 8-byte words are never torn, so a
-// reader that sees the expected tag in both halves has the whole value; no fence and no separate flag are needed
-// (the producer's tag is the step number, unique within a solve phase).
+// A double with a 32-bit tag in each 8-byte half: {lo, tag, hi, tag}.  ASSUMPTION (the NCCL "LL" idiom): a 16-byte
+// vector store may become visible in two pieces, but each naturally aligned 8-byte half {payload word, tag} is
+// single-copy atomic, so a reader that sees the expected tag in BOTH halves has the whole value; no fence and no
+// separate flag are needed (the producer's tag is the step number, unique within a solve phase).
 __device__ __forceinline__ void ll_store(uint4* p, double v, unsigned tag) {
     const unsigned lo = (unsigned)__double2loint(v), hi = (unsigned)__double2hiint(v);
     asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag)
@@ -163,7 +164,7 @@ struct BoxEngine {
                                                 int nthreads) {
         for (int r = tid; r < BH; r += nthreads) {
             exR[r * LS + 0] = 0.0;                                              // west of the box (cW = 0 on the axis)
-            exL[r * LS + TXN + 1] = (bx + BW == g.nr) ? bE[by + r] : 0.0;       // east
+            exL[r * LS + TXN + 1] = (bx + BW == g.nr && by + r < g.nz) ? bE[by + r] : 0.0;   // east (rows past nz: ragged halo tile)
             exL[r * LS + 0] = 0.0;
             exR[r * LS + TXN + 1] = 0.0;
         }

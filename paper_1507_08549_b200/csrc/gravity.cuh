@@ -8,12 +8,12 @@
 
 namespace snp {
 
-// Four consecutive cells of one row per thread (nr % 4 == 0, 16-byte aligned arrays).  grid = (ceil(nr/4/128), nz, nb).
-__global__ void __launch_bounds__(128) k_gravity4(Geom g, const double* __restrict__ phi, const double* __restrict__ bE,
+// Four consecutive cells of one row per thread (nr % 4 == 0, 16-byte aligned arrays).  grid = (ceil(nr/4/128) * nz, 1, nb).
+__global__ void __launch_bounds__(128) k_gravity4(Geom g, int qx, const double* __restrict__ phi, const double* __restrict__ bE,
                                                   const double* __restrict__ bN, const double* __restrict__ bS,
                                                   double* __restrict__ gr, double* __restrict__ gz) {
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;       // quad index in the row
-    const int j = blockIdx.y, b = blockIdx.z;
+    const int j = blockIdx.x / qx, b = blockIdx.z;             // grid.x = qx blocks per row x nz rows
+    const int q = (blockIdx.x - j * qx) * blockDim.x + threadIdx.x;       // quad index in the row
     const int i0 = 4 * q;
     if (i0 >= g.nr) return;
     const size_t ncell = (size_t)g.nr * g.nz;
@@ -56,12 +56,12 @@ __global__ void __launch_bounds__(128) k_gravity4(Geom g, const double* __restri
     *reinterpret_cast<double2*>(zrow + 2) = make_double2(z4[2], z4[3]);
 }
 
-// One cell per thread: any grid, any alignment.  grid = (ceil(nr/128), nz, nb).
-__global__ void __launch_bounds__(128) k_gravity1(Geom g, const double* __restrict__ phi, const double* __restrict__ bE,
+// One cell per thread: any grid, any alignment.  grid = (ceil(nr/128) * nz, 1, nb).
+__global__ void __launch_bounds__(128) k_gravity1(Geom g, int qx, const double* __restrict__ phi, const double* __restrict__ bE,
                                                   const double* __restrict__ bN, const double* __restrict__ bS,
                                                   double* __restrict__ gr, double* __restrict__ gz) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y, b = blockIdx.z;
+    const int j = blockIdx.x / qx, b = blockIdx.z;
+    const int i = (blockIdx.x - j * qx) * blockDim.x + threadIdx.x;
     if (i >= g.nr) return;
     const size_t ncell = (size_t)g.nr * g.nz;
     const double* p = phi + (size_t)b * ncell;

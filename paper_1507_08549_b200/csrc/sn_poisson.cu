@@ -16,6 +16,7 @@
 #include "common.cuh"
 #include "moments.cuh"
 #include "gravity.cuh"
+#include "probe.cuh"
 #include "sweep_stream.cuh"
 #include "sweep_blocked.cuh"
 #include "sweep_resident.cuh"
@@ -52,6 +53,20 @@ int dev_alloc(T** p, size_t n) {
 
 }  // namespace
 
+namespace {
+struct BlkPlan {
+    int shape = -1, m = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0, occ = 0;
+    double cost = 0;
+};
+struct ResPlan {
+    int shape = -1, halo = 0, ds = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
+    double cost = 0;
+};
+// Limits of the per-sweep bookkeeping (maxima slots + history: 32 B per sweep and member).
+constexpr int kMaxSweepsLimit = 1 << 22;                 // per solve
+constexpr long long kMaxSweepSlots = 1ll << 26;          // max_sweeps x nbatch (2 GiB of slots)
+}  // namespace
+
 struct sn_poisson {
     int nr = 0, nz = 0, symmetry = 0, lmax = 0;
     double dr = 0, dz = 0;
@@ -85,13 +100,28 @@ struct sn_poisson {
     size_t prof_cap = 0, prof_ctas = 0;
     double prof_mean[8] = {0}, prof_max[8] = {0};
     bool user_boundary = false;
+    int last_nbatch = 0;        // members whose ghost arrays are valid (last solve / set_boundary)
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
     cudaEvent_t ev_t[3] = {nullptr, nullptr, nullptr};
+    // host-buffer entry points: staging (grown on demand, kept), a copy stream and its events
+    size_t stage_cap = 0;       // doubles per staging array
+    double* d_snap[2] = {nullptr, nullptr};                  // sequence: phi snapshots for the overlapped D2H
+    size_t snap_cap = 0;
+    cudaStream_t st_copy = nullptr;
+    cudaEvent_t ev_io[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    // planner cache: the plan depends only on (nbatch, pointer alignment, options), not on the data
+    struct {
+        bool valid = false;
+        int nbatch = 0, aligned = 0;
+        ResPlan pl;
+        BlkPlan bp;
+        int group = 0;
+    } plan_cache;
 
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
     double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
-    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0, st_group = 0, st_ds = 0;
+    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0, st_group = 0, st_ds = 0, st_redund = 1;
     int last_sweeps0 = 0;
 };
 
@@ -132,6 +162,7 @@ void free_batch_ws(sn_poisson* h) {
     h->d_bE = h->d_bN = h->d_bS = h->d_M = h->d_partial = h->d_hist = nullptr;
     h->d_slots = nullptr; h->d_slots_f = nullptr; h->d_ctl = nullptr; h->h_ctl = nullptr;
     h->cap_batch = 0; h->cap_sweeps = 0;
+    h->last_nbatch = 0;
 }
 
 // Grow the per-member workspace.  Keeps injected boundary arrays of member 0 across a regrow.
@@ -250,10 +281,6 @@ const std::vector<BlkShapeInfo>& blk_shapes() {
     return v;
 }
 
-struct BlkPlan {
-    int shape = -1, m = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0, occ = 0;
-    double cost = 0;
-};
 
 // Pick (shape, m) minimising modelled clocks per sweep; honours the "shape"/"tblock" overrides.
 BlkPlan plan_blocked(sn_poisson* h, int nbatch, const double* rho, const double* phi) {
@@ -310,7 +337,8 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
         CU_TRY(cudaMalloc((void**)&h->d_work, sizeof(double) * ncell * nbatch));
         h->work_cap = ncell * nbatch;
     }
-    CU_TRY(cudaMemsetAsync(h->d_slots_f, 0, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
+    CU_TRY(cudaMemset2DAsync(h->d_slots_f, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps, 0,
+                             sizeof(unsigned int) * 2 * (size_t)std::max(1, max_sweeps), nbatch, st));
     BlkParams P;
     P.g = g;
     P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.max_sweeps = max_sweeps;
@@ -324,7 +352,6 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
     k_blocked_init<<<nbatch, 32, 0, st>>>(h->d_ctl, pl.m, max_sweeps, h->opt_exact);
     h->st_launches += 1;
     h->st_aux_launches += 1;
-    CU_TRY(cudaFuncSetAttribute(S.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
     void* args[] = {&P};
     const dim3 grid(pl.ntiles, nbatch), block(S.NT());
     // every advance may be followed by one exact re-run; plus replay and copy
@@ -355,6 +382,7 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
     h->st_path = 3;
     h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.m;
     h->st_shape = pl.shape;
+    h->st_redund = (double)pl.ntiles * S.BW() * S.BH() / ((double)h->nr * h->nz);
     return 0;
 }
 
@@ -396,10 +424,6 @@ const std::vector<ShapeInfo>& shapes() {
     return v;
 }
 
-struct ResPlan {
-    int shape = -1, halo = 0, ds = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
-    double cost = 0;
-};
 
 // Modelled SM clocks of one half-sweep of a box when `k` CTAs of that shape share an SM, calibrated with the
 // in-kernel profile ("prof" option; profiles/r01c_resident_inkernel.md): a warp needs `lat` clocks for its 2H cell
@@ -544,8 +568,8 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         h->sync_cap = need_sync;
     }
     CU_TRY(cudaMemsetAsync(h->d_sync, 0, sizeof(unsigned int) * need_sync, st));
-    CU_TRY(cudaMemsetAsync(h->d_slots_f + (size_t)member0 * 2 * h->cap_sweeps, 0,
-                           sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps * nbatch, st));
+    CU_TRY(cudaMemset2DAsync(h->d_slots_f + (size_t)member0 * 2 * h->cap_sweeps, sizeof(unsigned int) * 2 * (size_t)h->cap_sweeps,
+                             0, sizeof(unsigned int) * 2 * (size_t)std::max(1, max_sweeps), nbatch, st));
     if ((pl.halo && !pl.ds) || pl.ll) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
     ResParams P;
     P.g = g;
@@ -582,7 +606,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     }
     void* args[] = {&P};
     const void* fn = S.fn[pl.ds ? 2 : pl.halo ? 1 : 0];
-    CU_TRY(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem));
+    // (the planner has already set the kernel's shared-memory attribute; plans are cached on the handle)
     if (pl.ds) {
         // one cluster per member (gang-scheduled, so its CTAs are co-resident by construction; the clusters of a batch
         // were checked against cudaOccupancyMaxActiveClusters by the planner)
@@ -604,41 +628,33 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     h->st_path = 2;
     h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.Q;
     h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch; h->st_ds = pl.ds;
+    h->st_redund = pl.halo ? 1.0 : (double)pl.ntiles * S.BW() * S.BH() / ((double)h->nr * h->nz);
     return 0;
 }
 
-int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double tol, int max_sweeps,
-               cudaStream_t st, sn_poisson_result* out) {
-    CU_TRY(cudaSetDevice(h->device));
-    if (int rc = ensure_ws(h, nbatch, max_sweeps)) return rc;
-    if (!h->omega_user) h->omega = default_omega(h->nr, h->nz, h->dr, h->dz, h->symmetry);
-    const Geom g = make_geom(h, tol);
-    h->st_launches = 0;
-    h->st_aux_launches = 0;
-    h->st_path = 1;
-    h->st_halo = 0;
-    h->st_ds = 0;
+// Hooks of the host-buffer entry points into one solve: an event the relaxation must wait for (phi's H2D on the copy
+// stream) and a device -> host copy enqueued right after the relaxation, before the call's single synchronisation.
+struct HostIO {
+    cudaEvent_t wait_before_relax = nullptr;
+    double* d2h_dst = nullptr;
+    const double* d2h_src = nullptr;
+    size_t d2h_bytes = 0;
+};
 
-    CU_TRY(cudaEventRecord(h->ev_t[0], st));
-    CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl) * nbatch, st));
-    CU_TRY(cudaMemsetAsync(h->d_slots, 0, sizeof(unsigned long long) * 2 * (size_t)h->cap_sweeps * nbatch, st));
-    // a-1: moments (+ max|4 pi rho|), a-1b: boundary fill (skipped when ghosts were injected by the test hook)
-    if (int rc = launch_moments(h, g, nbatch, rho, st)) return rc;
-    h->st_launches += 1;
-    h->st_aux_launches += 1;
-    if (!h->user_boundary) {
-        k_boundary<<<nbatch, 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN,
-                                           h->d_bS, 0);
-        CU_TRY(cudaGetLastError());
-        h->st_launches += 1;
-        h->st_aux_launches += 1;
+// The plan of a solve depends only on (nbatch, pointer alignment, options): planned once, cached on the handle
+// (set_option invalidates).  The planners also set the kernels' shared-memory attributes, once.
+void plan_solve(sn_poisson* h, int nbatch, const double* rho, const double* phi, ResPlan* pl_out, BlkPlan* bp_out,
+                int* group_out) {
+    const int aligned = ((((uintptr_t)rho | (uintptr_t)phi) & 15) == 0) ? 1 : 0;
+    auto& pc = h->plan_cache;
+    if (pc.valid && pc.nbatch == nbatch && pc.aligned == aligned) {
+        *pl_out = pc.pl; *bp_out = pc.bp; *group_out = pc.group;
+        return;
     }
-    CU_TRY(cudaEventRecord(h->ev_t[1], st));
-    // a-2 + a-3
     ResPlan pl;
     BlkPlan bp;
     int group = nbatch;          // members per resident launch
-    if ((h->opt_path == 0 || h->opt_path == 2) && max_sweeps > 0) {
+    if (h->opt_path == 0 || h->opt_path == 2) {
         pl = plan_resident(h, nbatch, rho, phi);
         // A batch whose tiles cannot all be co-resident: solve it in groups of G members, one resident launch after
         // the other, if a group fills the chip (otherwise the blocked path streams the whole batch).  "group"
@@ -659,12 +675,52 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
             if (pl.shape < 0) group = nbatch;
         }
     }
+    if ((h->opt_path == 0 || h->opt_path == 3) && pl.shape < 0) bp = plan_blocked(h, nbatch, rho, phi);
+    pc.valid = true; pc.nbatch = nbatch; pc.aligned = aligned; pc.pl = pl; pc.bp = bp; pc.group = group;
+    *pl_out = pl; *bp_out = bp; *group_out = group;
+}
+
+int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double tol, int max_sweeps,
+               cudaStream_t st, sn_poisson_result* out, const HostIO* io = nullptr) {
+    CU_TRY(cudaSetDevice(h->device));
+    if (int rc = ensure_ws(h, nbatch, max_sweeps)) return rc;
+    if (!h->omega_user) h->omega = default_omega(h->nr, h->nz, h->dr, h->dz, h->symmetry);
+    const Geom g = make_geom(h, tol);
+    h->st_launches = 0;
+    h->st_aux_launches = 0;
+    h->st_path = 1;
+    h->st_halo = 0;
+    h->st_ds = 0;
+    h->st_redund = 1;
+
+    CU_TRY(cudaEventRecord(h->ev_t[0], st));
+    CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl) * nbatch, st));
+    CU_TRY(cudaMemset2DAsync(h->d_slots, sizeof(unsigned long long) * 2 * (size_t)h->cap_sweeps, 0,
+                             sizeof(unsigned long long) * 2 * (size_t)std::max(1, max_sweeps), nbatch, st));
+    // a-1: moments (+ max|4 pi rho|), a-1b: boundary fill (skipped when ghosts were injected by the test hook)
+    if (int rc = launch_moments(h, g, nbatch, rho, st)) return rc;
+    h->st_launches += 1;
+    h->st_aux_launches += 1;
+    if (!h->user_boundary) {
+        k_boundary<<<nbatch, 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN,
+                                           h->d_bS, 0);
+        CU_TRY(cudaGetLastError());
+        h->st_launches += 1;
+        h->st_aux_launches += 1;
+    }
+    h->last_nbatch = h->user_boundary ? h->cap_batch : nbatch;
+    CU_TRY(cudaEventRecord(h->ev_t[1], st));
+    if (io && io->wait_before_relax) CU_TRY(cudaStreamWaitEvent(st, io->wait_before_relax, 0));
+    // a-2 + a-3
+    ResPlan pl;
+    BlkPlan bp;
+    int group = nbatch;
+    if (max_sweeps > 0) plan_solve(h, nbatch, rho, phi, &pl, &bp, &group);
     if (h->opt_path == 2 && pl.shape < 0 && max_sweeps > 0) {
         set_err("resident path requested but not eligible (needs nr%%4==0, nz%%H==0, grid >= one box, 16-byte aligned "
                 "pointers, tiles x batch <= co-resident CTAs)");
         return -1;
     }
-    if ((h->opt_path == 0 || h->opt_path == 3) && pl.shape < 0 && max_sweeps > 0) bp = plan_blocked(h, nbatch, rho, phi);
     if (h->opt_path == 3 && bp.shape < 0 && max_sweeps > 0) {
         set_err("blocked path requested but not eligible (needs nr%%4==0, nz%%H==0, grid >= one box, 16-byte aligned "
                 "pointers)");
@@ -681,6 +737,8 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
         if (int rc = run_stream(h, g, nbatch, rho, phi, max_sweeps, st)) return rc;
     }
     CU_TRY(cudaEventRecord(h->ev_t[2], st));
+    if (io && io->d2h_dst)
+        CU_TRY(cudaMemcpyAsync(io->d2h_dst, io->d2h_src, io->d2h_bytes, cudaMemcpyDeviceToHost, st));
     CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl) * nbatch, cudaMemcpyDeviceToHost, st));
     CU_TRY(cudaStreamSynchronize(st));
     float ms = 0;
@@ -719,12 +777,33 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     return 0;
 }
 
-bool check_solve_args(sn_poisson* h, const void* rho, const void* phi, double tol, int max_sweeps) {
+bool check_solve_args(sn_poisson* h, const void* rho, const void* phi, double tol, int max_sweeps, int nbatch = 1) {
     if (!h) { set_err("NULL handle"); return false; }
     if (!rho || !phi) { set_err("NULL rho / phi pointer"); return false; }
     if (max_sweeps < 0) { set_err("max_sweeps < 0"); return false; }
+    if (max_sweeps > kMaxSweepsLimit || (long long)max_sweeps * nbatch > kMaxSweepSlots) {
+        set_err("max_sweeps too large: the per-sweep bookkeeping allows max_sweeps <= %d and max_sweeps x nbatch <= %lld",
+                kMaxSweepsLimit, kMaxSweepSlots);
+        return false;
+    }
     if (tol != tol) { set_err("tol is NaN"); return false; }
     return true;
+}
+
+// Device staging of the host-buffer entry points: `n` doubles each for rho and phi, grown on demand and kept.
+int ensure_stage(sn_poisson* h, size_t n) {
+    if (!h->st_copy) {
+        CU_TRY(cudaStreamCreateWithFlags(&h->st_copy, cudaStreamNonBlocking));
+        for (auto& e : h->ev_io) CU_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    if (h->stage_cap >= n) return 0;
+    cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage);
+    h->d_rho_stage = h->d_phi_stage = nullptr;
+    h->stage_cap = 0;
+    CU_TRY(cudaMalloc((void**)&h->d_rho_stage, sizeof(double) * n));
+    CU_TRY(cudaMalloc((void**)&h->d_phi_stage, sizeof(double) * n));
+    h->stage_cap = n;
+    return 0;
 }
 
 }  // namespace
@@ -789,7 +868,9 @@ void sn_poisson_destroy(sn_poisson* h) {
     if (!h) return;
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
-    cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage);
+    cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage); cudaFree(h->d_snap[0]); cudaFree(h->d_snap[1]);
+    if (h->st_copy) cudaStreamDestroy(h->st_copy);
+    for (auto& e : h->ev_io) if (e) cudaEventDestroy(e);
     cudaFree(h->d_prof); cudaFree(h->d_ring); cudaFree(h->d_mail); cudaFree(h->d_sync); cudaFree(h->d_work);
     for (auto& e : h->ev_poll) if (e) cudaEventDestroy(e);
     for (auto& e : h->ev_t) if (e) cudaEventDestroy(e);
@@ -809,9 +890,9 @@ sn_poisson_result sn_poisson_solve(sn_poisson* h, const double* rho, double* phi
 int sn_poisson_solve_batch(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double tol,
                            int max_sweeps, void* stream, sn_poisson_result* out) {
     g_err.clear();
-    if (!check_solve_args(h, rho, phi_inout, tol, max_sweeps)) return -1;
     if (nbatch < 1 || !out) { set_err("nbatch < 1 or NULL out"); return -1; }
     if (nbatch > 65535) { set_err("nbatch > 65535"); return -1; }
+    if (!check_solve_args(h, rho, phi_inout, tol, max_sweeps, nbatch)) return -1;
     return solve_impl(h, nbatch, rho, phi_inout, tol, max_sweeps, (cudaStream_t)stream, out);
 }
 
@@ -820,34 +901,96 @@ sn_poisson_result sn_poisson_solve_host(sn_poisson* h, const double* rho_host, d
     g_err.clear();
     sn_poisson_result r = {0, -1, 0.0};
     if (!check_solve_args(h, rho_host, phi_inout_host, tol, max_sweeps)) return r;
-    cudaStream_t st = (cudaStream_t)stream;
-    const size_t bytes = sizeof(double) * (size_t)h->nr * h->nz;
-    auto fail = [&](cudaError_t e, const char* what) {
-        set_err("%s failed: %s", what, cudaGetErrorString(e));
-        r.status = -2;
-        return r;
-    };
-    cudaError_t e;
-    if ((e = cudaSetDevice(h->device)) != cudaSuccess) return fail(e, "cudaSetDevice");
-    if (!h->d_rho_stage) {
-        if ((e = cudaMalloc((void**)&h->d_rho_stage, bytes)) != cudaSuccess) return fail(e, "cudaMalloc");
-        if ((e = cudaMalloc((void**)&h->d_phi_stage, bytes)) != cudaSuccess) return fail(e, "cudaMalloc");
-    }
-    if ((e = cudaMemcpyAsync(h->d_rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e, "H2D rho");
-    if ((e = cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return fail(e, "H2D phi");
-    const int rc = solve_impl(h, 1, h->d_rho_stage, h->d_phi_stage, tol, max_sweeps, st, &r);
+    sn_poisson_result out;
+    const int rc = sn_poisson_solve_batch_host(h, 1, rho_host, phi_inout_host, tol, max_sweeps, stream, &out);
     if (rc) { r.sweeps = 0; r.status = rc; r.residual = 0.0; return r; }
-    if ((e = cudaMemcpyAsync(phi_inout_host, h->d_phi_stage, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return fail(e, "D2H phi");
-    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return fail(e, "cudaStreamSynchronize");
-    return r;
+    return out;
+}
+
+int sn_poisson_solve_batch_host(sn_poisson* h, int nbatch, const double* rho_host, double* phi_inout_host, double tol,
+                                int max_sweeps, void* stream, sn_poisson_result* out) {
+    g_err.clear();
+    if (nbatch < 1 || !out) { set_err("nbatch < 1 or NULL out"); return -1; }
+    if (nbatch > 65535) { set_err("nbatch > 65535"); return -1; }
+    if (!check_solve_args(h, rho_host, phi_inout_host, tol, max_sweeps, nbatch)) return -1;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)h->nr * h->nz * nbatch, bytes = sizeof(double) * n;
+    CU_TRY(cudaSetDevice(h->device));
+    if (int rc = ensure_stage(h, n)) return rc;
+    // rho goes first on the caller's stream (the moments need it); phi's upload rides on the copy stream behind the
+    // moments / boundary kernels and is waited for just before the relaxation; phi's download is enqueued right
+    // after the relaxation, before the call's single synchronisation.
+    CU_TRY(cudaEventRecord(h->ev_io[0], st));                          // order the copy stream after the caller's work
+    CU_TRY(cudaStreamWaitEvent(h->st_copy, h->ev_io[0], 0));
+    CU_TRY(cudaMemcpyAsync(h->d_rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, h->st_copy));
+    CU_TRY(cudaEventRecord(h->ev_io[1], h->st_copy));
+    HostIO io;
+    io.wait_before_relax = h->ev_io[1];
+    io.d2h_dst = phi_inout_host; io.d2h_src = h->d_phi_stage; io.d2h_bytes = bytes;
+    return solve_impl(h, nbatch, h->d_rho_stage, h->d_phi_stage, tol, max_sweeps, st, out, &io);
+}
+
+int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_seq_host, double* phi_inout_host,
+                                   double* phi_seq_host, double tol, int max_sweeps, void* stream,
+                                   sn_poisson_result* out) {
+    g_err.clear();
+    if (nsteps < 1 || !out) { set_err("nsteps < 1 or NULL out"); return -1; }
+    if (!check_solve_args(h, rho_seq_host, phi_inout_host, tol, max_sweeps)) return -1;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)h->nr * h->nz, bytes = sizeof(double) * n;
+    CU_TRY(cudaSetDevice(h->device));
+    if (int rc = ensure_stage(h, 2 * n)) return rc;                    // rho double-buffered in d_rho_stage[2][n]
+    if (phi_seq_host && h->snap_cap < n) {
+        for (auto& d : h->d_snap) { cudaFree(d); d = nullptr; }
+        h->snap_cap = 0;
+        for (auto& d : h->d_snap) CU_TRY(cudaMalloc((void**)&d, bytes));
+        h->snap_cap = n;
+    }
+    cudaEvent_t ev_h2d[2] = {h->ev_io[0], h->ev_io[1]}, ev_snap[2] = {h->ev_io[2], h->ev_io[3]},
+                ev_d2h[2] = {h->ev_io[4], h->ev_io[5]};
+    CU_TRY(cudaMemcpyAsync(h->d_rho_stage, rho_seq_host, bytes, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaEventRecord(ev_h2d[0], st));
+    CU_TRY(cudaStreamWaitEvent(h->st_copy, ev_h2d[0], 0));             // the copy stream starts behind the caller's work
+    bool d2h_pending[2] = {false, false};
+    for (int t = 0; t < nsteps; ++t) {
+        const int cur = t & 1, nxt = cur ^ 1;
+        // upload rho_{t+1} on the copy stream while solve t runs (its buffer was last read by solve t-1: complete,
+        // every solve ends with a stream synchronisation)
+        if (t + 1 < nsteps) {
+            CU_TRY(cudaMemcpyAsync(h->d_rho_stage + (size_t)nxt * n, rho_seq_host + (size_t)(t + 1) * n, bytes,
+                                   cudaMemcpyHostToDevice, h->st_copy));
+            CU_TRY(cudaEventRecord(ev_h2d[nxt], h->st_copy));
+        }
+        if (t > 0) CU_TRY(cudaStreamWaitEvent(st, ev_h2d[cur], 0));
+        if (int rc = solve_impl(h, 1, h->d_rho_stage + (size_t)cur * n, h->d_phi_stage, tol, max_sweeps, st, out + t)) return rc;
+        if (out[t].status < 0) return 0;                                // the caller sees which step failed
+        if (phi_seq_host) {
+            // snapshot on the caller's stream (the next solve updates phi in place), download on the copy stream
+            // while solve t+1 runs
+            if (d2h_pending[cur]) CU_TRY(cudaStreamWaitEvent(st, ev_d2h[cur], 0));
+            CU_TRY(cudaMemcpyAsync(h->d_snap[cur], h->d_phi_stage, bytes, cudaMemcpyDeviceToDevice, st));
+            CU_TRY(cudaEventRecord(ev_snap[cur], st));
+            CU_TRY(cudaStreamWaitEvent(h->st_copy, ev_snap[cur], 0));
+            CU_TRY(cudaMemcpyAsync(phi_seq_host + (size_t)t * n, h->d_snap[cur], bytes, cudaMemcpyDeviceToHost, h->st_copy));
+            CU_TRY(cudaEventRecord(ev_d2h[cur], h->st_copy));
+            d2h_pending[cur] = true;
+        }
+    }
+    CU_TRY(cudaMemcpyAsync(phi_inout_host, h->d_phi_stage, bytes, cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    CU_TRY(cudaStreamSynchronize(h->st_copy));
+    return 0;
 }
 
 int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr, double* gz, void* stream) {
     g_err.clear();
     if (!h || !phi || !gr || !gz) { set_err("NULL argument"); return -1; }
     if (nbatch < 1 || nbatch > 65535) { set_err("nbatch must be in [1, 65535]"); return -1; }
-    if (!h->d_bE || nbatch > h->cap_batch) {
-        set_err("no ghost values for %d member(s): solve (or set_boundary) on this handle first", nbatch);
+    if (!h->d_bE || nbatch > h->last_nbatch) {
+        set_err("no ghost values for %d member(s): the last solve / set_boundary on this handle covered %d", nbatch,
+                h->d_bE ? h->last_nbatch : 0);
         return -1;
     }
     CU_TRY(cudaSetDevice(h->device));
@@ -855,14 +998,64 @@ int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr,
     cudaStream_t st = (cudaStream_t)stream;
     const bool vec = h->nr % 4 == 0 && ((((uintptr_t)phi | (uintptr_t)gr | (uintptr_t)gz) & 15) == 0);
     if (vec) {
-        const dim3 grid((h->nr / 4 + 127) / 128, h->nz, nbatch);
-        k_gravity4<<<grid, 128, 0, st>>>(g, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
+        const unsigned qx = (h->nr / 4 + 127) / 128;                       // rows folded into grid.x: no 65535 limit on nz
+        const dim3 grid(qx * (unsigned)h->nz, 1, nbatch);
+        k_gravity4<<<grid, 128, 0, st>>>(g, (int)qx, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
     } else {
-        const dim3 grid((h->nr + 127) / 128, h->nz, nbatch);
-        k_gravity1<<<grid, 128, 0, st>>>(g, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
+        const unsigned qx = (h->nr + 127) / 128;
+        const dim3 grid(qx * (unsigned)h->nz, 1, nbatch);
+        k_gravity1<<<grid, 128, 0, st>>>(g, (int)qx, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
     }
     CU_TRY(cudaGetLastError());
     return 0;
+}
+
+int sn_poisson_probe_l2(int mib, double* copy_gbs, double* read_gbs, void* stream) {
+    g_err.clear();
+    if (mib < 1 || mib > 1024 || !copy_gbs || !read_gbs) { set_err("bad argument"); return -1; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CU_TRY(cudaGetDevice(&dev));
+    CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t n2 = (size_t)mib * (1u << 20) / 16;                   // double2 elements per array
+    const int grid = 2 * sms, reps = 20;
+    double2 *a = nullptr, *b = nullptr;
+    double* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = 0;
+    auto body = [&]() -> int {
+        CU_TRY(cudaMalloc((void**)&a, 16 * n2));
+        CU_TRY(cudaMalloc((void**)&b, 16 * n2));
+        CU_TRY(cudaMalloc((void**)&sink, sizeof(double) * grid * kProbeThreads));
+        CU_TRY(cudaMemsetAsync(a, 0, 16 * n2, st));
+        CU_TRY(cudaEventCreate(&e0));
+        CU_TRY(cudaEventCreate(&e1));
+        double best_c = 0, best_r = 0;
+        for (int it = 0; it < 6; ++it) {                               // first pass of each kind warms L2 and clocks
+            float ms = 0;
+            CU_TRY(cudaEventRecord(e0, st));
+            k_probe_l2_copy<<<grid, kProbeThreads, 0, st>>>(a, b, n2, reps);
+            CU_TRY(cudaEventRecord(e1, st));
+            CU_TRY(cudaEventSynchronize(e1));
+            CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            if (it > 0) best_c = std::max(best_c, 2.0 * 16.0 * n2 * reps / (ms * 1e-3) / 1e9);
+            CU_TRY(cudaEventRecord(e0, st));
+            k_probe_l2_read<<<grid, kProbeThreads, 0, st>>>(a, n2, reps, sink);
+            CU_TRY(cudaEventRecord(e1, st));
+            CU_TRY(cudaEventSynchronize(e1));
+            CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            if (it > 0) best_r = std::max(best_r, 16.0 * n2 * reps / (ms * 1e-3) / 1e9);
+        }
+        CU_TRY(cudaGetLastError());
+        *copy_gbs = best_c;
+        *read_gbs = best_r;
+        return 0;
+    };
+    rc = body();
+    cudaFree(a); cudaFree(b); cudaFree(sink);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    return rc;
 }
 
 int sn_poisson_set_omega(sn_poisson* h, double omega) {
@@ -902,6 +1095,7 @@ int sn_poisson_set_boundary(sn_poisson* h, const double* bE, const double* bN, c
             CU_TRY(cudaMemcpy(h->d_bS + (size_t)b * h->nr, bS, sizeof(double) * h->nr, cudaMemcpyHostToDevice));
     }
     h->user_boundary = true;
+    h->last_nbatch = h->cap_batch;
     return 0;
 }
 
@@ -927,6 +1121,7 @@ int sn_poisson_get_history(sn_poisson* h, double* R, int n) {
 int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     g_err.clear();
     if (!h || !key) { set_err("NULL argument"); return -1; }
+    h->plan_cache.valid = false;
     if (!strcmp(key, "path")) { if (value < 0 || value > 3) { set_err("path must be 0..3"); return -1; } h->opt_path = (int)value; return 0; }
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
@@ -957,6 +1152,7 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "halo")) { *out = h->st_halo; return 0; }
     if (!strcmp(key, "ds")) { *out = h->st_ds; return 0; }
     if (!strcmp(key, "group")) { *out = h->st_group; return 0; }
+    if (!strcmp(key, "redundancy")) { *out = h->st_redund; return 0; }
     if (!strncmp(key, "prof_mean", 9) && key[9] >= '0' && key[9] <= '7' && !key[10]) { *out = h->prof_mean[key[9] - '0']; return 0; }
     if (!strncmp(key, "prof_max", 8) && key[8] >= '0' && key[8] <= '7' && !key[9]) { *out = h->prof_max[key[8] - '0']; return 0; }
     set_err("unknown stat '%s'", key);

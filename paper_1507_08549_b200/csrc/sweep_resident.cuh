@@ -479,10 +479,13 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 const int t = (nby0 + i / (nbx1 - nbx0 + 1)) * p.ntx + nbx0 + i % (nbx1 - nbx0 + 1);
                 if (t == tile) continue;
                 unsigned spins = 0;
-                // relaxed polls (an acquire would invalidate L1 on every iteration); the margins are then read
-                // with ld.global.cg, which is served by L2 where the release made the tile visible before the flag
+                // relaxed polls (an acquire would invalidate L1 on every iteration)
                 while (ld_relaxed_u32(flags + t) < want && !poll_giveup(pc, spins, 5, (int)want)) {}
             }
+            // ONE acquire fence after the relaxed spin (not one per poll): relaxed load that observed the neighbour's
+            // st.release + fence.acq_rel = acquire pattern of the PTX memory model, so the ring stores of every tile
+            // polled above happen-before the margin loads of the whole CTA (ordered after this warp by the barrier).
+            asm volatile("fence.acq_rel.gpu;" ::: "memory");
         }
         const long long tp0 = tick();
         Engine::sync();

@@ -36,6 +36,15 @@ class PoissonSolver:
         if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
             raise ValueError("expected a contiguous float64 CUDA tensor")
 
+    @staticmethod
+    def _raise_if_failed(results, what):
+        """Same rule for single solves, batches and sequences: any status < 0 raises; the results ride on the error."""
+        bad = [(i, r.status) for i, r in enumerate(results) if r.status < 0]
+        if bad:
+            e = B.SnPoissonError(f"{what}: status {bad[0][1]} (member/step {bad[0][0]}): {B.sn_poisson_last_error()}")
+            e.results = list(results)
+            raise e
+
     def solve(self, rho, phi, tol, max_sweeps):
         """In-place on ``phi``.  Returns sn_poisson_result (or a list for a 3-D batch)."""
         import torch
@@ -45,23 +54,56 @@ class PoissonSolver:
         if rho.dim() == 3:
             if rho.shape != phi.shape or tuple(rho.shape[1:]) != (self.nz, self.nr):
                 raise ValueError("shape mismatch")
-            return B.sn_poisson_solve_batch(self.h, rho.shape[0], rho.data_ptr(), phi.data_ptr(), tol, max_sweeps,
-                                            stream)
+            res = B.sn_poisson_solve_batch(self.h, rho.shape[0], rho.data_ptr(), phi.data_ptr(), tol, max_sweeps,
+                                           stream)
+            self._raise_if_failed(res, "sn_poisson_solve_batch")
+            return res
         if tuple(rho.shape) != (self.nz, self.nr) or rho.shape != phi.shape:
             raise ValueError("shape mismatch")
         r = B.sn_poisson_solve(self.h, rho.data_ptr(), phi.data_ptr(), tol, max_sweeps, stream)
-        if r.status < 0:
-            raise B.SnPoissonError(f"sn_poisson_solve status {r.status}: {B.sn_poisson_last_error()}")
+        self._raise_if_failed([r], "sn_poisson_solve")
         return r
 
+    def _check_host(self, a, shape, writeable=False):
+        import numpy as np
+        if not isinstance(a, np.ndarray) or a.dtype != np.float64 or not a.flags.c_contiguous or tuple(a.shape) != shape:
+            raise ValueError(f"expected a C-contiguous float64 numpy array of shape {shape}")
+        if writeable and not a.flags.writeable:
+            raise ValueError("output array is read-only")
+
     def solve_host(self, rho_np, phi_np, tol, max_sweeps):
-        """Host numpy arrays (C-contiguous float64); phi_np is updated in place.  H2D/D2H inside the call."""
+        """Host numpy arrays (C-contiguous float64, (nz, nr) or (nbatch, nz, nr)); phi_np is updated in place.
+        H2D/D2H inside the call (sn_poisson_solve_host / sn_poisson_solve_batch_host)."""
         import torch
         stream = torch.cuda.current_stream().cuda_stream
+        if rho_np.ndim == 3:
+            shape = (rho_np.shape[0], self.nz, self.nr)
+            self._check_host(rho_np, shape)
+            self._check_host(phi_np, shape, writeable=True)
+            res = B.sn_poisson_solve_batch_host(self.h, shape[0], rho_np.ctypes.data, phi_np.ctypes.data, tol,
+                                                max_sweeps, stream)
+            self._raise_if_failed(res, "sn_poisson_solve_batch_host")
+            return res
+        self._check_host(rho_np, (self.nz, self.nr))
+        self._check_host(phi_np, (self.nz, self.nr), writeable=True)
         r = B.sn_poisson_solve_host(self.h, rho_np.ctypes.data, phi_np.ctypes.data, tol, max_sweeps, stream)
-        if r.status < 0:
-            raise B.SnPoissonError(f"sn_poisson_solve_host status {r.status}: {B.sn_poisson_last_error()}")
+        self._raise_if_failed([r], "sn_poisson_solve_host")
         return r
+
+    def solve_sequence_host(self, rho_seq_np, phi_np, tol, max_sweeps, phi_seq_np=None):
+        """Warm-started sequence ([CFG 3]): rho_seq_np (nsteps, nz, nr); phi_np (nz, nr) initial guess in / last
+        potential out; phi_seq_np (nsteps, nz, nr) optional, every step's potential.  Returns the list of results."""
+        import torch
+        n = rho_seq_np.shape[0]
+        self._check_host(rho_seq_np, (n, self.nz, self.nr))
+        self._check_host(phi_np, (self.nz, self.nr), writeable=True)
+        if phi_seq_np is not None:
+            self._check_host(phi_seq_np, (n, self.nz, self.nr), writeable=True)
+        res = B.sn_poisson_solve_sequence_host(self.h, n, rho_seq_np.ctypes.data, phi_np.ctypes.data,
+                                               0 if phi_seq_np is None else phi_seq_np.ctypes.data, tol, max_sweeps,
+                                               torch.cuda.current_stream().cuda_stream)
+        self._raise_if_failed(res, "sn_poisson_solve_sequence_host")      # steps after a failed one stay at -1
+        return res
 
     def gravity(self, phi, gr=None, gz=None):
         """(g_r, g_z) = -grad phi with the ghost values of the last solve; enqueued on the current stream."""

@@ -19,7 +19,7 @@ def lib():
 def header_symbols():
     src = open(os.path.join(ROOT, "include", "sn_poisson.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(sn_poisson_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(sn_poisson_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_and_binding_agree():

@@ -50,6 +50,20 @@ def relmax(a, b):
     return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
 
 
+def assert_field_matches(oracle, w, got, r, ref, rho=None, phi0=None):
+    """north_star: same converged sweep count within +-1 AND phi equal to <= 1e-11 after an IDENTICAL sweep count.
+    The field comparison is unconditional: if the counts differ by one, the oracle is re-run for exactly the GPU's
+    count from the same start (never observed; a regression that shifts a crossing must still be compared)."""
+    assert abs(r.sweeps - ref["sweeps"]) <= 1, (r, ref["sweeps"])
+    want = ref["phi"]
+    if r.sweeps != ref["sweeps"]:
+        rho = w.rho if rho is None else rho
+        phi0 = np.zeros_like(rho) if phi0 is None else phi0
+        want = oracle.solve(rho, phi0, w.dr, w.dz, w.symmetry, w.lmax, 0.0, r.sweeps, omega=w.omega)["phi"]
+    err = relmax(got, want)
+    assert err <= REL, err
+
+
 PATHS = [{"path": 1}, {"path": 1, "chunk": 3}]
 
 
@@ -358,9 +372,8 @@ def test_config_parity_small(P, torch_cuda, oracle, name):
     ref = oracle.solve_workload(w, history=True)
     s, got, r = gpu_solve(P, torch_cuda, w)
     assert r.status == ref["status"] == 0
-    assert abs(r.sweeps - ref["sweeps"]) <= 1
+    assert_field_matches(oracle, w, got, r, ref)
     if r.sweeps == ref["sweeps"]:
-        assert relmax(got, ref["phi"]) <= REL
         assert r.residual == pytest.approx(ref["residual"], rel=1e-6)
     # identical sweep count, fixed: k = 1, 10, 100 (the end state alone tests little once stagnated)
     for k in (1, 10, 100):
@@ -375,9 +388,8 @@ def test_cfg1_full_size_parity_and_closed_form(P, torch_cuda, oracle):
     w = W.cfg1()
     ref = oracle.solve_workload(w)
     s, got, r = gpu_solve(P, torch_cuda, w)
-    assert r.status == 0 and abs(r.sweeps - ref["sweeps"]) <= 1
-    if r.sweeps == ref["sweeps"]:
-        assert relmax(got, ref["phi"]) <= REL
+    assert r.status == 0
+    assert_field_matches(oracle, w, got, r, ref)
     rr, zz = W.cell_centres(w.nr, w.nz, w.dr, w.dz, 1)
     sph = np.hypot(rr[None, :], zz[:, None])
     R = 0.8
@@ -391,9 +403,8 @@ def test_cfg2_full_size_parity(P, torch_cuda, oracle):
     w = W.cfg2()
     ref = oracle.solve_workload(w)
     s, got, r = gpu_solve(P, torch_cuda, w)
-    assert r.status == 0 and abs(r.sweeps - ref["sweeps"]) <= 1
-    if r.sweeps == ref["sweeps"]:
-        assert relmax(got, ref["phi"]) <= REL
+    assert r.status == 0
+    assert_field_matches(oracle, w, got, r, ref)
 
 
 def test_cfg3_warm_started_sequence_reduced(P, torch_cuda, oracle):
@@ -410,42 +421,50 @@ def test_cfg3_warm_started_sequence_reduced(P, torch_cuda, oracle):
             rho = seq.step(rho, t)
         ref = oracle.solve(rho, phi_ref, w.dr, w.dz, 0, w.lmax, w.tol, w.max_sweeps)
         r = s.solve(torch_cuda.from_numpy(rho).cuda(), phi_gpu, w.tol, w.max_sweeps)
-        assert r.status == 0 and abs(r.sweeps - ref["sweeps"]) <= 1
-        if r.sweeps == ref["sweeps"]:
-            assert relmax(phi_gpu.cpu().numpy(), ref["phi"]) <= REL
+        assert r.status == 0
+        assert_field_matches(oracle, w, phi_gpu.cpu().numpy(), r, ref, rho=rho, phi0=phi_ref)
         phi_ref = ref["phi"]
         phi_gpu.copy_(torch_cuda.from_numpy(phi_ref))      # keep both on the same trajectory
         counts.append(r.sweeps)
     assert counts[1] < counts[0] and counts[2] < counts[0]      # warm start helps
 
 
-def test_cfg3_full_size_fixed_sweeps_and_converged_property(P, torch_cuda, oracle):
-    """[CFG 3] 1024x2048, lmax 32 (a full oracle solve would take ~1 h): 12 sweeps element by element, then the
-    converged solve is checked by properties the oracle can compute at this size:
-      * the oracle's plain-arithmetic operator residual of the returned field is tiny;
-      * the history crosses tol exactly once, at the returned sweep k* (first crossing);
-      * ONE oracle sweep applied to the returned field equals, element by element, the GPU's own field after a
-        fixed k*+1 sweeps, and its ratio R_{k*+1} equals the GPU's history entry.  (R_k is not monotone -- the
-        oracle's own histories rise by up to x2.4 between consecutive sweeps -- so R_{k*+1} <= tol is NOT a property.)"""
-    w = W.cfg3().first
+def test_cfg3_full_size_converged_and_warm_started(P, torch_cuda, oracle):
+    """[CFG 3] 1024x2048 full plane, lmax 32, in the launch configuration bench.py times: 12 sweeps element by element,
+    then the CONVERGED cold solve against a full oracle solve (5161 sweeps x 2.1 M cells, ~30 s of oracle), then two
+    warm-started steps of the sequence at full size, each against the oracle started from the same field.
+    Sweep counts equal, phi <= 1e-11 relative max-norm, history tail and residual equal to the oracle's (the two
+    differ only through the summation order of the moments, ~1e-15 in the ghost values)."""
+    seq = W.cfg3(nsteps=3)
+    w = seq.first
     ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, 0, w.lmax, 0.0, 12)
     s, got, r = gpu_solve(P, torch_cuda, w, tol=0.0, max_sweeps=12)
     assert r.sweeps == 12 and relmax(got, ref["phi"]) <= REL
-    s, got, r = gpu_solve(P, torch_cuda, w)
-    assert r.status == 0 and 3000 < r.sweeps < 8000
-    hist = s.history(r.sweeps)
-    assert len(hist) == r.sweeps and hist[-1] == r.residual <= w.tol and np.all(hist[:-1] > w.tol)
-    bE, bN, bS = s.boundary()
-    f = 12.566370614359172 * w.rho
-    res = oracle.apply_operator(got, w.dr, w.dz, 0, bE, bN, bS) - f
-    D = 2 / w.dr ** 2 + 2 / w.dz ** 2
-    assert np.max(np.abs(res)) / (np.max(np.abs(f)) + D * np.max(np.abs(got))) < 5e-10
-    nxt, Rabs, Pk = oracle.sweeps(w.rho, got, w.dr, w.dz, 0, s.omega, bE, bN, bS, 1)
-    s2, got2, r2 = gpu_solve(P, torch_cuda, w, tol=0.0, max_sweeps=r.sweeps + 1)
-    assert r2.sweeps == r.sweeps + 1
-    assert relmax(got2, nxt) <= REL
-    want = oracle.ratio(Rabs[0], Pk[0], np.max(np.abs(f)), w.dr, w.dz)
-    assert s2.history(r2.sweeps)[-1] == pytest.approx(want, rel=1e-9)
+    s = P.PoissonSolver.for_workload(w)
+    rho = w.rho
+    phi_ref = np.zeros_like(rho)
+    phi_gpu = torch_cuda.zeros(rho.shape, dtype=torch_cuda.float64, device="cuda")
+    counts = []
+    for t in range(3):
+        if t > 0:
+            rho = seq.step(rho, t)
+        ref = oracle.solve(rho, phi_ref, w.dr, w.dz, 0, w.lmax, w.tol, w.max_sweeps, history=True)
+        r = s.solve(torch_cuda.from_numpy(rho).cuda(), phi_gpu, w.tol, w.max_sweeps)
+        got = phi_gpu.cpu().numpy()
+        assert r.status == 0 and ref["status"] == 0
+        assert s.stat("path") == 2 and s.stat("halo") == 1            # the bench's launch configuration
+        assert_field_matches(oracle, w, got, r, ref, rho=rho, phi0=phi_ref)
+        assert r.sweeps == ref["sweeps"]                               # equal in every run so far; +-1 is the bar
+        assert r.residual == pytest.approx(ref["residual"], rel=1e-6)
+        hist = s.history(r.sweeps)
+        assert len(hist) == r.sweeps and hist[-1] == r.residual <= w.tol
+        # entries before the exactly tracked endgame are lower bounds within 2^-19 (sn_poisson.h)
+        assert np.allclose(hist, ref["hist"], rtol=4e-6, atol=0.0)
+        assert np.all(hist[:-1] > w.tol)
+        phi_ref = ref["phi"]
+        phi_gpu.copy_(torch_cuda.from_numpy(phi_ref))                  # keep both on the same trajectory
+        counts.append(r.sweeps)
+    assert 3000 < counts[0] < 8000 and counts[1] < counts[0] and counts[2] < counts[0]
 
 
 def test_batch_matches_individual_oracle_solves(P, torch_cuda, oracle):
@@ -460,31 +479,39 @@ def test_batch_matches_individual_oracle_solves(P, torch_cuda, oracle):
     sweeps = set()
     for b, w in enumerate(ws):
         ref = oracle.solve_workload(w)
-        assert res[b].status == 0 and abs(res[b].sweeps - ref["sweeps"]) <= 1
-        if res[b].sweeps == ref["sweeps"]:
-            assert relmax(got[b], ref["phi"]) <= REL
+        assert res[b].status == 0
+        assert_field_matches(oracle, w, got[b], res[b], ref)
         sweeps.add(res[b].sweeps)
     assert len(sweeps) > 1
 
 
-def test_batch_full_size_sampled_members(P, torch_cuda, oracle):
-    """[CFG 4a] 64 x 512x512 in the launch configuration bench.py uses; 2 sampled members vs the oracle."""
+def test_batch_full_size_all_members(P, torch_cuda, oracle):
+    """[CFG 4a] 64 x 512x512 in the launch configuration bench.py uses; EVERY member against its own oracle solve
+    (64 single-thread oracle solves, spread over the host cores: ctypes releases the GIL)."""
+    from concurrent.futures import ThreadPoolExecutor
+    import os
     ws = W.cfg4a(64)
     s = P.PoissonSolver.for_workload(ws[0])
     rho = torch_cuda.from_numpy(np.stack([w.rho for w in ws])).cuda()
     phi = torch_cuda.zeros_like(rho)
     res = s.solve(rho, phi, ws[0].tol, ws[0].max_sweeps)
     assert all(r.status == 0 for r in res)
-    for b in (5, 41):
-        ref = oracle.solve_workload(ws[b])
-        assert abs(res[b].sweeps - ref["sweeps"]) <= 1
-        if res[b].sweeps == ref["sweeps"]:
-            assert relmax(phi[b].cpu().numpy(), ref["phi"]) <= REL
+    got = phi.cpu().numpy()
+    oracle.lib()
+    with ThreadPoolExecutor(max_workers=max(1, min(16, os.cpu_count() or 1))) as ex:
+        refs = list(ex.map(oracle.solve_workload, ws))
+    for b, (w, ref) in enumerate(zip(ws, refs)):
+        assert ref["status"] == 0
+        assert_field_matches(oracle, w, got[b], res[b], ref)
+        assert res[b].sweeps == ref["sweeps"], b
+        assert res[b].residual == pytest.approx(ref["residual"], rel=1e-6)
+    assert len({r.sweeps for r in res}) > 8                            # members converge at different counts
 
 
 def test_size_sweep_points_fixed_sweeps(P, torch_cuda, oracle):
-    """[CFG 4b] fixed-sweep throughput points: 30 sweeps at 1024 and 2048 vs the oracle, element by element."""
-    for n in (1024, 2048):
+    """[CFG 4b] fixed-sweep throughput points: 30 sweeps at 1024, 2048 and 4096 (the HBM-bound point: 1849 tiles on the
+    blocked path) vs the oracle, element by element."""
+    for n in (1024, 2048, 4096):
         w = W.cfg4b(n, max_sweeps=30)
         ref = oracle.solve_workload(w)
         _, got, r = gpu_solve(P, torch_cuda, w)
@@ -543,6 +570,74 @@ def test_solve_host_equals_device_solve(P, torch_cuda, oracle):
     assert (r2.sweeps, r2.status, r2.residual) == (r.sweeps, r.status, r.residual)
     assert np.array_equal(phi_h, got)
     assert s.stat("launches") > 0 and s.stat("sweep_ms") > 0
+
+
+def test_batch_host_and_sequence_host_equal_device_solves(P, torch_cuda, oracle):
+    """The HOST-buffer entry points (what bench.py's e2e times) give bit-identical results to the device-pointer calls:
+    sn_poisson_solve_batch_host vs sn_poisson_solve_batch, sn_poisson_solve_sequence_host vs a loop of warm-started
+    sn_poisson_solve calls (with and without the per-step potentials); the first step is also checked against the oracle."""
+    ws = [W.cfg4a_member(b, 128) for b in range(5)]
+    s = P.PoissonSolver.for_workload(ws[0])
+    rho_h = np.stack([w.rho for w in ws])
+    rho = torch_cuda.from_numpy(rho_h).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    res = s.solve(rho, phi, ws[0].tol, ws[0].max_sweeps)
+    phi_h = np.zeros_like(rho_h)
+    res_h = s.solve_host(rho_h, phi_h, ws[0].tol, ws[0].max_sweeps)
+    assert [(a.sweeps, a.status, a.residual) for a in res] == [(a.sweeps, a.status, a.residual) for a in res_h]
+    assert np.array_equal(phi_h, phi.cpu().numpy())
+    with pytest.raises(ValueError):
+        s.solve_host(rho_h.astype(np.float32), phi_h, 1e-10, 10)
+    with pytest.raises(ValueError):
+        s.solve_host(rho_h[:, ::2], phi_h[:, ::2], 1e-10, 10)
+
+    seq = W.cfg3(128, nsteps=4)
+    w = seq.first
+    rhos, r_t = [w.rho], w.rho
+    for t in range(1, 4):
+        r_t = seq.step(r_t, t)
+        rhos.append(r_t)
+    rho_seq = np.stack(rhos)
+    s = P.PoissonSolver.for_workload(w)
+    phi_d = torch_cuda.zeros(w.rho.shape, dtype=torch_cuda.float64, device="cuda")
+    want_res, want_phi = [], []
+    for t in range(4):
+        want_res.append(s.solve(torch_cuda.from_numpy(rhos[t]).cuda(), phi_d, w.tol, w.max_sweeps))
+        want_phi.append(phi_d.cpu().numpy())
+    ref0 = oracle.solve_workload(w)
+    assert want_res[0].sweeps == ref0["sweeps"] and relmax(want_phi[0], ref0["phi"]) <= REL
+    for keep in (True, False):
+        phi_io = np.zeros_like(w.rho)
+        phi_all = np.full_like(rho_seq, np.nan) if keep else None
+        got = s.solve_sequence_host(rho_seq, phi_io, w.tol, w.max_sweeps, phi_all)
+        assert [(a.sweeps, a.status, a.residual) for a in got] == [(a.sweeps, a.status, a.residual) for a in want_res]
+        assert np.array_equal(phi_io, want_phi[-1])
+        if keep:
+            for t in range(4):
+                assert np.array_equal(phi_all[t], want_phi[t]), t
+
+
+def test_limits_and_stale_ghosts_are_rejected(P, torch_cuda):
+    """max_sweeps beyond the documented bookkeeping limit -> -1 (no allocation attempt); gravity for more members than
+    the last solve covered -> error."""
+    w = W.cfg2(128)
+    s = P.PoissonSolver.for_workload(w)
+    rho = torch_cuda.from_numpy(np.stack([w.rho] * 3)).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    r = P.sn_poisson_solve(s.h, rho.data_ptr(), phi.data_ptr(), 1e-10, 2 ** 31 - 1, 0)
+    assert r.status == -1 and "max_sweeps" in P.sn_poisson_last_error()
+    with pytest.raises(P.SnPoissonError):
+        P.sn_poisson_solve_batch(s.h, 3, rho.data_ptr(), phi.data_ptr(), 1e-10, 2 ** 25, 0)
+    s.solve(rho, phi, w.tol, 50)                       # 3 members
+    s.solve(rho[0], phi[0], w.tol, 50)                 # then 1 member: ghosts of members 1, 2 are stale
+    s.gravity(phi[0])
+    with pytest.raises(P.SnPoissonError):
+        s.gravity(phi)
+
+
+def test_l2_probe_reports_plausible_bandwidth(P, torch_cuda):
+    copy_gbs, read_gbs = P.sn_poisson_probe_l2(32)
+    assert 3000 < copy_gbs < 40000 and 3000 < read_gbs < 40000
 
 
 def test_rho_is_never_modified_and_stream_is_respected(P, torch_cuda):
