@@ -35,6 +35,8 @@ struct BoxShape {
     static constexpr size_t lat_doubles = (size_t)BH * LS;
     static constexpr size_t vert_doubles = (size_t)(TYN + 2) * BW;
     static constexpr size_t engine_doubles = f_doubles + 2 * lat_doubles + 2 * vert_doubles;
+    // ring duty (halo mode): second-layer columns / rows + the ring threads' private copies of their two edge cells
+    static constexpr size_t ring_doubles = (size_t)4 * (BH + BW);
     static_assert(NT % 32 == 0 && H % 2 == 0, "shape");
 };
 
@@ -53,6 +55,13 @@ __device__ __forceinline__ uint4 ll_load(const uint4* p) {
                  : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
                  : "l"(p)
                  : "memory");
+    return v;
+}
+// Same load, but not a compiler barrier for ordinary memory accesses: used to put a poll IN FLIGHT early (its result
+// is validated by the tags when it is consumed), so that the L2 round trip overlaps the patch update.
+__device__ __forceinline__ uint4 ll_load_early(const uint4* p) {
+    uint4 v;
+    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
     return v;
 }
 __device__ __forceinline__ bool ll_ready(const uint4& v, unsigned tag) { return v.y == tag && v.w == tag; }
@@ -105,6 +114,20 @@ struct BoxEngine {
     double* exR;    // [BH][LS]        column 3 of thread a at [row][a+1]
     double* exB;    // [TYN+2][2][PW]  bottom row of thread-row b at [b+1]
     double* exT;    // [TYN+2][2][PW]  top row of thread-row b at [b+1]
+    double *l2W = nullptr, *l2E = nullptr, *l2S = nullptr, *l2N = nullptr, *stash = nullptr;   // ring duty only
+
+    // Inbox of one tile: tagged packets it receives from its four neighbours, [E: BH][W: BH][N: BW][S: BW], each edge
+    // split by colour so that the packets of one half-sweep are contiguous: slot(i) = (i & 1) * n/2 + (i >> 1).
+    // A slot is written once per sweep with a strictly increasing tag, and its reader consumes tag t before the
+    // writer can produce t + 2, so one buffer is enough.
+    static constexpr int kInboxE = 0, kInboxW = BH, kInboxN = 2 * BH, kInboxS = 2 * BH + BW, kInboxPackets = 2 * (BH + BW);
+
+    // Which neighbours exist and where their inboxes are.
+    struct HaloLinks {
+        uint4* own;                  // this tile's inbox
+        uint4 *w, *e, *s, *n;        // neighbours' inboxes (NULL: no neighbour on that side)
+        int rows;                    // box rows inside the grid (== BH except in the ragged last tile row), even
+    };
 
     // per-thread state
     int a, b, rowbase;
@@ -125,6 +148,14 @@ struct BoxEngine {
         exR = exL + S::lat_doubles;
         exB = exR + S::lat_doubles;
         exT = exB + S::vert_doubles;
+    }
+    // ring-duty arrays; `base` = first double after everything else the kernel keeps in dynamic shared memory
+    __device__ __forceinline__ void carve_ring(double* base) {
+        l2W = base;            // [BH]        column 1 of the box (second layer behind the west edge)
+        l2E = l2W + BH;        // [BH]        column BW-2
+        l2S = l2E + BH;        // [2][PW]     row 1, parity planes like exB
+        l2N = l2S + BW;        // [2][PW]     row BH-2
+        stash = l2N + BW;      // [2][BH+BW]  per colour: the ring thread's own edge cell
     }
     __device__ __forceinline__ void bind_thread(int tid) {
         a = tid % TXN;
@@ -194,7 +225,23 @@ struct BoxEngine {
         }
     }
     // publish every edge value of the patch (both colours) to the exchange arrays
+    template <bool RING = false>
     __device__ __forceinline__ void publish_all() {
+        if (RING) {
+#pragma unroll
+            for (int q = 0; q < H; ++q) {
+                if (a == 0) l2W[rowbase + q] = phi[q][1];
+                if (a == TXN - 1) l2E[rowbase + q] = phi[q][2];
+            }
+            if (b == 0) {
+                *reinterpret_cast<double2*>(l2S + 2 * a) = make_double2(phi[1][0], phi[1][2]);
+                *reinterpret_cast<double2*>(l2S + PW + 2 * a) = make_double2(phi[1][1], phi[1][3]);
+            }
+            if (b == TYN - 1) {
+                *reinterpret_cast<double2*>(l2N + 2 * a) = make_double2(phi[H - 2][0], phi[H - 2][2]);
+                *reinterpret_cast<double2*>(l2N + PW + 2 * a) = make_double2(phi[H - 2][1], phi[H - 2][3]);
+            }
+        }
 #pragma unroll
         for (int q = 0; q < H; ++q) {
             exL[(rowbase + q) * LS + a + 1] = phi[q][0];
@@ -226,29 +273,33 @@ struct BoxEngine {
     }
 
     // One half-sweep of colour COL over the patch, then publish the updated edge cells and (SYNC) the barrier.
-    template <int COL, int TRACK, bool SYNC = true>
+    template <int COL, int TRACK, bool SYNC = true, bool RING = false>
     __device__ __forceinline__ void half_sweep() {
         if (active) {
             update_cells<COL, TRACK, 0>();
-            publish_colour<COL>();
+            publish_colour<COL, RING>();
         }
         if (SYNC) sync();
     }
-    // Halo mode: the cells a neighbouring TILE may need (first and last patch row, first / last patch column) are
-    // updated first and sent at once, so that the packets travel while the rest of the patch is updated.  The order
-    // of a colour's updates is free (they are mutually independent, R10).  No barrier here.
-    template <int COL, int TRACK, bool DS = false>
-    __device__ __forceinline__ void half_sweep_halo(unsigned tag) {
-        if (!active) return;
-        update_cells<COL, TRACK, 1>();
-        if (DS) ds_send<COL>();
-        else halo_send<COL>(tag);
-        update_cells<COL, TRACK, 2>();
-        publish_colour<COL>();
+    // ring variant: the packets of this half-sweep were sent by the neighbours' ring duty at its start, so the poll can
+    // be put in flight in the middle of the patch update; returns what it fetched (tags 0 if nothing was fetched)
+    template <int COL, int TRACK>
+    __device__ __forceinline__ uint4 half_sweep_ring(const HaloLinks& L) {
+        uint4 pf = make_uint4(0u, 0u, 0u, 0u);
+        const uint4* src = h_edge >= 0 ? recv_src<COL>(L) : nullptr;
+        if (active) {
+            update_cells<COL, TRACK, 0, true>(src, &pf);
+            publish_colour<COL, true>();
+        } else if (src) {
+            pf = ll_load_early(src);
+        }
+        return pf;
     }
     // WHICH: 0 all cells of colour COL, 1 only the patch-edge cells (rows 0 and H-1, column 0 / 3), 2 the others
-    template <int COL, int TRACK, int WHICH>
-    __device__ __forceinline__ void update_cells() {
+    // PF (ring duty): after the first half of the rows, put this thread's poll of the neighbour's packet in flight
+    // (pf_src may be NULL: nothing to receive); halo_recv consumes *pf.
+    template <int COL, int TRACK, int WHICH, bool PF = false>
+    __device__ __forceinline__ void update_cells(const uint4* pf_src = nullptr, uint4* pf = nullptr) {
         // vertical outer neighbours of the bottom (q=0) and top (q=H-1) rows: other-colour cells of the rows outside
         constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;                 // column parity updated in those rows
         double2 So = make_double2(0.0, 0.0), No = make_double2(0.0, 0.0);
@@ -258,6 +309,7 @@ struct BoxEngine {
         }
 #pragma unroll
         for (int q = 0; q < H; ++q) {
+            if (PF && q == H / 2) { if (pf_src) *pf = ll_load_early(pf_src); }
             const int pq = (q + COL) & 1;                                   // compile-time after unrolling
             const bool edge_row = q == 0 || q == H - 1;
             const bool any0 = WHICH == 0 || (WHICH == 1 ? (edge_row || pq == 0) : (!edge_row && pq != 0));   // cc = 0
@@ -286,9 +338,20 @@ struct BoxEngine {
         }
     }
     // publish the updated patch-edge cells of colour COL to the exchange arrays of the CTA
-    template <int COL>
+    template <int COL, bool RING = false>
     __device__ __forceinline__ void publish_colour() {
         constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;
+        if (RING) {            // second layer behind the box edges: what the ring duty of the NEXT half-sweep reads
+            constexpr int p1 = (1 + COL) & 1, pn = (H - 2 + COL) & 1;
+#pragma unroll
+            for (int q = 0; q < H; ++q) {
+                const int pq = (q + COL) & 1;
+                if (pq == 1) { if (a == 0) l2W[rowbase + q] = phi[q][1]; }
+                else { if (a == TXN - 1) l2E[rowbase + q] = phi[q][2]; }
+            }
+            if (b == 0) *reinterpret_cast<double2*>(l2S + p1 * PW + 2 * a) = make_double2(phi[1][p1], phi[1][p1 + 2]);
+            if (b == TYN - 1) *reinterpret_cast<double2*>(l2N + pn * PW + 2 * a) = make_double2(phi[H - 2][pn], phi[H - 2][pn + 2]);
+        }
 #pragma unroll
         for (int q = 0; q < H; ++q) {
             const int pq = (q + COL) & 1;
@@ -334,58 +397,49 @@ struct BoxEngine {
         }
     }
 
-    // Inbox of one tile: tagged packets it receives from its four neighbours, [E: BH][W: BH][N: BW][S: BW], each edge
-    // split by colour so that the packets of one half-sweep are contiguous: slot(i) = (i & 1) * n/2 + (i >> 1).
-    // A slot is written once per sweep with a strictly increasing tag, and its reader consumes tag t before the
-    // writer can produce t + 2, so one buffer is enough.
-    static constexpr int kInboxE = 0, kInboxW = BH, kInboxN = 2 * BH, kInboxS = 2 * BH + BW, kInboxPackets = 2 * (BH + BW);
-
-    // Which neighbours exist and where their inboxes are.
-    struct HaloLinks {
-        uint4* own;                  // this tile's inbox
-        uint4 *w, *e, *s, *n;        // neighbours' inboxes (NULL: no neighbour on that side)
-        int rows;                    // box rows inside the grid (== BH except in the ragged last tile row), even
-    };
-
-    // Per-thread halo state, computed once (halo_bind) so that the per-half-sweep exchange is a handful of
-    // instructions.  Receive: thread tid < BH + BW fetches ONE packet per half-sweep; for colour 0 it reads h_src
-    // and writes h_dst, for colour 1 both move by the deltas.  Send: a box-edge thread keeps the base of its slots
-    // in the neighbour's inbox (a thread sits on at most one column edge and one row edge: TXN, TYN >= 2).
-    const uint4* h_src = nullptr;
-    double* h_dst = nullptr;
-    int h_edge = 0;                  // 0 E, 1 W, 2 N, 3 S: fixes the two deltas
+    // Per-thread halo state, computed once (halo_bind).  RECEIVE: thread (edge, j) fetches ONE packet per half-sweep
+    // from this tile's inbox and drops it into the engine's border slot:
+    //   E (j < BH/2): the east tile's column 0,  row 2j + COL      W: the west tile's column BW-1, row 2j + 1 - COL
+    //   N (j < BW/2): the north tile's row 0,    plane COL, pos j  S: the south tile's row BH-1,   plane 1 - COL, pos j
+    // (plane p, position j <-> box column 4 (j >> 1) + 2 (j & 1) + p).  Where the CTA has enough warps every edge gets
+    // whole warps of its own (no divergence between the four cases), else the threads are packed E | W | N | S.
+    // SEND, plain variant: the owners of the box-edge cells send after their patch update (h_scol / h_srow).
+    // SEND, ring variant: see ring_duty().
+    int h_edge = -1;                 // 0 E, 1 W, 2 N, 3 S; -1: this thread receives nothing
+    int h_j = 0;
     uint4* h_scol = nullptr;         // column edge: west (h_west) or east
     uint4* h_srow = nullptr;         // row edge: south (h_south) or north
     bool h_west = false, h_south = false;
 
+    static constexpr int kWE = (BH / 2 + 31) / 32, kWB = (BW / 2 + 31) / 32;       // warps per column / row edge
+    static constexpr bool kWarpEdges = (2 * kWE + 2 * kWB) * 32 <= S::NT;
+
+    template <bool RING>
     __device__ __forceinline__ void halo_bind(const HaloLinks& L, int tid) {
         static_assert(BH + BW <= S::NT && TXN >= 2 && TYN >= 2, "halo mode: one packet per thread, one edge per axis");
-        if (tid < BH / 2) {                                  // east tile's column 0
-            const int j = tid;
-            if (L.e && 2 * j < L.rows) {
-                h_src = L.own + kInboxE + j; h_edge = 0;
-                h_dst = exL + 2 * j * LS + TXN + 1;
-            }
-        } else if (tid < BH) {                               // west tile's column 3
-            const int j = tid - BH / 2;
-            if (L.w && 2 * j < L.rows) {
-                h_src = L.own + kInboxW + BH / 2 + j; h_edge = 1;
-                h_dst = exR + (2 * j + 1) * LS;
-            }
-        } else if (tid < BH + BW / 2) {                      // north tile's bottom row
-            const int j = tid - BH;
-            if (L.n) {
-                h_src = L.own + kInboxN + j; h_edge = 2;
-                h_dst = exB + (size_t)(TYN + 1) * BW + j;
-            }
-        } else if (tid < BH + BW) {                          // south tile's top row
-            const int j = tid - BH - BW / 2;
-            if (L.s) {
-                h_src = L.own + kInboxS + BW / 2 + j; h_edge = 3;
-                h_dst = exT + PW + j;
-            }
+        int e = -1, j = 0;
+        if (kWarpEdges) {
+            const int w = tid >> 5, l = tid & 31;
+            if (w < kWE) { e = 0; j = w * 32 + l; }
+            else if (w < 2 * kWE) { e = 1; j = (w - kWE) * 32 + l; }
+            else if (w < 2 * kWE + kWB) { e = 2; j = (w - 2 * kWE) * 32 + l; }
+            else if (w < 2 * kWE + 2 * kWB) { e = 3; j = (w - 2 * kWE - kWB) * 32 + l; }
+            if (e >= 0 && j >= (e < 2 ? BH / 2 : BW / 2)) e = -1;
+        } else {
+            if (tid < BH / 2) { e = 0; j = tid; }
+            else if (tid < BH) { e = 1; j = tid - BH / 2; }
+            else if (tid < BH + BW / 2) { e = 2; j = tid - BH; }
+            else if (tid < BH + BW) { e = 3; j = tid - BH - BW / 2; }
         }
-        if (active) {
+        const bool have = e == 0 ? (L.e != nullptr && 2 * j < L.rows) : e == 1 ? (L.w != nullptr && 2 * j < L.rows)
+                        : e == 2 ? L.n != nullptr : e == 3 ? L.s != nullptr : false;
+        h_edge = have ? e : -1;
+        h_j = j;
+        if (e == 0) { h_src0 = kInboxE + j; h_sdelta = BH / 2; h_dst0 = (int)(exL - fs) + 2 * j * LS + TXN + 1; h_ddelta = LS; }
+        else if (e == 1) { h_src0 = kInboxW + BH / 2 + j; h_sdelta = -(BH / 2); h_dst0 = (int)(exR - fs) + (2 * j + 1) * LS; h_ddelta = -LS; }
+        else if (e == 2) { h_src0 = kInboxN + j; h_sdelta = BW / 2; h_dst0 = (int)(exB - fs) + (TYN + 1) * BW + j; h_ddelta = PW; }
+        else if (e == 3) { h_src0 = kInboxS + BW / 2 + j; h_sdelta = -(BW / 2); h_dst0 = (int)(exT - fs) + PW + j; h_ddelta = -PW; }
+        if (!RING && active) {
             if (a == 0 && L.w) { h_scol = L.w + kInboxE + rowbase / 2; h_west = true; }
             else if (a == TXN - 1 && L.e) { h_scol = L.e + kInboxW + rowbase / 2; }
             if (b == 0 && L.s) { h_srow = L.s + kInboxN + 2 * a; h_south = true; }
@@ -421,23 +475,130 @@ struct BoxEngine {
 
     // ... and every receiving thread fetches its ONE packet (coalesced, all four sides in flight at once) into the
     // border slot.  The poll gives up when the context says so.
+    // receive addressing, linear in the colour: packet index in the inbox and border slot (doubles from fs)
+    int h_src0 = 0, h_sdelta = 0, h_dst0 = 0, h_ddelta = 0;
     template <int COL>
-    __device__ __forceinline__ void halo_recv(unsigned tag, const PollCtx& pc) {
-        if (!h_src) return;
-        const uint4* src = h_src;
-        double* dst = h_dst;
-        if (COL) {                           // deltas of the colour-1 slot / border element (see halo_bind)
-            const int dsrc = h_edge == 0 ? BH / 2 : h_edge == 1 ? -(BH / 2) : h_edge == 2 ? BW / 2 : -(BW / 2);
-            const int ddst = h_edge == 0 ? LS : h_edge == 1 ? -LS : h_edge == 2 ? PW : -PW;
-            src += dsrc;
-            dst += ddst;
-        }
+    __device__ __forceinline__ const uint4* recv_src(const HaloLinks& L) const { return L.own + (h_src0 + COL * h_sdelta); }
+    template <int COL>
+    __device__ __forceinline__ double* recv_dst() const { return fs + (h_dst0 + COL * h_ddelta); }
+    // `first`: a poll already in flight (half_sweep_ring), consumed before any new load is issued
+    template <int COL>
+    __device__ __forceinline__ void halo_recv(const HaloLinks& L, unsigned tag, const PollCtx& pc,
+                                              uint4 first = make_uint4(0u, 0u, 0u, 0u)) {
+        if (h_edge < 0) return;
+        double* dst = recv_dst<COL>();
+        if (ll_ready(first, tag)) { *dst = ll_value(first); return; }       // tags start at 1: all-zero never matches
+        const uint4* src = recv_src<COL>(L);
         unsigned spins = 0;
         for (;;) {
             const uint4 v = ll_load(src);
             if (ll_ready(v, tag)) { *dst = ll_value(v); break; }
             if (poll_giveup(pc, spins, 1, (int)tag)) break;
         }
+    }
+
+    // ---- ring duty (halo mode): the box-edge cells are ALSO updated, one per thread, by the thread that receives on
+    // that edge, FIRST THING in the half-sweep and straight from shared memory, and sent at once.  The packets then
+    // travel while the patch update runs, so the neighbours find them when their own patch update is done: the period
+    // of a half-sweep becomes max(patch update, ring duty + packet flight) instead of their sum.  The patch owners
+    // update the same cells again later in the half-sweep from the same inputs with the same expression tree: the two
+    // results are the same bits (R10), the owners' copy is the one the maxima and the result come from.
+    //   Thread (edge, j), colour COL:   E: cell (BW-1, 2j + 1 - COL)    W: cell (0, 2j + COL)
+    //                                   N: cell (plane 1 - COL pos j, BH-1)    S: cell (plane COL pos j, 0)
+    // Inputs: the border slot (the neighbour tile's cell, received in the previous half-sweep), the two other-colour
+    // cells along the edge (published by their owners in the previous half-sweep; the corner's comes from the other
+    // edge's border slot), the second-layer cell behind it (l2*: published by its owner), f, and the cell's own old
+    // value from the thread's private stash (the owner overwrites the published copy DURING this half-sweep).
+    // CTA-uniform ring constants, kept in shared memory by the kernel
+    struct RingConst {
+        double cE_e, cW_e;           // coefficients of the box's last column (east edge)
+        double cE_w, cW_w;           // ... first column (west edge)
+        const double *cE, *cW;       // g.cE + bx, g.cW + bx (row-edge threads index them with their column)
+        int mirror_box;              // the box's row 0 is the reflecting equator row
+    };
+
+    // stash <- the current values of this thread's two edge cells; call after publish_all() + sync, then sync again
+    __device__ __forceinline__ void ring_init() {
+        if (h_edge < 0) return;
+        const int j = h_j;
+#pragma unroll
+        for (int col = 0; col < 2; ++col) {
+            double v;
+            if (h_edge == 0) v = exR[(2 * j + 1 - col) * LS + TXN];
+            else if (h_edge == 1) v = exL[(2 * j + col) * LS + 1];
+            else if (h_edge == 2) v = exT[(size_t)TYN * BW + (1 - col) * PW + j];
+            else v = exB[(size_t)BW + col * PW + j];
+            stash[col * (BH + BW) + ring_slot()] = v;
+        }
+    }
+    __device__ __forceinline__ int ring_slot() const {
+        return h_edge == 0 ? h_j : h_edge == 1 ? BH / 2 + h_j : h_edge == 2 ? BH + h_j : BH + BW / 2 + h_j;
+    }
+
+    // One specialised straight-line body per edge: every address is (compile-time constant) + (stride) * j.
+    template <int COL, int EDGE>
+    __device__ __forceinline__ void ring_cell(const HaloLinks& L, const RingConst& rc, unsigned tag) {
+        const int j = h_j;
+        double pE, pW, pN, pS, fv, cE, cW;
+        double cS = iz2, dg = D, ww = wD;
+        double* st;
+        uint4* out;
+        if (EDGE < 2) {
+            constexpr bool east = EDGE == 0;
+            constexpr int r0 = east ? 1 - COL : COL;                         // r = 2 j + r0
+            const int r = 2 * j + r0;
+            const double* own_col = east ? exR + TXN : exL + 1;              // this edge column as published by its owners
+            constexpr int pc = east ? BW - 1 : 0;                            // position of the column in a row of f / exB / exT
+            cE = east ? rc.cE_e : rc.cE_w;
+            cW = east ? rc.cW_e : rc.cW_w;
+            st = stash + COL * (BH + BW) + (east ? 0 : BH / 2) + j;
+            fv = fs[(size_t)r * BW + pc];
+            pE = east ? exL[r * LS + TXN + 1] : l2W[r];
+            pW = east ? l2E[r] : exR[r * LS];
+            // the corner cells take their vertical neighbour from the row border (the neighbouring tile / the ghosts)
+            pN = own_col[(r + 1 < BH ? r + 1 : r) * LS];
+            if (r0 == 1 && r + 1 == BH) pN = exB[(size_t)(TYN + 1) * BW + pc];
+            pS = own_col[(r > 0 ? r - 1 : r) * LS];
+            if (r0 == 0 && r == 0) {
+                pS = exT[pc];
+                if (rc.mirror_box) { cS = 0.0; dg = D0; ww = wD0; }
+            }
+            out = east ? L.e + kInboxW + (1 - COL) * (BH / 2) + j : L.w + kInboxE + COL * (BH / 2) + j;
+        } else {
+            constexpr bool north = EDGE == 2;
+            constexpr int pl = north ? 1 - COL : COL;                        // parity plane of my cell; column c = 2 j + pl
+            constexpr int r = north ? BH - 1 : 0;
+            const int pp = pl * PW + j;
+            const double* own_row = north ? exT + (size_t)TYN * BW : exB + BW;   // this edge row as published by its owners
+            cE = __ldg(rc.cE + 2 * j + pl);
+            cW = __ldg(rc.cW + 2 * j + pl);
+            st = stash + COL * (BH + BW) + BH + (north ? 0 : BW / 2) + j;
+            fv = fs[(size_t)r * BW + pp];
+            pN = north ? exB[(size_t)(TYN + 1) * BW + pp] : l2S[pp];
+            pS = north ? l2N[pp] : exT[pp];
+            if (pl == 1) {           // odd column: west neighbour = plane 0 [j], east = plane 0 [j + 1] or the east border
+                pW = own_row[j];
+                pE = own_row[j + 1 < PW ? j + 1 : j];
+                if (j + 1 == PW) pE = exL[r * LS + TXN + 1];
+            } else {                 // even column: west = plane 1 [j - 1] or the west border, east = plane 1 [j]
+                pE = own_row[PW + j];
+                pW = own_row[PW + (j > 0 ? j - 1 : j)];
+                if (j == 0) pW = exR[r * LS];
+            }
+            out = north ? L.n + kInboxS + (1 - COL) * (BW / 2) + j : L.s + kInboxN + COL * (BW / 2) + j;
+        }
+        double res;
+        const double pn = sor_update(cE, cW, iz2, cS, dg, ww, pE, pW, pN, pS, *st, fv, res);
+        ll_store(out, pn, tag);
+        *st = pn;
+    }
+
+    template <int COL>
+    __device__ __forceinline__ void ring_duty(const HaloLinks& L, const RingConst& rc, unsigned tag) {
+        if (h_edge == 0) ring_cell<COL, 0>(L, rc, tag);
+        else if (h_edge == 1) ring_cell<COL, 1>(L, rc, tag);
+        else if (h_edge == 2) ring_cell<COL, 2>(L, rc, tag);
+        else if (h_edge == 3) ring_cell<COL, 3>(L, rc, tag);
     }
 
     // ---- halo mode inside ONE thread-block cluster: distributed shared memory instead of L2 packets ----------------

@@ -59,7 +59,7 @@ struct BlkPlan {
     double cost = 0;
 };
 struct ResPlan {
-    int shape = -1, halo = 0, ds = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
+    int shape = -1, halo = 0, ds = 0, ring = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
     double cost = 0;
 };
 // Limits of the per-sweep bookkeeping (maxima slots + history: 32 B per sweep and member).
@@ -78,7 +78,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1, opt_ring = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -121,7 +121,7 @@ struct sn_poisson {
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
     double st_launches = 0, st_sweep_ms = 0, st_setup_ms = 0, st_path = 0;
-    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0, st_group = 0, st_ds = 0, st_redund = 1;
+    double st_ctas = 0, st_tile_w = 0, st_tile_h = 0, st_tblock = 0, st_shape = -1, st_halo = 0, st_group = 0, st_ds = 0, st_redund = 1, st_ring = 0;
     int last_sweeps0 = 0;
 };
 
@@ -390,40 +390,42 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
 // ---- resident path: shapes, planner, launcher ------------------------------------------------------------------
 struct ShapeInfo {
     int H, TXN, TYN, minb;
-    size_t smem;
-    const void* fn[3];          // [0] block mode, [1] halo mode, [2] halo mode inside one cluster (DSMEM) or NULL
+    size_t smem, smem_ring;
+    const void* fn[4];          // [0] block mode, [1] halo mode, [2] halo mode inside one cluster (DSMEM) or NULL,
+                                // [3] halo mode with ring duty
     int BW() const { return 4 * TXN; }
     int BH() const { return H * TYN; }
     int NT() const { return TXN * TYN; }
     int threads() const { return TXN * TYN + 32; }     // + the service warp
+    size_t smem_of(int f) const { return f == 3 ? smem_ring : smem; }
 };
 
-template <int H, int TXN, int TYN, int MINB, bool EF = true, bool DS = EF>
+template <int H, int TXN, int TYN, int MINB, bool DS = true>
 ShapeInfo shape_of() {
     const void* ds = nullptr;
-    if constexpr (DS) ds = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false, true>;   // no edge-first: one
-    // DSMEM hop is shorter than the extra pass costs (measured)
-    return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes,
+    if constexpr (DS) ds = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false, true>;
+    return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes, ResShape<H, TXN, TYN>::smem_bytes_ring,
             {(const void*)k_sor_resident<H, TXN, TYN, MINB, false, false>,
-             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, EF>, ds}};
+             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false>, ds,
+             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, true>}};
 }
 
 const std::vector<ShapeInfo>& shapes() {
     static const std::vector<ShapeInfo> v = {
-        shape_of<8, 32, 14, 1, false, false>(),   // 0: box 128 x 112, 448 threads (128-register cap: no edge-first)
-        shape_of<8, 32, 8, 1, true, false>(),    // 1: box 128 x 64,  256 threads
+        shape_of<8, 32, 14, 1, false>(),   // 0: box 128 x 112, 448 threads
+        shape_of<8, 32, 8, 1, false>(),    // 1: box 128 x 64,  256 threads
         shape_of<8, 16, 8, 2>(),    // 2: box 64 x 64,   128 threads
         shape_of<4, 16, 8, 2>(),    // 3: box 64 x 32,   128 threads
         shape_of<4, 8, 8, 2>(),     // 4: box 32 x 32,    64 threads
         shape_of<2, 8, 16, 2>(),    // 5: box 32 x 32,   128 threads
-        shape_of<8, 32, 7, 2, false, false>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
+        shape_of<8, 32, 7, 2, false>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
         shape_of<4, 16, 16, 1>(),   // 7: box 64 x 64,   256 threads
         shape_of<6, 12, 8, 2>(),    // 8: box 48 x 48,    96 threads
         shape_of<4, 12, 16, 1>(),   // 9: box 48 x 64,   192 threads
+        shape_of<2, 16, 32, 1>(),   // 10: box 64 x 64,  512 threads of 2 x 4 patches (shortest half-sweep: small grids)
     };
     return v;
 }
-
 
 // Modelled SM clocks of one half-sweep of a box when `k` CTAs of that shape share an SM, calibrated with the
 // in-kernel profile ("prof" option; profiles/r01c_resident_inkernel.md): a warp needs `lat` clocks for its 2H cell
@@ -469,11 +471,13 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
     for (int si = 0; si < (int)sh.size(); ++si) {
         if (h->opt_shape >= 0 && si != h->opt_shape) continue;
         const ShapeInfo& S = sh[si];
+        const int halo_fn = h->opt_ring != 0 ? 3 : 1;      // halo mode through L2 packets: ring duty unless switched off
         long long max_ctas_mode[2] = {0, 0};
         for (int md = 0; md < 2; ++md) {
+            const int f = md == 0 ? 0 : halo_fn;
             int occ = 0;
-            if (cudaFuncSetAttribute(S.fn[md], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
-                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn[md], S.threads(), S.smem) != cudaSuccess) {
+            if (cudaFuncSetAttribute(S.fn[f], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem_of(f)) != cudaSuccess ||
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn[f], S.threads(), S.smem_of(f)) != cudaSuccess) {
                 cudaGetLastError();
                 occ = 0;
             }
@@ -482,7 +486,7 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
         // halo mode: box == tile on a regular lattice, ragged last tile row allowed
         if (h->opt_halo != 0 && h->nr % S.BW() == 0 && h->nz % S.H == 0) {
             ResPlan p;
-            p.shape = si; p.halo = 1;
+            p.shape = si; p.halo = 1; p.ring = halo_fn == 3;
             p.ntx = h->nr / S.BW(); p.nty = (h->nz + S.BH() - 1) / S.BH();
             p.ow = S.BW(); p.oh = S.BH();
             p.ntiles = p.ntx * p.nty;
@@ -605,7 +609,9 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         h->prof_ctas = (size_t)pl.ntiles * nbatch;
     }
     void* args[] = {&P};
-    const void* fn = S.fn[pl.ds ? 2 : pl.halo ? 1 : 0];
+    const int fi = pl.ds ? 2 : pl.halo ? (pl.ring ? 3 : 1) : 0;
+    const void* fn = S.fn[fi];
+    const size_t smem = S.smem_of(fi);
     // (the planner has already set the kernel's shared-memory attribute; plans are cached on the handle)
     if (pl.ds) {
         // one cluster per member (gang-scheduled, so its CTAs are co-resident by construction; the clusters of a batch
@@ -614,7 +620,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(pl.ntiles, nbatch);
         cfg.blockDim = dim3(S.threads());
-        cfg.dynamicSmemBytes = S.smem;
+        cfg.dynamicSmemBytes = smem;
         cfg.stream = st;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
@@ -622,12 +628,12 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         cfg.attrs = at; cfg.numAttrs = 1;
         CU_TRY(cudaLaunchKernelExC(&cfg, fn, args));
     } else {
-        CU_TRY(cudaLaunchCooperativeKernel(fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, S.smem, st));
+        CU_TRY(cudaLaunchCooperativeKernel(fn, dim3(pl.ntiles, nbatch), dim3(S.threads()), args, smem, st));
     }
     h->st_launches += 1;
     h->st_path = 2;
     h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.Q;
-    h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch; h->st_ds = pl.ds;
+    h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch; h->st_ds = pl.ds; h->st_ring = pl.ring && !pl.ds;
     h->st_redund = pl.halo ? 1.0 : (double)pl.ntiles * S.BW() * S.BH() / ((double)h->nr * h->nz);
     return 0;
 }
@@ -691,6 +697,7 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     h->st_path = 1;
     h->st_halo = 0;
     h->st_ds = 0;
+    h->st_ring = 0;
     h->st_redund = 1;
 
     CU_TRY(cudaEventRecord(h->ev_t[0], st));
@@ -1126,6 +1133,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
     if (!strcmp(key, "prof")) { h->opt_prof = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "ring")) { if (value < -1 || value > 1) { set_err("ring must be -1, 0 or 1"); return -1; } h->opt_ring = (int)value; return 0; }
     if (!strcmp(key, "ds")) { if (value < -1 || value > 1) { set_err("ds must be -1, 0 or 1"); return -1; } h->opt_ds = (int)value; return 0; }
     if (!strcmp(key, "group")) { if (value < -1 || value > 65535) { set_err("group must be -1, 0 or a member count"); return -1; } h->opt_group = (int)value; return 0; }
     if (!strcmp(key, "ll")) { if (value < -1 || value > 1) { set_err("ll must be -1, 0 or 1"); return -1; } h->opt_ll = (int)value; return 0; }
@@ -1151,6 +1159,7 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "shape")) { *out = h->st_shape; return 0; }
     if (!strcmp(key, "halo")) { *out = h->st_halo; return 0; }
     if (!strcmp(key, "ds")) { *out = h->st_ds; return 0; }
+    if (!strcmp(key, "ring")) { *out = h->st_ring; return 0; }
     if (!strcmp(key, "group")) { *out = h->st_group; return 0; }
     if (!strcmp(key, "redundancy")) { *out = h->st_redund; return 0; }
     if (!strncmp(key, "prof_mean", 9) && key[9] >= '0' && key[9] <= '7' && !key[10]) { *out = h->prof_mean[key[9] - '0']; return 0; }

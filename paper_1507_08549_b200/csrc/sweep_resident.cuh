@@ -118,13 +118,16 @@ struct ResShape {
     static constexpr int NT = S::NT, NW = S::NW, NTHREADS = S::NT + 32;
     static constexpr size_t smax_entries = (size_t)2 * 2 * kMaxTB * NW;       // [parity][2Q][NW]
     static constexpr size_t smem_bytes = sizeof(double) * S::engine_doubles + sizeof(unsigned long long) * smax_entries;
+    static constexpr size_t smem_bytes_ring = smem_bytes + sizeof(double) * S::ring_doubles;
 };
 
 // grid = (ntx*nty, nbatch), block = TXN*TYN + 32 threads (the last warp is the service warp), cooperative launch.
-// EF (halo mode): update and send the patch-edge cells first (half_sweep_halo); only where registers allow it.
+// RING (halo mode through L2 packets): ring duty -- every box-edge cell is also updated and sent by a receiving thread
+// at the very start of the half-sweep, so that the packets travel during the patch update (BoxEngine::ring_duty).
 // DS (halo mode, all tiles of a member in one thread-block cluster): edges travel through distributed shared memory.
-template <int H, int TXN, int TYN, int MINB, bool HALO, bool EF, bool DS = false>
+template <int H, int TXN, int TYN, int MINB, bool HALO, bool RING, bool DS = false>
 __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResParams p) {
+    static_assert(!RING || (HALO && !DS), "ring duty belongs to the L2-packet halo mode");
     using S = BoxShape<H, TXN, TYN>;
     using RS = ResShape<H, TXN, TYN>;
     constexpr int BW = S::BW, BH = S::BH, NT = S::NT, NW = S::NW;
@@ -138,6 +141,8 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     __shared__ int s_zero;         // a quit word that never fires (endgame / replay polls)
     __shared__ __align__(8) unsigned long long s_mbar[2];   // DS: one mbarrier per colour, credited by the neighbours' st.async
     __shared__ long long s_pf[8];  // in-kernel profile of thread 0 ("prof" option)
+    __shared__ typename BoxEngine<H, TXN, TYN, 1>::HaloLinks s_links;   // halo mode: inboxes of this tile and its neighbours
+    __shared__ typename BoxEngine<H, TXN, TYN, 1>::RingConst s_ring;    // ring duty: CTA-uniform constants
 
     const Geom& g = p.g;
     const int member = blockIdx.y;
@@ -267,6 +272,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     // =============================================================================================================
     Engine E;
     E.carve(reinterpret_cast<double*>(smem_raw));
+    if (RING) E.carve_ring(reinterpret_cast<double*>(smem_raw + RS::smem_bytes));
     E.bind_thread(tid);
 
     const int tx = tile % p.ntx, ty = tile / p.ntx;
@@ -289,6 +295,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     double* phi_io = p.phi + (size_t)member * ncell;
     double* ring = p.ring + (size_t)member * kResRing * ncell;
     // halo mode: inboxes of this tile and of its four neighbours
+    const bool mirror_box = g.symmetry == 1 && by == 0;
     if (HALO) {
         typename Engine::HaloLinks links;
         uint4* mb = p.mail + (size_t)member * ntiles * Engine::kInboxPackets;
@@ -300,7 +307,16 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         links.n = (ty + 1 < p.nty) ? inbox(tile + p.ntx) : nullptr;
         links.rows = min(BH, g.nz - by);
         if (DS) E.ds_bind(links, s_mbar, tile, p.ntx);
-        else E.halo_bind(links, tid);
+        else E.template halo_bind<RING>(links, tid);
+        if (tid == 0) {                        // CTA-uniform: read from shared memory in the sweep loop, not kept in registers
+            s_links = links;
+            if (RING) {
+                s_ring.cE_e = g.cE[bx + BW - 1]; s_ring.cW_e = g.cW[bx + BW - 1];
+                s_ring.cE_w = g.cE[bx]; s_ring.cW_w = g.cW[bx];
+                s_ring.cE = g.cE + bx; s_ring.cW = g.cW + bx;
+                s_ring.mirror_box = mirror_box ? 1 : 0;
+            }
+        }
     }
     // block mode: the tiles whose owned cells this box overlaps (their flags gate the margin refill)
     unsigned int* flags = p.flags + (size_t)member * ntiles;
@@ -331,8 +347,12 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         E.set_borders(g, bx, by, bE, bN, bS, tid, NT);
         Engine::sync();                                          // borders first: halo loads overwrite some of them
         if (HALO) E.load_halo_borders(src, g.nr, g.nz, bx, by);
-        E.publish_all();
+        E.template publish_all<RING>();
         Engine::sync();
+        if (RING) {                                              // the ring threads' private copies of their edge cells
+            E.ring_init();
+            Engine::sync();
+        }
     };
 
     auto panicked = [&]() -> bool { return *(volatile int*)&s_panic != 0; };
@@ -387,8 +407,10 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             E.reset_maxima();
             const long long t0 = tick();
             const unsigned tag0 = tagbase + 2u * (unsigned)(k0 + s) + 1u;
-            if (HALO && EF) {
-                E.template half_sweep_halo<0, TRACK, DS>(tag0);
+            uint4 pf = make_uint4(0u, 0u, 0u, 0u);
+            if (RING) {
+                E.template ring_duty<0>(s_links, s_ring, tag0);
+                pf = E.template half_sweep_ring<0, TRACK>(s_links);
             } else {
                 E.template half_sweep<0, TRACK, false>();
                 if (HALO && DS) E.template ds_send<0>();
@@ -396,12 +418,13 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             }
             const long long t1 = tick();
             if (HALO && DS) E.template ds_recv<0>(ds_expect, tid == 0, pc_end);      // never abandoned: see box_engine.cuh
-            else if (HALO) E.template halo_recv<0>(tag0, pc);
+            else if (HALO) E.template halo_recv<0>(s_links, tag0, pc, pf);
             const long long t2 = tick();
             Engine::sync();
             const long long t3 = tick();
-            if (HALO && EF) {
-                E.template half_sweep_halo<1, TRACK, DS>(tag0 + 1u);
+            if (RING) {
+                E.template ring_duty<1>(s_links, s_ring, tag0 + 1u);
+                pf = E.template half_sweep_ring<1, TRACK>(s_links);
             } else {
                 E.template half_sweep<1, TRACK, false>();
                 if (HALO && DS) E.template ds_send<1>();
@@ -426,7 +449,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 }
             }
             if (HALO && DS) E.template ds_recv<1>(ds_expect, tid == 0, pc_end);
-            else if (HALO) E.template halo_recv<1>(tag0 + 1u, pc);
+            else if (HALO) E.template halo_recv<1>(s_links, tag0 + 1u, pc, pf);
             const long long t5 = tick();
             Engine::sync();
             const long long t6 = tick();

@@ -13,6 +13,7 @@ import workloads as W
 pytestmark = pytest.mark.gpu
 
 REL = 1e-11          # north_star tolerance, relative max-norm
+RES_ABS = 1e-13      # |R_k - oracle's R_k| when the ghosts differ in the last bits (own moments): see the cfg3 test
 
 
 @pytest.fixture(scope="module")
@@ -114,6 +115,14 @@ RESIDENT_CASES = [
     (256, 120, 1, 0, 6, 1),      # 128x112 boxes, second tile row has 8 of 112 rows
     (96, 108, 0, 8, 4, 1),       # 48x48 boxes, H=6, ragged (12 rows)
     (128, 56, 1, 6, 8, 1),       # a single tile row
+    (128, 64, 1, 10, 3, 1),      # 64x64 boxes of 2x4 patches (512 threads), 2 tiles
+    (128, 128, 0, 10, 4, 0),     # ... block mode
+    (64, 64, 1, 10, 12, 0),      # ... ONE tile: cfg0's plan (no inter-CTA traffic at all)
+    # halo = 3: halo mode WITHOUT ring duty (the owners of the box-edge cells send after their patch update)
+    (96, 80, 0, 4, 3, 3),
+    (256, 200, 1, 6, 7, 3),
+    (128, 192, 0, 2, 2, 3),
+    (256, 120, 1, 0, 6, 3),
     # halo = 2: halo mode with all tiles in ONE thread-block cluster, edges through distributed shared memory
     (96, 80, 0, 4, 3, 2),        # 3 x 3 tiles of 32x32, ragged last tile row
     (128, 128, 1, 5, 4, 2),      # 16 tiles (non-portable cluster size), H=2 patches
@@ -126,7 +135,10 @@ RESIDENT_CASES = [
 
 
 def res_opts(shape, tb, halo, **kw):
-    return {"path": 2, "shape": shape, "tblock": tb, "halo": min(halo, 1), "ds": 1 if halo == 2 else 0, **kw}
+    """halo: 0 block mode, 1 halo mode through L2 packets with ring duty (the default), 2 cluster / DSMEM, 3 halo mode
+    through L2 packets without ring duty."""
+    return {"path": 2, "shape": shape, "tblock": tb, "halo": min(halo, 1), "ds": 1 if halo == 2 else 0,
+            "ring": 0 if halo == 3 else -1, **kw}
 
 
 @pytest.mark.parametrize("nr,nz,symmetry,shape,tb,halo", RESIDENT_CASES)
@@ -148,6 +160,7 @@ def test_resident_kernel_bit_exact_fixed_sweeps(P, torch_cuda, oracle, nr, nz, s
         s, got, r = gpu_solve(P, torch_cuda, w, phi0=phi0, tol=0.0, max_sweeps=k, boundary=bnd, options=opts)
         assert s.stat("path") == 2 and s.stat("tblock") == tb and s.stat("shape") == shape
         assert s.stat("halo") == min(halo, 1) and s.stat("ds") == (1 if halo == 2 else 0)
+        assert s.stat("ring") == (1 if halo == 1 else 0)
         assert r.sweeps == k and r.status == 0
         assert np.array_equal(got, want), f"k={k}: max diff {np.max(np.abs(got - want))}"
         want_hist = np.array([oracle.ratio(Rabs[q], Pk[q], maxf, w.dr, w.dz) for q in range(k)])
@@ -204,7 +217,7 @@ def test_resident_batch_members_finish_independently(P, torch_cuda, oracle, halo
         ref = oracle.solve_workload(w)
         assert (res[b].sweeps, res[b].status) == (ref["sweeps"], 0)
         assert relmax(got[b], ref["phi"]) <= REL
-        assert res[b].residual == pytest.approx(ref["residual"], rel=1e-6)
+        assert res[b].residual == pytest.approx(ref["residual"], rel=0, abs=RES_ABS)
     assert len({r.sweeps for r in res}) > 1
 
 
@@ -340,7 +353,7 @@ def test_blocked_batch_members_finish_independently(P, torch_cuda, oracle):
         ref = oracle.solve_workload(w)
         assert (res[b].sweeps, res[b].status) == (ref["sweeps"], 0)
         assert relmax(got[b], ref["phi"]) <= REL
-        assert res[b].residual == pytest.approx(ref["residual"], rel=1e-6)
+        assert res[b].residual == pytest.approx(ref["residual"], rel=0, abs=RES_ABS)
     assert len({r.sweeps for r in res}) > 1
 
 
@@ -374,7 +387,7 @@ def test_config_parity_small(P, torch_cuda, oracle, name):
     assert r.status == ref["status"] == 0
     assert_field_matches(oracle, w, got, r, ref)
     if r.sweeps == ref["sweeps"]:
-        assert r.residual == pytest.approx(ref["residual"], rel=1e-6)
+        assert r.residual == pytest.approx(ref["residual"], rel=0, abs=RES_ABS)
     # identical sweep count, fixed: k = 1, 10, 100 (the end state alone tests little once stagnated)
     for k in (1, 10, 100):
         refk = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, w.symmetry, w.lmax, 0.0, k, omega=w.omega)
@@ -433,8 +446,8 @@ def test_cfg3_full_size_converged_and_warm_started(P, torch_cuda, oracle):
     """[CFG 3] 1024x2048 full plane, lmax 32, in the launch configuration bench.py times: 12 sweeps element by element,
     then the CONVERGED cold solve against a full oracle solve (5161 sweeps x 2.1 M cells, ~30 s of oracle), then two
     warm-started steps of the sequence at full size, each against the oracle started from the same field.
-    Sweep counts equal, phi <= 1e-11 relative max-norm, history tail and residual equal to the oracle's (the two
-    differ only through the summation order of the moments, ~1e-15 in the ghost values)."""
+    Sweep counts equal, phi <= 1e-11 relative max-norm, residual history within the bound derived below; with the
+    oracle's ghost values injected the cold solve is bit-identical (field, count, residual, history tail)."""
     seq = W.cfg3(nsteps=3)
     w = seq.first
     ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, 0, w.lmax, 0.0, 12)
@@ -455,12 +468,25 @@ def test_cfg3_full_size_converged_and_warm_started(P, torch_cuda, oracle):
         assert s.stat("path") == 2 and s.stat("halo") == 1            # the bench's launch configuration
         assert_field_matches(oracle, w, got, r, ref, rho=rho, phi0=phi_ref)
         assert r.sweeps == ref["sweeps"]                               # equal in every run so far; +-1 is the bar
-        assert r.residual == pytest.approx(ref["residual"], rel=1e-6)
+        # The library's own moments differ from the oracle's in summation order (~1e-15 in the ghosts); a 1e-15
+        # relative change of phi moves R_k by ~1e-15 ABSOLUTE (res = f - L phi cancels to ~1e-10 of its terms), i.e.
+        # ~1e-5 of R_k near tol: compare with an absolute bound of 1e-3 tol, plus the documented 2^-19 lower-bound
+        # slack of the entries tracked on the upper words only (sn_poisson.h, get_history).
         hist = s.history(r.sweeps)
         assert len(hist) == r.sweeps and hist[-1] == r.residual <= w.tol
-        # entries before the exactly tracked endgame are lower bounds within 2^-19 (sn_poisson.h)
-        assert np.allclose(hist, ref["hist"], rtol=4e-6, atol=0.0)
+        assert abs(r.residual - ref["residual"]) <= RES_ABS
+        assert np.all(np.abs(hist - ref["hist"]) <= 4e-6 * ref["hist"] + RES_ABS)
         assert np.all(hist[:-1] > w.tol)
+        if t == 0:
+            # same solve with the ORACLE's ghost values injected: every bit must agree -- field, sweep count, residual,
+            # the exactly tracked history tail; entries before the endgame are lower bounds within 2^-19
+            bnd = oracle.boundary(w.nr, w.nz, w.dr, w.dz, 0, w.lmax, oracle.moments(rho, w.dr, w.dz, 0, w.lmax))
+            s2, got2, r2 = gpu_solve(P, torch_cuda, w, boundary=bnd)
+            assert (r2.sweeps, r2.status) == (ref["sweeps"], 0) and r2.residual == ref["residual"]
+            assert np.array_equal(got2, ref["phi"])
+            h2 = s2.history(r2.sweeps)
+            assert h2[-1] == ref["hist"][-1]
+            assert np.all(h2 <= ref["hist"]) and np.all(h2 >= ref["hist"] * (1 - 4e-6))
         phi_ref = ref["phi"]
         phi_gpu.copy_(torch_cuda.from_numpy(phi_ref))                  # keep both on the same trajectory
         counts.append(r.sweeps)
@@ -504,7 +530,7 @@ def test_batch_full_size_all_members(P, torch_cuda, oracle):
         assert ref["status"] == 0
         assert_field_matches(oracle, w, got[b], res[b], ref)
         assert res[b].sweeps == ref["sweeps"], b
-        assert res[b].residual == pytest.approx(ref["residual"], rel=1e-6)
+        assert res[b].residual == pytest.approx(ref["residual"], rel=0, abs=RES_ABS)
     assert len({r.sweeps for r in res}) > 8                            # members converge at different counts
 
 
