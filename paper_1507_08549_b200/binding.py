@@ -10,7 +10,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsn_poisson.so")
+LIB_PATH = os.environ.get("SN_POISSON_LIB") or os.path.join(_HERE, "libsn_poisson.so")   # override: A/B builds
 
 # every symbol include/sn_poisson.h declares
 EXPORTS = (

@@ -36,7 +36,7 @@ struct BoxShape {
     static constexpr size_t vert_doubles = (size_t)(TYN + 2) * BW;
     static constexpr size_t engine_doubles = f_doubles + 2 * lat_doubles + 2 * vert_doubles;
     // ring duty (halo mode): second-layer columns / rows + the ring threads' private copies of their two edge cells
-    static constexpr size_t ring_doubles = (size_t)4 * (BH + BW);
+    static constexpr size_t ring_doubles = (size_t)2 * (BH + BW);    // + the static stash, 2 (BH + BW)
     static_assert(NT % 32 == 0 && H % 2 == 0, "shape");
 };
 
@@ -48,6 +48,11 @@ __device__ __forceinline__ void ll_store(uint4* p, double v, unsigned tag) {
     const unsigned lo = (unsigned)__double2loint(v), hi = (unsigned)__double2hiint(v);
     asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag)
                  : "memory");
+}
+// the same store without the compiler barrier (the payload comes from registers; nothing has to be ordered before it)
+__device__ __forceinline__ void ll_store_early(uint4* p, double v, unsigned tag) {
+    const unsigned lo = (unsigned)__double2loint(v), hi = (unsigned)__double2hiint(v);
+    asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(lo), "r"(tag), "r"(hi), "r"(tag));
 }
 __device__ __forceinline__ uint4 ll_load(const uint4* p) {
     uint4 v;
@@ -155,8 +160,10 @@ struct BoxEngine {
         l2E = l2W + BH;        // [BH]        column BW-2
         l2S = l2E + BH;        // [2][PW]     row 1, parity planes like exB
         l2N = l2S + BW;        // [2][PW]     row BH-2
-        stash = l2N + BW;      // [2][BH+BW]  per colour: the ring thread's own edge cell
     }
+    // [2][BH+BW] per colour: the ring thread's own edge cell.  A static __shared__ array of the kernel (a distinct
+    // object: its stores do not hold back the loads of the patch update that follows the ring duty).
+    __device__ __forceinline__ void bind_stash(double* p) { stash = p; }
     __device__ __forceinline__ void bind_thread(int tid) {
         a = tid % TXN;
         b = tid / TXN;
@@ -309,7 +316,7 @@ struct BoxEngine {
         }
 #pragma unroll
         for (int q = 0; q < H; ++q) {
-            if (PF && q == H / 2) { if (pf_src) *pf = ll_load_early(pf_src); }
+            if (PF && q == kPfRow) { if (pf_src) *pf = ll_load_early(pf_src); }
             const int pq = (q + COL) & 1;                                   // compile-time after unrolling
             const bool edge_row = q == 0 || q == H - 1;
             const bool any0 = WHICH == 0 || (WHICH == 1 ? (edge_row || pq == 0) : (!edge_row && pq != 0));   // cc = 0
@@ -336,6 +343,7 @@ struct BoxEngine {
                 track<TRACK>(res, pn);
             }
         }
+        if (PF && kPfRow >= H) { if (pf_src) *pf = ll_load_early(pf_src); }
     }
     // publish the updated patch-edge cells of colour COL to the exchange arrays of the CTA
     template <int COL, bool RING = false>
@@ -405,6 +413,9 @@ struct BoxEngine {
     // whole warps of its own (no divergence between the four cases), else the threads are packed E | W | N | S.
     // SEND, plain variant: the owners of the box-edge cells send after their patch update (h_scol / h_srow).
     // SEND, ring variant: see ring_duty().
+    // Patch row before which the first poll is issued (H: after the last row).  Measured (profiles/r02_ring.md): any
+    // earlier position changes nothing, because ptxas sinks the load to its first use whatever the source order is.
+    static constexpr int kPfRow = H;
     int h_edge = -1;                 // 0 E, 1 W, 2 N, 3 S; -1: this thread receives nothing
     int h_j = 0;
     uint4* h_scol = nullptr;         // column edge: west (h_west) or east
@@ -589,7 +600,7 @@ struct BoxEngine {
         }
         double res;
         const double pn = sor_update(cE, cW, iz2, cS, dg, ww, pE, pW, pN, pS, *st, fv, res);
-        ll_store(out, pn, tag);
+        ll_store_early(out, pn, tag);
         *st = pn;
     }
 

@@ -78,7 +78,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1, opt_ring = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1, opt_ring = -1, opt_pfq = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -582,6 +582,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.Q = pl.Q;
     P.max_sweeps = max_sweeps;
     P.force_exact = h->opt_exact;
+    P.pfq = h->opt_pfq;
     P.rho = rho + (size_t)member0 * ncell; P.phi = phi + (size_t)member0 * ncell;
     P.ring = h->d_ring;
     P.mail = reinterpret_cast<uint4*>(h->d_mail);
@@ -1133,6 +1134,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
     if (!strcmp(key, "prof")) { h->opt_prof = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "pfq")) { h->opt_pfq = (int)value; return 0; }
     if (!strcmp(key, "ring")) { if (value < -1 || value > 1) { set_err("ring must be -1, 0 or 1"); return -1; } h->opt_ring = (int)value; return 0; }
     if (!strcmp(key, "ds")) { if (value < -1 || value > 1) { set_err("ds must be -1, 0 or 1"); return -1; } h->opt_ds = (int)value; return 0; }
     if (!strcmp(key, "group")) { if (value < -1 || value > 65535) { set_err("group must be -1, 0 or a member count"); return -1; } h->opt_group = (int)value; return 0; }

@@ -55,6 +55,7 @@ struct ResParams {
     int Q;                     // sweeps per interval (report / checkpoint / decision granularity)
     int max_sweeps;
     int force_exact;           // 1: exact maxima in every interval (exact history; every interval decided before the next)
+    int pfq;                   // ring duty: patch row before which the early poll is issued (-1: H/2)
     const double* rho;         // [nb][ncell]
     double* phi;               // [nb][ncell]  initial guess in, result out
     double* ring;              // [nb][kResRing][ncell]  checkpoints: state after interval r in ring[r % kResRing]
@@ -143,6 +144,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     __shared__ long long s_pf[8];  // in-kernel profile of thread 0 ("prof" option)
     __shared__ typename BoxEngine<H, TXN, TYN, 1>::HaloLinks s_links;   // halo mode: inboxes of this tile and its neighbours
     __shared__ typename BoxEngine<H, TXN, TYN, 1>::RingConst s_ring;    // ring duty: CTA-uniform constants
+    __shared__ double s_stash[RING ? 2 * (BoxShape<H, TXN, TYN>::BH + BoxShape<H, TXN, TYN>::BW) : 1];
 
     const Geom& g = p.g;
     const int member = blockIdx.y;
@@ -272,7 +274,10 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     // =============================================================================================================
     Engine E;
     E.carve(reinterpret_cast<double*>(smem_raw));
-    if (RING) E.carve_ring(reinterpret_cast<double*>(smem_raw + RS::smem_bytes));
+    if (RING) {
+        E.carve_ring(reinterpret_cast<double*>(smem_raw + RS::smem_bytes));
+        E.bind_stash(s_stash);
+    }
     E.bind_thread(tid);
 
     const int tx = tile % p.ntx, ty = tile / p.ntx;
@@ -418,7 +423,10 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             }
             const long long t1 = tick();
             if (HALO && DS) E.template ds_recv<0>(ds_expect, tid == 0, pc_end);      // never abandoned: see box_engine.cuh
-            else if (HALO) E.template halo_recv<0>(s_links, tag0, pc, pf);
+            else if (HALO) {
+                if (RING && prof_on && !ll_ready(pf, tag0)) s_pf[5] += 1;      // early poll came back empty
+                E.template halo_recv<0>(s_links, tag0, pc, pf);
+            }
             const long long t2 = tick();
             Engine::sync();
             const long long t3 = tick();
@@ -449,7 +457,10 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 }
             }
             if (HALO && DS) E.template ds_recv<1>(ds_expect, tid == 0, pc_end);
-            else if (HALO) E.template halo_recv<1>(s_links, tag0 + 1u, pc, pf);
+            else if (HALO) {
+                if (RING && prof_on && !ll_ready(pf, tag0 + 1u)) s_pf[5] += 1;
+                E.template halo_recv<1>(s_links, tag0 + 1u, pc, pf);
+            }
             const long long t5 = tick();
             Engine::sync();
             const long long t6 = tick();
