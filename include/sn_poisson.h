@@ -146,6 +146,10 @@ int sn_poisson_get_history(sn_poisson* h, double* R, int n);
  *   "ds"          path 2 halo mode: 1 = all tiles of a member in one thread-block cluster (<= 16 tiles), edges through
  *                 distributed shared memory (st.async + mbarrier), one cluster per batch member (any batch size: the
  *                 clusters are independent); 0 = never; -1 = planner's choice
+ *   "ring"        path 2 halo mode: 1 = ring duty (every box-edge cell is also updated, first thing in the half-sweep,
+ *                 by the thread that receives on that edge, and sent at once, so that the packets travel during the
+ *                 patch update), 0 = the owners of the edge cells send after their patch update, -1 = planner's
+ *                 choice (on through L2 packets, off inside a cluster)
  *   "ll"          path 2 block mode: 1 = margins travel as tagged packets, 0 = tile flags + ring loads, -1 = auto
  *   "group"       batches on path 2: G > 0 = solve the batch in groups of G members, one resident launch after the
  *                 other; 0 = never group (all members co-resident or another path); -1 = group when the whole batch
@@ -158,7 +162,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value);
 
 /* Counters of the last solve / batch: "launches" (kernels launched), "sweep_launches" (those that ran relaxation
  * sweeps), "sweep_ms" (device time of the relaxation phase, CUDA events on the caller's stream), "setup_ms"
- * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo", "ds",
+ * (moments + boundary), "path" (1, 2 or 3 as above), "ctas", "tile_w", "tile_h", "tblock", "shape", "halo", "ds", "ring",
  * "group" (members per resident launch), "redundancy" (cells updated per half-sweep / cells of the grid: 1 in halo
  * mode and on the streaming path, box cells / tile cells with temporal blocking).
  * Returns 0 or -1. */

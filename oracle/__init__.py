@@ -24,11 +24,32 @@ _lib = None
 _dp = C.POINTER(C.c_double)
 
 
+_EXTRA = {name: (os.path.join(_HERE, name + "_oracle.cpp"), os.path.join(_HERE, "lib" + name + "_oracle.so"))
+          for name in ("levelset", "weno")}
+_extra_libs = {}
+
+
+def _compile(src, lib, force):
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        subprocess.check_call(["g++", *CXXFLAGS, "-o", lib, src])
+    return lib
+
+
 def build(force: bool = False) -> str:
-    """Compile the oracle with g++ (single translation unit)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", *CXXFLAGS, "-o", _LIB, _SRC])
+    """Compile every oracle with g++ (one translation unit, one shared library each)."""
+    _compile(_SRC, _LIB, force)
+    for src, lib in _EXTRA.values():
+        if os.path.exists(src):
+            _compile(src, lib, force)
     return _LIB
+
+
+def extra_lib(name):
+    """ctypes handle of oracle/<name>_oracle.cpp (NEXT rows: level-set re-initialisation, WENO)."""
+    if name not in _extra_libs:
+        src, lib = _EXTRA[name]
+        _extra_libs[name] = C.CDLL(_compile(src, lib, False))
+    return _extra_libs[name]
 
 
 def lib():
@@ -158,3 +179,38 @@ def solve_workload(w, phi0=None, history=False):
     phi0 = np.zeros_like(w.rho) if phi0 is None else phi0
     return solve(w.rho, phi0, w.dr, w.dz, w.symmetry, w.lmax, w.tol, w.max_sweeps, omega=w.omega,
                  history=history)
+
+
+# ---- NEXT-2: level-set re-initialisation (oracle/levelset_oracle.cpp) ------------------------------------------------
+def _ls():
+    L = extra_lib("levelset")
+    L.lso_H.restype = C.c_double
+    L.lso_H.argtypes = [C.c_double, C.c_double]
+    L.lso_crossings.restype = C.c_long
+    L.lso_crossings.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp, _dp]
+    L.lso_reinit.restype = C.c_long
+    L.lso_reinit.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp]
+    return L
+
+
+def levelset_H(d, delta) -> float:
+    return _ls().lso_H(float(d), float(delta))
+
+
+def levelset_crossings(S, dr, dz):
+    """(cx, cy) of every grid-edge crossing of the zero contour, in the oracle's enumeration order."""
+    S = _f64(S)
+    ny, nx = S.shape
+    cx, cy = np.zeros(2 * nx * ny), np.zeros(2 * nx * ny)
+    n = _ls().lso_crossings(nx, ny, dr, dz, _p(S), _p(cx), _p(cy))
+    return cx[:n].copy(), cy[:n].copy()
+
+
+def levelset_reinit(S, dr, dz, delta=None):
+    """Returns dict(S=S_new, dist=signed minimum distance, crossings=count)."""
+    S = _f64(S)
+    ny, nx = S.shape
+    out, dist = np.zeros_like(S), np.zeros_like(S)
+    n = _ls().lso_reinit(nx, ny, dr, dz, dr if delta is None else delta, _p(S), _p(out), _p(dist))
+    assert n >= 0
+    return {"S": out, "dist": dist, "crossings": int(n)}

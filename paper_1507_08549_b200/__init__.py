@@ -2,13 +2,14 @@
 
 The product is the C-ABI library ``libsn_poisson.so`` (include/sn_poisson.h); this package is its thin binding.
 """
-from .binding import (EXPORTS, LIB_PATH, SnPoissonError, load, sn_poisson_create, sn_poisson_destroy,
+from .binding import (EXPORTS, EXPORTS_LEVELSET, sn_levelset_create, sn_levelset_destroy, sn_levelset_get_stat,
+                      sn_levelset_last_error, sn_levelset_reinit, sn_levelset_reinit_host, LIB_PATH, SnPoissonError, load, sn_poisson_create, sn_poisson_destroy,
                       sn_poisson_get_boundary, sn_poisson_get_history, sn_poisson_get_moments,
                       sn_poisson_get_omega, sn_poisson_get_stat, sn_poisson_gravity, sn_poisson_last_error,
                       sn_poisson_result,
                       sn_poisson_set_boundary, sn_poisson_set_omega, sn_poisson_set_option, sn_poisson_solve,
                       sn_poisson_solve_batch, sn_poisson_solve_batch_host, sn_poisson_solve_host,
                       sn_poisson_solve_sequence_host, sn_poisson_probe_l2, sn_poisson_version)
-from .solver import PoissonSolver
+from .solver import LevelSet, PoissonSolver
 
-__all__ = ["PoissonSolver", "SnPoissonError", "EXPORTS", "LIB_PATH", "load", "sn_poisson_result"] + list(EXPORTS)
+__all__ = ["PoissonSolver", "LevelSet", "SnPoissonError", "EXPORTS", "LIB_PATH", "load", "sn_poisson_result"] + list(EXPORTS) + list(EXPORTS_LEVELSET)

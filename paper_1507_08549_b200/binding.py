@@ -22,6 +22,13 @@ EXPORTS = (
 )
 
 
+# every symbol include/sn_levelset.h declares (NEXT-2)
+EXPORTS_LEVELSET = (
+    "sn_levelset_create", "sn_levelset_reinit", "sn_levelset_reinit_host", "sn_levelset_get_stat",
+    "sn_levelset_destroy", "sn_levelset_last_error",
+)
+
+
 class sn_poisson_result(C.Structure):
     _fields_ = [("sweeps", C.c_int32), ("status", C.c_int32), ("residual", C.c_double)]
 
@@ -88,6 +95,18 @@ def load():
     lib.sn_poisson_last_error.argtypes = []
     lib.sn_poisson_version.restype = C.c_char_p
     lib.sn_poisson_version.argtypes = []
+    lib.sn_levelset_create.restype = _vp
+    lib.sn_levelset_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]
+    lib.sn_levelset_reinit.restype = C.c_int64
+    lib.sn_levelset_reinit.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.sn_levelset_reinit_host.restype = C.c_int64
+    lib.sn_levelset_reinit_host.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.sn_levelset_get_stat.restype = C.c_int
+    lib.sn_levelset_get_stat.argtypes = [_vp, C.c_char_p, _dp]
+    lib.sn_levelset_destroy.restype = None
+    lib.sn_levelset_destroy.argtypes = [_vp]
+    lib.sn_levelset_last_error.restype = C.c_char_p
+    lib.sn_levelset_last_error.argtypes = []
     _lib = lib
     return lib
 
@@ -224,4 +243,43 @@ def sn_poisson_set_option(h, key: str, value: int) -> int:
 def sn_poisson_get_stat(h, key: str) -> float:
     out = C.c_double(0.0)
     _check(load().sn_poisson_get_stat(h, key.encode(), C.byref(out)), f"sn_poisson_get_stat({key})")
+    return out.value
+
+
+# ---- NEXT-2: level-set re-initialisation (include/sn_levelset.h) ------------------------------------------------------
+def sn_levelset_last_error() -> str:
+    return load().sn_levelset_last_error().decode()
+
+
+def sn_levelset_create(nx, ny, dr, dz, delta):
+    h = load().sn_levelset_create(int(nx), int(ny), float(dr), float(dz), float(delta))
+    if not h:
+        raise SnPoissonError("sn_levelset_create failed: " + sn_levelset_last_error())
+    return h
+
+
+def sn_levelset_destroy(h):
+    load().sn_levelset_destroy(h)
+
+
+def sn_levelset_reinit(h, s_old_ptr, s_new_ptr, dist_ptr=0, stream=0) -> int:
+    """DEVICE addresses; returns the number of crossings."""
+    n = load().sn_levelset_reinit(h, s_old_ptr, s_new_ptr, dist_ptr or None, stream or None)
+    if n < 0:
+        raise SnPoissonError(f"sn_levelset_reinit failed ({n}): " + sn_levelset_last_error())
+    return n
+
+
+def sn_levelset_reinit_host(h, s_old_ptr, s_new_ptr, dist_ptr=0, stream=0) -> int:
+    """HOST addresses; returns the number of crossings."""
+    n = load().sn_levelset_reinit_host(h, s_old_ptr, s_new_ptr, dist_ptr or None, stream or None)
+    if n < 0:
+        raise SnPoissonError(f"sn_levelset_reinit_host failed ({n}): " + sn_levelset_last_error())
+    return n
+
+
+def sn_levelset_get_stat(h, key: str) -> float:
+    out = C.c_double(0.0)
+    if load().sn_levelset_get_stat(h, key.encode(), C.byref(out)) != 0:
+        raise SnPoissonError("sn_levelset_get_stat: " + sn_levelset_last_error())
     return out.value

@@ -37,6 +37,7 @@ struct BoxShape {
     static constexpr size_t engine_doubles = f_doubles + 2 * lat_doubles + 2 * vert_doubles;
     // ring duty (halo mode): second-layer columns / rows + the ring threads' private copies of their two edge cells
     static constexpr size_t ring_doubles = (size_t)2 * (BH + BW);    // + the static stash, 2 (BH + BW)
+    static constexpr size_t ring_ds_doubles = ring_doubles + (size_t)2 * (BH + BW);   // + the DSMEM landing zone
     static_assert(NT % 32 == 0 && H % 2 == 0, "shape");
 };
 
@@ -119,7 +120,7 @@ struct BoxEngine {
     double* exR;    // [BH][LS]        column 3 of thread a at [row][a+1]
     double* exB;    // [TYN+2][2][PW]  bottom row of thread-row b at [b+1]
     double* exT;    // [TYN+2][2][PW]  top row of thread-row b at [b+1]
-    double *l2W = nullptr, *l2E = nullptr, *l2S = nullptr, *l2N = nullptr, *stash = nullptr;   // ring duty only
+    double *l2W = nullptr, *l2E = nullptr, *l2S = nullptr, *l2N = nullptr, *stash = nullptr, *land = nullptr;   // ring duty only
 
     // Inbox of one tile: tagged packets it receives from its four neighbours, [E: BH][W: BH][N: BW][S: BW], each edge
     // split by colour so that the packets of one half-sweep are contiguous: slot(i) = (i & 1) * n/2 + (i >> 1).
@@ -160,6 +161,7 @@ struct BoxEngine {
         l2E = l2W + BH;        // [BH]        column BW-2
         l2S = l2E + BH;        // [2][PW]     row 1, parity planes like exB
         l2N = l2S + BW;        // [2][PW]     row BH-2
+        land = l2N + BW;       // [2][BH+BW]  cluster mode only: where the neighbours' st.async land, per colour
     }
     // [2][BH+BW] per colour: the ring thread's own edge cell.  A static __shared__ array of the kernel (a distinct
     // object: its stores do not hold back the loads of the patch update that follows the ring duty).
@@ -526,6 +528,7 @@ struct BoxEngine {
         double cE_w, cW_w;           // ... first column (west edge)
         const double *cE, *cW;       // g.cE + bx, g.cW + bx (row-edge threads index them with their column)
         int mirror_box;              // the box's row 0 is the reflecting equator row
+        int tile, ntx;               // cluster mode: rank of this tile in the cluster, tiles per tile row
     };
 
     // stash <- the current values of this thread's two edge cells; call after publish_all() + sync, then sync again
@@ -547,7 +550,7 @@ struct BoxEngine {
     }
 
     // One specialised straight-line body per edge: every address is (compile-time constant) + (stride) * j.
-    template <int COL, int EDGE>
+    template <int COL, int EDGE, bool DSM = false>
     __device__ __forceinline__ void ring_cell(const HaloLinks& L, const RingConst& rc, unsigned tag) {
         const int j = h_j;
         double pE, pW, pN, pS, fv, cE, cW;
@@ -600,16 +603,31 @@ struct BoxEngine {
         }
         double res;
         const double pn = sor_update(cE, cW, iz2, cS, dg, ww, pE, pW, pN, pS, *st, fv, res);
-        ll_store_early(out, pn, tag);
+        if (DSM) {
+            // cluster mode: straight into the neighbour's landing zone (the slot of ITS receiving thread on the
+            // opposite edge, same j) through distributed shared memory; the bytes are credited to its mbarrier[COL].
+            // A landing slot of colour COL is rewritten two half-sweeps later, after the neighbour's packets of the
+            // half-sweep in between have arrived here, which it sends only after it has consumed this one.
+            const int nslot = EDGE == 0 ? BH / 2 + j : EDGE == 1 ? j : EDGE == 2 ? BH + BW / 2 + j : BH + j;
+            const unsigned rank = (unsigned)(EDGE == 0 ? rc.tile + 1 : EDGE == 1 ? rc.tile - 1 : EDGE == 2 ? rc.tile + rc.ntx : rc.tile - rc.ntx);
+            ds_store(ds_mapa(smem_u32(land + COL * (BH + BW) + nslot), rank), pn, ds_mapa(ds_bar + 8u * COL, rank));
+        } else {
+            ll_store_early(out, pn, tag);
+        }
         *st = pn;
     }
 
-    template <int COL>
+    template <int COL, bool DSM = false>
     __device__ __forceinline__ void ring_duty(const HaloLinks& L, const RingConst& rc, unsigned tag) {
-        if (h_edge == 0) ring_cell<COL, 0>(L, rc, tag);
-        else if (h_edge == 1) ring_cell<COL, 1>(L, rc, tag);
-        else if (h_edge == 2) ring_cell<COL, 2>(L, rc, tag);
-        else if (h_edge == 3) ring_cell<COL, 3>(L, rc, tag);
+        if (h_edge == 0) ring_cell<COL, 0, DSM>(L, rc, tag);
+        else if (h_edge == 1) ring_cell<COL, 1, DSM>(L, rc, tag);
+        else if (h_edge == 2) ring_cell<COL, 2, DSM>(L, rc, tag);
+        else if (h_edge == 3) ring_cell<COL, 3, DSM>(L, rc, tag);
+    }
+    // cluster mode, after ds_recv<COL>: every receiving thread moves its value from the landing zone to the border slot
+    template <int COL>
+    __device__ __forceinline__ void ds_ring_copy() {
+        if (h_edge >= 0) *recv_dst<COL>() = land[COL * (BH + BW) + ring_slot()];
     }
 
     // ---- halo mode inside ONE thread-block cluster: distributed shared memory instead of L2 packets ----------------

@@ -78,7 +78,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1, opt_ring = -1, opt_pfq = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1, opt_ring = -1;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -390,24 +390,28 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
 // ---- resident path: shapes, planner, launcher ------------------------------------------------------------------
 struct ShapeInfo {
     int H, TXN, TYN, minb;
-    size_t smem, smem_ring;
-    const void* fn[4];          // [0] block mode, [1] halo mode, [2] halo mode inside one cluster (DSMEM) or NULL,
-                                // [3] halo mode with ring duty
+    size_t smem, smem_ring, smem_ring_ds;
+    const void* fn[5];          // [0] block mode, [1] halo mode, [2] halo mode inside one cluster (DSMEM) or NULL,
+                                // [3] halo mode with ring duty, [4] cluster halo mode with ring duty or NULL
     int BW() const { return 4 * TXN; }
     int BH() const { return H * TYN; }
     int NT() const { return TXN * TYN; }
     int threads() const { return TXN * TYN + 32; }     // + the service warp
-    size_t smem_of(int f) const { return f == 3 ? smem_ring : smem; }
+    size_t smem_of(int f) const { return f == 3 ? smem_ring : f == 4 ? smem_ring_ds : smem; }
 };
 
 template <int H, int TXN, int TYN, int MINB, bool DS = true>
 ShapeInfo shape_of() {
-    const void* ds = nullptr;
-    if constexpr (DS) ds = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false, true>;
+    const void *ds = nullptr, *dsr = nullptr;
+    if constexpr (DS) {
+        ds = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false, true>;
+        dsr = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, true, true>;
+    }
     return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes, ResShape<H, TXN, TYN>::smem_bytes_ring,
+            ResShape<H, TXN, TYN>::smem_bytes_ring_ds,
             {(const void*)k_sor_resident<H, TXN, TYN, MINB, false, false>,
              (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false>, ds,
-             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, true>}};
+             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, true>, dsr}};
 }
 
 const std::vector<ShapeInfo>& shapes() {
@@ -436,15 +440,18 @@ double model_half_sweep(const ShapeInfo& S, int k) {
     const double lat = S.H <= 2 ? 215.0 : S.H <= 4 ? 420.0 : S.H <= 6 ? 480.0 : 545.0;
     const double warps_per_smsp = std::ceil(k * (S.NT() / 32.0) / 4.0);
     // CTAs sharing an SM also share its latency-bound phases (measured: ~ +50 % per extra CTA)
-    double t = std::max(lat * (1.0 + 0.5 * (k - 1)), warps_per_smsp * dpw * 2.0 / 0.62 + 100.0);
+    // ... and every half-sweep costs each warp ~70 + 22 H issue slots (SASS of the sweep loops: 102 instructions per
+    // half-sweep at H = 2, ~250 at H = 8), one per clock and sub-partition: the limit of the many-warp small-patch shapes
+    const double issue = warps_per_smsp * (70.0 + 22.0 * S.H);
+    double t = std::max(std::max(lat * (1.0 + 0.5 * (k - 1)), warps_per_smsp * dpw * 2.0 / 0.62 + 100.0), issue);
     if (S.threads() * S.minb > 448 && k == 1 && S.H == 8 && S.NT() < 448) t = std::max(t, 1400.0);   // 128-register cap
     return t;
 }
 
 // Can `nclusters` clusters of `csize` CTAs of this shape be resident at once?
-bool cluster_fits(sn_poisson* h, const ShapeInfo& S, int csize, int nclusters) {
-    const void* fn = S.fn[2];
-    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem) != cudaSuccess ||
+bool cluster_fits(sn_poisson* h, const ShapeInfo& S, int fi, int csize, int nclusters) {
+    const void* fn = S.fn[fi];
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem_of(fi)) != cudaSuccess ||
         (csize > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
         cudaGetLastError();
         return false;
@@ -452,7 +459,7 @@ bool cluster_fits(sn_poisson* h, const ShapeInfo& S, int csize, int nclusters) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(csize, nclusters);
     cfg.blockDim = dim3(S.threads());
-    cfg.dynamicSmemBytes = S.smem;
+    cfg.dynamicSmemBytes = S.smem_of(fi);
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = csize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
@@ -496,14 +503,18 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
                 const int k = (int)((p.ntiles * (long long)nbatch + h->num_sms - 1) / h->num_sms);
                 // per half-sweep: compute + the exposed part of the edge exchange (poll round trips, barrier, the
                 // neighbour's slowest warp) + the checkpoint / report of the interval
-                p.cost = 2.0 * (model_half_sweep(S, k) + 1500.0 + 0.1 * S.BW() * S.BH());
+                // (ring duty: the packet flight overlaps the patch update; what stays exposed is the ring duty itself, one
+                // L2 round trip of the poll and the barrier skew -- calibrated on profiles/r02_ring.md)
+                p.cost = 2.0 * (model_half_sweep(S, k) + (p.ring ? 1350.0 + 0.05 * S.BW() * S.BH() : 1500.0 + 0.1 * S.BW() * S.BH()));
                 if (best.shape < 0 || p.cost < best.cost) best = p;
             }
         }
         // halo mode with all tiles of a member in ONE thread-block cluster: edges through distributed shared memory
         if (h->opt_halo != 0 && h->opt_ds != 0 && S.fn[2] && h->nr % S.BW() == 0 && h->nz % S.H == 0) {
             ResPlan p;
-            p.shape = si; p.halo = 1; p.ds = 1;
+            // ring duty in cluster mode only on request: a DSMEM st.async needs ~550 clocks until the mbarrier fires,
+            // more than the patch update of the small boxes this mode serves, so sending first gains nothing there
+            p.shape = si; p.halo = 1; p.ds = 1; p.ring = h->opt_ring == 1;
             p.ntx = h->nr / S.BW(); p.nty = (h->nz + S.BH() - 1) / S.BH();
             p.ow = S.BW(); p.oh = S.BH();
             p.ntiles = p.ntx * p.nty;
@@ -511,7 +522,7 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
             p.m = p.Q;
             // members are independent and a cluster is gang-scheduled, so the clusters of a batch need not be
             // co-resident with each other: any batch size runs, in waves of clusters if it has to
-            if (p.ntiles > 1 && p.ntiles <= 16 && cluster_fits(h, S, p.ntiles, 1)) {
+            if (p.ntiles > 1 && p.ntiles <= 16 && cluster_fits(h, S, p.ring ? 4 : 2, p.ntiles, 1)) {
                 // per half-sweep: compute + the edge threads' st.async (~250 clocks) + one DSMEM hop and the mbarrier
                 // wake-up (~300); 420 puts the model where the measurements are (128^2: wins; 64^2, 256^2: block mode)
                 p.cost = 2.0 * (model_half_sweep(S, 1) + 420.0);
@@ -582,7 +593,6 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.Q = pl.Q;
     P.max_sweeps = max_sweeps;
     P.force_exact = h->opt_exact;
-    P.pfq = h->opt_pfq;
     P.rho = rho + (size_t)member0 * ncell; P.phi = phi + (size_t)member0 * ncell;
     P.ring = h->d_ring;
     P.mail = reinterpret_cast<uint4*>(h->d_mail);
@@ -610,7 +620,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
         h->prof_ctas = (size_t)pl.ntiles * nbatch;
     }
     void* args[] = {&P};
-    const int fi = pl.ds ? 2 : pl.halo ? (pl.ring ? 3 : 1) : 0;
+    const int fi = pl.ds ? (pl.ring ? 4 : 2) : pl.halo ? (pl.ring ? 3 : 1) : 0;
     const void* fn = S.fn[fi];
     const size_t smem = S.smem_of(fi);
     // (the planner has already set the kernel's shared-memory attribute; plans are cached on the handle)
@@ -634,7 +644,7 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     h->st_launches += 1;
     h->st_path = 2;
     h->st_ctas = (double)pl.ntiles * nbatch; h->st_tile_w = pl.ow; h->st_tile_h = pl.oh; h->st_tblock = pl.Q;
-    h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch; h->st_ds = pl.ds; h->st_ring = pl.ring && !pl.ds;
+    h->st_shape = pl.shape; h->st_halo = pl.halo; h->st_group = nbatch; h->st_ds = pl.ds; h->st_ring = pl.ring;
     h->st_redund = pl.halo ? 1.0 : (double)pl.ntiles * S.BW() * S.BH() / ((double)h->nr * h->nz);
     return 0;
 }
@@ -1134,7 +1144,6 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "chunk")) { if (value < 1) { set_err("chunk must be >= 1"); return -1; } h->opt_chunk = (int)value; return 0; }
     if (!strcmp(key, "exact")) { h->opt_exact = value ? 1 : 0; return 0; }
     if (!strcmp(key, "prof")) { h->opt_prof = value ? 1 : 0; return 0; }
-    if (!strcmp(key, "pfq")) { h->opt_pfq = (int)value; return 0; }
     if (!strcmp(key, "ring")) { if (value < -1 || value > 1) { set_err("ring must be -1, 0 or 1"); return -1; } h->opt_ring = (int)value; return 0; }
     if (!strcmp(key, "ds")) { if (value < -1 || value > 1) { set_err("ds must be -1, 0 or 1"); return -1; } h->opt_ds = (int)value; return 0; }
     if (!strcmp(key, "group")) { if (value < -1 || value > 65535) { set_err("group must be -1, 0 or a member count"); return -1; } h->opt_group = (int)value; return 0; }

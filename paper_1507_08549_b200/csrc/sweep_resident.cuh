@@ -55,7 +55,6 @@ struct ResParams {
     int Q;                     // sweeps per interval (report / checkpoint / decision granularity)
     int max_sweeps;
     int force_exact;           // 1: exact maxima in every interval (exact history; every interval decided before the next)
-    int pfq;                   // ring duty: patch row before which the early poll is issued (-1: H/2)
     const double* rho;         // [nb][ncell]
     double* phi;               // [nb][ncell]  initial guess in, result out
     double* ring;              // [nb][kResRing][ncell]  checkpoints: state after interval r in ring[r % kResRing]
@@ -120,6 +119,7 @@ struct ResShape {
     static constexpr size_t smax_entries = (size_t)2 * 2 * kMaxTB * NW;       // [parity][2Q][NW]
     static constexpr size_t smem_bytes = sizeof(double) * S::engine_doubles + sizeof(unsigned long long) * smax_entries;
     static constexpr size_t smem_bytes_ring = smem_bytes + sizeof(double) * S::ring_doubles;
+    static constexpr size_t smem_bytes_ring_ds = smem_bytes + sizeof(double) * S::ring_ds_doubles;
 };
 
 // grid = (ntx*nty, nbatch), block = TXN*TYN + 32 threads (the last warp is the service warp), cooperative launch.
@@ -128,7 +128,7 @@ struct ResShape {
 // DS (halo mode, all tiles of a member in one thread-block cluster): edges travel through distributed shared memory.
 template <int H, int TXN, int TYN, int MINB, bool HALO, bool RING, bool DS = false>
 __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResParams p) {
-    static_assert(!RING || (HALO && !DS), "ring duty belongs to the L2-packet halo mode");
+    static_assert(!RING || HALO, "ring duty belongs to the halo mode");
     using S = BoxShape<H, TXN, TYN>;
     using RS = ResShape<H, TXN, TYN>;
     constexpr int BW = S::BW, BH = S::BH, NT = S::NT, NW = S::NW;
@@ -312,7 +312,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
         links.n = (ty + 1 < p.nty) ? inbox(tile + p.ntx) : nullptr;
         links.rows = min(BH, g.nz - by);
         if (DS) E.ds_bind(links, s_mbar, tile, p.ntx);
-        else E.template halo_bind<RING>(links, tid);
+        if (!DS || RING) E.template halo_bind<RING>(links, tid);
         if (tid == 0) {                        // CTA-uniform: read from shared memory in the sweep loop, not kept in registers
             s_links = links;
             if (RING) {
@@ -320,6 +320,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 s_ring.cE_w = g.cE[bx]; s_ring.cW_w = g.cW[bx];
                 s_ring.cE = g.cE + bx; s_ring.cW = g.cW + bx;
                 s_ring.mirror_box = mirror_box ? 1 : 0;
+                s_ring.tile = tile; s_ring.ntx = p.ntx;
             }
         }
     }
@@ -413,30 +414,42 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             const long long t0 = tick();
             const unsigned tag0 = tagbase + 2u * (unsigned)(k0 + s) + 1u;
             uint4 pf = make_uint4(0u, 0u, 0u, 0u);
-            if (RING) {
+            if (RING && DS) {
+                E.template ring_duty<0, true>(s_links, s_ring, tag0);
+                if (prof_on) s_pf[5] += tick() - t0;                         // ring duty alone (slot 5: block mode's refill)
+                E.template half_sweep<0, TRACK, false, true>();
+            } else if (RING) {
                 E.template ring_duty<0>(s_links, s_ring, tag0);
+                if (prof_on) s_pf[5] += tick() - t0;
                 pf = E.template half_sweep_ring<0, TRACK>(s_links);
             } else {
                 E.template half_sweep<0, TRACK, false>();
-                if (HALO && DS) E.template ds_send<0>();
-                else if (HALO) E.template halo_send<0>(tag0);
+                if (HALO && DS && !RING) E.template ds_send<0>();
+                else if (HALO && !DS) E.template halo_send<0>(tag0);
             }
             const long long t1 = tick();
-            if (HALO && DS) E.template ds_recv<0>(ds_expect, tid == 0, pc_end);      // never abandoned: see box_engine.cuh
+            if (HALO && DS) {
+                E.template ds_recv<0>(ds_expect, tid == 0, pc_end);      // never abandoned: see box_engine.cuh
+                if (RING) E.template ds_ring_copy<0>();
+            }
             else if (HALO) {
-                if (RING && prof_on && !ll_ready(pf, tag0)) s_pf[5] += 1;      // early poll came back empty
                 E.template halo_recv<0>(s_links, tag0, pc, pf);
             }
             const long long t2 = tick();
             Engine::sync();
             const long long t3 = tick();
-            if (RING) {
+            if (RING && DS) {
+                E.template ring_duty<1, true>(s_links, s_ring, tag0 + 1u);
+                if (prof_on) s_pf[5] += tick() - t3;
+                E.template half_sweep<1, TRACK, false, true>();
+            } else if (RING) {
                 E.template ring_duty<1>(s_links, s_ring, tag0 + 1u);
+                if (prof_on) s_pf[5] += tick() - t3;
                 pf = E.template half_sweep_ring<1, TRACK>(s_links);
             } else {
                 E.template half_sweep<1, TRACK, false>();
-                if (HALO && DS) E.template ds_send<1>();
-                else if (HALO) E.template halo_send<1>(tag0 + 1u);
+                if (HALO && DS && !RING) E.template ds_send<1>();
+                else if (HALO && !DS) E.template halo_send<1>(tag0 + 1u);
             }
             const long long t4 = tick();
             // the sweep's maxima are complete: reduce them across the warp BEFORE the last wait / barrier of the sweep,
@@ -456,9 +469,11 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                     smax[((size_t)par * 2 * kMaxTB + 2 * s + 1) * NW + warp] = wp;
                 }
             }
-            if (HALO && DS) E.template ds_recv<1>(ds_expect, tid == 0, pc_end);
+            if (HALO && DS) {
+                E.template ds_recv<1>(ds_expect, tid == 0, pc_end);
+                if (RING) E.template ds_ring_copy<1>();
+            }
             else if (HALO) {
-                if (RING && prof_on && !ll_ready(pf, tag0 + 1u)) s_pf[5] += 1;
                 E.template halo_recv<1>(s_links, tag0 + 1u, pc, pf);
             }
             const long long t5 = tick();

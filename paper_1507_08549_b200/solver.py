@@ -141,3 +141,44 @@ class PoissonSolver:
     @property
     def omega(self):
         return B.sn_poisson_get_omega(self.h)
+
+
+class LevelSet:
+    """Owns one sn_levelset handle (NEXT-2: level-set re-initialisation).  ``S``: float64 CUDA tensor (ny, nx) of the
+    scalar field on the cell corners."""
+
+    def __init__(self, nx, ny, dr, dz, delta=None):
+        self.nx, self.ny = nx, ny
+        self.h = B.sn_levelset_create(nx, ny, dr, dz, dr if delta is None else delta)
+
+    def close(self):
+        if getattr(self, "h", None) and getattr(B, "sn_levelset_destroy", None):
+            B.sn_levelset_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def reinit(self, S, want_dist=False):
+        """Returns (S_new, dist or None, crossings); enqueued on the current stream, synchronised by the library."""
+        import torch
+        if not (S.is_cuda and S.dtype == torch.float64 and S.is_contiguous() and tuple(S.shape) == (self.ny, self.nx)):
+            raise ValueError("expected a contiguous float64 CUDA tensor of shape (ny, nx)")
+        out = torch.empty_like(S)
+        dist = torch.empty_like(S) if want_dist else None
+        n = B.sn_levelset_reinit(self.h, S.data_ptr(), out.data_ptr(), dist.data_ptr() if want_dist else 0,
+                                 torch.cuda.current_stream().cuda_stream)
+        return out, dist, n
+
+    def reinit_host(self, S_np, want_dist=False):
+        import numpy as np
+        import torch
+        if S_np.dtype != np.float64 or not S_np.flags.c_contiguous or tuple(S_np.shape) != (self.ny, self.nx):
+            raise ValueError("expected a C-contiguous float64 numpy array of shape (ny, nx)")
+        out = np.empty_like(S_np)
+        dist = np.empty_like(S_np) if want_dist else None
+        n = B.sn_levelset_reinit_host(self.h, S_np.ctypes.data, out.ctypes.data, dist.ctypes.data if want_dist else 0,
+                                      torch.cuda.current_stream().cuda_stream)
+        return out, dist, n
+
+    def stat(self, key):
+        return B.sn_levelset_get_stat(self.h, key)

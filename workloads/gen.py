@@ -295,3 +295,29 @@ def random_smooth(nr: int, nz: int, symmetry: int, seed: int, lmax: int = 8,
                             np.exp(-((r - rk) ** 2) / (2 * w * w)))
     return Workload(f"smooth_{nr}x{nz}_s{symmetry}_{seed}", nr, nz, dr, dz, symmetry, lmax,
                     1e-10, 20000, np.ascontiguousarray(rho), meta={"seed": seed})
+
+
+# ----------------------------------------------------------------------------
+# NEXT-2: a flame front for the level-set re-initialisation ("An initial three-finger flame front is
+# imposed, which is comparable with the c3 flame"; "500 grids in each direction")
+# ----------------------------------------------------------------------------
+def levelset_front(ncells: int = 500, seed: int = 7, distort: float = 0.5):
+    """S on the (ncells+1)^2 cell CORNERS of the unit (r,z) quadrant, dr = dz = 1/ncells.  Zero contour: three fingers,
+    s = R0 (1 + A cos(12 theta - pi)) (maxima at theta = pi/12, pi/4, 5 pi/12 from the z axis; dR/dtheta = 0 on the axis
+    and on the equator).  S > 0 inside (ash).  The magnitude is distorted by a smooth seeded factor 1 + distort * u(r,z),
+    |u| <= 1, so that |grad S| != 1 -- what an advection step leaves behind and re-initialisation has to repair.
+    Returns (S, dr)."""
+    n = ncells + 1
+    dr = 1.0 / ncells
+    x = np.arange(n) * dr
+    X, Y = np.meshgrid(x, x)                      # X: r (fastest index), Y: z
+    s = np.hypot(X, Y)
+    theta = np.arctan2(X, Y)                      # from the +z axis
+    R = 0.3 * (1.0 + 0.25 * np.cos(12.0 * theta - math.pi))
+    u = np.zeros_like(s)
+    for k in range(4):
+        kx = uniform(seed, 1, 3 * k, 2.0, 9.0)
+        ky = uniform(seed, 1, 3 * k + 1, 2.0, 9.0)
+        ph = uniform(seed, 1, 3 * k + 2, 0.0, 2.0 * math.pi)
+        u += 0.25 * np.sin(kx * X * math.pi + ph) * np.cos(ky * Y * math.pi)
+    return np.ascontiguousarray((R - s) * (1.0 + distort * u)), dr
