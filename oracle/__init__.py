@@ -68,6 +68,10 @@ def lib():
                                     _dp, _dp, C.c_int, _dp, _dp]
         _lib.sno_solve.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, _dp,
                                    _dp, C.c_double, C.c_int, C.POINTER(C.c_int), _dp, _dp, _dp, _dp, _dp]
+        _lib.sno_solve_rule.argtypes = [C.c_int] + _lib.sno_solve.argtypes
+        _lib.sno_sweeps_chg.argtypes = _lib.sno_sweeps.argtypes + [_dp]
+        _lib.sno_relchange.restype = C.c_double
+        _lib.sno_relchange.argtypes = [C.c_double, C.c_double]
         _lib.sno_gravity.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib.sno_apply_operator.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp,
                                             _dp, _dp]
@@ -134,9 +138,29 @@ def sweeps(rho, phi, dr, dz, symmetry, omega, bE, bN, bS, nsweeps):
     return phi, Rabs[:nsweeps], P[:nsweeps]
 
 
+def sweeps_chg(rho, phi, dr, dz, symmetry, omega, bE, bN, bS, nsweeps):
+    """sweeps() plus Chg[k] = max |w_j res| of every sweep (R16).  Returns (phi_new, Rabs, P, Chg)."""
+    rho = _f64(rho)
+    nz, nr = rho.shape
+    phi = np.array(phi, dtype=np.float64, order="C", copy=True)
+    bE, bN = _f64(bE), _f64(bN)
+    bS = _f64(bS) if bS is not None else np.zeros(nr)
+    n = max(nsweeps, 1)
+    Rabs, P, Chg = np.zeros(n), np.zeros(n), np.zeros(n)
+    rc = lib().sno_sweeps_chg(nr, nz, dr, dz, symmetry, omega, _p(rho), _p(bE), _p(bN), _p(bS), _p(phi), nsweeps,
+                              _p(Rabs), _p(P), _p(Chg))
+    assert rc == 0
+    return phi, Rabs[:nsweeps], P[:nsweeps], Chg[:nsweeps]
+
+
+def relchange(Chg, P) -> float:
+    return lib().sno_relchange(Chg, P)
+
+
 def solve(rho, phi0, dr, dz, symmetry, lmax, tol, max_sweeps, omega=None, boundary_arrays=None,
-          history=False):
-    """Whole path.  Returns dict(phi, sweeps, residual, status[, hist])."""
+          history=False, rule=0):
+    """Whole path.  rule 0: residual rule R9; rule 1: the paper-literal relative-change rule R16.
+    Returns dict(phi, sweeps, residual, status[, hist])."""
     rho = _f64(rho)
     nz, nr = rho.shape
     phi = np.array(phi0, dtype=np.float64, order="C", copy=True)
@@ -147,8 +171,9 @@ def solve(rho, phi0, dr, dz, symmetry, lmax, tol, max_sweeps, omega=None, bounda
         bE, bN, bS = boundary_arrays
         bE, bN = _f64(bE), _f64(bN)
         bS = _f64(bS) if bS is not None else np.zeros(nr)
-    rc = lib().sno_solve(nr, nz, dr, dz, symmetry, lmax, -1.0 if omega is None else float(omega), _p(rho),
-                         _p(phi), tol, max_sweeps, C.byref(nsw), C.byref(res), _p(hist), _p(bE), _p(bN), _p(bS))
+    rc = lib().sno_solve_rule(int(rule), nr, nz, dr, dz, symmetry, lmax, -1.0 if omega is None else float(omega),
+                              _p(rho), _p(phi), tol, max_sweeps, C.byref(nsw), C.byref(res), _p(hist), _p(bE), _p(bN),
+                              _p(bS))
     out = {"phi": phi, "sweeps": nsw.value, "residual": res.value, "status": rc}
     if history:
         out["hist"] = hist[: nsw.value]

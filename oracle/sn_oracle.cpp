@@ -160,9 +160,22 @@ int sno_boundary(int nr, int nz, double dr, double dz, int symmetry, int lmax, c
 //   res = f - t;  pC <- fma(-(omega/diag), res, pC),  f = FOURPI*rho.
 // Per sweep k (1-based) records Rabs[k-1] = max |res| seen (pre-update, both colours) and
 // P[k-1] = max |p_new| [R9].  bS is ignored when symmetry=1.
+int sno_sweeps_chg(int nr, int nz, double dr, double dz, int symmetry, double omega, const double* rho,
+                   const double* bE, const double* bN, const double* bS, double* phi, int nsweeps,
+                   double* Rabs_hist, double* P_hist, double* Chg_hist);
+
 int sno_sweeps(int nr, int nz, double dr, double dz, int symmetry, double omega, const double* rho,
                const double* bE, const double* bN, const double* bS, double* phi, int nsweeps,
                double* Rabs_hist, double* P_hist) {
+    return sno_sweeps_chg(nr, nz, dr, dz, symmetry, omega, rho, bE, bN, bS, phi, nsweeps, Rabs_hist, P_hist, nullptr);
+}
+
+// The same sweeps; additionally Chg[k-1] = max over the cells of |w_j * res| [R16]: the change of phi the update of
+// sweep k applies to a cell is dphi = -(omega/diag_j) res (the update is phi <- fma(-w_j, res, phi))
+// "relative changes of all grids".
+int sno_sweeps_chg(int nr, int nz, double dr, double dz, int symmetry, double omega, const double* rho,
+                   const double* bE, const double* bN, const double* bS, double* phi, int nsweeps,
+                   double* Rabs_hist, double* P_hist, double* Chg_hist) {
     if (nr < 1 || nz < 1 || !rho || !bE || !bN || !phi || (symmetry == 0 && !bS)) return -1;
     const double ir2 = 1.0 / (dr * dr);
     const double iz2 = 1.0 / (dz * dz);
@@ -176,7 +189,7 @@ int sno_sweeps(int nr, int nz, double dr, double dz, int symmetry, double omega,
         cW[i] = (i / (i + 0.5)) * ir2;
     }
     for (int k = 0; k < nsweeps; ++k) {
-        double Rabs = 0.0, P = 0.0;
+        double Rabs = 0.0, P = 0.0, Chg = 0.0;
         for (int colour = 0; colour < 2; ++colour) {
             for (int j = 0; j < nz; ++j) {
                 const bool mirror_row = (symmetry == 1 && j == 0);
@@ -202,11 +215,14 @@ int sno_sweeps(int nr, int nz, double dr, double dz, int symmetry, double omega,
                     const double ares = std::fabs(res), apn = std::fabs(pnew);
                     if (ares > Rabs || ares != ares) Rabs = ares;
                     if (apn > P || apn != apn) P = apn;
+                    const double achg = std::fabs(w * res);
+                    if (achg > Chg || achg != achg) Chg = achg;
                 }
             }
         }
         if (Rabs_hist) Rabs_hist[k] = Rabs;
         if (P_hist) P_hist[k] = P;
+        if (Chg_hist) Chg_hist[k] = Chg;
     }
     return 0;
 }
@@ -226,9 +242,29 @@ double sno_ratio(double Rabs, double P, double maxf, double dr, double dz) {
 // taken from the caller (test hook mirroring sn_poisson_set_boundary) and the moment step is skipped.
 // Outputs: *sweeps (full sweeps applied), *residual (R_k of the last sweep), hist[k] = R_{k+1} (nullable,
 // max_sweeps entries).  Returns 0 converged / fixed-sweep completed, 1 hit max_sweeps, -1 bad args, -3 non-finite.
+int sno_solve_rule(int rule, int nr, int nz, double dr, double dz, int symmetry, int lmax, double omega,
+                   const double* rho, double* phi, double tol, int max_sweeps, int* sweeps, double* residual,
+                   double* hist, const double* bE_in, const double* bN_in, const double* bS_in);
+
 int sno_solve(int nr, int nz, double dr, double dz, int symmetry, int lmax, double omega, const double* rho,
               double* phi, double tol, int max_sweeps, int* sweeps, double* residual, double* hist,
               const double* bE_in, const double* bN_in, const double* bS_in) {
+    return sno_solve_rule(0, nr, nz, dr, dz, symmetry, lmax, omega, rho, phi, tol, max_sweeps, sweeps, residual, hist,
+                          bE_in, bN_in, bS_in);
+}
+
+// [R16] the paper-literal stopping rule (rule = 1): "The iteration is stopped by default when the relative
+// changes of all grids reach below 1e-8":  E_k = max|dphi| / max|phi_new| of sweep k, stop after the first sweep with
+// E_k <= tol; max|dphi| == 0 gives 0.  rule = 0 is the residual rule R9 above.  `residual` / hist hold E_k then.
+double sno_relchange(double Chg, double P) {
+    if (Chg == 0.0) return 0.0;
+    return Chg / P;
+}
+
+int sno_solve_rule(int rule, int nr, int nz, double dr, double dz, int symmetry, int lmax, double omega,
+                   const double* rho, double* phi, double tol, int max_sweeps, int* sweeps, double* residual,
+                   double* hist, const double* bE_in, const double* bN_in, const double* bS_in) {
+    if (rule != 0 && rule != 1) return -1;
     if (nr < 2 || nz < 2 || !(dr > 0) || !(dz > 0) || (symmetry != 0 && symmetry != 1) || lmax < 0 ||
         !rho || !phi || max_sweeps < 0 || !sweeps || !residual)
         return -1;
@@ -250,9 +286,9 @@ int sno_solve(int nr, int nz, double dr, double dz, int symmetry, int lmax, doub
     *sweeps = 0;
     *residual = 0.0;
     for (int k = 0; k < max_sweeps; ++k) {
-        double Rabs, P;
-        sno_sweeps(nr, nz, dr, dz, symmetry, omega, rho, bE.data(), bN.data(), bS.data(), phi, 1, &Rabs, &P);
-        const double Rk = sno_ratio(Rabs, P, maxf, dr, dz);
+        double Rabs, P, Chg;
+        sno_sweeps_chg(nr, nz, dr, dz, symmetry, omega, rho, bE.data(), bN.data(), bS.data(), phi, 1, &Rabs, &P, &Chg);
+        const double Rk = rule == 0 ? sno_ratio(Rabs, P, maxf, dr, dz) : sno_relchange(Chg, P);
         *sweeps = k + 1;
         *residual = Rk;
         if (hist) hist[k] = Rk;

@@ -410,6 +410,45 @@ def test_relative_change_relation_to_paper_rule(oracle):
     assert np.max(np.abs(p1 - p0)) == pytest.approx(omega / D * Rabs[0], rel=1e-9)
 
 
+@pytest.mark.parametrize("symmetry", [0, 1])
+def test_paper_literal_rule_picks_the_sweep_of_a_bruteforce_python_sor(oracle, symmetry):
+    """R16 / PAPER.md:99 "stopped ... when the relative changes of all grids reach below 1e-8": an independent pure-Python
+    red-black SOR that measures max|phi_new - phi_old| / max|phi_new| sweep by sweep stops at the same sweep as the
+    oracle's rule 1, and the oracle's E_k equals that ratio to the rounding of the difference (|dphi| ~ 1e-5 |phi| here,
+    so ~1e-11 relative); with symmetry = 1 the mirror row (diag = D - 1/dz^2, larger omega/diag) is part of the maximum."""
+    nr, nz, tol = 10, 8, 1e-5
+    w = W.random_smooth(nr, nz, symmetry, seed=60 + symmetry, lmax=4)
+    M = oracle.moments(w.rho, w.dr, w.dz, symmetry, 4)
+    bnd = oracle.boundary(nr, nz, w.dr, w.dz, symmetry, 4, M)
+    omega = oracle.default_omega(nr, nz, w.dr, w.dz, symmetry)
+    ref = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, symmetry, 4, tol, 500, boundary_arrays=bnd, rule=1,
+                       history=True)
+    assert ref["status"] == 0 and 10 < ref["sweeps"] < 500
+    phi = np.zeros_like(w.rho)
+    stop = None
+    for k in range(1, 500):
+        new = python_rb_sor(w.rho, phi, w.dr, w.dz, symmetry, omega, bnd[0], bnd[1], bnd[2], 1)
+        E = np.max(np.abs(new - phi)) / np.max(np.abs(new))
+        assert ref["hist"][k - 1] == pytest.approx(E, rel=1e-8)
+        phi = new
+        if E <= tol:
+            stop = k
+            break
+    assert stop == ref["sweeps"] and ref["residual"] == ref["hist"][-1] <= tol
+    assert np.max(np.abs(phi - ref["phi"])) <= 1e-12 * np.max(np.abs(phi))
+    # the change is (omega/diag_j) |res| cell by cell: max over the rows with their own diag (mirror row: D0 < D)
+    p1, Rabs, Pk, Chg = oracle.sweeps_chg(w.rho, np.zeros_like(w.rho), w.dr, w.dz, symmetry, omega, *bnd, 3)
+    assert oracle.relchange(Chg[2], Pk[2]) == ref["hist"][2] and oracle.relchange(0.0, 0.0) == 0.0
+    D = 2 / w.dr ** 2 + 2 / w.dz ** 2
+    assert Chg[0] >= omega / D * Rabs[0] * (1 - 1e-15)
+    if symmetry == 0:
+        assert Chg[0] == omega / D * Rabs[0]
+    # rule 0 is untouched by the new argument
+    a = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, symmetry, 4, 1e-9, 500, boundary_arrays=bnd)
+    b = oracle.solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, symmetry, 4, 1e-9, 500, boundary_arrays=bnd, rule=0)
+    assert a["sweeps"] == b["sweeps"] and np.array_equal(a["phi"], b["phi"])
+
+
 def test_degenerate_inputs(oracle):
     z = np.zeros((8, 8))
     out = oracle.solve(z, z, 0.1, 0.1, 1, 4, 1e-10, 50)
