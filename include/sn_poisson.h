@@ -111,6 +111,14 @@ void sn_poisson_destroy(sn_poisson* h);
 int sn_poisson_set_omega(sn_poisson* h, double omega);
 double sn_poisson_get_omega(const sn_poisson* h);
 
+/* NEXT-1: the paper-literal stopping rule.  rule = 0 (default): the residual ratio R_k of
+ * DESIGN.md R9.  rule = 1: "The iteration is stopped by default when the relative changes of all grids reach
+ * below 1e-8" -- reading R16: E_k = max|dphi| / max|phi_new| of sweep k, dphi = (omega/diag_j) res the change the update
+ * applies to a cell; stop after the first sweep with E_k <= tol (the paper's default is tol = 1e-8; with lmax = 0 the
+ * boundary is the paper's Roche formula).  `residual` and get_history then hold E_k.  All three sweep paths support
+ * both rules.  Returns 0 or -1. */
+int sn_poisson_set_stop_rule(sn_poisson* h, int rule);
+
 /* NEXT-1: the gravity field g = -grad phi at the cell centres, the source term of the paper's
  * momentum and energy equations (eqs. 2-4).  Centred differences with the solver's boundary handling
  * (R15): reflecting axis, reflecting equator when symmetry = 1, elsewhere the ghost values of the LAST solve

@@ -16,6 +16,7 @@ LIB_PATH = os.environ.get("SN_POISSON_LIB") or os.path.join(_HERE, "libsn_poisso
 EXPORTS = (
     "sn_poisson_create", "sn_poisson_solve", "sn_poisson_solve_host", "sn_poisson_solve_batch",
     "sn_poisson_solve_batch_host", "sn_poisson_solve_sequence_host", "sn_poisson_probe_l2",
+    "sn_poisson_set_stop_rule",
     "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
     "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
@@ -75,6 +76,8 @@ def load():
     lib.sn_poisson_destroy.argtypes = [_vp]
     lib.sn_poisson_gravity.restype = C.c_int
     lib.sn_poisson_gravity.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp]
+    lib.sn_poisson_set_stop_rule.restype = C.c_int
+    lib.sn_poisson_set_stop_rule.argtypes = [_vp, C.c_int]
     lib.sn_poisson_set_omega.restype = C.c_int
     lib.sn_poisson_set_omega.argtypes = [_vp, C.c_double]
     lib.sn_poisson_get_omega.restype = C.c_double
@@ -184,6 +187,11 @@ def sn_poisson_gravity(h, nbatch, phi_ptr, gr_ptr, gz_ptr, stream=0):
     if rc != 0:
         raise SnPoissonError(f"sn_poisson_gravity failed ({rc}): " + sn_poisson_last_error())
     return rc
+
+
+def sn_poisson_set_stop_rule(h, rule) -> int:
+    """0 = residual ratio R_k (R9), 1 = the paper-literal relative change E_k (R16)."""
+    return _check(load().sn_poisson_set_stop_rule(h, int(rule)), "sn_poisson_set_stop_rule")
 
 
 def sn_poisson_set_omega(h, omega) -> int:

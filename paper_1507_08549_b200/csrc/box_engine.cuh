@@ -147,6 +147,8 @@ struct BoxEngine {
     // running maxima of the current sweep
     unsigned long long mres_k, mphi_k;     // exact keys
     float mres_f, mphi_f;                  // fast: |upper word| compared as fp32 (same order for finite values)
+    unsigned long long mres0_k;            // the same maxima of |res| over the reflecting-equator row alone (rule 1, R16)
+    float mres0_f;
 
     __device__ __forceinline__ void carve(double* base) {
         fs = base;
@@ -267,6 +269,7 @@ struct BoxEngine {
     __device__ __forceinline__ void reset_maxima() {
         mres_k = 0ull; mphi_k = 0ull;
         mres_f = 0.0f; mphi_f = 0.0f;
+        mres0_k = 0ull; mres0_f = 0.0f;
     }
 
     template <int TRACK>
@@ -343,6 +346,10 @@ struct BoxEngine {
                                              cc == 0 ? fv.x : fv.y, res);
                 phi[q][c] = pn;
                 track<TRACK>(res, pn);
+                if (q == 0 && mirror0) {             // q is a compile-time constant: two predicated maxima per half-sweep
+                    if (TRACK == kTrackExact) { const unsigned long long kr = abs_key(res); mres0_k = kr > mres0_k ? kr : mres0_k; }
+                    else if (TRACK == kTrackFast) mres0_f = fmaxf(mres0_f, fabsf(__int_as_float(__double2hiint(res))));
+                }
             }
         }
         if (PF && kPfRow >= H) { if (pf_src) *pf = ll_load_early(pf_src); }

@@ -45,6 +45,12 @@ struct Geom {
     double tol;
     const double* cE;  // [nr]  ((i+1)/(i+1/2))/dr^2
     const double* cW;  // [nr]  (i/(i+1/2))/dr^2, cW[0] = 0: regular axis
+    // stopping rule (R9 / R16): 0 = residual ratio R_k, 1 = the paper-literal relative change E_k.  Rule 1 with
+    // symmetry = 1 also needs the maximum of |res| over the reflecting-equator row alone (its omega/diag differs):
+    int rule;
+    int slots0_stride;                  // per member
+    unsigned int* slots0_f;             // [nb][cap]  upper words (FAST)
+    unsigned long long* slots0_x;       // [nb][cap]  exact keys
 };
 
 __device__ __forceinline__ unsigned long long dbits(double x) { return (unsigned long long)__double_as_longlong(x); }
@@ -69,6 +75,23 @@ __device__ __forceinline__ double stop_ratio(unsigned long long rabs_key, unsign
     const double Rabs = bits2d(rabs_key);
     if (Rabs == 0.0) return 0.0;
     return __ddiv_rn(Rabs, __fma_rn(D, bits2d(p_key), maxf));
+}
+
+// The value the stopping rule compares with tol after a sweep (keys: max|res|, max|phi_new| over all cells, max|res|
+// over the reflecting-equator row).  Rule 0: R_k (above).  Rule 1 (R16; "relative changes of all
+// grids"): E_k = max|dphi| / max|phi_new| with dphi = w_j (x) res.  Rounded multiplication by a positive constant is
+// monotone, so max_j |w_j (x) res| = max(wD (x) max|res|, wD0 (x) max_row0|res|) EXACTLY (wD0 > wD makes the row-0 cells
+// inside the first maximum harmless); max|dphi| == 0 -> 0.
+__device__ __forceinline__ double stop_value(const Geom& g, unsigned long long rabs_key, unsigned long long p_key,
+                                             unsigned long long r0_key, double maxf) {
+    if (g.rule == 0) return stop_ratio(rabs_key, p_key, maxf, g.D);
+    unsigned long long c = abs_key(__dmul_rn(g.wD, bits2d(rabs_key)));
+    if (g.symmetry == 1) {
+        const unsigned long long c0 = abs_key(__dmul_rn(g.wD0, bits2d(r0_key)));
+        c = c0 > c ? c0 : c;                         // keys: NaN sorts highest (sticky)
+    }
+    if (c == 0ull) return 0.0;
+    return __ddiv_rn(bits2d(c), bits2d(p_key));
 }
 
 __device__ __forceinline__ bool is_nonfinite(double x) { return !(x == x) || x == INFINITY || x == -INFINITY; }

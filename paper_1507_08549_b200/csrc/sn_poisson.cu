@@ -78,7 +78,7 @@ struct sn_poisson {
     int mom_blocks = 0;
 
     // options
-    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1, opt_ring = -1;
+    int opt_path = 0, opt_chunk = 32, opt_tblock = 0, opt_shape = -1, opt_exact = 0, opt_halo = -1, opt_prof = 0, opt_ll = -1, opt_group = -1, opt_ds = -1, opt_ring = -1, opt_rule = 0;
 
     // device workspace (sized for `cap_batch` members)
     int cap_batch = 0, cap_sweeps = 0;
@@ -86,6 +86,8 @@ struct sn_poisson {
     double *d_bE = nullptr, *d_bN = nullptr, *d_bS = nullptr, *d_M = nullptr, *d_partial = nullptr;
     unsigned long long* d_slots = nullptr;
     unsigned int* d_slots_f = nullptr;                       // blocked path: FAST maxima (upper words)
+    unsigned long long* d_slots0 = nullptr;                  // rule 1: per-sweep maxima of |res| over the equator row
+    unsigned int* d_slots0_f = nullptr;
     double* d_work = nullptr;                                // blocked path: second phi buffer, work_cap doubles
     size_t work_cap = 0;
     double* d_hist = nullptr;
@@ -152,12 +154,18 @@ Geom make_geom(const sn_poisson* h, double tol) {
     g.tol = tol;
     g.cE = h->d_cE;
     g.cW = h->d_cW;
+    g.rule = h->opt_rule;
+    g.slots0_stride = h->cap_sweeps;
+    g.slots0_f = h->d_slots0_f;
+    g.slots0_x = h->d_slots0;
     return g;
 }
 
 void free_batch_ws(sn_poisson* h) {
     cudaFree(h->d_bE); cudaFree(h->d_bN); cudaFree(h->d_bS); cudaFree(h->d_M); cudaFree(h->d_partial);
     cudaFree(h->d_slots); cudaFree(h->d_slots_f); cudaFree(h->d_hist); cudaFree(h->d_ctl);
+    cudaFree(h->d_slots0); cudaFree(h->d_slots0_f);
+    h->d_slots0 = nullptr; h->d_slots0_f = nullptr;
     if (h->h_ctl) cudaFreeHost(h->h_ctl);
     h->d_bE = h->d_bN = h->d_bS = h->d_M = h->d_partial = h->d_hist = nullptr;
     h->d_slots = nullptr; h->d_slots_f = nullptr; h->d_ctl = nullptr; h->h_ctl = nullptr;
@@ -182,6 +190,7 @@ int ensure_ws(sn_poisson* h, int nbatch, int max_sweeps) {
     if (dev_alloc(&h->d_bE, (size_t)nb * h->nz) || dev_alloc(&h->d_bN, (size_t)nb * h->nr) ||
         dev_alloc(&h->d_bS, (size_t)nb * h->nr) || dev_alloc(&h->d_M, (size_t)nb * (kMaxL + 1)) ||
         dev_alloc(&h->d_partial, (size_t)nb * h->mom_blocks * h->NL) || dev_alloc(&h->d_slots, (size_t)nb * 2 * ns) || dev_alloc(&h->d_slots_f, (size_t)nb * 2 * ns) ||
+        dev_alloc(&h->d_slots0, (size_t)nb * ns) || dev_alloc(&h->d_slots0_f, (size_t)nb * ns) ||
         dev_alloc(&h->d_hist, (size_t)nb * ns) || dev_alloc(&h->d_ctl, (size_t)nb))
         return -2;
     CU_TRY(cudaMallocHost((void**)&h->h_ctl, sizeof(Ctl) * 2 * nb));
@@ -590,6 +599,8 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     if ((pl.halo && !pl.ds) || pl.ll) CU_TRY(cudaMemsetAsync(h->d_mail, 0, 16 * need_mail, st));   // packet tags start at 1
     ResParams P;
     P.g = g;
+    P.g.slots0_f += (size_t)member0 * h->cap_sweeps;         // the kernel indexes members from 0
+    P.g.slots0_x += (size_t)member0 * h->cap_sweeps;
     P.halo = pl.halo;
     P.ll = pl.ll;
     P.ntx = pl.ntx; P.nty = pl.nty; P.ow = pl.ow; P.oh = pl.oh; P.m = pl.m; P.Q = pl.Q;
@@ -717,6 +728,12 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl) * nbatch, st));
     CU_TRY(cudaMemset2DAsync(h->d_slots, sizeof(unsigned long long) * 2 * (size_t)h->cap_sweeps, 0,
                              sizeof(unsigned long long) * 2 * (size_t)std::max(1, max_sweeps), nbatch, st));
+    if (h->opt_rule != 0 && h->symmetry == 1) {
+        CU_TRY(cudaMemset2DAsync(h->d_slots0, sizeof(unsigned long long) * (size_t)h->cap_sweeps, 0,
+                                 sizeof(unsigned long long) * (size_t)std::max(1, max_sweeps), nbatch, st));
+        CU_TRY(cudaMemset2DAsync(h->d_slots0_f, sizeof(unsigned int) * (size_t)h->cap_sweeps, 0,
+                                 sizeof(unsigned int) * (size_t)std::max(1, max_sweeps), nbatch, st));
+    }
     // a-1: moments (+ max|4 pi rho|), a-1b: boundary fill (skipped when ghosts were injected by the test hook)
     if (int rc = launch_moments(h, g, nbatch, rho, st)) return rc;
     h->st_launches += 1;
@@ -1076,6 +1093,14 @@ int sn_poisson_probe_l2(int mib, double* copy_gbs, double* read_gbs, void* strea
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
     return rc;
+}
+
+int sn_poisson_set_stop_rule(sn_poisson* h, int rule) {
+    g_err.clear();
+    if (!h) { set_err("NULL handle"); return -1; }
+    if (rule != 0 && rule != 1) { set_err("rule must be 0 (residual ratio) or 1 (relative change)"); return -1; }
+    h->opt_rule = rule;
+    return 0;
 }
 
 int sn_poisson_set_omega(sn_poisson* h, double omega) {

@@ -59,9 +59,11 @@ __global__ void k_blocked_init(Ctl* __restrict__ ctl, int m, int max_sweeps, int
 
 // The director: called by ONE thread of the last CTA of member `c` after a launch that executed (action, src, k0,
 // n, track).  All maxima of the launch are final and visible.  Writes the next action (or the result).
-__device__ inline void blocked_direct(const BlkParams& p, Ctl* c, int action, int src, int k0, int n, int track,
+__device__ inline void blocked_direct(const BlkParams& p, Ctl* c, int member, int action, int src, int k0, int n, int track,
                                       const unsigned int* sf, const unsigned long long* sx, double* hist) {
     const Geom& g = p.g;
+    const unsigned int* s0f = g.slots0_f + (size_t)member * g.slots0_stride;      // rule 1: equator-row maxima
+    const unsigned long long* s0x = g.slots0_x + (size_t)member * g.slots0_stride;
     auto finish = [&](int final_buf, int sweeps, int status, double R) {
         if (final_buf == 0) {
             c->sweeps = sweeps; c->status = status; c->residual = R;
@@ -85,7 +87,8 @@ __device__ inline void blocked_direct(const BlkParams& p, Ctl* c, int action, in
     if (track == kTrackExact) {
         for (int s = 0; s < n; ++s) {
             const int k = k0 + s + 1;
-            const double R = stop_ratio(__ldcg(sx + 2 * (k - 1)), __ldcg(sx + 2 * (k - 1) + 1), c->maxf, g.D);
+            const double R = stop_value(g, __ldcg(sx + 2 * (k - 1)), __ldcg(sx + 2 * (k - 1) + 1),
+                                        g.rule != 0 ? __ldcg(s0x + k - 1) : 0ull, c->maxf);
             hist[k - 1] = R;
             Rlast = R;
             const bool bad = is_nonfinite(R);
@@ -110,7 +113,7 @@ __device__ inline void blocked_direct(const BlkParams& p, Ctl* c, int action, in
             const int k = k0 + s + 1;
             const unsigned long long kr = (unsigned long long)__ldcg(sf + 2 * (k - 1)) << 32;
             const unsigned long long kp = ((unsigned long long)__ldcg(sf + 2 * (k - 1) + 1) << 32) | 0xffffffffull;
-            const double R_lo = stop_ratio(kr, kp, c->maxf, g.D);
+            const double R_lo = stop_value(g, kr, kp, g.rule != 0 ? (unsigned long long)__ldcg(s0f + k - 1) << 32 : 0ull, c->maxf);
             hist[k - 1] = R_lo;
             if (is_nonfinite(R_lo) || (g.tol > 0.0 && R_lo <= g.tol * 1.000000001)) candidate = true;
         }
@@ -176,6 +179,7 @@ __global__ void __launch_bounds__(TXN* TYN, MINB) k_sor_blocked(const BlkParams 
     E.bind_thread(tid);
     const int gi0 = bx + 4 * E.a, gj0 = by + H * E.b;
     const bool own = gi0 >= x0 && gi0 < x1 && gj0 >= y0 && gj0 < y1;
+    const bool row0_warp = __any_sync(0xffffffffu, g.symmetry == 1 && gj0 == 0);     // holds equator-row cells
 
     const double* srcp = p.buf[src] + (size_t)member * ncell;
     double* dstp = p.buf[src ^ 1] + (size_t)member * ncell;
@@ -199,6 +203,10 @@ __global__ void __launch_bounds__(TXN* TYN, MINB) k_sor_blocked(const BlkParams 
                 E.template half_sweep<0, kTrackFast>();
                 E.template half_sweep<1, kTrackFast, false>();
                 // warp reduction BEFORE the sweep's last barrier: its latency hides in the barrier wait
+                if (g.rule != 0 && row0_warp) {          // rule 1 (R16): equator-row maximum, straight to its slot
+                    const unsigned w0 = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres0_f) : 0u);
+                    if (lane == 0) atomicMax(g.slots0_f + (size_t)member * g.slots0_stride + k0 + s, w0);
+                }
                 const unsigned wr = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres_f) : 0u);
                 const unsigned wp = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mphi_f) : 0u);
                 if (lane == 0) {
@@ -212,6 +220,10 @@ __global__ void __launch_bounds__(TXN* TYN, MINB) k_sor_blocked(const BlkParams 
                 E.reset_maxima();
                 E.template half_sweep<0, kTrackExact>();
                 E.template half_sweep<1, kTrackExact, false>();
+                if (g.rule != 0 && row0_warp) {
+                    const unsigned long long w0 = warp_max_key(own ? E.mres0_k : 0ull);
+                    if (lane == 0) atomicMax(g.slots0_x + (size_t)member * g.slots0_stride + k0 + s, w0);
+                }
                 const unsigned long long wr = warp_max_key(own ? E.mres_k : 0ull);
                 const unsigned long long wp = warp_max_key(own ? E.mphi_k : 0ull);
                 if (lane == 0) {
@@ -249,7 +261,7 @@ __global__ void __launch_bounds__(TXN* TYN, MINB) k_sor_blocked(const BlkParams 
     if (s_last == (unsigned)(ntiles - 1) && tid == 0) {
         __threadfence();
         c->arrived = 0u;
-        blocked_direct(p, c, action, src, k0, n, track, p.slots_f + (size_t)member * p.slot_stride,
+        blocked_direct(p, c, member, action, src, k0, n, track, p.slots_f + (size_t)member * p.slot_stride,
                        p.slots_x + (size_t)member * p.slot_stride, p.hist + (size_t)member * p.hist_stride);
     }
 }

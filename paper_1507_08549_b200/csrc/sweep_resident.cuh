@@ -225,15 +225,18 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
                 double R = 0.0;
                 if (lane < rep.n) {
                     const size_t slot = 2 * (size_t)(rep.k0 + lane);
+                    const size_t s0 = (size_t)member * g.slots0_stride + rep.k0 + lane;      // rule 1: equator-row maximum
                     if (rep.exact) {
-                        R = stop_ratio(__ldcg(slots_x + slot), __ldcg(slots_x + slot + 1), ctl->maxf, g.D);
+                        const unsigned long long k0x = g.rule != 0 ? __ldcg(g.slots0_x + s0) : 0ull;
+                        R = stop_value(g, __ldcg(slots_x + slot), __ldcg(slots_x + slot + 1), k0x, ctl->maxf);
                         bad = is_nonfinite(R);
                         fire = bad || (g.tol > 0.0 && R <= g.tol);
                     } else {
                         // upper words only: R_lo <= R_k (up to rounding, covered by the factor)
                         const unsigned long long kr = (unsigned long long)__ldcg(slots_f + slot) << 32;
                         const unsigned long long kp = ((unsigned long long)__ldcg(slots_f + slot + 1) << 32) | 0xffffffffull;
-                        R = stop_ratio(kr, kp, ctl->maxf, g.D);
+                        const unsigned long long k0f = g.rule != 0 ? (unsigned long long)__ldcg(g.slots0_f + s0) << 32 : 0ull;
+                        R = stop_value(g, kr, kp, k0f, ctl->maxf);
                         bad = is_nonfinite(R);
                         fire = bad || (g.tol > 0.0 && R <= g.tol * 1.000000001);
                     }
@@ -295,6 +298,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     const int gi0 = bx + 4 * E.a, gj0 = by + H * E.b;
     E.active = gj0 < g.nz;                                      // false only in the ragged last tile row (halo mode)
     const bool own = gi0 >= x0 && gi0 < x1 && gj0 >= y0 && gj0 < y1;
+    const bool row0_warp = __any_sync(0xffffffffu, g.symmetry == 1 && gj0 == 0 && E.active);   // holds equator-row cells
 
     const double* rho = p.rho + (size_t)member * ncell;
     double* phi_io = p.phi + (size_t)member * ncell;
@@ -454,6 +458,17 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
             const long long t4 = tick();
             // the sweep's maxima are complete: reduce them across the warp BEFORE the last wait / barrier of the sweep,
             // so that the REDUX latency (measured ~135 clocks per half-sweep when done after the barrier) hides in it
+            // rule 1 (R16): the maximum over the reflecting-equator row goes straight to its own per-sweep slot from the
+            // few warps that hold that row (ordered before the service warp's release by the barriers in between)
+            if (g.rule != 0 && row0_warp && TRACK != kTrackNone) {
+                if (TRACK == kTrackFast) {
+                    const unsigned w0 = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres0_f) : 0u);
+                    if (lane == 0) atomicMax(g.slots0_f + (size_t)member * g.slots0_stride + k0 + s, w0);
+                } else {
+                    const unsigned long long w0 = warp_max_key(own ? E.mres0_k : 0ull);
+                    if (lane == 0) atomicMax(g.slots0_x + (size_t)member * g.slots0_stride + k0 + s, w0);
+                }
+            }
             if (TRACK == kTrackFast) {
                 const unsigned wr = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mres_f) : 0u);
                 const unsigned wp = __reduce_max_sync(0xffffffffu, own ? __float_as_uint(E.mphi_f) : 0u);

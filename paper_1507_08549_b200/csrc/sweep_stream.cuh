@@ -15,11 +15,12 @@ constexpr int kStreamTileH = kStreamWarps * kStreamRows;
 // Device-side stopping decision for sweep k-1, evaluated redundantly (and identically) by every block at the start
 // of both half-sweeps of sweep k: all blocks read the same final slot values, so all take the same branch.
 // `writer` (one thread of the red launch) records it.  Returns true if no more updates may be applied.
-__device__ __forceinline__ bool member_finished(const Geom& g, int k, const unsigned long long* slots, Ctl* ctl,
+__device__ __forceinline__ bool member_finished(const Geom& g, int member, int k, const unsigned long long* slots, Ctl* ctl,
                                                 double* hist, bool writer) {
     if (k <= 1) return false;
     if (*(volatile int*)&ctl->done) return true;
-    const double R = stop_ratio(slots[2 * (k - 2)], slots[2 * (k - 2) + 1], ctl->maxf, g.D);
+    const double R = stop_value(g, slots[2 * (k - 2)], slots[2 * (k - 2) + 1],
+                                g.rule != 0 ? g.slots0_x[(size_t)member * g.slots0_stride + k - 2] : 0ull, ctl->maxf);
     const bool bad = is_nonfinite(R);
     const bool stop = bad || (g.tol > 0.0 && R <= g.tol);
     if (writer) {
@@ -49,7 +50,7 @@ __global__ void __launch_bounds__(kStreamWarps * 32)
     __shared__ unsigned long long s_red[2][kStreamWarps];
     if (threadIdx.x == 0) {
         const bool writer = colour == 0 && blockIdx.x == 0 && blockIdx.y == 0;
-        s_fin = member_finished(g, k, sl, ctl + b, hist + (size_t)b * hist_stride, writer) ? 1 : 0;
+        s_fin = member_finished(g, b, k, sl, ctl + b, hist + (size_t)b * hist_stride, writer) ? 1 : 0;
     }
     __syncthreads();
     if (s_fin) return;
@@ -64,7 +65,7 @@ __global__ void __launch_bounds__(kStreamWarps * 32)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int pair = blockIdx.x * 32 + lane;
     const int j0 = blockIdx.y * kStreamTileH + warp * kStreamRows;
-    unsigned long long mres = 0ull, mphi = 0ull;
+    unsigned long long mres = 0ull, mphi = 0ull, mres0 = 0ull;
 #pragma unroll
     for (int q = 0; q < kStreamRows; ++q) {
         const int j = j0 + q;
@@ -87,7 +88,12 @@ __global__ void __launch_bounds__(kStreamWarps * 32)
             const unsigned long long kr = abs_key(res), kp = abs_key(pn);
             mres = kr > mres ? kr : mres;
             mphi = kp > mphi ? kp : mphi;
+            if (mirror_row) mres0 = kr > mres0 ? kr : mres0;
         }
+    }
+    if (g.rule != 0 && g.symmetry == 1 && j0 == 0) {         // rule 1 (R16): the warp that holds the equator row
+        mres0 = warp_max_u64(mres0);
+        if (lane == 0) atomicMax(g.slots0_x + (size_t)b * g.slots0_stride + k - 1, mres0);
     }
     mres = warp_max_u64(mres);
     mphi = warp_max_u64(mphi);
@@ -117,7 +123,8 @@ __global__ void k_decide_last(Geom g, int k_last, int slot_stride, int hist_stri
         return;
     }
     const unsigned long long* sl = slots + (size_t)b * slot_stride;
-    const double R = stop_ratio(sl[2 * (k_last - 1)], sl[2 * (k_last - 1) + 1], c->maxf, g.D);
+    const double R = stop_value(g, sl[2 * (k_last - 1)], sl[2 * (k_last - 1) + 1],
+                                g.rule != 0 ? g.slots0_x[(size_t)b * g.slots0_stride + k_last - 1] : 0ull, c->maxf);
     hist[(size_t)b * hist_stride + k_last - 1] = R;
     c->sweeps = k_last;
     c->residual = R;

@@ -120,6 +120,9 @@ class PoissonSolver:
                              torch.cuda.current_stream().cuda_stream)
         return gr, gz
 
+    def set_stop_rule(self, rule):
+        return B.sn_poisson_set_stop_rule(self.h, rule)
+
     def set_option(self, key, value):
         return B.sn_poisson_set_option(self.h, key, value)
 
