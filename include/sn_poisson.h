@@ -127,6 +127,16 @@ int sn_poisson_set_stop_rule(sn_poisson* h, int rule);
  * Returns 0, -1 (bad argument, or no ghost values for nbatch members yet), -2 (CUDA error). */
 int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr, double* gz, void* stream);
 
+/* Solve (as sn_poisson_solve_batch; nbatch = 1 for a single grid) AND emit the gravity field of the result in the same
+ * call: gr, gz are DEVICE pointers to nbatch consecutive grids receiving g_r, g_z = -grad phi (definition and boundary
+ * handling as sn_poisson_gravity).  On the resident path the epilogue is fused into the relaxation kernel: every thread
+ * differences the patch of phi it still holds in registers right after its final store (neighbours outside the patch
+ * from the stored result, after one grid barrier); on the blocked / streaming paths the standalone gravity kernel is
+ * enqueued right behind the last sweep.  Bit-identical to sn_poisson_gravity on the returned phi.  gr, gz, phi_inout
+ * must not alias.  Returns 0 or a negative status. */
+int sn_poisson_solve_gravity(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double* gr, double* gz,
+                             double tol, int max_sweeps, void* stream, sn_poisson_result* out);
+
 /* Test hooks.  All pointers are HOST pointers.
  * get_moments : M[0..lmax] of batch member 0 of the last solve (odd entries 0 when symmetry = 1).
  * set_boundary: inject ghost values bE[nz], bN[nr], bS[nr] (bS ignored when symmetry = 1) and skip the moment and

@@ -16,7 +16,7 @@ LIB_PATH = os.environ.get("SN_POISSON_LIB") or os.path.join(_HERE, "libsn_poisso
 EXPORTS = (
     "sn_poisson_create", "sn_poisson_solve", "sn_poisson_solve_host", "sn_poisson_solve_batch",
     "sn_poisson_solve_batch_host", "sn_poisson_solve_sequence_host", "sn_poisson_probe_l2",
-    "sn_poisson_set_stop_rule",
+    "sn_poisson_set_stop_rule", "sn_poisson_solve_gravity",
     "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
     "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
@@ -76,6 +76,9 @@ def load():
     lib.sn_poisson_destroy.argtypes = [_vp]
     lib.sn_poisson_gravity.restype = C.c_int
     lib.sn_poisson_gravity.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp]
+    lib.sn_poisson_solve_gravity.restype = C.c_int
+    lib.sn_poisson_solve_gravity.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, C.c_double, C.c_int, _vp,
+                                             C.POINTER(sn_poisson_result)]
     lib.sn_poisson_set_stop_rule.restype = C.c_int
     lib.sn_poisson_set_stop_rule.argtypes = [_vp, C.c_int]
     lib.sn_poisson_set_omega.restype = C.c_int
@@ -180,6 +183,16 @@ def sn_poisson_probe_l2(mib=32, stream=0):
     c, r = C.c_double(0.0), C.c_double(0.0)
     _check(load().sn_poisson_probe_l2(int(mib), C.byref(c), C.byref(r), stream or None), "sn_poisson_probe_l2")
     return c.value, r.value
+
+
+def sn_poisson_solve_gravity(h, nbatch, rho_ptr, phi_ptr, gr_ptr, gz_ptr, tol, max_sweeps, stream=0):
+    """Solve + fused gravity epilogue; DEVICE addresses of nbatch consecutive grids.  Returns the list of results."""
+    out = (sn_poisson_result * int(nbatch))()
+    rc = load().sn_poisson_solve_gravity(h, int(nbatch), rho_ptr, phi_ptr, gr_ptr, gz_ptr, float(tol), int(max_sweeps),
+                                         stream or None, out)
+    if rc != 0:
+        raise SnPoissonError(f"sn_poisson_solve_gravity failed ({rc}): " + sn_poisson_last_error())
+    return list(out)
 
 
 def sn_poisson_gravity(h, nbatch, phi_ptr, gr_ptr, gz_ptr, stream=0):

@@ -570,7 +570,7 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
 
 // Members member0 .. member0 + nbatch - 1 of the caller's batch (rho, phi point at member 0 of the batch).
 int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, const double* rho, double* phi,
-                 int max_sweeps, cudaStream_t st, int member0 = 0) {
+                 int max_sweeps, cudaStream_t st, int member0 = 0, double* gr = nullptr, double* gz = nullptr) {
     const ShapeInfo& S = shapes()[pl.shape];
     const size_t ncell = (size_t)h->nr * h->nz;
     const size_t nint = (size_t)(max_sweeps + pl.Q - 1) / pl.Q;
@@ -620,6 +620,8 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
     P.flags = P.gbar + nbatch;
     P.ctl = h->d_ctl + member0; P.hist = h->d_hist + (size_t)member0 * h->cap_sweeps;
     P.prof = nullptr;
+    P.gr = gr ? gr + (size_t)member0 * ncell : nullptr;
+    P.gz = gz ? gz + (size_t)member0 * ncell : nullptr;
     h->prof_ctas = 0;
     if (h->opt_prof) {
         const size_t need = (size_t)pl.ntiles * nbatch * 8;
@@ -665,6 +667,8 @@ int run_resident(sn_poisson* h, const Geom& g, const ResPlan& pl, int nbatch, co
 // Hooks of the host-buffer entry points into one solve: an event the relaxation must wait for (phi's H2D on the copy
 // stream) and a device -> host copy enqueued right after the relaxation, before the call's single synchronisation.
 struct HostIO {
+    double* gr = nullptr;        // fused gravity epilogue: DEVICE outputs [nbatch][ncell] (NULL: none)
+    double* gz = nullptr;
     cudaEvent_t wait_before_relax = nullptr;
     double* d2h_dst = nullptr;
     const double* d2h_src = nullptr;
@@ -708,6 +712,21 @@ void plan_solve(sn_poisson* h, int nbatch, const double* rho, const double* phi,
     if ((h->opt_path == 0 || h->opt_path == 3) && pl.shape < 0) bp = plan_blocked(h, nbatch, rho, phi);
     pc.valid = true; pc.nbatch = nbatch; pc.aligned = aligned; pc.pl = pl; pc.bp = bp; pc.group = group;
     *pl_out = pl; *bp_out = bp; *group_out = group;
+}
+
+int launch_gravity(sn_poisson* h, const Geom& g, int nbatch, const double* phi, double* gr, double* gz, cudaStream_t st) {
+    const bool vec = h->nr % 4 == 0 && ((((uintptr_t)phi | (uintptr_t)gr | (uintptr_t)gz) & 15) == 0);
+    if (vec) {
+        const unsigned qx = (h->nr / 4 + 127) / 128;                       // rows folded into grid.x: no 65535 limit on nz
+        const dim3 grid(qx * (unsigned)h->nz, 1, nbatch);
+        k_gravity4<<<grid, 128, 0, st>>>(g, (int)qx, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
+    } else {
+        const unsigned qx = (h->nr + 127) / 128;
+        const dim3 grid(qx * (unsigned)h->nz, 1, nbatch);
+        k_gravity1<<<grid, 128, 0, st>>>(g, (int)qx, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
+    }
+    CU_TRY(cudaGetLastError());
+    return 0;
 }
 
 int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double tol, int max_sweeps,
@@ -765,13 +784,20 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     }
     if (pl.shape >= 0) {
         for (int m0 = 0; m0 < nbatch; m0 += group)
-            if (int rc = run_resident(h, g, pl, std::min(group, nbatch - m0), rho, phi, max_sweeps, st, m0)) return rc;
+            if (int rc = run_resident(h, g, pl, std::min(group, nbatch - m0), rho, phi, max_sweeps, st, m0,
+                                      io ? io->gr : nullptr, io ? io->gz : nullptr)) return rc;
         h->st_group = group;
         h->st_ctas = (double)pl.ntiles * group;
-    } else if (bp.shape >= 0) {
-        if (int rc = run_blocked(h, g, bp, nbatch, rho, phi, max_sweeps, st)) return rc;
     } else {
-        if (int rc = run_stream(h, g, nbatch, rho, phi, max_sweeps, st)) return rc;
+        if (bp.shape >= 0) {
+            if (int rc = run_blocked(h, g, bp, nbatch, rho, phi, max_sweeps, st)) return rc;
+        } else {
+            if (int rc = run_stream(h, g, nbatch, rho, phi, max_sweeps, st)) return rc;
+        }
+        // the streamed / blocked paths have no phi on chip at the end: the epilogue is the standalone kernel, enqueued
+        // right behind the last sweep (phi is still L2-resident for grids that fit)
+        if (io && io->gr)
+            if (int rc = launch_gravity(h, g, nbatch, phi, io->gr, io->gz, st)) return rc;
     }
     CU_TRY(cudaEventRecord(h->ev_t[2], st));
     if (io && io->d2h_dst)
@@ -1021,6 +1047,19 @@ int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_
     return 0;
 }
 
+int sn_poisson_solve_gravity(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double* gr, double* gz,
+                             double tol, int max_sweeps, void* stream, sn_poisson_result* out) {
+    g_err.clear();
+    if (nbatch < 1 || !out) { set_err("nbatch < 1 or NULL out"); return -1; }
+    if (nbatch > 65535) { set_err("nbatch > 65535"); return -1; }
+    if (!gr || !gz) { set_err("NULL gr / gz pointer"); return -1; }
+    if (gr == phi_inout || gz == phi_inout || gr == gz) { set_err("gr, gz and phi must not alias"); return -1; }
+    if (!check_solve_args(h, rho, phi_inout, tol, max_sweeps, nbatch)) return -1;
+    HostIO io;
+    io.gr = gr; io.gz = gz;
+    return solve_impl(h, nbatch, rho, phi_inout, tol, max_sweeps, (cudaStream_t)stream, out, &io);
+}
+
 int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr, double* gz, void* stream) {
     g_err.clear();
     if (!h || !phi || !gr || !gz) { set_err("NULL argument"); return -1; }
@@ -1033,18 +1072,7 @@ int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr,
     CU_TRY(cudaSetDevice(h->device));
     const Geom g = make_geom(h, 0.0);
     cudaStream_t st = (cudaStream_t)stream;
-    const bool vec = h->nr % 4 == 0 && ((((uintptr_t)phi | (uintptr_t)gr | (uintptr_t)gz) & 15) == 0);
-    if (vec) {
-        const unsigned qx = (h->nr / 4 + 127) / 128;                       // rows folded into grid.x: no 65535 limit on nz
-        const dim3 grid(qx * (unsigned)h->nz, 1, nbatch);
-        k_gravity4<<<grid, 128, 0, st>>>(g, (int)qx, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
-    } else {
-        const unsigned qx = (h->nr + 127) / 128;
-        const dim3 grid(qx * (unsigned)h->nz, 1, nbatch);
-        k_gravity1<<<grid, 128, 0, st>>>(g, (int)qx, phi, h->d_bE, h->d_bN, h->d_bS, gr, gz);
-    }
-    CU_TRY(cudaGetLastError());
-    return 0;
+    return launch_gravity(h, g, nbatch, phi, gr, gz, st);
 }
 
 int sn_poisson_probe_l2(int mib, double* copy_gbs, double* read_gbs, void* stream) {

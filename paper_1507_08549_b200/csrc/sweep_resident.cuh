@@ -72,6 +72,8 @@ struct ResParams {
     Ctl* ctl;                  // [nb]
     double* hist;              // [nb][cap]
     long long* prof;           // optional [ctas][8] SM-clock counters of thread 0 of every CTA ("prof" option), else NULL
+    double* gr;                // optional fused epilogue (NEXT-1, R15): [nb][ncell] g_r, g_z = -grad phi of the result, else NULL
+    double* gz;
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -642,6 +644,42 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     // make every CTA pass one more barrier before the result overwrites it.
     grid_barrier();
     if (own) E.store_patch(phi_io, g.nr, gi0, gj0);
+    // ---- fused gravity epilogue (NEXT-1; eqs. 2-4; R15): g = -grad phi of the result while
+    // phi is still in registers.  Neighbours inside the patch are registers; the ones outside come from the result
+    // just stored (L2), after one more grid barrier -- the same in every tile mode, and exact: centred differences with
+    // the pinned arithmetic (lo - hi) * (0.5 / d), reflecting axis / equator, ghosts elsewhere.
+    if (p.gr != nullptr) {
+        grid_barrier();
+        if (own && E.active) {
+            double* grm = p.gr + (size_t)member * ncell;
+            double* gzm = p.gz + (size_t)member * ncell;
+            const double hr = 0.5 / g.dr, hz = 0.5 / g.dz;
+#pragma unroll
+            for (int q = 0; q < H; ++q) {
+                const int row = gj0 + q;
+                const double* prow = phi_io + (size_t)row * g.nr;
+                const double west = gi0 > 0 ? __ldcg(prow + gi0 - 1) : E.phi[q][0];                 // reflecting axis
+                const double east = gi0 + 4 < g.nr ? __ldcg(prow + gi0 + 4) : bE[row];
+                double r4[4], z4[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const double pW = c == 0 ? west : E.phi[q][c == 0 ? 0 : c - 1];
+                    const double pE = c == 3 ? east : E.phi[q][c == 3 ? 3 : c + 1];
+                    const double pN = q < H - 1 ? E.phi[q < H - 1 ? q + 1 : q][c]
+                                                : (row + 1 < g.nz ? __ldcg(prow + g.nr + gi0 + c) : bN[gi0 + c]);
+                    const double pS = q > 0 ? E.phi[q > 0 ? q - 1 : 0][c]
+                                            : (row > 0 ? __ldcg(prow - g.nr + gi0 + c)
+                                                       : (g.symmetry == 1 ? E.phi[q][c] : bS[gi0 + c]));
+                    r4[c] = __dmul_rn(__dsub_rn(pW, pE), hr);
+                    z4[c] = __dmul_rn(__dsub_rn(pS, pN), hz);
+                }
+                double2* o = reinterpret_cast<double2*>(grm + (size_t)row * g.nr + gi0);
+                double2* z = reinterpret_cast<double2*>(gzm + (size_t)row * g.nr + gi0);
+                __stcs(o, make_double2(r4[0], r4[1])); __stcs(o + 1, make_double2(r4[2], r4[3]));
+                __stcs(z, make_double2(z4[0], z4[1])); __stcs(z + 1, make_double2(z4[2], z4[3]));
+            }
+        }
+    }
     ++seq;
     Engine::sync();
     if (tid == 0) s_rep[seq & 1].quit = 1;

@@ -105,6 +105,20 @@ class PoissonSolver:
         self._raise_if_failed(res, "sn_poisson_solve_sequence_host")      # steps after a failed one stay at -1
         return res
 
+    def solve_gravity(self, rho, phi, tol, max_sweeps):
+        """Solve in place on ``phi`` and return (results, g_r, g_z) from the fused epilogue (sn_poisson_solve_gravity)."""
+        import torch
+        self._check(rho)
+        self._check(phi)
+        if rho.shape != phi.shape or tuple(rho.shape[-2:]) != (self.nz, self.nr):
+            raise ValueError("shape mismatch")
+        nb = rho.shape[0] if rho.dim() == 3 else 1
+        gr, gz = torch.empty_like(phi), torch.empty_like(phi)
+        res = B.sn_poisson_solve_gravity(self.h, nb, rho.data_ptr(), phi.data_ptr(), gr.data_ptr(), gz.data_ptr(), tol,
+                                         max_sweeps, torch.cuda.current_stream().cuda_stream)
+        self._raise_if_failed(res, "sn_poisson_solve_gravity")
+        return (res if rho.dim() == 3 else res[0]), gr, gz
+
     def gravity(self, phi, gr=None, gz=None):
         """(g_r, g_z) = -grad phi with the ghost values of the last solve; enqueued on the current stream."""
         import torch

@@ -901,3 +901,38 @@ def test_paper_literal_configuration(P, torch_cuda, oracle):
         refb = oracle.solve(m.rho, np.zeros_like(m.rho), m.dr, m.dz, 1, m.lmax, 1e-8, 20000, rule=1)
         assert (res[b].sweeps, res[b].status) == (refb["sweeps"], 0)
         assert relmax(pb[b].cpu().numpy(), refb["phi"]) <= REL
+
+
+@pytest.mark.parametrize("opts", [{}, {"path": 2, "halo": 0}, {"path": 2, "halo": 1, "ds": 0, "shape": 4},
+                                  {"path": 2, "halo": 1, "ds": 1, "shape": 4}, {"path": 3}, {"path": 1}])
+@pytest.mark.parametrize("symmetry", [0, 1])
+def test_fused_gravity_epilogue_bit_exact(P, torch_cuda, oracle, symmetry, opts):
+    """sn_poisson_solve_gravity: the field emitted by the relaxation kernel itself (resident path: from the registers that
+    hold phi) equals, bit for bit, the oracle's gravity of the returned phi with the solve's own ghosts -- on every path,
+    on ragged tiles, and for a batch (every member with its own ghosts)."""
+    w = W.random_smooth(128, 104, symmetry, seed=950 + symmetry, lmax=6)
+    s = P.PoissonSolver(w.nr, w.nz, w.dr, w.dz, symmetry, w.lmax)
+    for k, v in opts.items():
+        s.set_option(k, v)
+    rho = torch_cuda.from_numpy(w.rho).cuda()
+    phi = torch_cuda.zeros_like(rho)
+    r, gr, gz = s.solve_gravity(rho, phi, 1e-7, 3000)
+    assert r.status == 0 and (not opts or s.stat("path") == opts["path"])
+    got = phi.cpu().numpy()
+    want_r, want_z = oracle.gravity(got, w.dr, w.dz, symmetry, *s.boundary())
+    assert np.array_equal(gr.cpu().numpy(), want_r) and np.array_equal(gz.cpu().numpy(), want_z)
+    # the solve itself is unchanged by the epilogue
+    phi2 = torch_cuda.zeros_like(rho)
+    r2 = s.solve(rho, phi2, 1e-7, 3000)
+    assert (r2.sweeps, r2.residual) == (r.sweeps, r.residual) and torch_cuda.equal(phi, phi2)
+    # batch of 3, fixed sweeps
+    ws = [W.random_smooth(128, 104, symmetry, seed=960 + b, lmax=6) for b in range(3)]
+    rb = torch_cuda.from_numpy(np.stack([m.rho for m in ws])).cuda()
+    pb = torch_cuda.zeros_like(rb)
+    res, grb, gzb = s.solve_gravity(rb, pb, 0.0, 25)
+    assert all(x.sweeps == 25 for x in res)
+    for b, m in enumerate(ws):
+        M = oracle.moments(m.rho, m.dr, m.dz, symmetry, m.lmax)
+        bnd = oracle.boundary(m.nr, m.nz, m.dr, m.dz, symmetry, m.lmax, M)
+        want_r, want_z = oracle.gravity(pb[b].cpu().numpy(), m.dr, m.dz, symmetry, *bnd)
+        assert relmax(grb[b].cpu().numpy(), want_r) <= REL and relmax(gzb[b].cpu().numpy(), want_z) <= REL
