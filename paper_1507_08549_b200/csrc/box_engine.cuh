@@ -104,7 +104,19 @@ __device__ __forceinline__ bool poll_giveup(const PollCtx& c, unsigned& n, int c
 
 // BAR = 0: the engine's barrier is __syncthreads(); BAR > 0: named barrier BAR over the first NT threads of the CTA
 // (the resident kernel runs an extra service warp that must not take part in it).
-template <int H, int TXN, int TYN, int BAR = 0>
+// Rows per update group (BoxEngine::update_cells) for a kernel of `threads` threads with `minb` CTAs per SM: every
+// chain in flight needs ~6 registers of temporaries and operands on top of the 8 H registers of phi, so the group
+// grows with the registers per thread the launch bounds leave (measured on B200: profiles/r02_ilp.md).
+#ifndef SNP_GROUP_ROWS_ROOMY
+#define SNP_GROUP_ROWS_ROOMY 4
+#endif
+__host__ __device__ constexpr int group_rows_for(int threads, int minb) {
+    const int warps = (threads + 63) / 64 * 2;                   // registers are allocated per pair of warps
+    const int regs = 65536 / (minb * warps * 32) > 255 ? 255 : 65536 / (minb * warps * 32);
+    return regs >= 160 ? SNP_GROUP_ROWS_ROOMY : 2;
+}
+
+template <int H, int TXN, int TYN, int BAR = 0, int GR = 2>
 struct BoxEngine {
     using S = BoxShape<H, TXN, TYN>;
     static constexpr int BW = S::BW, BH = S::BH, LS = S::LS, PW = S::PW;
@@ -307,52 +319,71 @@ struct BoxEngine {
         }
         return pf;
     }
-    // WHICH: 0 all cells of colour COL, 1 only the patch-edge cells (rows 0 and H-1, column 0 / 3), 2 the others
-    // PF (ring duty): after the first half of the rows, put this thread's poll of the neighbour's packet in flight
-    // (pf_src may be NULL: nothing to receive); halo_recv consumes *pf.
+    // All cells of colour COL of the patch.  The updates of one colour are mutually independent, so they are issued in
+    // groups of kGroupRows rows (2 cells each) STAGE BY STAGE: all operands of the group are fetched first, then the
+    // 7-deep fp64 chains of the group's cells advance in lock step, so that each warp has 2 kGroupRows independent
+    // dependency chains in flight instead of one (a single chain issues one fp64 instruction per ~8.4 clocks; measured
+    // in profiles/r02_ilp.md).  The expression tree of every cell is sor_update's (R10), only the issue order differs.
+    // PF (ring duty): after the last row, put this thread's poll of the neighbour's packet in flight (pf_src may be
+    // NULL: nothing to receive); halo_recv consumes *pf.
+    // GR (template argument): rows per group the kernel can afford with its register budget (group_rows_for below).
+    static constexpr int kGroupRows = H % GR == 0 ? GR : 2;
     template <int COL, int TRACK, int WHICH, bool PF = false>
     __device__ __forceinline__ void update_cells(const uint4* pf_src = nullptr, uint4* pf = nullptr) {
+        static_assert(WHICH == 0 && H % kGroupRows == 0, "whole patch, whole groups");
         // vertical outer neighbours of the bottom (q=0) and top (q=H-1) rows: other-colour cells of the rows outside
         constexpr int pb = COL & 1, pt = (H - 1 + COL) & 1;                 // column parity updated in those rows
-        double2 So = make_double2(0.0, 0.0), No = make_double2(0.0, 0.0);
-        if (WHICH != 2) {
-            So = *reinterpret_cast<const double2*>(exT + (size_t)b * BW + pb * PW + 2 * a);
-            No = *reinterpret_cast<const double2*>(exB + (size_t)(b + 2) * BW + pt * PW + 2 * a);
-        }
+        const double2 So = *reinterpret_cast<const double2*>(exT + (size_t)b * BW + pb * PW + 2 * a);
+        const double2 No = *reinterpret_cast<const double2*>(exB + (size_t)(b + 2) * BW + pt * PW + 2 * a);
+        constexpr int G = kGroupRows, NC = 2 * G;
 #pragma unroll
-        for (int q = 0; q < H; ++q) {
-            if (PF && q == kPfRow) { if (pf_src) *pf = ll_load_early(pf_src); }
-            const int pq = (q + COL) & 1;                                   // compile-time after unrolling
-            const bool edge_row = q == 0 || q == H - 1;
-            const bool any0 = WHICH == 0 || (WHICH == 1 ? (edge_row || pq == 0) : (!edge_row && pq != 0));   // cc = 0
-            const bool any1 = WHICH == 0 || (WHICH == 1 ? (edge_row || pq == 1) : (!edge_row && pq != 1));   // cc = 1
-            if (!any0 && !any1) continue;
-            const bool need_outer = (pq == 0 && any0) || (pq == 1 && any1);
-            const double outer = !need_outer ? 0.0 : pq == 0 ? exR[(rowbase + q) * LS + a] : exL[(rowbase + q) * LS + a + 2];
-            const double2 fv = *reinterpret_cast<const double2*>(fs + (size_t)(rowbase + q) * BW + pq * PW + 2 * a);
-            const double cS = (q == 0 && mirror0) ? 0.0 : iz2;
-            const double dg = (q == 0 && mirror0) ? D0 : D;
-            const double ww = (q == 0 && mirror0) ? wD0 : wD;
+        for (int q0 = 0; q0 < H; q0 += G) {
+            double pE[NC], pW[NC], pN[NC], pS[NC], pC[NC], ff[NC], t[NC];
+            // ---- operands
 #pragma unroll
-            for (int cc = 0; cc < 2; ++cc) {
-                if (!(cc == 0 ? any0 : any1)) continue;
-                const int c = pq + 2 * cc;
-                const double pW = c == 0 ? outer : phi[q][c == 0 ? 0 : c - 1];
-                const double pE = c == 3 ? outer : phi[q][c == 3 ? 3 : c + 1];
-                const double pN = q == H - 1 ? (cc == 0 ? No.x : No.y) : phi[q == H - 1 ? q : q + 1][c];
-                const double pS = q == 0 ? (cc == 0 ? So.x : So.y) : phi[q == 0 ? 0 : q - 1][c];
-                double res;
-                const double pn = sor_update(cEr[c], cWr[c], iz2, cS, dg, ww, pE, pW, pN, pS, phi[q][c],
-                                             cc == 0 ? fv.x : fv.y, res);
-                phi[q][c] = pn;
-                track<TRACK>(res, pn);
+            for (int gq = 0; gq < G; ++gq) {
+                const int q = q0 + gq;
+                const int pq = (q + COL) & 1;                               // compile-time after unrolling
+                const double outer = pq == 0 ? exR[(rowbase + q) * LS + a] : exL[(rowbase + q) * LS + a + 2];
+                const double2 fv = *reinterpret_cast<const double2*>(fs + (size_t)(rowbase + q) * BW + pq * PW + 2 * a);
+#pragma unroll
+                for (int cc = 0; cc < 2; ++cc) {
+                    const int c = pq + 2 * cc, i = 2 * gq + cc;
+                    pW[i] = c == 0 ? outer : phi[q][c == 0 ? 0 : c - 1];
+                    pE[i] = c == 3 ? outer : phi[q][c == 3 ? 3 : c + 1];
+                    pN[i] = q == H - 1 ? (cc == 0 ? No.x : No.y) : phi[q == H - 1 ? q : q + 1][c];
+                    pS[i] = q == 0 ? (cc == 0 ? So.x : So.y) : phi[q == 0 ? 0 : q - 1][c];
+                    pC[i] = phi[q][c];
+                    ff[i] = cc == 0 ? fv.x : fv.y;
+                }
+            }
+            // ---- the chains, stage by stage (sor_update's tree)
+#pragma unroll
+            for (int i = 0; i < NC; ++i) t[i] = __dmul_rn(cEr[((q0 + i / 2 + COL) & 1) + 2 * (i & 1)], pE[i]);
+#pragma unroll
+            for (int i = 0; i < NC; ++i) t[i] = __fma_rn(cWr[((q0 + i / 2 + COL) & 1) + 2 * (i & 1)], pW[i], t[i]);
+#pragma unroll
+            for (int i = 0; i < NC; ++i) t[i] = __fma_rn(iz2, pN[i], t[i]);
+#pragma unroll
+            for (int i = 0; i < NC; ++i) t[i] = __fma_rn((q0 + i / 2 == 0 && mirror0) ? 0.0 : iz2, pS[i], t[i]);
+#pragma unroll
+            for (int i = 0; i < NC; ++i) t[i] = __fma_rn(-((q0 + i / 2 == 0 && mirror0) ? D0 : D), pC[i], t[i]);
+#pragma unroll
+            for (int i = 0; i < NC; ++i) t[i] = __dsub_rn(ff[i], t[i]);                                   // res
+#pragma unroll
+            for (int i = 0; i < NC; ++i) pC[i] = __fma_rn(-((q0 + i / 2 == 0 && mirror0) ? wD0 : wD), t[i], pC[i]);
+#pragma unroll
+            for (int i = 0; i < NC; ++i) {
+                const int q = q0 + i / 2, c = ((q + COL) & 1) + 2 * (i & 1);
+                phi[q][c] = pC[i];
+                track<TRACK>(t[i], pC[i]);
                 if (q == 0 && mirror0) {             // q is a compile-time constant: two predicated maxima per half-sweep
-                    if (TRACK == kTrackExact) { const unsigned long long kr = abs_key(res); mres0_k = kr > mres0_k ? kr : mres0_k; }
-                    else if (TRACK == kTrackFast) mres0_f = fmaxf(mres0_f, fabsf(__int_as_float(__double2hiint(res))));
+                    if (TRACK == kTrackExact) { const unsigned long long kr = abs_key(t[i]); mres0_k = kr > mres0_k ? kr : mres0_k; }
+                    else if (TRACK == kTrackFast) mres0_f = fmaxf(mres0_f, fabsf(__int_as_float(__double2hiint(t[i]))));
                 }
             }
         }
-        if (PF && kPfRow >= H) { if (pf_src) *pf = ll_load_early(pf_src); }
+        if (PF) { if (pf_src) *pf = ll_load_early(pf_src); }
     }
     // publish the updated patch-edge cells of colour COL to the exchange arrays of the CTA
     template <int COL, bool RING = false>
@@ -422,9 +453,8 @@ struct BoxEngine {
     // whole warps of its own (no divergence between the four cases), else the threads are packed E | W | N | S.
     // SEND, plain variant: the owners of the box-edge cells send after their patch update (h_scol / h_srow).
     // SEND, ring variant: see ring_duty().
-    // Patch row before which the first poll is issued (H: after the last row).  Measured (profiles/r02_ring.md): any
-    // earlier position changes nothing, because ptxas sinks the load to its first use whatever the source order is.
-    static constexpr int kPfRow = H;
+    // (the first poll is issued after the last patch row: any earlier position in the source changes nothing, ptxas
+    // sinks the load to its first use -- profiles/r02_ring.md)
     int h_edge = -1;                 // 0 E, 1 W, 2 N, 3 S; -1: this thread receives nothing
     int h_j = 0;
     uint4* h_scol = nullptr;         // column edge: west (h_west) or east

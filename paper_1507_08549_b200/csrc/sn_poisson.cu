@@ -20,6 +20,7 @@
 #include "sweep_stream.cuh"
 #include "sweep_blocked.cuh"
 #include "sweep_resident.cuh"
+#include "shapes.cuh"
 
 using namespace snp;
 
@@ -264,29 +265,12 @@ int run_stream(sn_poisson* h, const Geom& g, int nbatch, const double* rho, doub
 
 
 // ---- blocked path: shapes, planner, launcher -------------------------------------------------------------------
-struct BlkShapeInfo {
-    int H, TXN, TYN, minb;
-    size_t smem;
-    const void* fn;
-    double hs_clk;             // measured clocks per half-sweep of one box with `minb` CTAs sharing an SM (cost model)
-    int BW() const { return 4 * TXN; }
-    int BH() const { return H * TYN; }
-    int NT() const { return TXN * TYN; }
-};
-
-template <int H, int TXN, int TYN, int MINB>
-BlkShapeInfo blk_shape_of(double hs_clk) {
-    return {H, TXN, TYN, MINB, BlkShape<H, TXN, TYN>::smem_bytes, (const void*)k_sor_blocked<H, TXN, TYN, MINB>, hs_clk};
-}
-
 const std::vector<BlkShapeInfo>& blk_shapes() {
-    static const std::vector<BlkShapeInfo> v = {
-        blk_shape_of<8, 32, 8, 2>(1853.0),    // 0: box 128 x 64,  256 threads, 2 CTAs / SM
-        blk_shape_of<8, 32, 14, 1>(1516.0),   // 1: box 128 x 112, 448 threads
-        blk_shape_of<16, 32, 8, 1>(1562.0),   // 2: box 128 x 128, 256 threads
-        blk_shape_of<8, 16, 8, 3>(1400.0),    // 3: box 64 x 64,   128 threads, 3 CTAs / SM
-        blk_shape_of<4, 16, 8, 4>(1200.0),    // 4: box 64 x 32,   128 threads, 4 CTAs / SM
-    };
+    static const std::vector<BlkShapeInfo> v = [] {
+        std::vector<BlkShapeInfo> t;
+        for (int i = 0; i < kNumBlkShapes; ++i) t.push_back(blk_shape(i));      // shape_tu.cu
+        return t;
+    }();
     return v;
 }
 
@@ -397,46 +381,12 @@ int run_blocked(sn_poisson* h, const Geom& g, const BlkPlan& pl, int nbatch, con
 
 
 // ---- resident path: shapes, planner, launcher ------------------------------------------------------------------
-struct ShapeInfo {
-    int H, TXN, TYN, minb;
-    size_t smem, smem_ring, smem_ring_ds;
-    const void* fn[5];          // [0] block mode, [1] halo mode, [2] halo mode inside one cluster (DSMEM) or NULL,
-                                // [3] halo mode with ring duty, [4] cluster halo mode with ring duty or NULL
-    int BW() const { return 4 * TXN; }
-    int BH() const { return H * TYN; }
-    int NT() const { return TXN * TYN; }
-    int threads() const { return TXN * TYN + 32; }     // + the service warp
-    size_t smem_of(int f) const { return f == 3 ? smem_ring : f == 4 ? smem_ring_ds : smem; }
-};
-
-template <int H, int TXN, int TYN, int MINB, bool DS = true>
-ShapeInfo shape_of() {
-    const void *ds = nullptr, *dsr = nullptr;
-    if constexpr (DS) {
-        ds = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false, true>;
-        dsr = (const void*)k_sor_resident<H, TXN, TYN, MINB, true, true, true>;
-    }
-    return {H, TXN, TYN, MINB, ResShape<H, TXN, TYN>::smem_bytes, ResShape<H, TXN, TYN>::smem_bytes_ring,
-            ResShape<H, TXN, TYN>::smem_bytes_ring_ds,
-            {(const void*)k_sor_resident<H, TXN, TYN, MINB, false, false>,
-             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, false>, ds,
-             (const void*)k_sor_resident<H, TXN, TYN, MINB, true, true>, dsr}};
-}
-
 const std::vector<ShapeInfo>& shapes() {
-    static const std::vector<ShapeInfo> v = {
-        shape_of<8, 32, 14, 1, false>(),   // 0: box 128 x 112, 448 threads
-        shape_of<8, 32, 8, 1, false>(),    // 1: box 128 x 64,  256 threads
-        shape_of<8, 16, 8, 2>(),    // 2: box 64 x 64,   128 threads
-        shape_of<4, 16, 8, 2>(),    // 3: box 64 x 32,   128 threads
-        shape_of<4, 8, 8, 2>(),     // 4: box 32 x 32,    64 threads
-        shape_of<2, 8, 16, 2>(),    // 5: box 32 x 32,   128 threads
-        shape_of<8, 32, 7, 2, false>(),    // 6: box 128 x 56,  224 threads, 2 CTAs / SM (halo mode on chip-filling grids)
-        shape_of<4, 16, 16, 1>(),   // 7: box 64 x 64,   256 threads
-        shape_of<6, 12, 8, 2>(),    // 8: box 48 x 48,    96 threads
-        shape_of<4, 12, 16, 1>(),   // 9: box 48 x 64,   192 threads
-        shape_of<2, 16, 32, 1>(),   // 10: box 64 x 64,  512 threads of 2 x 4 patches (shortest half-sweep: small grids)
-    };
+    static const std::vector<ShapeInfo> v = [] {
+        std::vector<ShapeInfo> t;
+        for (int i = 0; i < kNumResShapes; ++i) t.push_back(res_shape(i));      // shape_tu.cu: one translation unit per shape
+        return t;
+    }();
     return v;
 }
 
@@ -492,6 +442,7 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
         for (int md = 0; md < 2; ++md) {
             const int f = md == 0 ? 0 : halo_fn;
             int occ = 0;
+            if (!S.fn[f]) { max_ctas_mode[md] = 0; continue; }       // shape without this mode
             if (cudaFuncSetAttribute(S.fn[f], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S.smem_of(f)) != cudaSuccess ||
                 cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, S.fn[f], S.threads(), S.smem_of(f)) != cudaSuccess) {
                 cudaGetLastError();
@@ -500,7 +451,7 @@ ResPlan plan_resident(sn_poisson* h, int nbatch, const double* rho, const double
             max_ctas_mode[md] = (long long)occ * h->num_sms;
         }
         // halo mode: box == tile on a regular lattice, ragged last tile row allowed
-        if (h->opt_halo != 0 && h->nr % S.BW() == 0 && h->nz % S.H == 0) {
+        if (h->opt_halo != 0 && S.fn[halo_fn] && h->nr % S.BW() == 0 && h->nz % S.H == 0) {
             ResPlan p;
             p.shape = si; p.halo = 1; p.ring = halo_fn == 3;
             p.ntx = h->nr / S.BW(); p.nty = (h->nz + S.BH() - 1) / S.BH();

@@ -45,7 +45,7 @@ struct BlkParams {
 };
 
 // First action of a member (after the moments pass has written maxf).  grid = nbatch, 1 thread.
-__global__ void k_blocked_init(Ctl* __restrict__ ctl, int m, int max_sweeps, int force_exact) {
+static __global__ void k_blocked_init(Ctl* __restrict__ ctl, int m, int max_sweeps, int force_exact) {
     Ctl* c = ctl + blockIdx.x;
     if (threadIdx.x != 0) return;
     const int n = max_sweeps < m ? max_sweeps : m;
@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(TXN* TYN, MINB) k_sor_blocked(const BlkParams 
     const int bx = box_origin(x0, h, 4, BW, g.nr);
     const int by = box_origin(y0, h, H, BH, g.nz);
 
-    BoxEngine<H, TXN, TYN> E;
+    BoxEngine<H, TXN, TYN, 0, group_rows_for(TXN * TYN, MINB)> E;
     E.carve(reinterpret_cast<double*>(smem_raw));
     unsigned long long* smax = reinterpret_cast<unsigned long long*>(E.exT + S::vert_doubles);   // [2*kMaxTB][NW]
     E.bind_thread(tid);

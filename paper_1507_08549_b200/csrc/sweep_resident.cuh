@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     using S = BoxShape<H, TXN, TYN>;
     using RS = ResShape<H, TXN, TYN>;
     constexpr int BW = S::BW, BH = S::BH, NT = S::NT, NW = S::NW;
-    using Engine = BoxEngine<H, TXN, TYN, 1>;
+    using Engine = BoxEngine<H, TXN, TYN, 1, group_rows_for(TXN * TYN + 32, MINB)>;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ ResReport s_rep[2];
@@ -144,8 +144,8 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     __shared__ int s_zero;         // a quit word that never fires (endgame / replay polls)
     __shared__ __align__(8) unsigned long long s_mbar[2];   // DS: one mbarrier per colour, credited by the neighbours' st.async
     __shared__ long long s_pf[8];  // in-kernel profile of thread 0 ("prof" option)
-    __shared__ typename BoxEngine<H, TXN, TYN, 1>::HaloLinks s_links;   // halo mode: inboxes of this tile and its neighbours
-    __shared__ typename BoxEngine<H, TXN, TYN, 1>::RingConst s_ring;    // ring duty: CTA-uniform constants
+    __shared__ typename Engine::HaloLinks s_links;   // halo mode: inboxes of this tile and its neighbours
+    __shared__ typename Engine::RingConst s_ring;    // ring duty: CTA-uniform constants
     __shared__ double s_stash[RING ? 2 * (BoxShape<H, TXN, TYN>::BH + BoxShape<H, TXN, TYN>::BW) : 1];
 
     const Geom& g = p.g;
@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(TXN* TYN + 32, MINB) k_sor_resident(const ResP
     double* ring = p.ring + (size_t)member * kResRing * ncell;
     // halo mode: inboxes of this tile and of its four neighbours
     const bool mirror_box = g.symmetry == 1 && by == 0;
-    if (HALO) {
+    if constexpr (HALO) {
         typename Engine::HaloLinks links;
         uint4* mb = p.mail + (size_t)member * ntiles * Engine::kInboxPackets;
         auto inbox = [&](int t) { return mb + (size_t)t * Engine::kInboxPackets; };
