@@ -239,3 +239,79 @@ def levelset_reinit(S, dr, dz, delta=None):
     n = _ls().lso_reinit(nx, ny, dr, dz, dr if delta is None else delta, _p(S), _p(out), _p(dist))
     assert n >= 0
     return {"S": out, "dist": dist, "crossings": int(n)}
+
+
+# ---- NEXT-3: WENO-5 / global Lax-Friedrichs flux reconstruction (oracle/weno_oracle.cpp) ----------------------------
+_ip = C.POINTER(C.c_int)
+
+
+def _wn():
+    L = extra_lib("weno")
+    L.wno_weno5.restype = C.c_double
+    L.wno_weno5.argtypes = [C.c_double] * 5
+    L.wno_candidates.argtypes = [C.c_double] * 5 + [_dp, _dp]
+    L.wno_max_speeds.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _dp, _dp, _dp]
+    L.wno_rhs.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _dp, C.c_double, C.c_double, _dp]
+    L.wno_face_fluxes.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, _dp, _dp, _dp]
+    L.wno_step.restype = C.c_double
+    L.wno_step.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, C.c_double, _dp]
+    L.wno_evolve.restype = C.c_int
+    L.wno_evolve.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, _ip, C.c_double, C.c_double,
+                             C.c_int, _dp]
+    return L
+
+
+def _bc(bc):
+    return (C.c_int * 4)(*[int(b) for b in bc])
+
+
+def weno5(a, b, c, d, e) -> float:
+    return _wn().wno_weno5(float(a), float(b), float(c), float(d), float(e))
+
+
+def weno_candidates(a, b, c, d, e):
+    q, beta = np.zeros(3), np.zeros(3)
+    _wn().wno_candidates(float(a), float(b), float(c), float(d), float(e), _p(q), _p(beta))
+    return q, beta
+
+
+def _u4(U):
+    U = _f64(U)
+    assert U.ndim == 3 and U.shape[0] == 4, "U must be (4, nz, nr)"
+    return U
+
+
+def weno_max_speeds(U, dr, dz, gamma, bc):
+    U = _u4(U)
+    ar, az = C.c_double(), C.c_double()
+    _wn().wno_max_speeds(U.shape[2], U.shape[1], dr, dz, gamma, _bc(bc), _p(U), C.byref(ar), C.byref(az))
+    return ar.value, az.value
+
+
+def weno_rhs(U, dr, dz, gamma, bc, alpha=None):
+    """L(U) = -(dF/dr + dG/dz) (W6); alpha = (alpha_r, alpha_z) or None for the global maxima of U (W4)."""
+    U = _u4(U)
+    L = np.zeros_like(U)
+    ar, az = (-1.0, -1.0) if alpha is None else alpha
+    _wn().wno_rhs(U.shape[2], U.shape[1], dr, dz, gamma, _bc(bc), _p(U), ar, az, _p(L))
+    return L
+
+
+def weno_face_fluxes(U, dr, dz, gamma, bc):
+    U = _u4(U)
+    F, G = np.zeros_like(U), np.zeros_like(U)
+    _wn().wno_face_fluxes(U.shape[2], U.shape[1], dr, dz, gamma, _bc(bc), _p(U), _p(F), _p(G))
+    return F, G
+
+
+def weno_step(U, dr, dz, gamma, bc, cfl):
+    """One SSP-RK3 step (W8) on a copy; returns (U_new, dt)."""
+    U = _u4(U).copy()
+    dt = _wn().wno_step(U.shape[2], U.shape[1], dr, dz, gamma, _bc(bc), cfl, _p(U))
+    return U, dt
+
+
+def weno_evolve(U, dr, dz, gamma, bc, cfl, t_end, max_steps=1000000):
+    U = _u4(U).copy()
+    n = _wn().wno_evolve(U.shape[2], U.shape[1], dr, dz, gamma, _bc(bc), cfl, t_end, max_steps, _p(U))
+    return U, n

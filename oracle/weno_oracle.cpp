@@ -1,0 +1,255 @@
+// weno_oracle.cpp -- CPU oracle of the WENO-5 / global Lax-Friedrichs flux reconstruction.
+//
+// TEST INFRASTRUCTURE, NOT THE PRODUCT.  Plain, slow, single-threaded fp64; shares no code with
+// paper_1507_08549_b200/; only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+// load it.
+//
+// PAPER.md:79-89, eqs. (1)-(4): the conservative Euler equations; "The terms on the right hand side are regarded as
+// source terms" -- this oracle computes the LEFT-hand side only (the flux divergence), as the paper's "WENO scheme"
+// subroutine (Table 2) does.  PAPER.md:95: "This is a fifth-order scheme ... we use a finite-difference
+// formulation of the WENO scheme ... First we separate the hydro flux into a positive flux and a negative flux by a
+// global Lax-Friedrichs splitting.  Then we apply the WENO reconstruction on the two fluxes by an upwinding scheme.
+// The numerical flux is obtained by summing the reconstructed positive and negative fluxes."  PAPER.md:402 (section
+// 5.1): "we use a polytropic EOS with the ratio of specific heat gamma = 1.4 ... p = rho eps (gamma - 1) ... The
+// Courant number is fixed to be 0.5", Cartesian limit ("the volume of each grid is independent of the radial distance").
+//
+// Readings where the paper is silent (W1..W8):
+//   W1  state: U[c][j][i], c = 0..3 = (rho, rho v_r, rho v_z, tau), planes of nz x nr, r fastest; values at cell centres.
+//   W2  EOS: p = (gamma - 1) (tau - (m_r m_r + m_z m_z) / (2 rho)); sound speed c = sqrt(gamma p / rho).
+//   W3  fluxes: F = (m_r, m_r v_r + p, m_z v_r, (tau + p) v_r) in r, G = (m_z, m_r v_z, m_z v_z + p, (tau + p) v_z) in z,
+//       v = m / rho.
+//   W4  "global" splitting: alpha_r = max over ALL cells of (|v_r| + c), alpha_z likewise; F+- = 0.5 (F +- alpha U),
+//       component by component (the paper describes no characteristic projection).
+//   W5  reconstruction at the face i+1/2: the classic fifth-order WENO of Jiang & Shu (the paper's citation): candidates
+//       q0 = (2a - 7b + 11c)/6, q1 = (-b + 5c + 2d)/6, q2 = (2c + 5d - e)/6 on the cells (a..e) = (i-2..i+2) for F+,
+//       mirrored (i+3..i-1) for F-; smoothness b0 = 13/12 (a-2b+c)^2 + 1/4 (a-4b+3c)^2, b1 = 13/12 (b-2c+d)^2 +
+//       1/4 (b-d)^2, b2 = 13/12 (c-2d+e)^2 + 1/4 (3c-4d+e)^2; weights w_k = (d_k / (eps + b_k)^2) / sum, d = (0.1, 0.6, 0.3),
+//       eps = 1e-6.
+//   W6  L(U) = -(Fhat_{i+1/2} - Fhat_{i-1/2}) / dr - (Ghat_{j+1/2} - Ghat_{j-1/2}) / dz.
+//   W7  three ghost cells per side, per side one of: 0 outflow (copy of the edge cell), 1 reflecting (mirror image, the
+//       normal momentum changes sign), 2 periodic.
+//   W8  time step (for the shock-tube pins and the step entry point only): the paper's five-stage third-order RK is
+//       cited, not printed; the "original prescription" it names is used instead -- SSP-RK3 (Shu-Osher):
+//       U1 = U + dt L(U); U2 = 3/4 U + 1/4 (U1 + dt L(U1)); U' = 1/3 U + 2/3 (U2 + dt L(U2)); alpha recomputed per stage;
+//       dt = CFL / (alpha_r / dr + alpha_z / dz) from the state at the start of the step (a 1-D test is one row with a
+//       dz so large that the second term vanishes: the paper's 1-D Courant number).
+//   W9  Table 3 prints t0 = 0.5 for test 2, the text shows it at t0 = 0.15 (Toro's value; at 0.5 the
+//       rarefactions have left the unit interval): 0.15 is used.
+//   Pinned arithmetic (so that the CUDA path can match bit for bit): no FMA contraction (-ffp-contract=off), every
+//   expression typed out below in the order it is evaluated; max-reductions are exact in any order.
+//
+// Pins (tests/test_weno_pins.py): constant state -> L = 0 exactly; the reconstruction reproduces polynomials of degree
+// <= 2 exactly on every candidate and the 5th-order linear combination for degree <= 4 (smooth limit); fifth-order
+// convergence of L on a smooth periodic advection profile; conservation (sum L dV = boundary fluxes, 0 when periodic);
+// a brute-force pure-Python restatement on tiny grids; mirror symmetry; the paper's four shock tubes (Table 3,
+// PAPER.md:391-398) at the paper's resolution against an exact Riemann solver written independently in the test.
+#include <cmath>
+#include <cstddef>
+#include <vector>
+
+namespace {
+
+struct Grid {
+    int nr, nz;
+    double dr, dz, gamma;
+    int bc[4];        // r-low, r-high, z-low, z-high: 0 outflow, 1 reflecting, 2 periodic
+};
+
+// index of the source cell of ghost position i (may be outside [0, n)) and whether the normal momentum flips
+inline int ghost_index(int i, int n, int bc_lo, int bc_hi, bool* flip) {
+    *flip = false;
+    if (i < 0) {
+        if (bc_lo == 0) return 0;
+        if (bc_lo == 1) { *flip = true; return -1 - i; }
+        return i + n;
+    }
+    if (i >= n) {
+        if (bc_hi == 0) return n - 1;
+        if (bc_hi == 1) { *flip = true; return 2 * n - 1 - i; }
+        return i - n;
+    }
+    return i;
+}
+
+// conserved state of cell (i, j), ghosts included
+inline void cell_state(const Grid& g, const double* U, int i, int j, double u[4]) {
+    bool fr, fz;
+    const int si = ghost_index(i, g.nr, g.bc[0], g.bc[1], &fr);
+    const int sj = ghost_index(j, g.nz, g.bc[2], g.bc[3], &fz);
+    const size_t n = (size_t)g.nr * g.nz, k = (size_t)sj * g.nr + si;
+    u[0] = U[k];
+    u[1] = fr ? -U[n + k] : U[n + k];
+    u[2] = fz ? -U[2 * n + k] : U[2 * n + k];
+    u[3] = U[3 * n + k];
+}
+
+inline double pressure(const Grid& g, const double u[4]) {
+    const double ke = (u[1] * u[1] + u[2] * u[2]) / (2.0 * u[0]);
+    return (g.gamma - 1.0) * (u[3] - ke);
+}
+
+// flux in direction dir (0: r, 1: z) of the state u
+inline void flux(const Grid& g, const double u[4], int dir, double f[4]) {
+    const double p = pressure(g, u);
+    const double v = u[1 + dir] / u[0];
+    f[0] = u[1 + dir];
+    f[1] = u[1] * v;
+    f[2] = u[2] * v;
+    f[1 + dir] = f[1 + dir] + p;
+    f[3] = (u[3] + p) * v;
+}
+
+// fifth-order WENO value at the right face of cell c from the five cell values a..e (upwind side = a)
+inline double weno5(double a, double b, double c, double d, double e) {
+    const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) / 6.0;
+    const double q1 = (-b + 5.0 * c + 2.0 * d) / 6.0;
+    const double q2 = (2.0 * c + 5.0 * d - e) / 6.0;
+    const double s0 = a - 2.0 * b + c, t0 = a - 4.0 * b + 3.0 * c;
+    const double s1 = b - 2.0 * c + d, t1 = b - d;
+    const double s2 = c - 2.0 * d + e, t2 = 3.0 * c - 4.0 * d + e;
+    const double b0 = (13.0 / 12.0) * (s0 * s0) + 0.25 * (t0 * t0);
+    const double b1 = (13.0 / 12.0) * (s1 * s1) + 0.25 * (t1 * t1);
+    const double b2 = (13.0 / 12.0) * (s2 * s2) + 0.25 * (t2 * t2);
+    const double eps = 1.0e-6;
+    const double e0 = eps + b0, e1 = eps + b1, e2 = eps + b2;
+    const double a0 = 0.1 / (e0 * e0), a1 = 0.6 / (e1 * e1), a2 = 0.3 / (e2 * e2);
+    const double sum = (a0 + a1) + a2;
+    return ((a0 * q0 + a1 * q1) + a2 * q2) / sum;
+}
+
+void max_speeds(const Grid& g, const double* U, double* ar, double* az) {
+    double mr = 0.0, mz = 0.0;
+    for (int j = 0; j < g.nz; ++j)
+        for (int i = 0; i < g.nr; ++i) {
+            double u[4];
+            cell_state(g, U, i, j, u);
+            const double c = std::sqrt(g.gamma * pressure(g, u) / u[0]);
+            const double sr = std::fabs(u[1] / u[0]) + c, sz = std::fabs(u[2] / u[0]) + c;
+            if (sr > mr || sr != sr) mr = sr;
+            if (sz > mz || sz != sz) mz = sz;
+        }
+    *ar = mr;
+    *az = mz;
+}
+
+// numerical flux through the face between cell (i, j) and its + neighbour in direction dir
+void face_flux(const Grid& g, const double* U, int i, int j, int dir, double alpha, double fh[4]) {
+    double fp[6][4], fm[6][4];
+    for (int k = 0; k < 6; ++k) {          // cells -2 .. +3 relative to (i, j)
+        double u[4], f[4];
+        cell_state(g, U, dir == 0 ? i - 2 + k : i, dir == 0 ? j : j - 2 + k, u);
+        flux(g, u, dir, f);
+        for (int c = 0; c < 4; ++c) {
+            fp[k][c] = 0.5 * (f[c] + alpha * u[c]);
+            fm[k][c] = 0.5 * (f[c] - alpha * u[c]);
+        }
+    }
+    for (int c = 0; c < 4; ++c)
+        fh[c] = weno5(fp[0][c], fp[1][c], fp[2][c], fp[3][c], fp[4][c]) +
+                weno5(fm[5][c], fm[4][c], fm[3][c], fm[2][c], fm[1][c]);
+}
+
+void rhs(const Grid& g, const double* U, double ar, double az, double* L) {
+    const size_t n = (size_t)g.nr * g.nz;
+    for (int j = 0; j < g.nz; ++j)
+        for (int i = 0; i < g.nr; ++i) {
+            double fe[4], fw[4], gn[4], gs[4];
+            face_flux(g, U, i, j, 0, ar, fe);
+            face_flux(g, U, i - 1, j, 0, ar, fw);
+            face_flux(g, U, i, j, 1, az, gn);
+            face_flux(g, U, i, j - 1, 1, az, gs);
+            for (int c = 0; c < 4; ++c)
+                L[c * n + (size_t)j * g.nr + i] = -((fe[c] - fw[c]) / g.dr) - ((gn[c] - gs[c]) / g.dz);
+        }
+}
+
+}  // namespace
+
+extern "C" {
+
+double wno_weno5(double a, double b, double c, double d, double e) { return weno5(a, b, c, d, e); }
+
+// the three third-order candidates and the smoothness indicators (pins)
+void wno_candidates(double a, double b, double c, double d, double e, double* q, double* beta) {
+    q[0] = (2.0 * a - 7.0 * b + 11.0 * c) / 6.0;
+    q[1] = (-b + 5.0 * c + 2.0 * d) / 6.0;
+    q[2] = (2.0 * c + 5.0 * d - e) / 6.0;
+    const double s0 = a - 2.0 * b + c, t0 = a - 4.0 * b + 3.0 * c;
+    const double s1 = b - 2.0 * c + d, t1 = b - d;
+    const double s2 = c - 2.0 * d + e, t2 = 3.0 * c - 4.0 * d + e;
+    beta[0] = (13.0 / 12.0) * (s0 * s0) + 0.25 * (t0 * t0);
+    beta[1] = (13.0 / 12.0) * (s1 * s1) + 0.25 * (t1 * t1);
+    beta[2] = (13.0 / 12.0) * (s2 * s2) + 0.25 * (t2 * t2);
+}
+
+void wno_max_speeds(int nr, int nz, double dr, double dz, double gamma, const int* bc, const double* U, double* ar,
+                    double* az) {
+    const Grid g = {nr, nz, dr, dz, gamma, {bc[0], bc[1], bc[2], bc[3]}};
+    max_speeds(g, U, ar, az);
+}
+
+// L(U) with the given splitting speeds (alpha < 0: use the global maxima of U, W4)
+void wno_rhs(int nr, int nz, double dr, double dz, double gamma, const int* bc, const double* U, double alpha_r,
+             double alpha_z, double* L) {
+    const Grid g = {nr, nz, dr, dz, gamma, {bc[0], bc[1], bc[2], bc[3]}};
+    if (alpha_r < 0.0 || alpha_z < 0.0) max_speeds(g, U, &alpha_r, &alpha_z);
+    rhs(g, U, alpha_r, alpha_z, L);
+}
+
+// numerical fluxes through the + faces of every cell (Fhat: r direction, Ghat: z direction), for the conservation pin
+void wno_face_fluxes(int nr, int nz, double dr, double dz, double gamma, const int* bc, const double* U, double* Fhat,
+                     double* Ghat) {
+    const Grid g = {nr, nz, dr, dz, gamma, {bc[0], bc[1], bc[2], bc[3]}};
+    double ar, az;
+    max_speeds(g, U, &ar, &az);
+    const size_t n = (size_t)nr * nz;
+    for (int j = 0; j < nz; ++j)
+        for (int i = 0; i < nr; ++i) {
+            double f[4], h[4];
+            face_flux(g, U, i, j, 0, ar, f);
+            face_flux(g, U, i, j, 1, az, h);
+            for (int c = 0; c < 4; ++c) {
+                Fhat[c * n + (size_t)j * nr + i] = f[c];
+                Ghat[c * n + (size_t)j * nr + i] = h[c];
+            }
+        }
+}
+
+// One SSP-RK3 step (W8); returns dt.  U is updated in place.
+double wno_step(int nr, int nz, double dr, double dz, double gamma, const int* bc, double cfl, double* U) {
+    const Grid g = {nr, nz, dr, dz, gamma, {bc[0], bc[1], bc[2], bc[3]}};
+    const size_t n4 = (size_t)4 * nr * nz;
+    std::vector<double> L(n4), U1(n4), U2(n4);
+    double ar, az;
+    max_speeds(g, U, &ar, &az);
+    const double dt = cfl / (ar / dr + az / dz);
+    rhs(g, U, ar, az, L.data());
+    for (size_t k = 0; k < n4; ++k) U1[k] = U[k] + dt * L[k];
+    max_speeds(g, U1.data(), &ar, &az);
+    rhs(g, U1.data(), ar, az, L.data());
+    for (size_t k = 0; k < n4; ++k) U2[k] = 0.75 * U[k] + 0.25 * (U1[k] + dt * L[k]);
+    max_speeds(g, U2.data(), &ar, &az);
+    rhs(g, U2.data(), ar, az, L.data());
+    for (size_t k = 0; k < n4; ++k) U[k] = (1.0 / 3.0) * U[k] + (2.0 / 3.0) * (U2[k] + dt * L[k]);
+    return dt;
+}
+
+// March to t_end (the last step is shortened to land on it); returns the number of steps.
+int wno_evolve(int nr, int nz, double dr, double dz, double gamma, const int* bc, double cfl, double t_end, int max_steps,
+               double* U) {
+    const Grid g = {nr, nz, dr, dz, gamma, {bc[0], bc[1], bc[2], bc[3]}};
+    double t = 0.0;
+    int steps = 0;
+    while (t < t_end && steps < max_steps) {
+        double ar, az;
+        max_speeds(g, U, &ar, &az);
+        const double dt = cfl / (ar / dr + az / dz);
+        const double use = t + dt > t_end ? (t_end - t) / dt * cfl : cfl;
+        t += wno_step(nr, nz, dr, dz, gamma, bc, use, U);
+        ++steps;
+        if (use != cfl) break;
+    }
+    return steps;
+}
+
+}  // extern "C"
