@@ -24,7 +24,7 @@
 //       q0 = (2a - 7b + 11c)/6, q1 = (-b + 5c + 2d)/6, q2 = (2c + 5d - e)/6 on the cells (a..e) = (i-2..i+2) for F+,
 //       mirrored (i+3..i-1) for F-; smoothness b0 = 13/12 (a-2b+c)^2 + 1/4 (a-4b+3c)^2, b1 = 13/12 (b-2c+d)^2 +
 //       1/4 (b-d)^2, b2 = 13/12 (c-2d+e)^2 + 1/4 (3c-4d+e)^2; weights w_k = (d_k / (eps + b_k)^2) / sum, d = (0.1, 0.6, 0.3),
-//       eps = 1e-6.
+//       eps = 1e-6.  Pinned: the candidates' division by 6 is a multiplication by the fp64 constant 1.0/6.0.
 //   W6  L(U) = -(Fhat_{i+1/2} - Fhat_{i-1/2}) / dr - (Ghat_{j+1/2} - Ghat_{j-1/2}) / dz.
 //   W7  three ghost cells per side, per side one of: 0 outflow (copy of the edge cell), 1 reflecting (mirror image, the
 //       normal momentum changes sign), 2 periodic.
@@ -101,9 +101,10 @@ inline void flux(const Grid& g, const double u[4], int dir, double f[4]) {
 
 // fifth-order WENO value at the right face of cell c from the five cell values a..e (upwind side = a)
 inline double weno5(double a, double b, double c, double d, double e) {
-    const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) / 6.0;
-    const double q1 = (-b + 5.0 * c + 2.0 * d) / 6.0;
-    const double q2 = (2.0 * c + 5.0 * d - e) / 6.0;
+    const double k6 = 1.0 / 6.0;           // the /6 of the candidates as a multiplication by the rounded constant (W5)
+    const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) * k6;
+    const double q1 = (-b + 5.0 * c + 2.0 * d) * k6;
+    const double q2 = (2.0 * c + 5.0 * d - e) * k6;
     const double s0 = a - 2.0 * b + c, t0 = a - 4.0 * b + 3.0 * c;
     const double s1 = b - 2.0 * c + d, t1 = b - d;
     const double s2 = c - 2.0 * d + e, t2 = 3.0 * c - 4.0 * d + e;
@@ -171,9 +172,10 @@ double wno_weno5(double a, double b, double c, double d, double e) { return weno
 
 // the three third-order candidates and the smoothness indicators (pins)
 void wno_candidates(double a, double b, double c, double d, double e, double* q, double* beta) {
-    q[0] = (2.0 * a - 7.0 * b + 11.0 * c) / 6.0;
-    q[1] = (-b + 5.0 * c + 2.0 * d) / 6.0;
-    q[2] = (2.0 * c + 5.0 * d - e) / 6.0;
+    const double k6 = 1.0 / 6.0;
+    q[0] = (2.0 * a - 7.0 * b + 11.0 * c) * k6;
+    q[1] = (-b + 5.0 * c + 2.0 * d) * k6;
+    q[2] = (2.0 * c + 5.0 * d - e) * k6;
     const double s0 = a - 2.0 * b + c, t0 = a - 4.0 * b + 3.0 * c;
     const double s1 = b - 2.0 * c + d, t1 = b - d;
     const double s2 = c - 2.0 * d + e, t2 = 3.0 * c - 4.0 * d + e;
