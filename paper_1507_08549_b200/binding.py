@@ -30,6 +30,13 @@ EXPORTS_LEVELSET = (
 )
 
 
+# every symbol include/sn_weno.h declares (NEXT-3)
+EXPORTS_WENO = (
+    "sn_weno_create", "sn_weno_max_speeds", "sn_weno_rhs", "sn_weno_step", "sn_weno_evolve", "sn_weno_rhs_host",
+    "sn_weno_get_stat", "sn_weno_destroy", "sn_weno_last_error",
+)
+
+
 class sn_poisson_result(C.Structure):
     _fields_ = [("sweeps", C.c_int32), ("status", C.c_int32), ("residual", C.c_double)]
 
@@ -113,6 +120,24 @@ def load():
     lib.sn_levelset_destroy.argtypes = [_vp]
     lib.sn_levelset_last_error.restype = C.c_char_p
     lib.sn_levelset_last_error.argtypes = []
+    lib.sn_weno_create.restype = _vp
+    lib.sn_weno_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int)]
+    lib.sn_weno_max_speeds.restype = C.c_int
+    lib.sn_weno_max_speeds.argtypes = [_vp, _vp, _dp, _vp]
+    lib.sn_weno_rhs.restype = C.c_int
+    lib.sn_weno_rhs.argtypes = [_vp, _vp, _vp, C.c_double, C.c_double, _vp]
+    lib.sn_weno_step.restype = C.c_int
+    lib.sn_weno_step.argtypes = [_vp, _vp, C.c_double, _dp, _vp]
+    lib.sn_weno_evolve.restype = C.c_int
+    lib.sn_weno_evolve.argtypes = [_vp, _vp, C.c_double, C.c_double, C.c_int, _vp]
+    lib.sn_weno_rhs_host.restype = C.c_int
+    lib.sn_weno_rhs_host.argtypes = [_vp, _vp, _vp, _vp]
+    lib.sn_weno_get_stat.restype = C.c_int
+    lib.sn_weno_get_stat.argtypes = [_vp, C.c_char_p, _dp]
+    lib.sn_weno_destroy.restype = None
+    lib.sn_weno_destroy.argtypes = [_vp]
+    lib.sn_weno_last_error.restype = C.c_char_p
+    lib.sn_weno_last_error.argtypes = []
     _lib = lib
     return lib
 
@@ -303,4 +328,57 @@ def sn_levelset_get_stat(h, key: str) -> float:
     out = C.c_double(0.0)
     if load().sn_levelset_get_stat(h, key.encode(), C.byref(out)) != 0:
         raise SnPoissonError("sn_levelset_get_stat: " + sn_levelset_last_error())
+    return out.value
+
+
+# ---- NEXT-3: WENO-5 / global Lax-Friedrichs flux reconstruction (include/sn_weno.h) ------------------------------------
+def sn_weno_last_error() -> str:
+    return load().sn_weno_last_error().decode()
+
+
+def _wcheck(rc, what):
+    if rc < 0:
+        raise SnPoissonError(f"{what} failed ({rc}): " + sn_weno_last_error())
+    return rc
+
+
+def sn_weno_create(nr, nz, dr, dz, gamma, bc):
+    h = load().sn_weno_create(int(nr), int(nz), float(dr), float(dz), float(gamma), (C.c_int * 4)(*[int(b) for b in bc]))
+    if not h:
+        raise SnPoissonError("sn_weno_create failed: " + sn_weno_last_error())
+    return h
+
+
+def sn_weno_destroy(h):
+    load().sn_weno_destroy(h)
+
+
+def sn_weno_max_speeds(h, u_ptr, stream=0):
+    a = (C.c_double * 2)()
+    _wcheck(load().sn_weno_max_speeds(h, u_ptr, a, stream or None), "sn_weno_max_speeds")
+    return a[0], a[1]
+
+
+def sn_weno_rhs(h, u_ptr, l_ptr, alpha_r=-1.0, alpha_z=-1.0, stream=0) -> int:
+    return _wcheck(load().sn_weno_rhs(h, u_ptr, l_ptr, float(alpha_r), float(alpha_z), stream or None), "sn_weno_rhs")
+
+
+def sn_weno_step(h, u_ptr, cfl, stream=0, want_dt=True):
+    dt = C.c_double(0.0)
+    _wcheck(load().sn_weno_step(h, u_ptr, float(cfl), C.byref(dt) if want_dt else None, stream or None), "sn_weno_step")
+    return dt.value if want_dt else None
+
+
+def sn_weno_evolve(h, u_ptr, cfl, t_end, max_steps, stream=0) -> int:
+    return _wcheck(load().sn_weno_evolve(h, u_ptr, float(cfl), float(t_end), int(max_steps), stream or None),
+                   "sn_weno_evolve")
+
+
+def sn_weno_rhs_host(h, u_host_ptr, l_host_ptr, stream=0) -> int:
+    return _wcheck(load().sn_weno_rhs_host(h, u_host_ptr, l_host_ptr, stream or None), "sn_weno_rhs_host")
+
+
+def sn_weno_get_stat(h, key: str) -> float:
+    out = C.c_double(0.0)
+    _wcheck(load().sn_weno_get_stat(h, key.encode(), C.byref(out)), f"sn_weno_get_stat({key})")
     return out.value

@@ -32,7 +32,7 @@ def units():
 
 def _deps():
     return [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [
-        os.path.join(os.path.dirname(HERE), "include", f) for f in ("sn_poisson.h", "sn_levelset.h")]
+        os.path.join(os.path.dirname(HERE), "include", f) for f in ("sn_poisson.h", "sn_levelset.h", "sn_weno.h")]
 
 
 def _stale(target: str) -> bool:

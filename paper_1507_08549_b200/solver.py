@@ -199,3 +199,64 @@ class LevelSet:
 
     def stat(self, key):
         return B.sn_levelset_get_stat(self.h, key)
+
+
+class Weno:
+    """Owns one sn_weno handle (NEXT-3: WENO-5 / global Lax-Friedrichs flux reconstruction).  ``U``: float64 CUDA
+    tensor (4, nz, nr) of (rho, rho v_r, rho v_z, tau); bc = (r-low, r-high, z-low, z-high), 0 outflow / 1 reflecting /
+    2 periodic."""
+
+    def __init__(self, nr, nz, dr, dz, gamma, bc):
+        self.nr, self.nz = nr, nz
+        self.h = B.sn_weno_create(nr, nz, dr, dz, gamma, bc)
+
+    def close(self):
+        if getattr(self, "h", None) and getattr(B, "sn_weno_destroy", None):
+            B.sn_weno_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def _check(self, U):
+        import torch
+        if not (U.is_cuda and U.dtype == torch.float64 and U.is_contiguous() and tuple(U.shape) == (4, self.nz, self.nr)):
+            raise ValueError("expected a contiguous float64 CUDA tensor of shape (4, nz, nr)")
+
+    @staticmethod
+    def _stream():
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+
+    def max_speeds(self, U):
+        self._check(U)
+        return B.sn_weno_max_speeds(self.h, U.data_ptr(), self._stream())
+
+    def rhs(self, U, alpha=None, out=None):
+        """L(U); alpha = (alpha_r, alpha_z) or None for the device-computed global maxima.  Asynchronous."""
+        import torch
+        self._check(U)
+        out = torch.empty_like(U) if out is None else out
+        self._check(out)
+        ar, az = (-1.0, -1.0) if alpha is None else alpha
+        B.sn_weno_rhs(self.h, U.data_ptr(), out.data_ptr(), ar, az, self._stream())
+        return out
+
+    def step(self, U, cfl, want_dt=True):
+        """One SSP-RK3 step in place; returns dt (synchronises) or None."""
+        self._check(U)
+        return B.sn_weno_step(self.h, U.data_ptr(), cfl, self._stream(), want_dt)
+
+    def evolve(self, U, cfl, t_end, max_steps=1000000):
+        self._check(U)
+        return B.sn_weno_evolve(self.h, U.data_ptr(), cfl, t_end, max_steps, self._stream())
+
+    def rhs_host(self, U_np):
+        import numpy as np
+        if U_np.dtype != np.float64 or not U_np.flags.c_contiguous or tuple(U_np.shape) != (4, self.nz, self.nr):
+            raise ValueError("expected a C-contiguous float64 numpy array of shape (4, nz, nr)")
+        out = np.empty_like(U_np)
+        B.sn_weno_rhs_host(self.h, U_np.ctypes.data, out.ctypes.data, self._stream())
+        return out
+
+    def stat(self, key):
+        return B.sn_weno_get_stat(self.h, key)

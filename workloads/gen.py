@@ -321,3 +321,54 @@ def levelset_front(ncells: int = 500, seed: int = 7, distort: float = 0.5):
         ph = uniform(seed, 1, 3 * k + 2, 0.0, 2.0 * math.pi)
         u += 0.25 * np.sin(kx * X * math.pi + ph) * np.cos(ky * Y * math.pi)
     return np.ascontiguousarray((R - s) * (1.0 + distort * u)), dr
+
+
+# ----------------------------------------------------------------------------
+# NEXT-3: conserved hydro states for the WENO-5 / global Lax-Friedrichs flux reconstruction.  Inputs only:
+# the conversion primitive -> conserved is the definition of the state vector ("tau = rho eps + rho v^2 / 2"
+# with the gamma-law EOS of PAPER.md:402), not part of the method under test.
+# ----------------------------------------------------------------------------
+def hydro_state(rho, vr, vz, p, gamma: float = 1.4) -> np.ndarray:
+    """U = (rho, rho v_r, rho v_z, tau) of shape (4, nz, nr) from primitive fields."""
+    rho, vr, vz, p = np.broadcast_arrays(*(np.asarray(a, dtype=np.float64) for a in (rho, vr, vz, p)))
+    return np.ascontiguousarray(np.stack([rho, rho * vr, rho * vz, p / (gamma - 1.0) + 0.5 * rho * (vr * vr + vz * vz)]))
+
+
+def shock_tube(rho_l, v_l, p_l, rho_r, v_r, p_r, x0: float, n: int, rows: int = 1, axis: int = 0, gamma: float = 1.4):
+    """Left / right states meeting at x0 on n cells of [0, 1] (the values of the paper's Table 3 are in
+    tests/golden/paper_table3_shocktubes.txt), `rows` identical copies along the other axis.  Returns (U, dx)."""
+    x = (np.arange(n) + 0.5) / n
+    left = x < x0
+    rho, v, p = np.where(left, rho_l, rho_r), np.where(left, v_l, v_r), np.where(left, p_l, p_r)
+    if axis == 0:
+        U = hydro_state(np.tile(rho, (rows, 1)), np.tile(v, (rows, 1)), 0.0, np.tile(p, (rows, 1)), gamma)
+    else:
+        U = hydro_state(np.tile(rho[:, None], (1, rows)), 0.0, np.tile(v[:, None], (1, rows)), np.tile(p[:, None], (1, rows)), gamma)
+    return U, 1.0 / n
+
+
+def hydro_blobs(nr: int = 500, nz: int = 500, seed: int = 11, gamma: float = 1.4, jump: float = 0.0):
+    """2-D state on the unit (r, z) quadrant, dr = 1/nr, dz = 1/nz (the paper's hydro grids are 500 x 500):
+    a smooth background with seeded Gaussian over-densities / over-pressures and a seeded smooth velocity field; `jump`
+    > 0 adds a sharp circular density / pressure step (the nonlinear weights then matter).  Returns (U, dr, dz)."""
+    dr, dz = 1.0 / nr, 1.0 / nz
+    r = (np.arange(nr) + 0.5) * dr
+    z = (np.arange(nz) + 0.5) * dz
+    R, Z = np.meshgrid(r, z)
+    rho = np.full((nz, nr), 1.0)
+    p = np.full((nz, nr), 1.0)
+    for k in range(6):
+        A = uniform(seed, 21, 5 * k, 0.2, 1.5)
+        w = uniform(seed, 21, 5 * k + 1, 0.04, 0.15)
+        rk = uniform(seed, 21, 5 * k + 2, 0.1, 0.9)
+        zk = uniform(seed, 21, 5 * k + 3, 0.1, 0.9)
+        g = np.exp(-((R - rk) ** 2 + (Z - zk) ** 2) / (2 * w * w))
+        rho += A * g
+        p += uniform(seed, 21, 5 * k + 4, 0.5, 3.0) * A * g
+    vr = 0.6 * np.sin(2 * math.pi * R * uniform(seed, 22, 0, 0.5, 2.0)) * np.cos(math.pi * Z * uniform(seed, 22, 1, 0.5, 2.0))
+    vz = 0.6 * np.cos(math.pi * R * uniform(seed, 22, 2, 0.5, 2.0)) * np.sin(2 * math.pi * Z * uniform(seed, 22, 3, 0.5, 2.0))
+    if jump > 0.0:
+        inside = np.hypot(R - 0.4, Z - 0.45) < 0.2
+        rho = np.where(inside, rho * (1.0 + jump), rho)
+        p = np.where(inside, p * (1.0 + 3.0 * jump), p)
+    return hydro_state(rho, vr, vz, p, gamma), dr, dz
