@@ -13,7 +13,9 @@ workload is the [CFG 4a] batch of 64 x 512^2, its members dealt across the ranks
 
 The same line carries `per_config`: every other configuration of BASELINE.json (cfg0, cfg1, cfg2, cfg3 cold, cfg4a,
 the size sweep 128..4096) measured the same way in the same run (>= 3 warm-ups, L2 flushed between timed solves),
-each with its own value / time / sweeps / roofline fraction / fp64-pipe fraction / redundancy / e2e.
+each with its own value / time / sweeps / roofline fraction / fp64-pipe fraction / redundancy / e2e, and `next_rows`:
+the built NEXT rows of SURVEY.md section 8f (level-set re-initialisation, WENO-5 / LF flux reconstruction) on their
+paper-sized inputs with their own (fp64 ALU) rooflines.
 
 Timing: W warm-up steps, then K steps each bracketed by CUDA events on the launching stream (the call synchronises
 that stream itself); L2 is flushed (a 256 MiB write) and phi re-zeroed between steps, outside the events; the K-step
@@ -48,6 +50,9 @@ METRIC = "poisson_relaxation_cell_updates_per_s"
 UNIT = "cell-updates/s"
 BYTES_PER_UPDATE = 24.0     # phi read + f read + phi write
 FP64_UPDATES_PER_S = 148 * 64 * 1.965e9 / 7.0      # ALU ceiling: 7 fp64 instructions per update
+FP64_LANE_INSTR_PER_S = 148 * 64 * 1.965e9        # fp64 pipe: 64 lanes per clock and SM
+LS_FP64_PER_PAIR = 5.0                            # level-set distance kernel: fp64 instructions per node-crossing pair
+WENO_FP64_PER_CELL = 2750.0                       # flux reconstruction: fp64 instructions per cell, no redundant faces (profiles/r02_weno500_rhs.md)
 DEFAULT_WORKLOAD = "cfg3seq100"
 PER_CONFIG = ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "sweep128", "sweep256", "sweep512", "sweep1024", "sweep2048",
               "sweep4096"]
@@ -372,6 +377,81 @@ class Bench:
                 "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"}
 
 
+def next_rows(torch, P, flush):
+    """The NEXT rows of SURVEY.md section 8f that are built (level-set re-initialisation, WENO-5 / LF flux
+    reconstruction), each on its paper-sized synthetic input (500 x 500) with its own roofline: both are
+    bound by plain fp64 ALU work, so `frac` is fp64 instructions per second against the fp64 pipe's issue peak."""
+    rows = []
+
+    def timed(fn, reps, warm=3):
+        for _ in range(warm):
+            fn()
+        ms = []
+        for _ in range(reps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return float(np.mean(ms))
+
+    def wall(fn, reps):
+        fn()
+        t = []
+        for _ in range(reps):
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            fn()
+            t.append((time.perf_counter() - t0) * 1e3)
+        return float(np.mean(t))
+
+    # ---- NEXT-2: level-set re-initialisation (PAPER.md:131-141)
+    S, dr = W.levelset_front(500)
+    ls = P.LevelSet(S.shape[1], S.shape[0], dr, dr)
+    Sd = torch.from_numpy(S).cuda()
+    dist_ms = []
+    ms = timed(lambda: (ls.reinit(Sd), dist_ms.append(ls.stat("distance_ms"))), 10)
+    pairs, dms = ls.stat("pairs"), float(np.mean(dist_ms[3:]))
+    e2e_ms = wall(lambda: ls.reinit_host(S), 5)
+    ach = LS_FP64_PER_PAIR * pairs / (dms * 1e-3)
+    rows.append({"workload": "levelset500", "label": "NEXT-2: level-set re-initialisation, three-finger front on 501 x 501 nodes",
+                 "metric": "node_crossing_pairs_per_s", "value": pairs / (ms * 1e-3), "ms_per_step": ms,
+                 "crossings": int(ls.stat("crossings")), "pairs": pairs, "gpu_launches_per_step": int(ls.stat("launches")),
+                 "roofline": {"bound": "alu", "kernel": "k_ls_distance", "achieved": ach, "peak": FP64_LANE_INSTR_PER_S,
+                              "unit": "fp64 instr/s", "frac": ach / FP64_LANE_INSTR_PER_S, "launch_ms": dms,
+                              "alg_fp64_instr_per_launch": LS_FP64_PER_PAIR * pairs},
+                 "e2e": {"value": pairs / (e2e_ms * 1e-3), "ms_per_step": e2e_ms, "api": "sn_levelset_reinit_host",
+                         "h2d_bytes_per_step": S.nbytes, "d2h_bytes_per_step": S.nbytes}})
+    ls.close()
+    # ---- NEXT-3: WENO-5 / global Lax-Friedrichs flux reconstruction (PAPER.md:95)
+    U, dr, dz = W.hydro_blobs(500, 500, jump=0.5)
+    wn = P.Weno(500, 500, dr, dz, 1.4, [1, 0, 1, 0])
+    Ud = torch.from_numpy(U).cuda()
+    Ld = torch.empty_like(Ud)
+    rhs_ms = []
+    ms = timed(lambda: (wn.rhs(Ud, out=Ld), rhs_ms.append(wn.stat("rhs_ms"))), 20)
+    kms = float(np.mean(rhs_ms[3:]))
+    cells = 500 * 500
+    Us = Ud.clone()
+    step_ms = timed(lambda: wn.step(Us, 0.5, want_dt=False), 20)
+    e2e_ms = wall(lambda: wn.rhs_host(U), 5)
+    ach = WENO_FP64_PER_CELL * cells / (kms * 1e-3)
+    rows.append({"workload": "weno500", "label": "NEXT-3: WENO-5 / global LF flux divergence L(U), 500 x 500 cells, 4 components",
+                 "metric": "cells_per_s", "value": cells / (ms * 1e-3), "ms_per_step": ms, "rk3_step_ms": step_ms,
+                 "rk3_cells_per_s": cells / (step_ms * 1e-3), "gpu_launches_per_step": 2,
+                 "roofline": {"bound": "alu", "kernel": "k_weno_rhs", "achieved": ach, "peak": FP64_LANE_INSTR_PER_S,
+                              "unit": "fp64 instr/s", "frac": ach / FP64_LANE_INSTR_PER_S, "launch_ms": kms,
+                              "alg_fp64_instr_per_launch": WENO_FP64_PER_CELL * cells,
+                              "hbm_frac": 64.0 * cells / (kms * 1e-3) / 1e9 / measured_peaks()[0]},
+                 "e2e": {"value": cells / (e2e_ms * 1e-3), "ms_per_step": e2e_ms, "api": "sn_weno_rhs_host",
+                         "h2d_bytes_per_step": U.nbytes, "d2h_bytes_per_step": U.nbytes}})
+    wn.close()
+    return rows
+
+
 def spawn_ranks(args):
     """`--gpus N` without torchrun: start the N ranks (one process per GPU) the way the driver would."""
     import socket
@@ -393,6 +473,7 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 streaming kernels, 2 resident kernel, 3 blocked kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--next-only", action="store_true", help="only the NEXT rows (level set, WENO): for profiling")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     world_env = os.environ.get("WORLD_SIZE")
@@ -439,6 +520,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.next_only:
+        if rank == 0:
+            print(json.dumps({"next_rows": next_rows(torch, P, bench.flush)}))
+        return
     long_step = hasattr(mine[0], "first") or len(mine) > 1
     info = bench.measure(wl_name, mine, args.steps, args.warmup, min(args.steps, 3 if long_step else 20),
                          barrier=barrier, sampler=ClockSampler(local_rank))
@@ -499,6 +584,7 @@ def main():
                                  "h2d_bytes_per_step": inf["h2d"], "d2h_bytes_per_step": inf["d2h"]},
                          "gpu_launches_per_step": inf["launches"] // max(1, len(inf["step_ms"]))})
         out["per_config"] = rows
+        out["next_rows"] = next_rows(torch, P, bench.flush)
     if not args.no_cpu_baseline and world == 1:
         v, sample = oracle_rate([mine[0].first] if hasattr(mine[0], "first") else mine)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,

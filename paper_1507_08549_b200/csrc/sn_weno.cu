@@ -10,7 +10,7 @@
 //                   north face of its cell (4 components x 2 split fluxes x WENO-5 each); the west / south face values
 //                   come from the neighbouring thread (warp shuffle in r, shared memory in z; only the first column /
 //                   row of a tile recomputes them); the Runge-Kutta stage update is fused into the epilogue.
-// Bound: plain fp64 ALU work (~1.9 k fp64 instructions per cell against 64 B of compulsory traffic); no tensor cores
+// Bound: plain fp64 ALU work (~2.75 k fp64 instructions per cell -- an IEEE division is ~18 of them -- against 64 B of compulsory traffic); no tensor cores
 // (not a contraction).  Arithmetic pinned like the rest of the library: -fmad=false, expression trees typed out.
 #include "../../include/sn_weno.h"
 
