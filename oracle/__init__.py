@@ -25,7 +25,7 @@ _dp = C.POINTER(C.c_double)
 
 
 _EXTRA = {name: (os.path.join(_HERE, name + "_oracle.cpp"), os.path.join(_HERE, "lib" + name + "_oracle.so"))
-          for name in ("levelset", "weno")}
+          for name in ("levelset", "weno", "mg")}
 _extra_libs = {}
 
 
@@ -315,3 +315,65 @@ def weno_evolve(U, dr, dz, gamma, bc, cfl, t_end, max_steps=1000000):
     U = _u4(U).copy()
     n = _wn().wno_evolve(U.shape[2], U.shape[1], dr, dz, gamma, _bc(bc), cfl, t_end, max_steps, _p(U))
     return U, n
+
+
+# ---- NEXT-4: red-black-smoothed multigrid variant of the Poisson solve (oracle/mg_oracle.cpp) ------------------------
+def _mg():
+    L = extra_lib("mg")
+    L.mgo_levels.restype = C.c_int
+    L.mgo_levels.argtypes = [C.c_int, C.c_int]
+    L.mgo_beta.restype = C.c_double
+    L.mgo_beta.argtypes = [C.c_int]
+    L.mgo_restrict.argtypes = [C.c_int, C.c_int, _dp, _dp]
+    L.mgo_prolong.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, _dp, _dp]
+    L.mgo_solve.restype = C.c_int
+    L.mgo_solve.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp, _dp, _dp, _dp, C.c_double,
+                            C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), _dp, _dp]
+    return L
+
+
+def mg_levels(nr, nz) -> int:
+    return _mg().mgo_levels(int(nr), int(nz))
+
+
+def mg_beta(l) -> float:
+    return _mg().mgo_beta(int(l))
+
+
+def mg_restrict(res):
+    res = _f64(res)
+    nz, nr = res.shape
+    out = np.zeros((nz // 2, nr // 2))
+    _mg().mgo_restrict(nr, nz, _p(res), _p(out))
+    return out
+
+
+def mg_prolong(ec, symmetry, lc):
+    """Bilinear prolongation (M7) of the level-lc error ec onto a zero fine field."""
+    ec = _f64(ec)
+    nzc, nrc = ec.shape
+    out = np.zeros((2 * nzc, 2 * nrc))
+    _mg().mgo_prolong(nrc, nzc, int(symmetry), int(lc), _p(ec), _p(out))
+    return out
+
+
+def mg_solve(rho, phi0, dr, dz, symmetry, lmax, tol, max_cycles, nu1=1, nu2=1, nc=30, ghosts=None):
+    """Multigrid solve (M1-M8) with the multipole ghosts of the SOR oracle (or the given (bE, bN, bS)).
+    Returns dict(phi, cycles, status, residual, history)."""
+    rho, phi = _f64(rho), _f64(phi0).copy()
+    nz, nr = rho.shape
+    if ghosts is None:
+        M = moments(rho, dr, dz, symmetry, lmax)
+        ghosts = boundary(nr, nz, dr, dz, symmetry, lmax, M)
+    bE, bN, bS = (_f64(g) if g is not None else np.zeros(nr) for g in ghosts)
+    cyc, R = C.c_int(0), C.c_double(0.0)
+    hist = np.zeros(max(1, max_cycles))
+    st = _mg().mgo_solve(nr, nz, dr, dz, symmetry, _p(rho), _p(bE), _p(bN), _p(bS), _p(phi), tol, max_cycles, nu1, nu2,
+                         nc, C.byref(cyc), C.byref(R), _p(hist))
+    assert st >= -3 and st != -1, "bad argument"
+    return {"phi": phi, "cycles": cyc.value, "status": st, "residual": R.value, "history": hist[:cyc.value].copy()}
+
+
+def mg_solve_workload(w, phi0=None, **kw):
+    phi0 = np.zeros_like(w.rho) if phi0 is None else phi0
+    return mg_solve(w.rho, phi0, w.dr, w.dz, w.symmetry, w.lmax, w.tol, kw.pop("max_cycles", 60), **kw)
