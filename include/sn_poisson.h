@@ -196,6 +196,24 @@ int sn_poisson_probe_l2(int mib, double* copy_gbs, double* read_gbs, void* strea
 const char* sn_poisson_last_error(void);
 const char* sn_poisson_version(void);
 
+/* ---- NEXT-4: a faster-converging variant on the same stencil --------------------------------
+ * Red-black-smoothed geometric multigrid (not in the paper, which relaxes the same equation by SOR).  Same
+ * equation, discretisation, multipole ghosts and therefore the same converged potential as sn_poisson_solve; only the
+ * iteration differs (readings M1..M8): V-cycles over the levels (nr / 2^l) x (nz / 2^l) (coarsened
+ * while both counts are even and >= 8), red-black Gauss-Seidel smoothing (options "mg_nu1", "mg_nu2": sweeps before /
+ * after the coarse-grid correction, default 1 / 1; "mg_nc": sweeps on the coarsest level, default 30), volume-weighted
+ * restriction, bilinear prolongation, coarse Dirichlet ghosts extrapolated to the level-0 ghost centre.  After every
+ * cycle the ratio R (rule R9) of the TRUE residual of the iterate is evaluated on the device; the solve stops after the
+ * first cycle with R <= tol (tol <= 0: exactly max_cycles cycles).  Returns {cycles, status, R} like sn_poisson_solve
+ * (`sweeps` = V-cycles applied); sn_poisson_get_history then returns R after every cycle.  rho / phi_inout: DEVICE
+ * pointers as for sn_poisson_solve; any nr, nz >= 2 (a grid that cannot be coarsened runs plain Gauss-Seidel sweeps).
+ * The stopping rule option (sn_poisson_set_stop_rule) does not apply.  Synchronises `stream`. */
+sn_poisson_result sn_poisson_solve_mg(sn_poisson* h, const double* rho, double* phi_inout, double tol, int max_cycles,
+                                      void* stream);
+/* The same with HOST buffers (H2D of rho and phi, D2H of phi inside the call). */
+sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
+                                           int max_cycles, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

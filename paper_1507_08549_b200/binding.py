@@ -16,7 +16,7 @@ LIB_PATH = os.environ.get("SN_POISSON_LIB") or os.path.join(_HERE, "libsn_poisso
 EXPORTS = (
     "sn_poisson_create", "sn_poisson_solve", "sn_poisson_solve_host", "sn_poisson_solve_batch",
     "sn_poisson_solve_batch_host", "sn_poisson_solve_sequence_host", "sn_poisson_probe_l2",
-    "sn_poisson_set_stop_rule", "sn_poisson_solve_gravity",
+    "sn_poisson_set_stop_rule", "sn_poisson_solve_gravity", "sn_poisson_solve_mg", "sn_poisson_solve_mg_host",
     "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
     "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
@@ -68,6 +68,10 @@ def load():
     lib.sn_poisson_solve.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
     lib.sn_poisson_solve_host.restype = sn_poisson_result
     lib.sn_poisson_solve_host.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
+    lib.sn_poisson_solve_mg.restype = sn_poisson_result
+    lib.sn_poisson_solve_mg.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
+    lib.sn_poisson_solve_mg_host.restype = sn_poisson_result
+    lib.sn_poisson_solve_mg_host.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
     lib.sn_poisson_solve_batch.restype = C.c_int
     lib.sn_poisson_solve_batch.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, C.c_int, _vp,
                                            C.POINTER(sn_poisson_result)]
@@ -170,6 +174,16 @@ def sn_poisson_solve(h, rho_ptr, phi_ptr, tol, max_sweeps, stream=0) -> sn_poiss
 def sn_poisson_solve_host(h, rho_ptr, phi_ptr, tol, max_sweeps, stream=0) -> sn_poisson_result:
     """rho_ptr / phi_ptr: HOST addresses (ints, e.g. numpy ``arr.ctypes.data`` or a pinned tensor's data_ptr())."""
     return load().sn_poisson_solve_host(h, rho_ptr, phi_ptr, float(tol), int(max_sweeps), stream or None)
+
+
+def sn_poisson_solve_mg(h, rho_ptr, phi_ptr, tol, max_cycles, stream=0) -> sn_poisson_result:
+    """Multigrid variant (NEXT-4); DEVICE addresses; `sweeps` of the result = V-cycles."""
+    return load().sn_poisson_solve_mg(h, rho_ptr, phi_ptr, float(tol), int(max_cycles), stream or None)
+
+
+def sn_poisson_solve_mg_host(h, rho_ptr, phi_ptr, tol, max_cycles, stream=0) -> sn_poisson_result:
+    """Multigrid variant (NEXT-4); HOST addresses."""
+    return load().sn_poisson_solve_mg_host(h, rho_ptr, phi_ptr, float(tol), int(max_cycles), stream or None)
 
 
 def sn_poisson_solve_batch(h, nbatch, rho_ptr, phi_ptr, tol, max_sweeps, stream=0):

@@ -21,6 +21,7 @@
 #include "sweep_blocked.cuh"
 #include "sweep_resident.cuh"
 #include "shapes.cuh"
+#include "mg.cuh"
 
 using namespace snp;
 
@@ -120,6 +121,15 @@ struct sn_poisson {
         BlkPlan bp;
         int group = 0;
     } plan_cache;
+
+    // multigrid variant (NEXT-4): per-level coefficient tables, errors and right-hand sides (levels >= 1), the maxima slots
+    struct MgWs {
+        int nlev = 0;
+        std::vector<int> nr, nz;
+        std::vector<double*> cE, cW, phi, f;
+        unsigned long long* slots = nullptr;
+    } mg;
+    int opt_mg_nu1 = 1, opt_mg_nu2 = 1, opt_mg_nc = 30;
 
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
@@ -822,6 +832,164 @@ int ensure_stage(sn_poisson* h, size_t n) {
 
 }  // namespace
 
+namespace {
+
+// ---- multigrid variant (NEXT-4; mg.cuh, readings M1..M8) ---------------------------------------------------------
+int mg_num_levels(int nr, int nz) {                                  // M1
+    int n = 1;
+    while (nr % 2 == 0 && nz % 2 == 0 && nr / 2 >= 4 && nz / 2 >= 4) { nr /= 2; nz /= 2; ++n; }
+    return n;
+}
+
+int ensure_mg(sn_poisson* h) {
+    if (h->mg.nlev) return 0;
+    auto& W = h->mg;
+    const int nlev = mg_num_levels(h->nr, h->nz);
+    W.nr.resize(nlev); W.nz.resize(nlev);
+    W.cE.assign(nlev, nullptr); W.cW.assign(nlev, nullptr); W.phi.assign(nlev, nullptr); W.f.assign(nlev, nullptr);
+    for (int l = 0; l < nlev; ++l) {
+        const int nr = h->nr >> l, nz = h->nz >> l;
+        W.nr[l] = nr; W.nz[l] = nz;
+        const double dr = std::ldexp(h->dr, l);
+        const double ir2 = 1.0 / (dr * dr);
+        std::vector<double> cE(nr), cW(nr);
+        for (int i = 0; i < nr; ++i) {
+            cE[i] = ((i + 1.0) / (i + 0.5)) * ir2;
+            cW[i] = (i / (i + 0.5)) * ir2;
+        }
+        if (int rc = dev_alloc(&W.cE[l], (size_t)nr)) return rc;
+        if (int rc = dev_alloc(&W.cW[l], (size_t)nr)) return rc;
+        CU_TRY(cudaMemcpy(W.cE[l], cE.data(), sizeof(double) * nr, cudaMemcpyHostToDevice));
+        CU_TRY(cudaMemcpy(W.cW[l], cW.data(), sizeof(double) * nr, cudaMemcpyHostToDevice));
+        if (l > 0) {
+            if (int rc = dev_alloc(&W.phi[l], (size_t)nr * nz)) return rc;
+            if (int rc = dev_alloc(&W.f[l], (size_t)nr * nz)) return rc;
+        }
+    }
+    if (int rc = dev_alloc(&W.slots, (size_t)2)) return rc;
+    W.nlev = nlev;
+    return 0;
+}
+
+MgLevel mg_level(const sn_poisson* h, int l, const double* rho, double* phi) {
+    const auto& W = h->mg;
+    MgLevel L;
+    L.nr = W.nr[l]; L.nz = W.nz[l]; L.symmetry = h->symmetry;
+    const double dr = std::ldexp(h->dr, l), dz = std::ldexp(h->dz, l);
+    const double ir2 = 1.0 / (dr * dr);
+    L.iz2 = 1.0 / (dz * dz);
+    L.D = 2.0 * ir2 + 2.0 * L.iz2;
+    L.D0 = L.D - L.iz2;
+    L.wD = 1.0 / L.D;
+    L.wD0 = 1.0 / L.D0;
+    const double s = std::ldexp(1.0, -l);
+    L.beta = (1.0 - s) / (1.0 + s);
+    L.scale = l == 0 ? kFourPi : 1.0;
+    L.cE = W.cE[l]; L.cW = W.cW[l];
+    L.phi = l == 0 ? phi : W.phi[l];
+    L.src = l == 0 ? rho : W.f[l];
+    L.bE = l == 0 ? h->d_bE : nullptr;
+    L.bN = l == 0 ? h->d_bN : nullptr;
+    L.bS = l == 0 ? h->d_bS : nullptr;
+    return L;
+}
+
+inline int mg_blocks(size_t n, int num_sms) { return (int)std::max<size_t>(1, std::min<size_t>((n + 255) / 256, (size_t)num_sms * 16)); }
+
+int mg_smooth(sn_poisson* h, const MgLevel& L, int nsweeps, cudaStream_t st) {
+    const int blocks = mg_blocks((size_t)((L.nr + 1) / 2) * L.nz, h->num_sms);
+    for (int k = 0; k < nsweeps; ++k) {
+        k_mg_halfsweep<0><<<blocks, 256, 0, st>>>(L);
+        k_mg_halfsweep<1><<<blocks, 256, 0, st>>>(L);
+        h->st_launches += 2;
+    }
+    CU_TRY(cudaGetLastError());
+    return 0;
+}
+
+// one V-cycle from level 0, then the true residual's maxima and the decision of the cycle (M8)
+int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int cycle, int max_cycles, cudaStream_t st) {
+    const auto& W = h->mg;
+    const int nu1 = h->opt_mg_nu1, nu2 = h->opt_mg_nu2;
+    std::vector<MgLevel> Ls;
+    for (int l = 0; l < W.nlev; ++l) Ls.push_back(mg_level(h, l, rho, phi));
+    if (W.nlev == 1) {
+        if (int rc = mg_smooth(h, Ls[0], nu1 + nu2, st)) return rc;
+    } else {
+        for (int l = 0; l + 1 < W.nlev; ++l) {                       // down
+            if (int rc = mg_smooth(h, Ls[l], nu1, st)) return rc;
+            const size_t nc = (size_t)W.nr[l + 1] * W.nz[l + 1];
+            k_mg_residual<true, false><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr);
+            h->st_launches += 1;
+        }
+        k_mg_coarse<<<1, 1024, 0, st>>>(Ls[W.nlev - 1], h->opt_mg_nc);
+        h->st_launches += 1;
+        for (int l = W.nlev - 2; l >= 0; --l) {                      // up
+            const size_t nf = (size_t)W.nr[l] * W.nz[l];
+            k_mg_prolong_add<<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l]);
+            h->st_launches += 1;
+            if (int rc = mg_smooth(h, Ls[l], nu2, st)) return rc;
+        }
+    }
+    const size_t nb = (size_t)((W.nr[0] + 1) / 2) * ((W.nz[0] + 1) / 2);
+    k_mg_residual<false, true><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], nullptr, nullptr, W.slots);
+    k_mg_decide<<<1, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, cycle, max_cycles, h->d_hist);
+    h->st_launches += 2;
+    CU_TRY(cudaGetLastError());
+    return 0;
+}
+
+int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int max_cycles, cudaStream_t st,
+                  sn_poisson_result* out, const HostIO* io = nullptr) {
+    CU_TRY(cudaSetDevice(h->device));
+    if (int rc = ensure_ws(h, 1, max_cycles)) return rc;
+    if (int rc = ensure_mg(h)) return rc;
+    const Geom g = make_geom(h, tol);
+    h->st_launches = 0; h->st_aux_launches = 0;
+    h->st_path = 4; h->st_halo = 0; h->st_ds = 0; h->st_ring = 0; h->st_redund = 1;
+    h->st_ctas = 0; h->st_tile_w = h->nr; h->st_tile_h = h->nz; h->st_tblock = 0; h->st_shape = -1; h->st_group = 1;
+    CU_TRY(cudaEventRecord(h->ev_t[0], st));
+    CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), st));
+    CU_TRY(cudaMemsetAsync(h->mg.slots, 0, 2 * sizeof(unsigned long long), st));
+    if (int rc = launch_moments(h, g, 1, rho, st)) return rc;         // a-1 (+ max|4 pi rho|), a-1b as in the SOR path
+    h->st_launches += 1; h->st_aux_launches += 1;
+    if (!h->user_boundary) {
+        k_boundary<<<1, 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN, h->d_bS, 0);
+        CU_TRY(cudaGetLastError());
+        h->st_launches += 1; h->st_aux_launches += 1;
+    }
+    h->last_nbatch = h->user_boundary ? h->cap_batch : 1;
+    CU_TRY(cudaEventRecord(h->ev_t[1], st));
+    if (io && io->wait_before_relax) CU_TRY(cudaStreamWaitEvent(st, io->wait_before_relax, 0));
+    if (max_cycles == 0) {
+        h->h_ctl[0] = Ctl();
+        h->h_ctl[0].done = 1; h->h_ctl[0].status = tol > 0.0 ? 1 : 0;
+    }
+    // The decision of a cycle is taken on the device (k_mg_decide, M8); the host reads it back after every cycle (a
+    // solve is ~8 cycles, so this is ~8 stream synchronisations per solve).
+    for (int c = 1; c <= max_cycles; ++c) {
+        if (int rc = mg_cycle(h, rho, phi, tol, c, max_cycles, st)) return rc;
+        CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
+        if (h->h_ctl[0].done) break;
+    }
+    CU_TRY(cudaEventRecord(h->ev_t[2], st));
+    if (io && io->d2h_dst) CU_TRY(cudaMemcpyAsync(io->d2h_dst, io->d2h_src, io->d2h_bytes, cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    float ms = 0;
+    CU_TRY(cudaEventElapsedTime(&ms, h->ev_t[0], h->ev_t[1]));
+    h->st_setup_ms = ms;
+    CU_TRY(cudaEventElapsedTime(&ms, h->ev_t[1], h->ev_t[2]));
+    h->st_sweep_ms = ms;
+    out->sweeps = h->h_ctl[0].sweeps;
+    out->status = h->h_ctl[0].status;
+    out->residual = h->h_ctl[0].residual;
+    h->last_sweeps0 = out->sweeps;
+    return 0;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char* sn_poisson_last_error(void) { return g_err.c_str(); }
@@ -880,6 +1048,9 @@ sn_poisson* sn_poisson_create(int nr, int nz, double dr, double dz, int symmetry
 
 void sn_poisson_destroy(sn_poisson* h) {
     if (!h) return;
+    for (auto& v : {&h->mg.cE, &h->mg.cW, &h->mg.phi, &h->mg.f})
+        for (double* p : *v) cudaFree(p);
+    cudaFree(h->mg.slots);
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
     cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage); cudaFree(h->d_snap[0]); cudaFree(h->d_snap[1]);
@@ -918,6 +1089,43 @@ sn_poisson_result sn_poisson_solve_host(sn_poisson* h, const double* rho_host, d
     sn_poisson_result out;
     const int rc = sn_poisson_solve_batch_host(h, 1, rho_host, phi_inout_host, tol, max_sweeps, stream, &out);
     if (rc) { r.sweeps = 0; r.status = rc; r.residual = 0.0; return r; }
+    return out;
+}
+
+sn_poisson_result sn_poisson_solve_mg(sn_poisson* h, const double* rho, double* phi_inout, double tol, int max_cycles,
+                                      void* stream) {
+    g_err.clear();
+    sn_poisson_result r = {0, -1, 0.0};
+    if (!check_solve_args(h, rho, phi_inout, tol, max_cycles)) return r;
+    sn_poisson_result out = {0, 0, 0.0};
+    const int rc = solve_mg_impl(h, rho, phi_inout, tol, max_cycles, (cudaStream_t)stream, &out);
+    if (rc) { r.status = rc; return r; }
+    return out;
+}
+
+sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
+                                           int max_cycles, void* stream) {
+    g_err.clear();
+    sn_poisson_result r = {0, -1, 0.0};
+    if (!check_solve_args(h, rho_host, phi_inout_host, tol, max_cycles)) return r;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)h->nr * h->nz, bytes = sizeof(double) * n;
+    auto fail = [&](int rc) { r.status = rc; return r; };
+    if (cudaSetDevice(h->device) != cudaSuccess) { set_err("cudaSetDevice failed"); return fail(-2); }
+    if (int rc = ensure_stage(h, n)) return fail(rc);
+    if (cudaEventRecord(h->ev_io[0], st) != cudaSuccess || cudaStreamWaitEvent(h->st_copy, h->ev_io[0], 0) != cudaSuccess ||
+        cudaMemcpyAsync(h->d_rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, h->st_copy) != cudaSuccess ||
+        cudaEventRecord(h->ev_io[1], h->st_copy) != cudaSuccess) {
+        set_err("host staging failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return fail(-2);
+    }
+    HostIO io;
+    io.wait_before_relax = h->ev_io[1];
+    io.d2h_dst = phi_inout_host; io.d2h_src = h->d_phi_stage; io.d2h_bytes = bytes;
+    sn_poisson_result out = {0, 0, 0.0};
+    const int rc = solve_mg_impl(h, h->d_rho_stage, h->d_phi_stage, tol, max_cycles, st, &out, &io);
+    if (rc) return fail(rc);
     return out;
 }
 
@@ -1156,6 +1364,9 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "ll")) { if (value < -1 || value > 1) { set_err("ll must be -1, 0 or 1"); return -1; } h->opt_ll = (int)value; return 0; }
     if (!strcmp(key, "halo")) { if (value < -1 || value > 1) { set_err("halo must be -1, 0 or 1"); return -1; } h->opt_halo = (int)value; return 0; }
     if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)std::max(shapes().size(), blk_shapes().size())) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
+    if (!strcmp(key, "mg_nu1")) { if (value < 0 || value > 8) { set_err("mg_nu1 must be 0..8"); return -1; } h->opt_mg_nu1 = (int)value; return 0; }
+    if (!strcmp(key, "mg_nu2")) { if (value < 0 || value > 8) { set_err("mg_nu2 must be 0..8"); return -1; } h->opt_mg_nu2 = (int)value; return 0; }
+    if (!strcmp(key, "mg_nc")) { if (value < 1 || value > 1000) { set_err("mg_nc must be 1..1000"); return -1; } h->opt_mg_nc = (int)value; return 0; }
     if (!strcmp(key, "tblock")) { if (value < 0 || value > kMaxTB) { set_err("tblock must be 0..%d", kMaxTB); return -1; } h->opt_tblock = (int)value; return 0; }
     set_err("unknown option '%s'", key);
     return -1;
@@ -1179,6 +1390,7 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
     if (!strcmp(key, "ring")) { *out = h->st_ring; return 0; }
     if (!strcmp(key, "group")) { *out = h->st_group; return 0; }
     if (!strcmp(key, "redundancy")) { *out = h->st_redund; return 0; }
+    if (!strcmp(key, "mg_levels")) { *out = h->mg.nlev; return 0; }
     if (!strncmp(key, "prof_mean", 9) && key[9] >= '0' && key[9] <= '7' && !key[10]) { *out = h->prof_mean[key[9] - '0']; return 0; }
     if (!strncmp(key, "prof_max", 8) && key[8] >= '0' && key[8] <= '7' && !key[9]) { *out = h->prof_max[key[8] - '0']; return 0; }
     set_err("unknown stat '%s'", key);

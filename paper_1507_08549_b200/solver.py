@@ -64,6 +64,27 @@ class PoissonSolver:
         self._raise_if_failed([r], "sn_poisson_solve")
         return r
 
+    def solve_mg(self, rho, phi, tol, max_cycles=60):
+        """Multigrid variant (NEXT-4): in place on ``phi``; the result's ``sweeps`` counts V-cycles."""
+        import torch
+        self._check(rho)
+        self._check(phi)
+        if tuple(rho.shape) != (self.nz, self.nr) or rho.shape != phi.shape:
+            raise ValueError("shape mismatch")
+        r = B.sn_poisson_solve_mg(self.h, rho.data_ptr(), phi.data_ptr(), tol, max_cycles,
+                                  torch.cuda.current_stream().cuda_stream)
+        self._raise_if_failed([r], "sn_poisson_solve_mg")
+        return r
+
+    def solve_mg_host(self, rho_np, phi_np, tol, max_cycles=60):
+        import torch
+        self._check_host(rho_np, (self.nz, self.nr))
+        self._check_host(phi_np, (self.nz, self.nr), writeable=True)
+        r = B.sn_poisson_solve_mg_host(self.h, rho_np.ctypes.data, phi_np.ctypes.data, tol, max_cycles,
+                                       torch.cuda.current_stream().cuda_stream)
+        self._raise_if_failed([r], "sn_poisson_solve_mg_host")
+        return r
+
     def _check_host(self, a, shape, writeable=False):
         import numpy as np
         if not isinstance(a, np.ndarray) or a.dtype != np.float64 or not a.flags.c_contiguous or tuple(a.shape) != shape:
