@@ -449,6 +449,28 @@ def next_rows(torch, P, flush):
                  "e2e": {"value": cells / (e2e_ms * 1e-3), "ms_per_step": e2e_ms, "api": "sn_weno_rhs_host",
                          "h2d_bytes_per_step": U.nbytes, "d2h_bytes_per_step": U.nbytes}})
     wn.close()
+    # ---- NEXT-4: multigrid variant on the same stencil (time to the same residual tolerance, next to the SOR path)
+    for name in ("cfg1", "cfg2", "cfg3"):
+        lab, mem = make_workload(name)
+        w0 = mem[0]
+        sv = P.PoissonSolver.for_workload(w0)
+        rho = torch.from_numpy(w0.rho).cuda()
+        phi = torch.zeros_like(rho)
+        res = []
+        ms = timed(lambda: (phi.zero_(), res.append(sv.solve_mg(rho, phi, w0.tol, 60))), 5)
+        zero_ms = timed(lambda: phi.zero_(), 5)
+        launches = int(sv.stat("launches"))
+        phi_h = np.zeros_like(w0.rho)
+        e2e_ms = wall(lambda: (phi_h.fill(0.0), sv.solve_mg_host(w0.rho, phi_h, w0.tol, 60)), 3)
+        r = res[-1]
+        # cells touched per V(1,1) cycle on level 0: 2 sweeps + 2 residual passes + 1 prolongation; x 4/3 for the coarse levels
+        rows.append({"workload": "mg_" + name, "label": "NEXT-4: multigrid V(1,1) on " + lab, "metric": "time_to_residual_ms",
+                     "value": ms - zero_ms, "cycles": r.sweeps, "final_residual": r.residual, "levels": int(sv.stat("mg_levels")),
+                     "higher_is_better": False, "gpu_launches_per_step": launches,
+                     "fine_cell_updates_per_s": 2.0 * r.sweeps * w0.cells / ((ms - zero_ms) * 1e-3),
+                     "e2e": {"value": e2e_ms, "unit": "ms", "api": "sn_poisson_solve_mg_host",
+                             "h2d_bytes_per_step": 2 * w0.rho.nbytes, "d2h_bytes_per_step": w0.rho.nbytes}})
+        sv.close()
     return rows
 
 

@@ -201,7 +201,7 @@ const char* sn_poisson_version(void);
  * equation, discretisation, multipole ghosts and therefore the same converged potential as sn_poisson_solve; only the
  * iteration differs (readings M1..M8): V-cycles over the levels (nr / 2^l) x (nz / 2^l) (coarsened
  * while both counts are even and >= 8), red-black Gauss-Seidel smoothing (options "mg_nu1", "mg_nu2": sweeps before /
- * after the coarse-grid correction, default 1 / 1; "mg_nc": sweeps on the coarsest level, default 30), volume-weighted
+ * after the coarse-grid correction, default 1 / 1; "mg_nc": sweeps on the coarsest level, default 12), volume-weighted
  * restriction, bilinear prolongation, coarse Dirichlet ghosts extrapolated to the level-0 ghost centre.  After every
  * cycle the ratio R (rule R9) of the TRUE residual of the iterate is evaluated on the device; the solve stops after the
  * first cycle with R <= tol (tol <= 0: exactly max_cycles cycles).  Returns {cycles, status, R} like sn_poisson_solve

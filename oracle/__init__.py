@@ -357,7 +357,7 @@ def mg_prolong(ec, symmetry, lc):
     return out
 
 
-def mg_solve(rho, phi0, dr, dz, symmetry, lmax, tol, max_cycles, nu1=1, nu2=1, nc=30, ghosts=None):
+def mg_solve(rho, phi0, dr, dz, symmetry, lmax, tol, max_cycles, nu1=1, nu2=1, nc=12, ghosts=None):
     """Multigrid solve (M1-M8) with the multipole ghosts of the SOR oracle (or the given (bE, bN, bS)).
     Returns dict(phi, cycles, status, residual, history)."""
     rho, phi = _f64(rho), _f64(phi0).copy()

@@ -24,7 +24,8 @@
 //   M4  residual: res = f - t with the same tree.
 //   M5  restriction (volume weighted, the volume of a cell is proportional to r_i = i + 1/2):
 //       f_c(I,J) = ((r_a res(a,2J) + r_b res(b,2J)) + (r_a res(a,2J+1) + r_b res(b,2J+1))) / (2 (r_a + r_b)), a = 2I, b = 2I+1.
-//   M6  coarsest level: nc red-black Gauss-Seidel sweeps from zero (default 30).
+//   M6  coarsest level: nc red-black Gauss-Seidel sweeps from zero (default 12: 10 already give the cycle count of 30,
+//       below 8 the V-cycle degrades -- the coarsest grid with its reflecting sides relaxes slowly).
 //   M7  prolongation: bilinear, e_f(2I+a, 2J+b) = (((9 C + 3 H) + 3 V) + Dg) / 16 with H / V / Dg the coarse neighbours
 //       towards the fine cell; the coarse error is extended by one ghost layer: reflected at the axis (and at the equator
 //       when symmetry = 1), -beta_{l+1} times the edge value at the outer edges (rows first, then columns, so a corner

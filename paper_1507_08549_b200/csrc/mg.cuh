@@ -45,54 +45,39 @@ __device__ __forceinline__ double mg_apply_at(const MgLevel& L, int i, int j, do
     return t;
 }
 
-// M3: one half-sweep of colour COL; one thread per cell of that colour
-template <int COL>
-__global__ void __launch_bounds__(256) k_mg_halfsweep(const MgLevel L) {
-    const int half = (L.nr + 1) / 2;
-    const size_t n = (size_t)half * L.nz;
-    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x) {
-        const int j = (int)(idx / half), i = 2 * (int)(idx - (size_t)j * half) + ((j + COL) & 1);
-        if (i >= L.nr) continue;
-        const size_t c = (size_t)j * L.nr + i;
-        const double pC = L.phi[c];
-        double diag, w;
-        const double t = mg_apply_at(L, i, j, pC, diag, w);
-        const double res = __dsub_rn(__dmul_rn(L.scale, L.src[c]), t);
-        L.phi[c] = __fma_rn(-w, res, pC);
-    }
+// M3: the Gauss-Seidel update of the idx-th cell of colour col (cells of one colour are numbered row by row)
+// (IDX: size_t in the streaming kernels, unsigned in the one-CTA tail, where a 64-bit division per cell would dominate)
+template <typename IDX>
+__device__ __forceinline__ void mg_update_cell(const MgLevel& L, IDX idx, int col) {
+    const IDX half = (IDX)((L.nr + 1) / 2);
+    const int j = (int)(idx / half), i = 2 * (int)(idx - (IDX)j * half) + ((j + col) & 1);
+    if (i >= L.nr) return;
+    const size_t c = (size_t)j * L.nr + i;
+    const double pC = L.phi[c];
+    double diag, w;
+    const double t = mg_apply_at(L, i, j, pC, diag, w);
+    const double res = __dsub_rn(__dmul_rn(L.scale, L.src[c]), t);
+    L.phi[c] = __fma_rn(-w, res, pC);
 }
 
-// M6: the coarsest level, nc sweeps by ONE CTA (the level is a few dozen cells; any size works)
-__global__ void __launch_bounds__(1024) k_mg_coarse(const MgLevel L, int nc) {
-    const int half = (L.nr + 1) / 2;
-    const int n = half * L.nz;
-    for (int s = 0; s < 2 * nc; ++s) {
-        const int col = s & 1;
-        for (int idx = threadIdx.x; idx < n; idx += blockDim.x) {
-            const int j = idx / half, i = 2 * (idx - j * half) + ((j + col) & 1);
-            if (i >= L.nr) continue;
-            const size_t c = (size_t)j * L.nr + i;
-            const double pC = L.phi[c];
-            double diag, w;
-            const double t = mg_apply_at(L, i, j, pC, diag, w);
-            const double res = __dsub_rn(__dmul_rn(L.scale, L.src[c]), t);
-            L.phi[c] = __fma_rn(-w, res, pC);
-        }
-        __syncthreads();
-    }
+// M3: one half-sweep of colour COL; one thread per cell of that colour
+template <int COL>
+__global__ void __launch_bounds__(256) k_mg_halfsweep(const MgLevel L, const Ctl* __restrict__ ctl) {
+    if (ctl->done) return;               // a finished solve: cycles enqueued ahead of the host's poll do nothing
+    const size_t n = (size_t)((L.nr + 1) / 2) * L.nz;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
+        mg_update_cell<size_t>(L, idx, COL);
 }
 
 // M4 + M5 + M8: one thread per 2 x 2 block of the level.  RESTRICT: the volume-weighted average of the four residuals
 // becomes the right-hand side of the next coarser level, whose error is zeroed.  MAXIMA: max|res| and max|phi| of the
 // level as order-preserving keys (warp REDUX, one atomicMax per warp) for the stopping ratio.
-template <bool RESTRICT, bool MAXIMA>
-__global__ void __launch_bounds__(256) k_mg_residual(const MgLevel L, double* __restrict__ fc, double* __restrict__ ec,
-                                                     unsigned long long* __restrict__ slots) {
-    const int nrc = (L.nr + 1) / 2, nzc = (L.nz + 1) / 2;
-    const size_t n = (size_t)nrc * nzc;
-    unsigned long long kr = 0ull, kp = 0ull;
-    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x) {
-        const int J = (int)(idx / nrc), I = (int)(idx - (size_t)J * nrc);
+template <bool RESTRICT, bool MAXIMA, typename IDX>
+__device__ __forceinline__ void mg_residual_block(const MgLevel& L, IDX idx, double* __restrict__ fc,
+                                                  double* __restrict__ ec, unsigned long long& kr, unsigned long long& kp) {
+    const IDX nrc = (IDX)((L.nr + 1) / 2);
+    {
+        const int J = (int)(idx / nrc), I = (int)(idx - (IDX)J * nrc);
         double r[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
         for (int b = 0; b < 2; ++b)
@@ -119,6 +104,16 @@ __global__ void __launch_bounds__(256) k_mg_residual(const MgLevel L, double* __
             ec[idx] = 0.0;
         }
     }
+}
+
+template <bool RESTRICT, bool MAXIMA>
+__global__ void __launch_bounds__(256) k_mg_residual(const MgLevel L, double* __restrict__ fc, double* __restrict__ ec,
+                                                     unsigned long long* __restrict__ slots, const Ctl* __restrict__ ctl) {
+    if (ctl->done) return;
+    const size_t n = (size_t)((L.nr + 1) / 2) * ((L.nz + 1) / 2);
+    unsigned long long kr = 0ull, kp = 0ull;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
+        mg_residual_block<RESTRICT, MAXIMA, size_t>(L, idx, fc, ec, kr, kp);
     if (MAXIMA) {
         kr = warp_max_key(kr);
         kp = warp_max_key(kp);
@@ -148,23 +143,105 @@ __device__ __forceinline__ double mg_ext(const MgLevel& Lc, int I, int J) {
     return v;
 }
 
-// M7: phi_f += bilinear interpolation of the coarse error; one thread per fine cell
-__global__ void __launch_bounds__(256) k_mg_prolong_add(const MgLevel Lc, double* __restrict__ phi_f, int nr_f, int nz_f) {
+// M7: phi_f += bilinear interpolation of the coarse error, fine cell idx
+template <typename IDX>
+__device__ __forceinline__ void mg_prolong_cell(const MgLevel& Lc, double* phi_f, int nr_f, IDX idx) {
+    const int j = (int)(idx / (IDX)nr_f), i = (int)(idx - (IDX)j * (IDX)nr_f);
+    const int I = i >> 1, J = j >> 1, di = (i & 1) ? 1 : -1, dj = (j & 1) ? 1 : -1;
+    const double C = mg_ext(Lc, I, J), H = mg_ext(Lc, I + di, J), V = mg_ext(Lc, I, J + dj), Dg = mg_ext(Lc, I + di, J + dj);
+    const double e = __dmul_rn(__dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(9.0, C), __dmul_rn(3.0, H)), __dmul_rn(3.0, V)), Dg), 0.0625);
+    phi_f[idx] = __dadd_rn(phi_f[idx], e);
+}
+
+// one thread per fine cell
+__global__ void __launch_bounds__(256) k_mg_prolong_add(const MgLevel Lc, double* phi_f, int nr_f, int nz_f,
+                                                        const Ctl* __restrict__ ctl) {
+    if (ctl->done) return;
     const size_t n = (size_t)nr_f * nz_f;
-    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x) {
-        const int j = (int)(idx / nr_f), i = (int)(idx - (size_t)j * nr_f);
-        const int I = i >> 1, J = j >> 1, di = (i & 1) ? 1 : -1, dj = (j & 1) ? 1 : -1;
-        const double C = mg_ext(Lc, I, J), H = mg_ext(Lc, I + di, J), V = mg_ext(Lc, I, J + dj), Dg = mg_ext(Lc, I + di, J + dj);
-        const double e = __dmul_rn(__dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(9.0, C), __dmul_rn(3.0, H)), __dmul_rn(3.0, V)), Dg), 0.0625);
-        phi_f[idx] = __dadd_rn(phi_f[idx], e);
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
+        mg_prolong_cell<size_t>(Lc, phi_f, nr_f, idx);
+}
+
+// The tail of the V-cycle -- every level small enough for ONE CTA (<= kMgTailCells cells) down to the coarsest and back
+// up -- as a single launch: these levels are a few thousand cells and purely launch / latency bound as separate
+// kernels (six launches per level and cycle, plus 2 nc half-sweeps on the coarsest).  The error and the right-hand side
+// of every tail level live in SHARED memory for the duration of the launch (<= 171 KB), the phases are the same device
+// functions as above, separated by CTA barriers.  L[0] is the finest level of the tail, L[n-1] the coarsest (M6).
+constexpr int kMgMaxLevels = 14;
+constexpr int kMgTailCells = 8192;
+struct MgTail {
+    int n, nu1, nu2, nc;
+    MgLevel L[kMgMaxLevels];
+};
+// doubles of dynamic shared memory the tail needs: phi and f of every level
+inline size_t mg_tail_smem_doubles(const MgTail& T) {
+    size_t d = 0;
+    for (int l = 0; l < T.n; ++l) d += 2 * (size_t)T.L[l].nr * T.L[l].nz;
+    return d;
+}
+
+__global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __restrict__ ctl) {
+    extern __shared__ __align__(16) double mg_sm[];
+    __shared__ MgLevel L[kMgMaxLevels];           // the levels with their arrays re-pointed to shared memory
+    __shared__ double* fw[kMgMaxLevels];
+    if (ctl->done) return;
+    {
+        if (threadIdx.x == 0) {
+            double* p = mg_sm;
+            for (int l = 0; l < T.n; ++l) {
+                const size_t n = (size_t)T.L[l].nr * T.L[l].nz;
+                L[l] = T.L[l];
+                L[l].phi = p; fw[l] = p + n; L[l].src = fw[l];
+                p += 2 * n;
+            }
+        }
+        __syncthreads();
+        const size_t n0 = (size_t)T.L[0].nr * T.L[0].nz;
+        for (size_t i = threadIdx.x; i < n0; i += blockDim.x) { L[0].phi[i] = T.L[0].phi[i]; fw[0][i] = T.L[0].src[i]; }
+        __syncthreads();
     }
+    auto smooth = [&](const MgLevel& Lv, int nsweeps) {
+        const unsigned n = (unsigned)((Lv.nr + 1) / 2) * (unsigned)Lv.nz;
+        if (n <= 32u) {                           // a level of <= 64 cells: one warp, warp barriers instead of CTA barriers
+            if (threadIdx.x < 32u) {
+                for (int s = 0; s < 2 * nsweeps; ++s) {
+                    if (threadIdx.x < n) mg_update_cell<unsigned>(Lv, threadIdx.x, s & 1);
+                    __syncwarp();
+                }
+            }
+            __syncthreads();
+            return;
+        }
+        for (int s = 0; s < 2 * nsweeps; ++s) {
+            for (unsigned idx = threadIdx.x; idx < n; idx += blockDim.x) mg_update_cell<unsigned>(Lv, idx, s & 1);
+            __syncthreads();
+        }
+    };
+    unsigned long long kr = 0ull, kp = 0ull;
+    for (int l = 0; l + 1 < T.n; ++l) {                              // down
+        smooth(L[l], T.nu1);
+        const unsigned nc = (unsigned)L[l + 1].nr * (unsigned)L[l + 1].nz;
+        for (unsigned idx = threadIdx.x; idx < nc; idx += blockDim.x)
+            mg_residual_block<true, false, unsigned>(L[l], idx, fw[l + 1], L[l + 1].phi, kr, kp);
+        __syncthreads();
+    }
+    smooth(L[T.n - 1], T.n == 1 ? T.nu1 + T.nu2 : T.nc);             // coarsest (a single-level grid: plain Gauss-Seidel)
+    for (int l = T.n - 2; l >= 0; --l) {                             // up
+        const unsigned nf = (unsigned)L[l].nr * (unsigned)L[l].nz;
+        for (unsigned idx = threadIdx.x; idx < nf; idx += blockDim.x) mg_prolong_cell<unsigned>(L[l + 1], L[l].phi, L[l].nr, idx);
+        __syncthreads();
+        smooth(L[l], T.nu2);
+    }
+    const size_t n0 = (size_t)T.L[0].nr * T.L[0].nz;
+    for (size_t i = threadIdx.x; i < n0; i += blockDim.x) T.L[0].phi[i] = L[0].phi[i];
 }
 
 // M8: the stopping ratio of the cycle just finished; resets the maxima for the next one
-__global__ void k_mg_decide(Ctl* __restrict__ ctl, unsigned long long* __restrict__ slots, double D, double tol, int cycle,
+__global__ void k_mg_decide(Ctl* __restrict__ ctl, unsigned long long* __restrict__ slots, double D, double tol,
                             int max_cycles, double* __restrict__ hist) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     if (ctl->done) return;
+    const int cycle = ctl->sweeps + 1;
     const double R = stop_ratio(slots[0], slots[1], ctl->maxf, D);
     slots[0] = 0ull;
     slots[1] = 0ull;

@@ -128,8 +128,10 @@ struct sn_poisson {
         std::vector<int> nr, nz;
         std::vector<double*> cE, cW, phi, f;
         unsigned long long* slots = nullptr;
+        bool tail_attr = false;
+        double* h_hist = nullptr;     // pinned: the last two ratios, for the host's chunk prediction
     } mg;
-    int opt_mg_nu1 = 1, opt_mg_nu2 = 1, opt_mg_nc = 30;
+    int opt_mg_nu1 = 1, opt_mg_nu2 = 1, opt_mg_nc = 12;
 
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
@@ -844,7 +846,7 @@ int mg_num_levels(int nr, int nz) {                                  // M1
 int ensure_mg(sn_poisson* h) {
     if (h->mg.nlev) return 0;
     auto& W = h->mg;
-    const int nlev = mg_num_levels(h->nr, h->nz);
+    const int nlev = std::min(mg_num_levels(h->nr, h->nz), kMgMaxLevels);
     W.nr.resize(nlev); W.nz.resize(nlev);
     W.cE.assign(nlev, nullptr); W.cW.assign(nlev, nullptr); W.phi.assign(nlev, nullptr); W.f.assign(nlev, nullptr);
     for (int l = 0; l < nlev; ++l) {
@@ -899,8 +901,8 @@ inline int mg_blocks(size_t n, int num_sms) { return (int)std::max<size_t>(1, st
 int mg_smooth(sn_poisson* h, const MgLevel& L, int nsweeps, cudaStream_t st) {
     const int blocks = mg_blocks((size_t)((L.nr + 1) / 2) * L.nz, h->num_sms);
     for (int k = 0; k < nsweeps; ++k) {
-        k_mg_halfsweep<0><<<blocks, 256, 0, st>>>(L);
-        k_mg_halfsweep<1><<<blocks, 256, 0, st>>>(L);
+        k_mg_halfsweep<0><<<blocks, 256, 0, st>>>(L, h->d_ctl);
+        k_mg_halfsweep<1><<<blocks, 256, 0, st>>>(L, h->d_ctl);
         h->st_launches += 2;
     }
     CU_TRY(cudaGetLastError());
@@ -908,32 +910,45 @@ int mg_smooth(sn_poisson* h, const MgLevel& L, int nsweeps, cudaStream_t st) {
 }
 
 // one V-cycle from level 0, then the true residual's maxima and the decision of the cycle (M8)
-int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int cycle, int max_cycles, cudaStream_t st) {
+int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_cycles, cudaStream_t st) {
     const auto& W = h->mg;
     const int nu1 = h->opt_mg_nu1, nu2 = h->opt_mg_nu2;
     std::vector<MgLevel> Ls;
     for (int l = 0; l < W.nlev; ++l) Ls.push_back(mg_level(h, l, rho, phi));
-    if (W.nlev == 1) {
-        if (int rc = mg_smooth(h, Ls[0], nu1 + nu2, st)) return rc;
-    } else {
-        for (int l = 0; l + 1 < W.nlev; ++l) {                       // down
-            if (int rc = mg_smooth(h, Ls[l], nu1, st)) return rc;
-            const size_t nc = (size_t)W.nr[l + 1] * W.nz[l + 1];
-            k_mg_residual<true, false><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr);
-            h->st_launches += 1;
-        }
-        k_mg_coarse<<<1, 1024, 0, st>>>(Ls[W.nlev - 1], h->opt_mg_nc);
+    // levels 0 .. top-1 run as separate launches; the tail (every level of <= kMgTailCells cells) is ONE launch
+    int k = W.nlev;
+    for (int l = 0; l < W.nlev; ++l)
+        if ((long long)W.nr[l] * W.nz[l] <= kMgTailCells) { k = l; break; }
+    const int top = k < W.nlev ? k : W.nlev - 1;
+    for (int l = 0; l < top; ++l) {                                  // down
+        if (int rc = mg_smooth(h, Ls[l], nu1, st)) return rc;
+        const size_t nc = (size_t)W.nr[l + 1] * W.nz[l + 1];
+        k_mg_residual<true, false><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl);
         h->st_launches += 1;
-        for (int l = W.nlev - 2; l >= 0; --l) {                      // up
-            const size_t nf = (size_t)W.nr[l] * W.nz[l];
-            k_mg_prolong_add<<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l]);
-            h->st_launches += 1;
-            if (int rc = mg_smooth(h, Ls[l], nu2, st)) return rc;
+    }
+    if (k < W.nlev) {
+        MgTail T;
+        T.n = W.nlev - k; T.nu1 = nu1; T.nu2 = nu2; T.nc = h->opt_mg_nc;
+        for (int l = k; l < W.nlev; ++l) T.L[l - k] = Ls[l];
+        const size_t smem = sizeof(double) * mg_tail_smem_doubles(T);
+        if (!h->mg.tail_attr) {
+            CU_TRY(cudaFuncSetAttribute(k_mg_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            h->mg.tail_attr = true;
         }
+        k_mg_tail<<<1, 1024, smem, st>>>(T, h->d_ctl);
+        h->st_launches += 1;
+    } else {                                                         // a coarsest level too large for one CTA
+        if (int rc = mg_smooth(h, Ls[W.nlev - 1], W.nlev == 1 ? nu1 + nu2 : h->opt_mg_nc, st)) return rc;
+    }
+    for (int l = top - 1; l >= 0; --l) {                             // up
+        const size_t nf = (size_t)W.nr[l] * W.nz[l];
+        k_mg_prolong_add<<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl);
+        h->st_launches += 1;
+        if (int rc = mg_smooth(h, Ls[l], nu2, st)) return rc;
     }
     const size_t nb = (size_t)((W.nr[0] + 1) / 2) * ((W.nz[0] + 1) / 2);
-    k_mg_residual<false, true><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], nullptr, nullptr, W.slots);
-    k_mg_decide<<<1, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, cycle, max_cycles, h->d_hist);
+    k_mg_residual<false, true><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], nullptr, nullptr, W.slots, h->d_ctl);
+    k_mg_decide<<<1, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, max_cycles, h->d_hist);
     h->st_launches += 2;
     CU_TRY(cudaGetLastError());
     return 0;
@@ -965,13 +980,31 @@ int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int
         h->h_ctl[0] = Ctl();
         h->h_ctl[0].done = 1; h->h_ctl[0].status = tol > 0.0 ? 1 : 0;
     }
-    // The decision of a cycle is taken on the device (k_mg_decide, M8); the host reads it back after every cycle (a
-    // solve is ~8 cycles, so this is ~8 stream synchronisations per solve).
-    for (int c = 1; c <= max_cycles; ++c) {
-        if (int rc = mg_cycle(h, rho, phi, tol, c, max_cycles, st)) return rc;
-        CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
-        CU_TRY(cudaStreamSynchronize(st));
-        if (h->h_ctl[0].done) break;
+    // The decision of a cycle is taken on the device (k_mg_decide, M8); once `done` is set every later kernel of the
+    // variant returns at once, so cycles enqueued ahead neither touch phi nor cost more than their launches.  A host
+    // round trip costs about as much as a whole cycle of a small grid, so the host enqueues cycles in chunks: two
+    // first, then as many as the measured contraction per cycle predicts are still needed (a V-cycle contracts at a
+    // nearly constant rate), and looks at the decision only between chunks.  tol <= 0: all cycles at once.
+    if (max_cycles > 0) {
+        if (!h->mg.h_hist) CU_TRY(cudaMallocHost((void**)&h->mg.h_hist, 2 * sizeof(double)));
+        int enq = 0;
+        int chunk = tol > 0.0 ? std::min(2, max_cycles) : max_cycles;
+        for (;;) {
+            for (int c = 0; c < chunk; ++c)
+                if (int rc = mg_cycle(h, rho, phi, tol, max_cycles, st)) return rc;
+            enq += chunk;
+            CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
+            if (enq >= 2) CU_TRY(cudaMemcpyAsync(h->mg.h_hist, h->d_hist + (enq - 2), 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CU_TRY(cudaStreamSynchronize(st));
+            if (h->h_ctl[0].done || enq >= max_cycles) break;
+            chunk = 1;
+            if (enq >= 2 && h->mg.h_hist[0] > 0.0 && h->mg.h_hist[1] > 0.0) {
+                const double rate = std::min(0.5, std::max(0.02, h->mg.h_hist[1] / h->mg.h_hist[0]));
+                const double need = std::ceil(std::log(tol / h->mg.h_hist[1]) / std::log(rate));
+                chunk = (int)std::min(16.0, std::max(1.0, need));
+            }
+            chunk = std::min(chunk, max_cycles - enq);
+        }
     }
     CU_TRY(cudaEventRecord(h->ev_t[2], st));
     if (io && io->d2h_dst) CU_TRY(cudaMemcpyAsync(io->d2h_dst, io->d2h_src, io->d2h_bytes, cudaMemcpyDeviceToHost, st));
@@ -1051,6 +1084,7 @@ void sn_poisson_destroy(sn_poisson* h) {
     for (auto& v : {&h->mg.cE, &h->mg.cW, &h->mg.phi, &h->mg.f})
         for (double* p : *v) cudaFree(p);
     cudaFree(h->mg.slots);
+    if (h->mg.h_hist) cudaFreeHost(h->mg.h_hist);
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
     cudaFree(h->d_rho_stage); cudaFree(h->d_phi_stage); cudaFree(h->d_snap[0]); cudaFree(h->d_snap[1]);
