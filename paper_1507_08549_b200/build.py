@@ -18,6 +18,7 @@ NVCC_FLAGS = [
     "-fmad=false",                              # pinned fp64 expression trees (R10)
     "-Xcompiler", "-fPIC,-ffp-contract=off,-O2",
 ]
+NVCC_FLAGS += os.environ.get("SN_NVCC_EXTRA", "").split()      # e.g. -DSNP_GROUP_ROWS_ROOMY=2 for an A/B build
 SHAPE_TUS = list(range(11)) + [100, 200]        # csrc/shapes.cuh: kNumResShapes resident shapes, blocked, dispatch
 
 
