@@ -129,9 +129,15 @@ struct sn_poisson {
         std::vector<double*> cE, cW, phi, f;
         unsigned long long* slots = nullptr;
         bool tail_attr = false;
+        // one V-cycle captured as a CUDA graph (the cycle is ~15-27 short launches): valid for one (rho, phi, tol,
+        // max_cycles, options, ghost source) key, re-captured when the key changes
+        cudaGraphExec_t exec = nullptr;
+        cudaStream_t st = nullptr;        // runs the cycles when the caller hands in the (uncapturable) legacy stream
+        double nodes = 0;                 // kernel nodes per captured cycle
+        struct Key { const double* rho = nullptr; double* phi = nullptr; double tol = 0; int max_cycles = -1, nu1 = 0, nu2 = 0, nc = 0; } key;
         double* h_hist = nullptr;     // pinned: the last two ratios, for the host's chunk prediction
     } mg;
-    int opt_mg_nu1 = 1, opt_mg_nu2 = 1, opt_mg_nc = 12;
+    int opt_mg_nu1 = 1, opt_mg_nu2 = 1, opt_mg_nc = 12, opt_mg_graph = 1;
 
     // stats of the last solve
     double st_aux_launches = 0;   // launches that are not relaxation sweeps (moments, boundary, init, decide)
@@ -175,6 +181,7 @@ Geom make_geom(const sn_poisson* h, double tol) {
 }
 
 void free_batch_ws(sn_poisson* h) {
+    if (h->mg.exec) { cudaGraphExecDestroy(h->mg.exec); h->mg.exec = nullptr; }      // the captured cycle holds these pointers
     cudaFree(h->d_bE); cudaFree(h->d_bN); cudaFree(h->d_bS); cudaFree(h->d_M); cudaFree(h->d_partial);
     cudaFree(h->d_slots); cudaFree(h->d_slots_f); cudaFree(h->d_hist); cudaFree(h->d_ctl);
     cudaFree(h->d_slots0); cudaFree(h->d_slots0_f);
@@ -869,6 +876,8 @@ int ensure_mg(sn_poisson* h) {
         }
     }
     if (int rc = dev_alloc(&W.slots, (size_t)2)) return rc;
+    CU_TRY(cudaFuncSetAttribute(k_mg_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    W.tail_attr = true;
     W.nlev = nlev;
     return 0;
 }
@@ -931,10 +940,6 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
         T.n = W.nlev - k; T.nu1 = nu1; T.nu2 = nu2; T.nc = h->opt_mg_nc;
         for (int l = k; l < W.nlev; ++l) T.L[l - k] = Ls[l];
         const size_t smem = sizeof(double) * mg_tail_smem_doubles(T);
-        if (!h->mg.tail_attr) {
-            CU_TRY(cudaFuncSetAttribute(k_mg_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-            h->mg.tail_attr = true;
-        }
         k_mg_tail<<<1, 1024, smem, st>>>(T, h->d_ctl);
         h->st_launches += 1;
     } else {                                                         // a coarsest level too large for one CTA
@@ -951,6 +956,47 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
     k_mg_decide<<<1, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, max_cycles, h->d_hist);
     h->st_launches += 2;
     CU_TRY(cudaGetLastError());
+    return 0;
+}
+
+// One cycle through the cached graph ("mg_graph" option, default on; the legacy default stream cannot be captured
+// and takes the plain launches).
+int mg_launch_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_cycles, cudaStream_t st) {
+    auto& W = h->mg;
+    if (!h->opt_mg_graph || st == nullptr || st == cudaStreamLegacy) return mg_cycle(h, rho, phi, tol, max_cycles, st);
+    const auto& k = W.key;
+    const bool same = W.exec && k.rho == rho && k.phi == phi && k.tol == tol && k.max_cycles == max_cycles &&
+                      k.nu1 == h->opt_mg_nu1 && k.nu2 == h->opt_mg_nu2 && k.nc == h->opt_mg_nc;
+    if (!same) {
+        if (W.exec) { cudaGraphExecDestroy(W.exec); W.exec = nullptr; }
+        const double launches_before = h->st_launches;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+            cudaGetLastError();
+            return mg_cycle(h, rho, phi, tol, max_cycles, st);
+        }
+        const int rc = mg_cycle(h, rho, phi, tol, max_cycles, st);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(st, &graph);
+        W.nodes = h->st_launches - launches_before;
+        h->st_launches = launches_before;
+        if (rc || e != cudaSuccess || !graph) {
+            cudaGetLastError();
+            if (graph) cudaGraphDestroy(graph);
+            if (rc) return rc;
+            return mg_cycle(h, rho, phi, tol, max_cycles, st);
+        }
+        const cudaError_t ei = cudaGraphInstantiate(&W.exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ei != cudaSuccess) {
+            cudaGetLastError();
+            W.exec = nullptr;
+            return mg_cycle(h, rho, phi, tol, max_cycles, st);
+        }
+        W.key.rho = rho; W.key.phi = phi; W.key.tol = tol; W.key.max_cycles = max_cycles;
+        W.key.nu1 = h->opt_mg_nu1; W.key.nu2 = h->opt_mg_nu2; W.key.nc = h->opt_mg_nc;
+    }
+    CU_TRY(cudaGraphLaunch(W.exec, st));
+    h->st_launches += W.nodes;            // kernels of mine that run inside the graph
     return 0;
 }
 
@@ -987,11 +1033,20 @@ int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int
     // nearly constant rate), and looks at the decision only between chunks.  tol <= 0: all cycles at once.
     if (max_cycles > 0) {
         if (!h->mg.h_hist) CU_TRY(cudaMallocHost((void**)&h->mg.h_hist, 2 * sizeof(double)));
+        // The legacy default stream cannot be captured: the cycles then run on a stream of the handle, ordered after
+        // the caller's stream here and before it again below.
+        cudaStream_t caller = st;
+        if (h->opt_mg_graph && (st == nullptr || st == cudaStreamLegacy)) {
+            if (!h->mg.st) CU_TRY(cudaStreamCreateWithFlags(&h->mg.st, cudaStreamNonBlocking));
+            CU_TRY(cudaEventRecord(h->ev_poll[0], caller));
+            CU_TRY(cudaStreamWaitEvent(h->mg.st, h->ev_poll[0], 0));
+            st = h->mg.st;
+        }
         int enq = 0;
         int chunk = tol > 0.0 ? std::min(2, max_cycles) : max_cycles;
         for (;;) {
             for (int c = 0; c < chunk; ++c)
-                if (int rc = mg_cycle(h, rho, phi, tol, max_cycles, st)) return rc;
+                if (int rc = mg_launch_cycle(h, rho, phi, tol, max_cycles, st)) return rc;
             enq += chunk;
             CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
             if (enq >= 2) CU_TRY(cudaMemcpyAsync(h->mg.h_hist, h->d_hist + (enq - 2), 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -1004,6 +1059,11 @@ int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int
                 chunk = (int)std::min(16.0, std::max(1.0, need));
             }
             chunk = std::min(chunk, max_cycles - enq);
+        }
+        if (st != caller) {                  // the loop above ended with st synchronised: the caller's stream may go on
+            CU_TRY(cudaEventRecord(h->ev_poll[1], st));
+            CU_TRY(cudaStreamWaitEvent(caller, h->ev_poll[1], 0));
+            st = caller;
         }
     }
     CU_TRY(cudaEventRecord(h->ev_t[2], st));
@@ -1084,6 +1144,8 @@ void sn_poisson_destroy(sn_poisson* h) {
     for (auto& v : {&h->mg.cE, &h->mg.cW, &h->mg.phi, &h->mg.f})
         for (double* p : *v) cudaFree(p);
     cudaFree(h->mg.slots);
+    if (h->mg.exec) { cudaGraphExecDestroy(h->mg.exec); h->mg.exec = nullptr; }
+    if (h->mg.st) cudaStreamDestroy(h->mg.st);
     if (h->mg.h_hist) cudaFreeHost(h->mg.h_hist);
     free_batch_ws(h);
     cudaFree(h->d_cE); cudaFree(h->d_cW);
@@ -1400,6 +1462,7 @@ int sn_poisson_set_option(sn_poisson* h, const char* key, int64_t value) {
     if (!strcmp(key, "shape")) { if (value < -1 || value >= (int64_t)std::max(shapes().size(), blk_shapes().size())) { set_err("bad shape"); return -1; } h->opt_shape = (int)value; return 0; }
     if (!strcmp(key, "mg_nu1")) { if (value < 0 || value > 8) { set_err("mg_nu1 must be 0..8"); return -1; } h->opt_mg_nu1 = (int)value; return 0; }
     if (!strcmp(key, "mg_nu2")) { if (value < 0 || value > 8) { set_err("mg_nu2 must be 0..8"); return -1; } h->opt_mg_nu2 = (int)value; return 0; }
+    if (!strcmp(key, "mg_graph")) { h->opt_mg_graph = value ? 1 : 0; return 0; }
     if (!strcmp(key, "mg_nc")) { if (value < 1 || value > 1000) { set_err("mg_nc must be 1..1000"); return -1; } h->opt_mg_nc = (int)value; return 0; }
     if (!strcmp(key, "tblock")) { if (value < 0 || value > kMaxTB) { set_err("tblock must be 0..%d", kMaxTB); return -1; } h->opt_tblock = (int)value; return 0; }
     set_err("unknown option '%s'", key);
