@@ -69,7 +69,8 @@ __global__ void __launch_bounds__(kMomThreads) k_moments(const double* __restric
 // Fixed-order final sum over blocks (deterministic), symmetry rule, then the ghost values
 //   phi_b = -(1/L0) sum_l M_l I_l,  I_0 = 1/shat, I_1 = y/shat^3, (l+1) I_{l+1} = ((2l+1) y I_l - l I_{l-1})/shat^2
 // at east (r=(nr+1/2)dr, z_j), north (r_i, z_{nz-1}+dz) and, for symmetry=0, south (r_i, z_0-dz) ghost centres.
-// grid = nbatch blocks.
+// grid = (nbatch, slices): every block forms the moments itself (same fixed order, so every block gets the same bits;
+// slice 0 stores them) and fills its slice of the ghost points, one point per thread and pass.
 __global__ void __launch_bounds__(256) k_boundary(Geom g, double L0, int NL, int nblocks,
                                                   const double* __restrict__ partial, double* __restrict__ M,
                                                   double* __restrict__ bE, double* __restrict__ bN,
@@ -77,20 +78,22 @@ __global__ void __launch_bounds__(256) k_boundary(Geom g, double L0, int NL, int
     const int b = blockIdx.x;
     __shared__ double sM[kMaxL + 1];
     double* Mb = M + (size_t)b * (kMaxL + 1);
-    if (!have_moments) {
-        for (int l = threadIdx.x; l <= g.lmax; l += blockDim.x) {
-            double v = 0.0;
+    for (int l = threadIdx.x; l <= g.lmax; l += blockDim.x) {
+        double v;
+        if (!have_moments) {
+            v = 0.0;
             for (int k = 0; k < nblocks; ++k) v += partial[((size_t)b * nblocks + k) * NL + l];
             if (g.symmetry == 1) v = (l & 1) ? 0.0 : 2.0 * v;
-            Mb[l] = v;
+            if (blockIdx.y == 0) Mb[l] = v;
+        } else {
+            v = Mb[l];
         }
-        __syncthreads();
+        sM[l] = v;
     }
-    for (int l = threadIdx.x; l <= g.lmax; l += blockDim.x) sM[l] = Mb[l];
     __syncthreads();
     const double zoff = g.symmetry == 1 ? 0.5 : 0.5 - 0.5 * g.nz;
     const int npts = g.nz + g.nr + (g.symmetry == 0 ? g.nr : 0);
-    for (int p = threadIdx.x; p < npts; p += blockDim.x) {
+    for (int p = blockIdx.y * blockDim.x + threadIdx.x; p < npts; p += gridDim.y * blockDim.x) {
         double r, z;
         double* dst;
         if (p < g.nz) {

@@ -228,6 +228,12 @@ int ensure_ws(sn_poisson* h, int nbatch, int max_sweeps) {
     return 0;
 }
 
+// blocks per member of the boundary fill: one ghost point per thread, at most 32 slices
+inline int boundary_slices(const sn_poisson* h) {
+    const int npts = h->nz + h->nr * (h->symmetry == 0 ? 2 : 1);
+    return std::max(1, std::min(32, (npts + 255) / 256));
+}
+
 int launch_moments(sn_poisson* h, const Geom& g, int nbatch, const double* rho, cudaStream_t st) {
     dim3 grid(h->mom_blocks, nbatch);
     switch (h->NL) {
@@ -728,7 +734,7 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
     h->st_launches += 1;
     h->st_aux_launches += 1;
     if (!h->user_boundary) {
-        k_boundary<<<nbatch, 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN,
+        k_boundary<<<dim3(nbatch, boundary_slices(h)), 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN,
                                            h->d_bS, 0);
         CU_TRY(cudaGetLastError());
         h->st_launches += 1;
@@ -1015,7 +1021,7 @@ int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int
     if (int rc = launch_moments(h, g, 1, rho, st)) return rc;         // a-1 (+ max|4 pi rho|), a-1b as in the SOR path
     h->st_launches += 1; h->st_aux_launches += 1;
     if (!h->user_boundary) {
-        k_boundary<<<1, 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN, h->d_bS, 0);
+        k_boundary<<<dim3(1, boundary_slices(h)), 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN, h->d_bS, 0);
         CU_TRY(cudaGetLastError());
         h->st_launches += 1; h->st_aux_launches += 1;
     }
