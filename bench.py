@@ -471,6 +471,28 @@ def next_rows(torch, P, flush):
                      "e2e": {"value": e2e_ms, "unit": "ms", "api": "sn_poisson_solve_mg_host",
                              "h2d_bytes_per_step": 2 * w0.rho.nbytes, "d2h_bytes_per_step": w0.rho.nbytes}})
         sv.close()
+    # the [CFG 3] workload itself (warm-started sequence, here its first 20 solves) through the multigrid variant
+    seq = W.cfg3(nsteps=20)
+    w0 = seq.first
+    rhos, r_t = [w0.rho], w0.rho
+    for t in range(1, seq.nsteps):
+        r_t = seq.step(r_t, t)
+        rhos.append(r_t)
+    rho_d = torch.from_numpy(np.stack(rhos)).cuda()
+    phi = torch.zeros((w0.nz, w0.nr), dtype=torch.float64, device="cuda")
+    sv = P.PoissonSolver.for_workload(w0)
+    cyc = []
+
+    def run_seq():
+        phi.zero_()
+        cyc.clear()
+        for t in range(seq.nsteps):
+            cyc.append(sv.solve_mg(rho_d[t], phi, w0.tol, 60).sweeps)
+    ms = timed(run_seq, 3, warm=1)
+    rows.append({"workload": "mg_cfg3seq20", "label": "NEXT-4: multigrid V(1,1) on the first 20 warm-started solves of [CFG 3]",
+                 "metric": "time_to_residual_ms", "value": ms / seq.nsteps, "sequence_ms": ms, "cycles": list(cyc),
+                 "higher_is_better": False, "e2e": {"value": None, "api": None}})
+    sv.close()
     return rows
 
 

@@ -208,8 +208,7 @@ const char* sn_poisson_version(void);
  * (`sweeps` = V-cycles applied); sn_poisson_get_history then returns R after every cycle.  rho / phi_inout: DEVICE
  * pointers as for sn_poisson_solve; any nr, nz >= 2 (a grid that cannot be coarsened runs plain Gauss-Seidel sweeps).
  * The stopping rule option (sn_poisson_set_stop_rule) does not apply.  One V-cycle is captured as a CUDA graph and
- * re-launched per cycle (option "mg_graph", default 1; re-captured when rho / phi / tol / max_cycles / the options
- * change); with the legacy default stream the cycles run on a stream of the handle ordered between the caller's work.
+ * re-launched per cycle (option "mg_graph", default 1; re-captured when tol / max_cycles / the options change); with the legacy default stream the cycles run on a stream of the handle ordered between the caller's work.
  * Synchronises `stream`. */
 sn_poisson_result sn_poisson_solve_mg(sn_poisson* h, const double* rho, double* phi_inout, double tol, int max_cycles,
                                       void* stream);

@@ -25,6 +25,17 @@ struct MgLevel {
     const double *bE, *bN, *bS;     // level 0: multipole ghosts; coarse: NULL
 };
 
+// The caller's arrays of the current solve.  Level 0 reaches them through this device-side record (phi == NULL in its
+// MgLevel), so that a captured cycle (CUDA graph) stays valid when the next solve brings other pointers.
+struct MgPtrs {
+    const double* rho;
+    double* phi;
+};
+__device__ __forceinline__ MgLevel mg_resolve(MgLevel L, const MgPtrs* __restrict__ pp) {
+    if (L.phi == nullptr) { L.phi = pp->phi; L.src = pp->rho; }
+    return L;
+}
+
 // t = (A phi)(i, j) with the pinned tree (R10); ghosts per M2.  Also returns the row's diagonal and omega / diag.
 __device__ __forceinline__ double mg_apply_at(const MgLevel& L, int i, int j, double pC, double& diag, double& w) {
     const size_t c = (size_t)j * L.nr + i;
@@ -62,8 +73,10 @@ __device__ __forceinline__ void mg_update_cell(const MgLevel& L, IDX idx, int co
 
 // M3: one half-sweep of colour COL; one thread per cell of that colour
 template <int COL>
-__global__ void __launch_bounds__(256) k_mg_halfsweep(const MgLevel L, const Ctl* __restrict__ ctl) {
+__global__ void __launch_bounds__(256) k_mg_halfsweep(const MgLevel Larg, const Ctl* __restrict__ ctl,
+                                                      const MgPtrs* __restrict__ pp) {
     if (ctl->done) return;               // a finished solve: cycles enqueued ahead of the host's poll do nothing
+    const MgLevel L = mg_resolve(Larg, pp);
     const size_t n = (size_t)((L.nr + 1) / 2) * L.nz;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
         mg_update_cell<size_t>(L, idx, COL);
@@ -107,9 +120,11 @@ __device__ __forceinline__ void mg_residual_block(const MgLevel& L, IDX idx, dou
 }
 
 template <bool RESTRICT, bool MAXIMA>
-__global__ void __launch_bounds__(256) k_mg_residual(const MgLevel L, double* __restrict__ fc, double* __restrict__ ec,
-                                                     unsigned long long* __restrict__ slots, const Ctl* __restrict__ ctl) {
+__global__ void __launch_bounds__(256) k_mg_residual(const MgLevel Larg, double* __restrict__ fc, double* __restrict__ ec,
+                                                     unsigned long long* __restrict__ slots, const Ctl* __restrict__ ctl,
+                                                     const MgPtrs* __restrict__ pp) {
     if (ctl->done) return;
+    const MgLevel L = mg_resolve(Larg, pp);
     const size_t n = (size_t)((L.nr + 1) / 2) * ((L.nz + 1) / 2);
     unsigned long long kr = 0ull, kp = 0ull;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
@@ -155,8 +170,9 @@ __device__ __forceinline__ void mg_prolong_cell(const MgLevel& Lc, double* phi_f
 
 // one thread per fine cell
 __global__ void __launch_bounds__(256) k_mg_prolong_add(const MgLevel Lc, double* phi_f, int nr_f, int nz_f,
-                                                        const Ctl* __restrict__ ctl) {
+                                                        const Ctl* __restrict__ ctl, const MgPtrs* __restrict__ pp) {
     if (ctl->done) return;
+    if (phi_f == nullptr) phi_f = pp->phi;           // level 0
     const size_t n = (size_t)nr_f * nz_f;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
         mg_prolong_cell<size_t>(Lc, phi_f, nr_f, idx);
@@ -180,7 +196,7 @@ inline size_t mg_tail_smem_doubles(const MgTail& T) {
     return d;
 }
 
-__global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __restrict__ ctl) {
+__global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __restrict__ ctl, const MgPtrs* __restrict__ pp) {
     extern __shared__ __align__(16) double mg_sm[];
     __shared__ MgLevel L[kMgMaxLevels];           // the levels with their arrays re-pointed to shared memory
     __shared__ double* fw[kMgMaxLevels];
@@ -196,8 +212,9 @@ __global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __r
             }
         }
         __syncthreads();
+        const MgLevel G0 = mg_resolve(T.L[0], pp);
         const size_t n0 = (size_t)T.L[0].nr * T.L[0].nz;
-        for (size_t i = threadIdx.x; i < n0; i += blockDim.x) { L[0].phi[i] = T.L[0].phi[i]; fw[0][i] = T.L[0].src[i]; }
+        for (size_t i = threadIdx.x; i < n0; i += blockDim.x) { L[0].phi[i] = G0.phi[i]; fw[0][i] = G0.src[i]; }
         __syncthreads();
     }
     auto smooth = [&](const MgLevel& Lv, int nsweeps) {
@@ -232,8 +249,9 @@ __global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __r
         __syncthreads();
         smooth(L[l], T.nu2);
     }
+    double* out0 = mg_resolve(T.L[0], pp).phi;
     const size_t n0 = (size_t)T.L[0].nr * T.L[0].nz;
-    for (size_t i = threadIdx.x; i < n0; i += blockDim.x) T.L[0].phi[i] = L[0].phi[i];
+    for (size_t i = threadIdx.x; i < n0; i += blockDim.x) out0[i] = L[0].phi[i];
 }
 
 // M8: the stopping ratio of the cycle just finished; resets the maxima for the next one

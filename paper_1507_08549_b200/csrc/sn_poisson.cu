@@ -128,13 +128,14 @@ struct sn_poisson {
         std::vector<int> nr, nz;
         std::vector<double*> cE, cW, phi, f;
         unsigned long long* slots = nullptr;
+        MgPtrs* d_ptrs = nullptr;         // the caller's rho / phi of the current solve, read by the level-0 kernels
         bool tail_attr = false;
-        // one V-cycle captured as a CUDA graph (the cycle is ~15-27 short launches): valid for one (rho, phi, tol,
-        // max_cycles, options, ghost source) key, re-captured when the key changes
+        // one V-cycle captured as a CUDA graph (the cycle is ~15-27 short launches): valid for one (tol, max_cycles,
+        // options) key -- the caller's rho / phi reach the kernels through d_ptrs --, re-captured when the key changes
         cudaGraphExec_t exec = nullptr;
         cudaStream_t st = nullptr;        // runs the cycles when the caller hands in the (uncapturable) legacy stream
         double nodes = 0;                 // kernel nodes per captured cycle
-        struct Key { const double* rho = nullptr; double* phi = nullptr; double tol = 0; int max_cycles = -1, nu1 = 0, nu2 = 0, nc = 0; } key;
+        struct Key { double tol = 0; int max_cycles = -1, nu1 = 0, nu2 = 0, nc = 0; } key;
         double* h_hist = nullptr;     // pinned: the last two ratios, for the host's chunk prediction
     } mg;
     int opt_mg_nu1 = 1, opt_mg_nu2 = 1, opt_mg_nc = 12, opt_mg_graph = 1;
@@ -882,6 +883,7 @@ int ensure_mg(sn_poisson* h) {
         }
     }
     if (int rc = dev_alloc(&W.slots, (size_t)2)) return rc;
+    if (int rc = dev_alloc(&W.d_ptrs, (size_t)1)) return rc;
     CU_TRY(cudaFuncSetAttribute(k_mg_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     W.tail_attr = true;
     W.nlev = nlev;
@@ -903,8 +905,9 @@ MgLevel mg_level(const sn_poisson* h, int l, const double* rho, double* phi) {
     L.beta = (1.0 - s) / (1.0 + s);
     L.scale = l == 0 ? kFourPi : 1.0;
     L.cE = W.cE[l]; L.cW = W.cW[l];
-    L.phi = l == 0 ? phi : W.phi[l];
-    L.src = l == 0 ? rho : W.f[l];
+    L.phi = l == 0 ? nullptr : W.phi[l];          // level 0: resolved on the device through MgPtrs (mg.cuh)
+    L.src = l == 0 ? nullptr : W.f[l];
+    (void)rho; (void)phi;
     L.bE = l == 0 ? h->d_bE : nullptr;
     L.bN = l == 0 ? h->d_bN : nullptr;
     L.bS = l == 0 ? h->d_bS : nullptr;
@@ -916,8 +919,8 @@ inline int mg_blocks(size_t n, int num_sms) { return (int)std::max<size_t>(1, st
 int mg_smooth(sn_poisson* h, const MgLevel& L, int nsweeps, cudaStream_t st) {
     const int blocks = mg_blocks((size_t)((L.nr + 1) / 2) * L.nz, h->num_sms);
     for (int k = 0; k < nsweeps; ++k) {
-        k_mg_halfsweep<0><<<blocks, 256, 0, st>>>(L, h->d_ctl);
-        k_mg_halfsweep<1><<<blocks, 256, 0, st>>>(L, h->d_ctl);
+        k_mg_halfsweep<0><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
+        k_mg_halfsweep<1><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
         h->st_launches += 2;
     }
     CU_TRY(cudaGetLastError());
@@ -938,7 +941,7 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
     for (int l = 0; l < top; ++l) {                                  // down
         if (int rc = mg_smooth(h, Ls[l], nu1, st)) return rc;
         const size_t nc = (size_t)W.nr[l + 1] * W.nz[l + 1];
-        k_mg_residual<true, false><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl);
+        k_mg_residual<true, false><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
     }
     if (k < W.nlev) {
@@ -946,19 +949,19 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
         T.n = W.nlev - k; T.nu1 = nu1; T.nu2 = nu2; T.nc = h->opt_mg_nc;
         for (int l = k; l < W.nlev; ++l) T.L[l - k] = Ls[l];
         const size_t smem = sizeof(double) * mg_tail_smem_doubles(T);
-        k_mg_tail<<<1, 1024, smem, st>>>(T, h->d_ctl);
+        k_mg_tail<<<1, 1024, smem, st>>>(T, h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
     } else {                                                         // a coarsest level too large for one CTA
         if (int rc = mg_smooth(h, Ls[W.nlev - 1], W.nlev == 1 ? nu1 + nu2 : h->opt_mg_nc, st)) return rc;
     }
     for (int l = top - 1; l >= 0; --l) {                             // up
         const size_t nf = (size_t)W.nr[l] * W.nz[l];
-        k_mg_prolong_add<<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl);
+        k_mg_prolong_add<<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
         if (int rc = mg_smooth(h, Ls[l], nu2, st)) return rc;
     }
     const size_t nb = (size_t)((W.nr[0] + 1) / 2) * ((W.nz[0] + 1) / 2);
-    k_mg_residual<false, true><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], nullptr, nullptr, W.slots, h->d_ctl);
+    k_mg_residual<false, true><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], nullptr, nullptr, W.slots, h->d_ctl, W.d_ptrs);
     k_mg_decide<<<1, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, max_cycles, h->d_hist);
     h->st_launches += 2;
     CU_TRY(cudaGetLastError());
@@ -971,7 +974,7 @@ int mg_launch_cycle(sn_poisson* h, const double* rho, double* phi, double tol, i
     auto& W = h->mg;
     if (!h->opt_mg_graph || st == nullptr || st == cudaStreamLegacy) return mg_cycle(h, rho, phi, tol, max_cycles, st);
     const auto& k = W.key;
-    const bool same = W.exec && k.rho == rho && k.phi == phi && k.tol == tol && k.max_cycles == max_cycles &&
+    const bool same = W.exec && k.tol == tol && k.max_cycles == max_cycles &&
                       k.nu1 == h->opt_mg_nu1 && k.nu2 == h->opt_mg_nu2 && k.nc == h->opt_mg_nc;
     if (!same) {
         if (W.exec) { cudaGraphExecDestroy(W.exec); W.exec = nullptr; }
@@ -998,7 +1001,7 @@ int mg_launch_cycle(sn_poisson* h, const double* rho, double* phi, double tol, i
             W.exec = nullptr;
             return mg_cycle(h, rho, phi, tol, max_cycles, st);
         }
-        W.key.rho = rho; W.key.phi = phi; W.key.tol = tol; W.key.max_cycles = max_cycles;
+        W.key.tol = tol; W.key.max_cycles = max_cycles;
         W.key.nu1 = h->opt_mg_nu1; W.key.nu2 = h->opt_mg_nu2; W.key.nc = h->opt_mg_nc;
     }
     CU_TRY(cudaGraphLaunch(W.exec, st));
@@ -1018,6 +1021,10 @@ int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int
     CU_TRY(cudaEventRecord(h->ev_t[0], st));
     CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), st));
     CU_TRY(cudaMemsetAsync(h->mg.slots, 0, 2 * sizeof(unsigned long long), st));
+    {
+        const MgPtrs hp = {rho, phi};
+        CU_TRY(cudaMemcpyAsync(h->mg.d_ptrs, &hp, sizeof hp, cudaMemcpyHostToDevice, st));     // pageable: staged before return
+    }
     if (int rc = launch_moments(h, g, 1, rho, st)) return rc;         // a-1 (+ max|4 pi rho|), a-1b as in the SOR path
     h->st_launches += 1; h->st_aux_launches += 1;
     if (!h->user_boundary) {
@@ -1150,6 +1157,7 @@ void sn_poisson_destroy(sn_poisson* h) {
     for (auto& v : {&h->mg.cE, &h->mg.cW, &h->mg.phi, &h->mg.f})
         for (double* p : *v) cudaFree(p);
     cudaFree(h->mg.slots);
+    cudaFree(h->mg.d_ptrs);
     if (h->mg.exec) { cudaGraphExecDestroy(h->mg.exec); h->mg.exec = nullptr; }
     if (h->mg.st) cudaStreamDestroy(h->mg.st);
     if (h->mg.h_hist) cudaFreeHost(h->mg.h_hist);
