@@ -72,14 +72,14 @@ __device__ __forceinline__ void mg_update_cell(const MgLevel& L, IDX idx, int co
 }
 
 // M3: one half-sweep of colour COL; one thread per cell of that colour
-template <int COL>
+template <int COL, typename IDX>
 __global__ void __launch_bounds__(256) k_mg_halfsweep(const MgLevel Larg, const Ctl* __restrict__ ctl,
                                                       const MgPtrs* __restrict__ pp) {
     if (ctl->done) return;               // a finished solve: cycles enqueued ahead of the host's poll do nothing
     const MgLevel L = mg_resolve(Larg, pp);
-    const size_t n = (size_t)((L.nr + 1) / 2) * L.nz;
-    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
-        mg_update_cell<size_t>(L, idx, COL);
+    const IDX n = (IDX)((L.nr + 1) / 2) * (IDX)L.nz;
+    for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x)
+        mg_update_cell<IDX>(L, idx, COL);
 }
 
 // M4 + M5 + M8: one thread per 2 x 2 block of the level.  RESTRICT: the volume-weighted average of the four residuals
@@ -119,20 +119,56 @@ __device__ __forceinline__ void mg_residual_block(const MgLevel& L, IDX idx, dou
     }
 }
 
-template <bool RESTRICT, bool MAXIMA>
+template <bool RESTRICT, bool MAXIMA, typename IDX>
 __global__ void __launch_bounds__(256) k_mg_residual(const MgLevel Larg, double* __restrict__ fc, double* __restrict__ ec,
                                                      unsigned long long* __restrict__ slots, const Ctl* __restrict__ ctl,
                                                      const MgPtrs* __restrict__ pp) {
     if (ctl->done) return;
     const MgLevel L = mg_resolve(Larg, pp);
-    const size_t n = (size_t)((L.nr + 1) / 2) * ((L.nz + 1) / 2);
+    const IDX n = (IDX)((L.nr + 1) / 2) * (IDX)((L.nz + 1) / 2);
     unsigned long long kr = 0ull, kp = 0ull;
-    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
-        mg_residual_block<RESTRICT, MAXIMA, size_t>(L, idx, fc, ec, kr, kp);
+    for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x)
+        mg_residual_block<RESTRICT, MAXIMA, IDX>(L, idx, fc, ec, kr, kp);
     if (MAXIMA) {
         kr = warp_max_key(kr);
         kp = warp_max_key(kp);
         if ((threadIdx.x & 31) == 0) {
+            atomicMax(slots, kr);
+            atomicMax(slots + 1, kp);
+        }
+    }
+}
+
+// M8: max|res| and max|phi| of a level, one thread per CELL (coalesced rows; the 2 x 2 mapping above is only needed
+// where the restriction wants the four residuals in one thread)
+template <typename IDX>
+__global__ void __launch_bounds__(256) k_mg_resmax(const MgLevel Larg, unsigned long long* __restrict__ slots,
+                                                   const Ctl* __restrict__ ctl, const MgPtrs* __restrict__ pp) {
+    if (ctl->done) return;
+    const MgLevel L = mg_resolve(Larg, pp);
+    const IDX n = (IDX)L.nr * (IDX)L.nz;
+    unsigned long long kr = 0ull, kp = 0ull;
+    for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x) {
+        const int j = (int)(idx / (IDX)L.nr), i = (int)(idx - (IDX)j * (IDX)L.nr);
+        const double pC = L.phi[idx];
+        double diag, w;
+        const double t = mg_apply_at(L, i, j, pC, diag, w);
+        const double r = __dsub_rn(__dmul_rn(L.scale, L.src[idx]), t);
+        const unsigned long long a1 = abs_key(r), a2 = abs_key(pC);
+        kr = a1 > kr ? a1 : kr;
+        kp = a2 > kp ? a2 : kp;
+    }
+    // warp -> CTA -> ONE atomic pair per CTA (thousands of warps hitting the same two words serialise in L2)
+    __shared__ unsigned long long sk[2][8];
+    kr = warp_max_key(kr);
+    kp = warp_max_key(kp);
+    if ((threadIdx.x & 31) == 0) { sk[0][threadIdx.x >> 5] = kr; sk[1][threadIdx.x >> 5] = kp; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const unsigned nw = blockDim.x >> 5;
+        kr = warp_max_key(threadIdx.x < nw ? sk[0][threadIdx.x] : 0ull);
+        kp = warp_max_key(threadIdx.x < nw ? sk[1][threadIdx.x] : 0ull);
+        if (threadIdx.x == 0) {
             atomicMax(slots, kr);
             atomicMax(slots + 1, kp);
         }
@@ -169,13 +205,14 @@ __device__ __forceinline__ void mg_prolong_cell(const MgLevel& Lc, double* phi_f
 }
 
 // one thread per fine cell
+template <typename IDX>
 __global__ void __launch_bounds__(256) k_mg_prolong_add(const MgLevel Lc, double* phi_f, int nr_f, int nz_f,
                                                         const Ctl* __restrict__ ctl, const MgPtrs* __restrict__ pp) {
     if (ctl->done) return;
     if (phi_f == nullptr) phi_f = pp->phi;           // level 0
-    const size_t n = (size_t)nr_f * nz_f;
-    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x)
-        mg_prolong_cell<size_t>(Lc, phi_f, nr_f, idx);
+    const IDX n = (IDX)nr_f * (IDX)nz_f;
+    for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x)
+        mg_prolong_cell<IDX>(Lc, phi_f, nr_f, idx);
 }
 
 // The tail of the V-cycle -- every level small enough for ONE CTA (<= kMgTailCells cells) down to the coarsest and back

@@ -916,11 +916,20 @@ MgLevel mg_level(const sn_poisson* h, int l, const double* rho, double* phi) {
 
 inline int mg_blocks(size_t n, int num_sms) { return (int)std::max<size_t>(1, std::min<size_t>((n + 255) / 256, (size_t)num_sms * 16)); }
 
+// 32-bit cell indices (a 64-bit division per cell is a third of these kernels' instructions) where they suffice
+inline bool mg_small(int nr, int nz) { return (long long)nr * nz < (1ll << 30); }
+
 int mg_smooth(sn_poisson* h, const MgLevel& L, int nsweeps, cudaStream_t st) {
     const int blocks = mg_blocks((size_t)((L.nr + 1) / 2) * L.nz, h->num_sms);
+    const bool small = mg_small(L.nr, L.nz);
     for (int k = 0; k < nsweeps; ++k) {
-        k_mg_halfsweep<0><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
-        k_mg_halfsweep<1><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
+        if (small) {
+            k_mg_halfsweep<0, unsigned><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
+            k_mg_halfsweep<1, unsigned><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
+        } else {
+            k_mg_halfsweep<0, size_t><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
+            k_mg_halfsweep<1, size_t><<<blocks, 256, 0, st>>>(L, h->d_ctl, h->mg.d_ptrs);
+        }
         h->st_launches += 2;
     }
     CU_TRY(cudaGetLastError());
@@ -941,7 +950,10 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
     for (int l = 0; l < top; ++l) {                                  // down
         if (int rc = mg_smooth(h, Ls[l], nu1, st)) return rc;
         const size_t nc = (size_t)W.nr[l + 1] * W.nz[l + 1];
-        k_mg_residual<true, false><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
+        if (mg_small(W.nr[l], W.nz[l]))
+            k_mg_residual<true, false, unsigned><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
+        else
+            k_mg_residual<true, false, size_t><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
     }
     if (k < W.nlev) {
@@ -956,12 +968,16 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
     }
     for (int l = top - 1; l >= 0; --l) {                             // up
         const size_t nf = (size_t)W.nr[l] * W.nz[l];
-        k_mg_prolong_add<<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
+        if (mg_small(W.nr[l], W.nz[l]))
+            k_mg_prolong_add<unsigned><<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
+        else
+            k_mg_prolong_add<size_t><<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
         if (int rc = mg_smooth(h, Ls[l], nu2, st)) return rc;
     }
-    const size_t nb = (size_t)((W.nr[0] + 1) / 2) * ((W.nz[0] + 1) / 2);
-    k_mg_residual<false, true><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], nullptr, nullptr, W.slots, h->d_ctl, W.d_ptrs);
+    const size_t nb = (size_t)W.nr[0] * W.nz[0];
+    if (mg_small(W.nr[0], W.nz[0])) k_mg_resmax<unsigned><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], W.slots, h->d_ctl, W.d_ptrs);
+    else k_mg_resmax<size_t><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], W.slots, h->d_ctl, W.d_ptrs);
     k_mg_decide<<<1, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, max_cycles, h->d_hist);
     h->st_launches += 2;
     CU_TRY(cudaGetLastError());

@@ -3,7 +3,7 @@
 // reconstruction of both split fluxes), PAPER.md:402 (gamma-law EOS, Courant number 0.5); readings W1..W9 in DESIGN.md.
 // Kernels:
 //   k_weno_speeds   alpha_r, alpha_z = max over all cells of |v| + c_s: registers -> warp REDUX on the order-preserving
-//                   bit pattern -> one atomicMax per warp (exact, order-independent);
+//                   bit pattern -> shared memory -> one atomicMax per CTA (exact, order-independent);
 //   k_weno_dt       dt = cfl / (alpha_r/dr + alpha_z/dz) on the device, so that a Runge-Kutta step needs no host round trip;
 //   k_weno_rhs      one CTA per 32 x 8 tile: the tile plus its 3-cell halo (ghost cells by index mapping) goes to shared
 //                   memory once together with p, v_r, v_z; every thread reconstructs the fluxes through the east and the
@@ -115,11 +115,19 @@ __global__ void __launch_bounds__(256) k_weno_speeds(WenoGeom g, const double* _
         kr = br > kr ? br : kr;
         kz = bz > kz ? bz : kz;
     }
+    // warp -> CTA -> one atomic pair per CTA (warps hitting the same two words serialise in L2)
+    __shared__ unsigned long long sk[2][8];
     kr = warp_max_u64(kr);
     kz = warp_max_u64(kz);
-    if ((threadIdx.x & 31) == 0) {
-        atomicMax(alpha, kr);
-        atomicMax(alpha + 1, kz);
+    if ((threadIdx.x & 31) == 0) { sk[0][threadIdx.x >> 5] = kr; sk[1][threadIdx.x >> 5] = kz; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        kr = warp_max_u64(threadIdx.x < 8 ? sk[0][threadIdx.x] : 0ull);
+        kz = warp_max_u64(threadIdx.x < 8 ? sk[1][threadIdx.x] : 0ull);
+        if (threadIdx.x == 0) {
+            atomicMax(alpha, kr);
+            atomicMax(alpha + 1, kz);
+        }
     }
 }
 
