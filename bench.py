@@ -471,6 +471,21 @@ def next_rows(torch, P, flush):
                      "e2e": {"value": e2e_ms, "unit": "ms", "api": "sn_poisson_solve_mg_host",
                              "h2d_bytes_per_step": 2 * w0.rho.nbytes, "d2h_bytes_per_step": w0.rho.nbytes}})
         sv.close()
+    # the [CFG 4a] batch through the multigrid variant (one call, every kernel covers all 64 members)
+    lab, mem = make_workload("cfg4a")
+    w0 = mem[0]
+    sv = P.PoissonSolver.for_workload(w0)
+    rho = torch.from_numpy(np.stack([m.rho for m in mem])).cuda()
+    phi = torch.zeros_like(rho)
+    res = []
+    ms = timed(lambda: (phi.zero_(), res.clear(), res.extend(sv.solve_mg(rho, phi, w0.tol, 60))), 3)
+    zero_ms = timed(lambda: phi.zero_(), 3)
+    rows.append({"workload": "mg_cfg4a", "label": "NEXT-4: multigrid V(1,1) on " + lab, "metric": "time_to_residual_ms",
+                 "value": ms - zero_ms, "cycles": [r.sweeps for r in res][:8], "max_cycles": max(r.sweeps for r in res),
+                 "higher_is_better": False, "gpu_launches_per_step": int(sv.stat("launches")),
+                 "e2e": {"value": None, "api": None}})
+    sv.close()
+    del rho, phi
     # the [CFG 3] workload itself (warm-started sequence, here its first 20 solves) through the multigrid variant
     seq = W.cfg3(nsteps=20)
     w0 = seq.first

@@ -212,7 +212,12 @@ const char* sn_poisson_version(void);
  * Synchronises `stream`. */
 sn_poisson_result sn_poisson_solve_mg(sn_poisson* h, const double* rho, double* phi_inout, double tol, int max_cycles,
                                       void* stream);
-/* The same with HOST buffers (H2D of rho and phi, D2H of phi inside the call). */
+/* nbatch independent solves in one call (layout and `out` as for sn_poisson_solve_batch): every kernel of a cycle covers
+ * all members, each member stops on its own ratio, the call returns when the last one has.  Member b's result is the
+ * one sn_poisson_solve_mg gives for it alone, bit for bit.  Returns 0, or < 0 as sn_poisson_solve_batch. */
+int sn_poisson_solve_mg_batch(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double tol, int max_cycles,
+                              void* stream, sn_poisson_result* out);
+/* The same as sn_poisson_solve_mg with HOST buffers (H2D of rho and phi, D2H of phi inside the call). */
 sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
                                            int max_cycles, void* stream);
 

@@ -16,7 +16,7 @@ LIB_PATH = os.environ.get("SN_POISSON_LIB") or os.path.join(_HERE, "libsn_poisso
 EXPORTS = (
     "sn_poisson_create", "sn_poisson_solve", "sn_poisson_solve_host", "sn_poisson_solve_batch",
     "sn_poisson_solve_batch_host", "sn_poisson_solve_sequence_host", "sn_poisson_probe_l2",
-    "sn_poisson_set_stop_rule", "sn_poisson_solve_gravity", "sn_poisson_solve_mg", "sn_poisson_solve_mg_host",
+    "sn_poisson_set_stop_rule", "sn_poisson_solve_gravity", "sn_poisson_solve_mg", "sn_poisson_solve_mg_host", "sn_poisson_solve_mg_batch",
     "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
     "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
@@ -70,6 +70,8 @@ def load():
     lib.sn_poisson_solve_host.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
     lib.sn_poisson_solve_mg.restype = sn_poisson_result
     lib.sn_poisson_solve_mg.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
+    lib.sn_poisson_solve_mg_batch.restype = C.c_int
+    lib.sn_poisson_solve_mg_batch.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, C.c_int, _vp, C.POINTER(sn_poisson_result)]
     lib.sn_poisson_solve_mg_host.restype = sn_poisson_result
     lib.sn_poisson_solve_mg_host.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
     lib.sn_poisson_solve_batch.restype = C.c_int
@@ -179,6 +181,15 @@ def sn_poisson_solve_host(h, rho_ptr, phi_ptr, tol, max_sweeps, stream=0) -> sn_
 def sn_poisson_solve_mg(h, rho_ptr, phi_ptr, tol, max_cycles, stream=0) -> sn_poisson_result:
     """Multigrid variant (NEXT-4); DEVICE addresses; `sweeps` of the result = V-cycles."""
     return load().sn_poisson_solve_mg(h, rho_ptr, phi_ptr, float(tol), int(max_cycles), stream or None)
+
+
+def sn_poisson_solve_mg_batch(h, nbatch, rho_ptr, phi_ptr, tol, max_cycles, stream=0):
+    """Multigrid variant, nbatch independent solves; returns a list of sn_poisson_result."""
+    out = (sn_poisson_result * int(nbatch))()
+    rc = load().sn_poisson_solve_mg_batch(h, int(nbatch), rho_ptr, phi_ptr, float(tol), int(max_cycles), stream or None, out)
+    if rc != 0:
+        raise SnPoissonError(f"sn_poisson_solve_mg_batch failed ({rc}): " + sn_poisson_last_error())
+    return list(out)
 
 
 def sn_poisson_solve_mg_host(h, rho_ptr, phi_ptr, tol, max_cycles, stream=0) -> sn_poisson_result:

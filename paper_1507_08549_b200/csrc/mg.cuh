@@ -31,8 +31,17 @@ struct MgPtrs {
     const double* rho;
     double* phi;
 };
-__device__ __forceinline__ MgLevel mg_resolve(MgLevel L, const MgPtrs* __restrict__ pp) {
+// Batches: member m of a batch works on the m-th slice of every array (the members' slices are contiguous).
+__device__ __forceinline__ MgLevel mg_resolve(MgLevel L, const MgPtrs* __restrict__ pp, int member = 0) {
     if (L.phi == nullptr) { L.phi = pp->phi; L.src = pp->rho; }
+    const size_t off = (size_t)member * L.nr * L.nz;
+    L.phi += off;
+    L.src += off;
+    if (L.bE) {
+        L.bE += (size_t)member * L.nz;
+        L.bN += (size_t)member * L.nr;
+        if (L.bS) L.bS += (size_t)member * L.nr;
+    }
     return L;
 }
 
@@ -75,8 +84,8 @@ __device__ __forceinline__ void mg_update_cell(const MgLevel& L, IDX idx, int co
 template <int COL, typename IDX>
 __global__ void __launch_bounds__(256) k_mg_halfsweep(const MgLevel Larg, const Ctl* __restrict__ ctl,
                                                       const MgPtrs* __restrict__ pp) {
-    if (ctl->done) return;               // a finished solve: cycles enqueued ahead of the host's poll do nothing
-    const MgLevel L = mg_resolve(Larg, pp);
+    if (ctl[blockIdx.y].done) return;    // a finished solve: cycles enqueued ahead of the host's poll do nothing
+    const MgLevel L = mg_resolve(Larg, pp, blockIdx.y);
     const IDX n = (IDX)((L.nr + 1) / 2) * (IDX)L.nz;
     for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x)
         mg_update_cell<IDX>(L, idx, COL);
@@ -123,9 +132,11 @@ template <bool RESTRICT, bool MAXIMA, typename IDX>
 __global__ void __launch_bounds__(256) k_mg_residual(const MgLevel Larg, double* __restrict__ fc, double* __restrict__ ec,
                                                      unsigned long long* __restrict__ slots, const Ctl* __restrict__ ctl,
                                                      const MgPtrs* __restrict__ pp) {
-    if (ctl->done) return;
-    const MgLevel L = mg_resolve(Larg, pp);
+    if (ctl[blockIdx.y].done) return;
+    const MgLevel L = mg_resolve(Larg, pp, blockIdx.y);
     const IDX n = (IDX)((L.nr + 1) / 2) * (IDX)((L.nz + 1) / 2);
+    if (RESTRICT) { fc += (size_t)blockIdx.y * n; ec += (size_t)blockIdx.y * n; }
+    if (MAXIMA) slots += 2 * blockIdx.y;
     unsigned long long kr = 0ull, kp = 0ull;
     for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x)
         mg_residual_block<RESTRICT, MAXIMA, IDX>(L, idx, fc, ec, kr, kp);
@@ -144,9 +155,10 @@ __global__ void __launch_bounds__(256) k_mg_residual(const MgLevel Larg, double*
 template <typename IDX>
 __global__ void __launch_bounds__(256) k_mg_resmax(const MgLevel Larg, unsigned long long* __restrict__ slots,
                                                    const Ctl* __restrict__ ctl, const MgPtrs* __restrict__ pp) {
-    if (ctl->done) return;
-    const MgLevel L = mg_resolve(Larg, pp);
+    if (ctl[blockIdx.y].done) return;
+    const MgLevel L = mg_resolve(Larg, pp, blockIdx.y);
     const IDX n = (IDX)L.nr * (IDX)L.nz;
+    slots += 2 * blockIdx.y;
     unsigned long long kr = 0ull, kp = 0ull;
     for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x) {
         const int j = (int)(idx / (IDX)L.nr), i = (int)(idx - (IDX)j * (IDX)L.nr);
@@ -206,10 +218,12 @@ __device__ __forceinline__ void mg_prolong_cell(const MgLevel& Lc, double* phi_f
 
 // one thread per fine cell
 template <typename IDX>
-__global__ void __launch_bounds__(256) k_mg_prolong_add(const MgLevel Lc, double* phi_f, int nr_f, int nz_f,
+__global__ void __launch_bounds__(256) k_mg_prolong_add(const MgLevel Lcarg, double* phi_f, int nr_f, int nz_f,
                                                         const Ctl* __restrict__ ctl, const MgPtrs* __restrict__ pp) {
-    if (ctl->done) return;
+    if (ctl[blockIdx.y].done) return;
     if (phi_f == nullptr) phi_f = pp->phi;           // level 0
+    phi_f += (size_t)blockIdx.y * nr_f * nz_f;
+    const MgLevel Lc = mg_resolve(Lcarg, pp, blockIdx.y);
     const IDX n = (IDX)nr_f * (IDX)nz_f;
     for (IDX idx = (IDX)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (IDX)gridDim.x * blockDim.x)
         mg_prolong_cell<IDX>(Lc, phi_f, nr_f, idx);
@@ -237,19 +251,20 @@ __global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __r
     extern __shared__ __align__(16) double mg_sm[];
     __shared__ MgLevel L[kMgMaxLevels];           // the levels with their arrays re-pointed to shared memory
     __shared__ double* fw[kMgMaxLevels];
-    if (ctl->done) return;
+    const int member = blockIdx.x;               // one CTA per batch member
+    if (ctl[member].done) return;
     {
         if (threadIdx.x == 0) {
             double* p = mg_sm;
             for (int l = 0; l < T.n; ++l) {
                 const size_t n = (size_t)T.L[l].nr * T.L[l].nz;
-                L[l] = T.L[l];
+                L[l] = l == 0 ? mg_resolve(T.L[0], pp, member) : T.L[l];       // level 0 of the grid keeps its (member's) ghosts
                 L[l].phi = p; fw[l] = p + n; L[l].src = fw[l];
                 p += 2 * n;
             }
         }
         __syncthreads();
-        const MgLevel G0 = mg_resolve(T.L[0], pp);
+        const MgLevel G0 = mg_resolve(T.L[0], pp, member);
         const size_t n0 = (size_t)T.L[0].nr * T.L[0].nz;
         for (size_t i = threadIdx.x; i < n0; i += blockDim.x) { L[0].phi[i] = G0.phi[i]; fw[0][i] = G0.src[i]; }
         __syncthreads();
@@ -286,15 +301,18 @@ __global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __r
         __syncthreads();
         smooth(L[l], T.nu2);
     }
-    double* out0 = mg_resolve(T.L[0], pp).phi;
+    double* out0 = mg_resolve(T.L[0], pp, member).phi;
     const size_t n0 = (size_t)T.L[0].nr * T.L[0].nz;
     for (size_t i = threadIdx.x; i < n0; i += blockDim.x) out0[i] = L[0].phi[i];
 }
 
 // M8: the stopping ratio of the cycle just finished; resets the maxima for the next one
-__global__ void k_mg_decide(Ctl* __restrict__ ctl, unsigned long long* __restrict__ slots, double D, double tol,
-                            int max_cycles, double* __restrict__ hist) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+__global__ void k_mg_decide(Ctl* __restrict__ ctl_all, unsigned long long* __restrict__ slots_all, double D, double tol,
+                            int max_cycles, double* __restrict__ hist_all, int hist_stride) {
+    if (threadIdx.x != 0) return;
+    Ctl* ctl = ctl_all + blockIdx.x;                       // one block per batch member
+    unsigned long long* slots = slots_all + 2 * blockIdx.x;
+    double* hist = hist_all + (size_t)blockIdx.x * hist_stride;
     if (ctl->done) return;
     const int cycle = ctl->sweeps + 1;
     const double R = stop_ratio(slots[0], slots[1], ctl->maxf, D);

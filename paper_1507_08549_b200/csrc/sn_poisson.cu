@@ -130,13 +130,16 @@ struct sn_poisson {
         unsigned long long* slots = nullptr;
         MgPtrs* d_ptrs = nullptr;         // the caller's rho / phi of the current solve, read by the level-0 kernels
         bool tail_attr = false;
+        int cap_batch = 0;                // members the per-level arrays hold
+        int nb = 1;                       // members of the current solve
         // one V-cycle captured as a CUDA graph (the cycle is ~15-27 short launches): valid for one (tol, max_cycles,
         // options) key -- the caller's rho / phi reach the kernels through d_ptrs --, re-captured when the key changes
         cudaGraphExec_t exec = nullptr;
         cudaStream_t st = nullptr;        // runs the cycles when the caller hands in the (uncapturable) legacy stream
         double nodes = 0;                 // kernel nodes per captured cycle
-        struct Key { double tol = 0; int max_cycles = -1, nu1 = 0, nu2 = 0, nc = 0; } key;
-        double* h_hist = nullptr;     // pinned: the last two ratios, for the host's chunk prediction
+        struct Key { double tol = 0; int max_cycles = -1, nu1 = 0, nu2 = 0, nc = 0, nb = 0, cap_sweeps = 0; } key;
+        double* h_hist = nullptr;     // pinned: the last two ratios of every member, for the host's chunk prediction
+        int hist_cap = 0;
     } mg;
     int opt_mg_nu1 = 1, opt_mg_nu2 = 1, opt_mg_nc = 12, opt_mg_graph = 1;
 
@@ -857,9 +860,21 @@ int mg_num_levels(int nr, int nz) {                                  // M1
     return n;
 }
 
-int ensure_mg(sn_poisson* h) {
-    if (h->mg.nlev) return 0;
+int ensure_mg(sn_poisson* h, int nbatch) {
     auto& W = h->mg;
+    if (W.nlev && nbatch > W.cap_batch) {        // grow the per-member arrays (the captured cycle holds their addresses)
+        if (W.exec) { cudaGraphExecDestroy(W.exec); W.exec = nullptr; }
+        for (int l = 1; l < W.nlev; ++l) {
+            cudaFree(W.phi[l]); cudaFree(W.f[l]);
+            W.phi[l] = W.f[l] = nullptr;
+            if (int rc = dev_alloc(&W.phi[l], (size_t)nbatch * W.nr[l] * W.nz[l])) return rc;
+            if (int rc = dev_alloc(&W.f[l], (size_t)nbatch * W.nr[l] * W.nz[l])) return rc;
+        }
+        cudaFree(W.slots); W.slots = nullptr;
+        if (int rc = dev_alloc(&W.slots, (size_t)2 * nbatch)) return rc;
+        W.cap_batch = nbatch;
+    }
+    if (W.nlev) return 0;
     const int nlev = std::min(mg_num_levels(h->nr, h->nz), kMgMaxLevels);
     W.nr.resize(nlev); W.nz.resize(nlev);
     W.cE.assign(nlev, nullptr); W.cW.assign(nlev, nullptr); W.phi.assign(nlev, nullptr); W.f.assign(nlev, nullptr);
@@ -878,11 +893,12 @@ int ensure_mg(sn_poisson* h) {
         CU_TRY(cudaMemcpy(W.cE[l], cE.data(), sizeof(double) * nr, cudaMemcpyHostToDevice));
         CU_TRY(cudaMemcpy(W.cW[l], cW.data(), sizeof(double) * nr, cudaMemcpyHostToDevice));
         if (l > 0) {
-            if (int rc = dev_alloc(&W.phi[l], (size_t)nr * nz)) return rc;
-            if (int rc = dev_alloc(&W.f[l], (size_t)nr * nz)) return rc;
+            if (int rc = dev_alloc(&W.phi[l], (size_t)nbatch * nr * nz)) return rc;
+            if (int rc = dev_alloc(&W.f[l], (size_t)nbatch * nr * nz)) return rc;
         }
     }
-    if (int rc = dev_alloc(&W.slots, (size_t)2)) return rc;
+    if (int rc = dev_alloc(&W.slots, (size_t)2 * nbatch)) return rc;
+    W.cap_batch = nbatch;
     if (int rc = dev_alloc(&W.d_ptrs, (size_t)1)) return rc;
     CU_TRY(cudaFuncSetAttribute(k_mg_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     W.tail_attr = true;
@@ -914,13 +930,16 @@ MgLevel mg_level(const sn_poisson* h, int l, const double* rho, double* phi) {
     return L;
 }
 
-inline int mg_blocks(size_t n, int num_sms) { return (int)std::max<size_t>(1, std::min<size_t>((n + 255) / 256, (size_t)num_sms * 16)); }
+// blocks per member: one thread per unit, at most 16 CTAs per SM over the whole batch
+inline int mg_blocks(size_t n, int num_sms, int nb = 1) {
+    return (int)std::max<size_t>(1, std::min<size_t>((n + 255) / 256, std::max<size_t>(1, (size_t)num_sms * 16 / nb)));
+}
 
 // 32-bit cell indices (a 64-bit division per cell is a third of these kernels' instructions) where they suffice
 inline bool mg_small(int nr, int nz) { return (long long)nr * nz < (1ll << 30); }
 
 int mg_smooth(sn_poisson* h, const MgLevel& L, int nsweeps, cudaStream_t st) {
-    const int blocks = mg_blocks((size_t)((L.nr + 1) / 2) * L.nz, h->num_sms);
+    const dim3 blocks(mg_blocks((size_t)((L.nr + 1) / 2) * L.nz, h->num_sms, h->mg.nb), h->mg.nb);
     const bool small = mg_small(L.nr, L.nz);
     for (int k = 0; k < nsweeps; ++k) {
         if (small) {
@@ -951,9 +970,9 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
         if (int rc = mg_smooth(h, Ls[l], nu1, st)) return rc;
         const size_t nc = (size_t)W.nr[l + 1] * W.nz[l + 1];
         if (mg_small(W.nr[l], W.nz[l]))
-            k_mg_residual<true, false, unsigned><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
+            k_mg_residual<true, false, unsigned><<<dim3(mg_blocks(nc, h->num_sms, W.nb), W.nb), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
         else
-            k_mg_residual<true, false, size_t><<<mg_blocks(nc, h->num_sms), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
+            k_mg_residual<true, false, size_t><<<dim3(mg_blocks(nc, h->num_sms, W.nb), W.nb), 256, 0, st>>>(Ls[l], W.f[l + 1], W.phi[l + 1], nullptr, h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
     }
     if (k < W.nlev) {
@@ -961,7 +980,7 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
         T.n = W.nlev - k; T.nu1 = nu1; T.nu2 = nu2; T.nc = h->opt_mg_nc;
         for (int l = k; l < W.nlev; ++l) T.L[l - k] = Ls[l];
         const size_t smem = sizeof(double) * mg_tail_smem_doubles(T);
-        k_mg_tail<<<1, 1024, smem, st>>>(T, h->d_ctl, W.d_ptrs);
+        k_mg_tail<<<W.nb, 1024, smem, st>>>(T, h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
     } else {                                                         // a coarsest level too large for one CTA
         if (int rc = mg_smooth(h, Ls[W.nlev - 1], W.nlev == 1 ? nu1 + nu2 : h->opt_mg_nc, st)) return rc;
@@ -969,16 +988,16 @@ int mg_cycle(sn_poisson* h, const double* rho, double* phi, double tol, int max_
     for (int l = top - 1; l >= 0; --l) {                             // up
         const size_t nf = (size_t)W.nr[l] * W.nz[l];
         if (mg_small(W.nr[l], W.nz[l]))
-            k_mg_prolong_add<unsigned><<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
+            k_mg_prolong_add<unsigned><<<dim3(mg_blocks(nf, h->num_sms, W.nb), W.nb), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
         else
-            k_mg_prolong_add<size_t><<<mg_blocks(nf, h->num_sms), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
+            k_mg_prolong_add<size_t><<<dim3(mg_blocks(nf, h->num_sms, W.nb), W.nb), 256, 0, st>>>(Ls[l + 1], Ls[l].phi, W.nr[l], W.nz[l], h->d_ctl, W.d_ptrs);
         h->st_launches += 1;
         if (int rc = mg_smooth(h, Ls[l], nu2, st)) return rc;
     }
     const size_t nb = (size_t)W.nr[0] * W.nz[0];
-    if (mg_small(W.nr[0], W.nz[0])) k_mg_resmax<unsigned><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], W.slots, h->d_ctl, W.d_ptrs);
-    else k_mg_resmax<size_t><<<mg_blocks(nb, h->num_sms), 256, 0, st>>>(Ls[0], W.slots, h->d_ctl, W.d_ptrs);
-    k_mg_decide<<<1, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, max_cycles, h->d_hist);
+    if (mg_small(W.nr[0], W.nz[0])) k_mg_resmax<unsigned><<<dim3(mg_blocks(nb, h->num_sms, W.nb), W.nb), 256, 0, st>>>(Ls[0], W.slots, h->d_ctl, W.d_ptrs);
+    else k_mg_resmax<size_t><<<dim3(mg_blocks(nb, h->num_sms, W.nb), W.nb), 256, 0, st>>>(Ls[0], W.slots, h->d_ctl, W.d_ptrs);
+    k_mg_decide<<<W.nb, 32, 0, st>>>(h->d_ctl, W.slots, Ls[0].D, tol, max_cycles, h->d_hist, h->cap_sweeps);
     h->st_launches += 2;
     CU_TRY(cudaGetLastError());
     return 0;
@@ -991,7 +1010,8 @@ int mg_launch_cycle(sn_poisson* h, const double* rho, double* phi, double tol, i
     if (!h->opt_mg_graph || st == nullptr || st == cudaStreamLegacy) return mg_cycle(h, rho, phi, tol, max_cycles, st);
     const auto& k = W.key;
     const bool same = W.exec && k.tol == tol && k.max_cycles == max_cycles &&
-                      k.nu1 == h->opt_mg_nu1 && k.nu2 == h->opt_mg_nu2 && k.nc == h->opt_mg_nc;
+                      k.nu1 == h->opt_mg_nu1 && k.nu2 == h->opt_mg_nu2 && k.nc == h->opt_mg_nc && k.nb == W.nb &&
+                      k.cap_sweeps == h->cap_sweeps;
     if (!same) {
         if (W.exec) { cudaGraphExecDestroy(W.exec); W.exec = nullptr; }
         const double launches_before = h->st_launches;
@@ -1018,50 +1038,60 @@ int mg_launch_cycle(sn_poisson* h, const double* rho, double* phi, double tol, i
             return mg_cycle(h, rho, phi, tol, max_cycles, st);
         }
         W.key.tol = tol; W.key.max_cycles = max_cycles;
-        W.key.nu1 = h->opt_mg_nu1; W.key.nu2 = h->opt_mg_nu2; W.key.nc = h->opt_mg_nc;
+        W.key.nu1 = h->opt_mg_nu1; W.key.nu2 = h->opt_mg_nu2; W.key.nc = h->opt_mg_nc; W.key.nb = W.nb;
+        W.key.cap_sweeps = h->cap_sweeps;
     }
     CU_TRY(cudaGraphLaunch(W.exec, st));
     h->st_launches += W.nodes;            // kernels of mine that run inside the graph
     return 0;
 }
 
-int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int max_cycles, cudaStream_t st,
+int solve_mg_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double tol, int max_cycles, cudaStream_t st,
                   sn_poisson_result* out, const HostIO* io = nullptr) {
     CU_TRY(cudaSetDevice(h->device));
-    if (int rc = ensure_ws(h, 1, max_cycles)) return rc;
-    if (int rc = ensure_mg(h)) return rc;
+    if (int rc = ensure_ws(h, nbatch, max_cycles)) return rc;
+    if (int rc = ensure_mg(h, nbatch)) return rc;
+    h->mg.nb = nbatch;
     const Geom g = make_geom(h, tol);
     h->st_launches = 0; h->st_aux_launches = 0;
     h->st_path = 4; h->st_halo = 0; h->st_ds = 0; h->st_ring = 0; h->st_redund = 1;
-    h->st_ctas = 0; h->st_tile_w = h->nr; h->st_tile_h = h->nz; h->st_tblock = 0; h->st_shape = -1; h->st_group = 1;
+    h->st_ctas = 0; h->st_tile_w = h->nr; h->st_tile_h = h->nz; h->st_tblock = 0; h->st_shape = -1; h->st_group = nbatch;
     CU_TRY(cudaEventRecord(h->ev_t[0], st));
-    CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), st));
-    CU_TRY(cudaMemsetAsync(h->mg.slots, 0, 2 * sizeof(unsigned long long), st));
+    CU_TRY(cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl) * nbatch, st));
+    CU_TRY(cudaMemsetAsync(h->mg.slots, 0, 2 * sizeof(unsigned long long) * nbatch, st));
     {
         const MgPtrs hp = {rho, phi};
         CU_TRY(cudaMemcpyAsync(h->mg.d_ptrs, &hp, sizeof hp, cudaMemcpyHostToDevice, st));     // pageable: staged before return
     }
-    if (int rc = launch_moments(h, g, 1, rho, st)) return rc;         // a-1 (+ max|4 pi rho|), a-1b as in the SOR path
+    if (int rc = launch_moments(h, g, nbatch, rho, st)) return rc;    // a-1 (+ max|4 pi rho|), a-1b as in the SOR path
     h->st_launches += 1; h->st_aux_launches += 1;
     if (!h->user_boundary) {
-        k_boundary<<<dim3(1, boundary_slices(h)), 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN, h->d_bS, 0);
+        k_boundary<<<dim3(nbatch, boundary_slices(h)), 256, 0, st>>>(g, h->L0, h->NL, h->mom_blocks, h->d_partial, h->d_M, h->d_bE, h->d_bN, h->d_bS, 0);
         CU_TRY(cudaGetLastError());
         h->st_launches += 1; h->st_aux_launches += 1;
     }
-    h->last_nbatch = h->user_boundary ? h->cap_batch : 1;
+    h->last_nbatch = h->user_boundary ? h->cap_batch : nbatch;
     CU_TRY(cudaEventRecord(h->ev_t[1], st));
     if (io && io->wait_before_relax) CU_TRY(cudaStreamWaitEvent(st, io->wait_before_relax, 0));
     if (max_cycles == 0) {
-        h->h_ctl[0] = Ctl();
-        h->h_ctl[0].done = 1; h->h_ctl[0].status = tol > 0.0 ? 1 : 0;
+        for (int b = 0; b < nbatch; ++b) {
+            h->h_ctl[b] = Ctl();
+            h->h_ctl[b].done = 1; h->h_ctl[b].status = tol > 0.0 ? 1 : 0;
+        }
     }
-    // The decision of a cycle is taken on the device (k_mg_decide, M8); once `done` is set every later kernel of the
-    // variant returns at once, so cycles enqueued ahead neither touch phi nor cost more than their launches.  A host
-    // round trip costs about as much as a whole cycle of a small grid, so the host enqueues cycles in chunks: two
-    // first, then as many as the measured contraction per cycle predicts are still needed (a V-cycle contracts at a
-    // nearly constant rate), and looks at the decision only between chunks.  tol <= 0: all cycles at once.
+    // The decision of a cycle is taken on the device (k_mg_decide, M8), per member; once `done` is set every later
+    // kernel of the variant returns at once for that member, so cycles enqueued ahead neither touch its phi nor cost more
+    // than their launches.  A host round trip costs about as much as a whole cycle of a small grid, so the host enqueues
+    // cycles in chunks: two first, then as many as the measured contraction per cycle predicts the slowest member
+    // still needs (a V-cycle contracts at a nearly constant rate), and looks at the decisions only between chunks.
+    // tol <= 0: all cycles at once.
     if (max_cycles > 0) {
-        if (!h->mg.h_hist) CU_TRY(cudaMallocHost((void**)&h->mg.h_hist, 2 * sizeof(double)));
+        if (h->mg.hist_cap < nbatch) {
+            if (h->mg.h_hist) cudaFreeHost(h->mg.h_hist);
+            h->mg.h_hist = nullptr; h->mg.hist_cap = 0;
+            CU_TRY(cudaMallocHost((void**)&h->mg.h_hist, 2 * sizeof(double) * nbatch));
+            h->mg.hist_cap = nbatch;
+        }
         // The legacy default stream cannot be captured: the cycles then run on a stream of the handle, ordered after
         // the caller's stream here and before it again below.
         cudaStream_t caller = st;
@@ -1077,14 +1107,23 @@ int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int
             for (int c = 0; c < chunk; ++c)
                 if (int rc = mg_launch_cycle(h, rho, phi, tol, max_cycles, st)) return rc;
             enq += chunk;
-            CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
-            if (enq >= 2) CU_TRY(cudaMemcpyAsync(h->mg.h_hist, h->d_hist + (enq - 2), 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CU_TRY(cudaMemcpyAsync(h->h_ctl, h->d_ctl, sizeof(Ctl) * nbatch, cudaMemcpyDeviceToHost, st));
+            if (enq >= 2)
+                CU_TRY(cudaMemcpy2DAsync(h->mg.h_hist, 2 * sizeof(double), h->d_hist + (enq - 2), sizeof(double) * h->cap_sweeps,
+                                         2 * sizeof(double), nbatch, cudaMemcpyDeviceToHost, st));
             CU_TRY(cudaStreamSynchronize(st));
-            if (h->h_ctl[0].done || enq >= max_cycles) break;
+            bool all_done = true;
+            for (int b = 0; b < nbatch; ++b) all_done = all_done && h->h_ctl[b].done;
+            if (all_done || enq >= max_cycles) break;
             chunk = 1;
-            if (enq >= 2 && h->mg.h_hist[0] > 0.0 && h->mg.h_hist[1] > 0.0) {
-                const double rate = std::min(0.5, std::max(0.02, h->mg.h_hist[1] / h->mg.h_hist[0]));
-                const double need = std::ceil(std::log(tol / h->mg.h_hist[1]) / std::log(rate));
+            if (enq >= 2) {
+                double need = 1.0;
+                for (int b = 0; b < nbatch; ++b) {
+                    const double r0 = h->mg.h_hist[2 * b], r1 = h->mg.h_hist[2 * b + 1];
+                    if (h->h_ctl[b].done || !(r0 > 0.0) || !(r1 > 0.0)) continue;      // (a finished member's slots hold older cycles)
+                    const double rate = std::min(0.5, std::max(0.02, r1 / r0));
+                    need = std::max(need, std::ceil(std::log(tol / r1) / std::log(rate)));
+                }
                 chunk = (int)std::min(16.0, std::max(1.0, need));
             }
             chunk = std::min(chunk, max_cycles - enq);
@@ -1103,10 +1142,12 @@ int solve_mg_impl(sn_poisson* h, const double* rho, double* phi, double tol, int
     h->st_setup_ms = ms;
     CU_TRY(cudaEventElapsedTime(&ms, h->ev_t[1], h->ev_t[2]));
     h->st_sweep_ms = ms;
-    out->sweeps = h->h_ctl[0].sweeps;
-    out->status = h->h_ctl[0].status;
-    out->residual = h->h_ctl[0].residual;
-    h->last_sweeps0 = out->sweeps;
+    for (int b = 0; b < nbatch; ++b) {
+        out[b].sweeps = h->h_ctl[b].sweeps;
+        out[b].status = h->h_ctl[b].status;
+        out[b].residual = h->h_ctl[b].residual;
+    }
+    h->last_sweeps0 = out[0].sweeps;
     return 0;
 }
 
@@ -1224,9 +1265,18 @@ sn_poisson_result sn_poisson_solve_mg(sn_poisson* h, const double* rho, double* 
     sn_poisson_result r = {0, -1, 0.0};
     if (!check_solve_args(h, rho, phi_inout, tol, max_cycles)) return r;
     sn_poisson_result out = {0, 0, 0.0};
-    const int rc = solve_mg_impl(h, rho, phi_inout, tol, max_cycles, (cudaStream_t)stream, &out);
+    const int rc = solve_mg_impl(h, 1, rho, phi_inout, tol, max_cycles, (cudaStream_t)stream, &out);
     if (rc) { r.status = rc; return r; }
     return out;
+}
+
+int sn_poisson_solve_mg_batch(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double tol, int max_cycles,
+                              void* stream, sn_poisson_result* out) {
+    g_err.clear();
+    if (nbatch < 1 || !out) { set_err("nbatch < 1 or NULL out"); return -1; }
+    if (nbatch > 65535) { set_err("nbatch > 65535"); return -1; }
+    if (!check_solve_args(h, rho, phi_inout, tol, max_cycles, nbatch)) return -1;
+    return solve_mg_impl(h, nbatch, rho, phi_inout, tol, max_cycles, (cudaStream_t)stream, out);
 }
 
 sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
@@ -1250,7 +1300,7 @@ sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host
     io.wait_before_relax = h->ev_io[1];
     io.d2h_dst = phi_inout_host; io.d2h_src = h->d_phi_stage; io.d2h_bytes = bytes;
     sn_poisson_result out = {0, 0, 0.0};
-    const int rc = solve_mg_impl(h, h->d_rho_stage, h->d_phi_stage, tol, max_cycles, st, &out, &io);
+    const int rc = solve_mg_impl(h, 1, h->d_rho_stage, h->d_phi_stage, tol, max_cycles, st, &out, &io);
     if (rc) return fail(rc);
     return out;
 }

@@ -69,6 +69,13 @@ class PoissonSolver:
         import torch
         self._check(rho)
         self._check(phi)
+        if rho.dim() == 3:
+            if rho.shape != phi.shape or tuple(rho.shape[1:]) != (self.nz, self.nr):
+                raise ValueError("shape mismatch")
+            res = B.sn_poisson_solve_mg_batch(self.h, rho.shape[0], rho.data_ptr(), phi.data_ptr(), tol, max_cycles,
+                                              torch.cuda.current_stream().cuda_stream)
+            self._raise_if_failed(res, "sn_poisson_solve_mg_batch")
+            return res
         if tuple(rho.shape) != (self.nz, self.nr) or rho.shape != phi.shape:
             raise ValueError("shape mismatch")
         r = B.sn_poisson_solve_mg(self.h, rho.data_ptr(), phi.data_ptr(), tol, max_cycles,

@@ -126,3 +126,52 @@ def test_warm_start_host_entry_and_errors(P, torch_cuda, oracle):
     with pytest.raises(P.SnPoissonError):
         s.solve_mg(rho, p, w.tol, 5)                                 # status -3
     s.close()
+
+
+def test_batch_members_equal_single_solves_and_the_oracle(P, torch_cuda, oracle):
+    """sn_poisson_solve_mg_batch: members with different convergence histories in one call; each member's result is the
+    single-solve result bit for bit, and the oracle's within the north_star tolerance with the same cycle count."""
+    torch = torch_cuda
+    members = [W.cfg4a_member(b, 128) for b in (0, 1, 2, 3, 4)]
+    w0 = members[0]
+    rho = torch.from_numpy(np.stack([m.rho for m in members])).cuda()
+    phi = torch.zeros_like(rho)
+    s = P.PoissonSolver.for_workload(w0)
+    res = s.solve_mg(rho, phi, w0.tol, 60)
+    got = phi.cpu().numpy()
+    for b, m in enumerate(members):
+        ref = oracle.mg_solve_workload(m)
+        assert res[b].status == 0 and res[b].sweeps == ref["cycles"], (b, res[b], ref["cycles"])
+        assert np.abs(got[b] - ref["phi"]).max() <= 1e-11 * np.abs(ref["phi"]).max()
+        one = torch.zeros_like(rho[b])
+        r1 = s.solve_mg(rho[b].contiguous(), one, w0.tol, 60)
+        assert r1.sweeps == res[b].sweeps and r1.residual == res[b].residual
+        assert np.array_equal(one.cpu().numpy(), got[b])
+    # a member that needs no work next to ones that do: warm start of member 2 only
+    phi2 = torch.zeros_like(rho)
+    phi2[2] = phi[2]
+    res2 = s.solve_mg(rho, phi2, w0.tol, 60)
+    assert res2[2].sweeps == 1 and [r.sweeps for i, r in enumerate(res2) if i != 2] == [r.sweeps for i, r in enumerate(res) if i != 2]
+    assert np.array_equal(phi2.cpu().numpy()[[0, 1, 3, 4]], got[[0, 1, 3, 4]])
+    # fixed cycles, max_cycles reached
+    phi3 = torch.zeros_like(rho)
+    res3 = s.solve_mg(rho, phi3, w0.tol, 3)
+    assert all(r.sweeps == 3 and r.status == 1 for r in res3)
+    s.close()
+
+
+def test_batch_full_size_cfg4a(P, torch_cuda, oracle):
+    """All 64 members of [CFG 4a] (512 x 512) in one multigrid call against 64 oracle solves."""
+    torch = torch_cuda
+    members = W.cfg4a(64)
+    w0 = members[0]
+    rho = torch.from_numpy(np.stack([m.rho for m in members])).cuda()
+    phi = torch.zeros_like(rho)
+    s = P.PoissonSolver.for_workload(w0)
+    res = s.solve_mg(rho, phi, w0.tol, 60)
+    got = phi.cpu().numpy()
+    for b, m in enumerate(members):
+        ref = oracle.mg_solve_workload(m)
+        assert res[b].status == 0 and res[b].sweeps == ref["cycles"], (b, res[b], ref["cycles"])
+        assert np.abs(got[b] - ref["phi"]).max() <= 1e-11 * np.abs(ref["phi"]).max()
+    s.close()
