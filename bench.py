@@ -460,8 +460,9 @@ def next_rows(torch, P, flush):
         ms = timed(lambda: (phi.zero_(), res.append(sv.solve_mg(rho, phi, w0.tol, 60))), 5)
         zero_ms = timed(lambda: phi.zero_(), 5)
         launches = int(sv.stat("launches"))
-        phi_h = np.zeros_like(w0.rho)
-        e2e_ms = wall(lambda: (phi_h.fill(0.0), sv.solve_mg_host(w0.rho, phi_h, w0.tol, 60)), 3)
+        rho_pin = torch.from_numpy(w0.rho).pin_memory()
+        phi_pin = torch.zeros(w0.rho.shape, dtype=torch.float64).pin_memory()
+        e2e_ms = wall(lambda: (phi_pin.zero_(), sv.solve_mg_host(rho_pin.numpy(), phi_pin.numpy(), w0.tol, 60)), 3)
         r = res[-1]
         # cells touched per V(1,1) cycle on level 0: 2 sweeps + 2 residual passes + 1 prolongation; x 4/3 for the coarse levels
         rows.append({"workload": "mg_" + name, "label": "NEXT-4: multigrid V(1,1) on " + lab, "metric": "time_to_residual_ms",
