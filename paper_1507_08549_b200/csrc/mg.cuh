@@ -53,10 +53,22 @@ __device__ __forceinline__ double mg_apply_at(const MgLevel& L, int i, int j, do
     diag = mirror_row ? L.D0 : L.D;
     w = mirror_row ? L.wD0 : L.wD;
     const double ghost = -__dmul_rn(L.beta, pC);
-    const double pE = (i + 1 < L.nr) ? L.phi[c + 1] : (L.bE ? L.bE[j] : ghost);
-    const double pW = (i > 0) ? L.phi[c - 1] : 0.0;
-    const double pN = (j + 1 < L.nz) ? L.phi[c + L.nr] : (L.bN ? L.bN[i] : ghost);
-    const double pS = (j > 0) ? L.phi[c - L.nr] : (L.symmetry == 1 ? 0.0 : (L.bS ? L.bS[i] : ghost));
+    // the four neighbours are fetched UNCONDITIONALLY from clamped (always valid) positions and selected afterwards: as
+    // conditional loads the lanes of a boundary warp -- every warp of the small levels -- take them one branch after the
+    // other, each with its own load latency (measured: a warp-wide update of a 4 x 4 level took 720 clocks)
+    const int ie = i + 1 < L.nr ? 1 : 0, iw = i > 0 ? 1 : 0;
+    const int jn = j + 1 < L.nz ? L.nr : 0, js = j > 0 ? L.nr : 0;
+    const double vE = L.phi[c + ie], vW = L.phi[c - iw], vN = L.phi[c + jn], vS = L.phi[c - js];
+    double gE = ghost, gN = ghost, gS = ghost;
+    if (L.bE) {                                   // level 0: the multipole ghosts (uniform branch)
+        if (!ie) gE = L.bE[j];
+        if (!jn) gN = L.bN[i];
+        if (!js && L.bS) gS = L.bS[i];
+    }
+    const double pE = ie ? vE : gE;
+    const double pW = iw ? vW : 0.0;
+    const double pN = jn ? vN : gN;
+    const double pS = js ? vS : (L.symmetry == 1 ? 0.0 : gS);
     double t = __dmul_rn(L.cE[i], pE);
     t = __fma_rn(L.cW[i], pW, t);
     t = __fma_rn(L.iz2, pN, t);
@@ -243,7 +255,7 @@ struct MgTail {
 // doubles of dynamic shared memory the tail needs: phi and f of every level
 inline size_t mg_tail_smem_doubles(const MgTail& T) {
     size_t d = 0;
-    for (int l = 0; l < T.n; ++l) d += 2 * (size_t)T.L[l].nr * T.L[l].nz;
+    for (int l = 0; l < T.n; ++l) d += 2 * (size_t)T.L[l].nr * T.L[l].nz + 2 * (size_t)T.L[l].nr;      // phi, f, cE, cW
     return d;
 }
 
@@ -251,6 +263,7 @@ __global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __r
     extern __shared__ __align__(16) double mg_sm[];
     __shared__ MgLevel L[kMgMaxLevels];           // the levels with their arrays re-pointed to shared memory
     __shared__ double* fw[kMgMaxLevels];
+    __shared__ double* cw[kMgMaxLevels];
     const int member = blockIdx.x;               // one CTA per batch member
     if (ctl[member].done) return;
     {
@@ -261,15 +274,26 @@ __global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __r
                 L[l] = l == 0 ? mg_resolve(T.L[0], pp, member) : T.L[l];       // level 0 of the grid keeps its (member's) ghosts
                 L[l].phi = p; fw[l] = p + n; L[l].src = fw[l];
                 p += 2 * n;
+                cw[l] = p;                        // the coefficient tables too: cE [nr], cW [nr]
+                p += 2 * T.L[l].nr;
             }
         }
         __syncthreads();
+        for (int l = 0; l < T.n; ++l) {
+            for (int i = threadIdx.x; i < T.L[l].nr; i += blockDim.x) { cw[l][i] = T.L[l].cE[i]; cw[l][T.L[l].nr + i] = T.L[l].cW[i]; }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0)
+            for (int l = 0; l < T.n; ++l) { L[l].cE = cw[l]; L[l].cW = cw[l] + T.L[l].nr; }
         const MgLevel G0 = mg_resolve(T.L[0], pp, member);
         const size_t n0 = (size_t)T.L[0].nr * T.L[0].nz;
         for (size_t i = threadIdx.x; i < n0; i += blockDim.x) { L[0].phi[i] = G0.phi[i]; fw[0][i] = G0.src[i]; }
         __syncthreads();
     }
-    auto smooth = [&](const MgLevel& Lv, int nsweeps) {
+    // (every phase works on a LOCAL copy of its level descriptor: read through the shared-memory struct, each field would
+    // be re-fetched after every store to phi, which may alias it as far as the compiler knows)
+    auto smooth = [&](const MgLevel& Lshared, int nsweeps) {
+        const MgLevel Lv = Lshared;
         const unsigned n = (unsigned)((Lv.nr + 1) / 2) * (unsigned)Lv.nz;
         if (n <= 32u) {                           // a level of <= 64 cells: one warp, warp barriers instead of CTA barriers
             if (threadIdx.x < 32u) {
@@ -290,14 +314,24 @@ __global__ void __launch_bounds__(1024) k_mg_tail(const MgTail T, const Ctl* __r
     for (int l = 0; l + 1 < T.n; ++l) {                              // down
         smooth(L[l], T.nu1);
         const unsigned nc = (unsigned)L[l + 1].nr * (unsigned)L[l + 1].nz;
-        for (unsigned idx = threadIdx.x; idx < nc; idx += blockDim.x)
-            mg_residual_block<true, false, unsigned>(L[l], idx, fw[l + 1], L[l + 1].phi, kr, kp);
+        {
+            const MgLevel Lf = L[l];
+            double* const fcw = fw[l + 1];
+            double* const ecw = L[l + 1].phi;
+            for (unsigned idx = threadIdx.x; idx < nc; idx += blockDim.x)
+                mg_residual_block<true, false, unsigned>(Lf, idx, fcw, ecw, kr, kp);
+        }
         __syncthreads();
     }
     smooth(L[T.n - 1], T.n == 1 ? T.nu1 + T.nu2 : T.nc);             // coarsest (a single-level grid: plain Gauss-Seidel)
     for (int l = T.n - 2; l >= 0; --l) {                             // up
         const unsigned nf = (unsigned)L[l].nr * (unsigned)L[l].nz;
-        for (unsigned idx = threadIdx.x; idx < nf; idx += blockDim.x) mg_prolong_cell<unsigned>(L[l + 1], L[l].phi, L[l].nr, idx);
+        {
+            const MgLevel Lc = L[l + 1];
+            double* const pf = L[l].phi;
+            const int nrf = L[l].nr;
+            for (unsigned idx = threadIdx.x; idx < nf; idx += blockDim.x) mg_prolong_cell<unsigned>(Lc, pf, nrf, idx);
+        }
         __syncthreads();
         smooth(L[l], T.nu2);
     }
