@@ -175,3 +175,14 @@ def test_batch_full_size_cfg4a(P, torch_cuda, oracle):
         assert res[b].status == 0 and res[b].sweeps == ref["cycles"], (b, res[b], ref["cycles"])
         assert np.abs(got[b] - ref["phi"]).max() <= 1e-11 * np.abs(ref["phi"]).max()
     s.close()
+
+
+def test_largest_size_sweep_point_two_cycles_bit_exact(P, torch_cuda, oracle):
+    """4096 x 4096 (the largest grid of BASELINE.json's size sweep; 11 levels, 64-bit-free index path, 256 MiB working
+    set): two V-cycles with injected ghosts, every element against the oracle."""
+    w = W.cfg4b(4096, 2)
+    g = ghosts_of(oracle, w)
+    ref = oracle.mg_solve(w.rho, np.zeros_like(w.rho), w.dr, w.dz, w.symmetry, w.lmax, 0.0, 2, ghosts=g)
+    r, phi, hist, lev = gpu_mg(P, torch_cuda, w, 0.0, 2, ghosts=g)
+    assert lev == oracle.mg_levels(4096, 4096) == 11 and r.sweeps == 2
+    assert np.array_equal(phi, ref["phi"]) and np.array_equal(hist, ref["history"])

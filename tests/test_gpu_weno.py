@@ -153,3 +153,18 @@ def test_weno_argument_errors(P, torch_cuda):
     with pytest.raises(ValueError):
         w.rhs(U[:, :4])
     w.close()
+
+
+def test_paper_test1_at_the_papers_resolution(P, torch_cuda, oracle):
+    """PAPER.md:402 "2000 computing cells": test 1 of Table 3 evolved to t0 = 0.2 on both sides, bit for bit (the oracle
+    needs ~20 s; its distance to the exact Riemann solution at this resolution is pinned in tests/test_weno_pins.py)."""
+    torch = torch_cuda
+    row = table3()[0]
+    n = 2000
+    U, dx = W.shock_tube(*row[3:9], x0=row[2], n=n)
+    ref, steps_ref = oracle.weno_evolve(U, dx, 1.0e30, GAMMA, [0, 0, 0, 0], 0.5, row[1])
+    w = P.Weno(n, 1, dx, 1.0e30, GAMMA, [0, 0, 0, 0])
+    Ud = torch.from_numpy(U).cuda()
+    assert w.evolve(Ud, 0.5, row[1]) == steps_ref
+    assert np.array_equal(Ud.cpu().numpy(), ref)
+    w.close()
