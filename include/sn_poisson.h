@@ -221,6 +221,45 @@ int sn_poisson_solve_mg_batch(sn_poisson* h, int nbatch, const double* rho, doub
 sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
                                            int max_cycles, void* stream);
 
+/* ---- Multipole moments without any device allocation ----------------------------------------------------------------
+ * Who this is for.  Every other entry point works through a handle, and a handle gets its workspace from cudaMalloc
+ * (at sn_poisson_create and again on the first solve).  Some hosts cannot do that: a hydro code that sized its grids to
+ * fill the GPU at start-up and left no free memory to ask for; a framework in which all device memory belongs to one
+ * pool and stray cudaMalloc calls are banned; a time-step loop that cannot accept cudaMalloc / cudaFree stalling the
+ * whole device while other streams are busy.  For them this one call computes step (a-1) -- M_l, l = 0..lmax, and
+ * max|4 pi rho| -- with no handle and without calling cudaMalloc, cudaFree or anything else that allocates.
+ *
+ * How.  The reduction needs a little global scratch between its two kernels (per-block partial sums and one control
+ * block per member).  Here that scratch is a fixed array built into the library image: 520 KiB of device memory on
+ * every GPU that loads the library, held until the process exits, whether or not this function is ever called.
+ *
+ * Arguments.  rho: DEVICE pointer, nbatch consecutive grids in the layout above (read only).  nr, nz, dr, dz, symmetry,
+ * lmax: as for sn_poisson_create.  M_out: DEVICE pointer to nbatch * (lmax + 1) doubles, member b's M_l at
+ * M_out[b * (lmax + 1) + l] (odd l are 0 when symmetry = 1).  maxf_out: DEVICE pointer to nbatch doubles receiving
+ * max|4 pi rho| per member, or NULL.  The caller owns all three buffers.  stream: cudaStream_t or NULL.
+ * The work is enqueued on `stream` and the call returns without waiting; results are valid once the stream reaches
+ * that point.  Same kernels, block count and summation order as a handle uses, so M equals what
+ * sn_poisson_get_moments reports after a solve of the same grid (the tests compare at the 1e-13 bar of the moment tests).
+ *
+ * Limits, checked up front.  1 <= nbatch <= SN_POISSON_STATIC_MAX_BATCH, and nbatch * B * NL <=
+ * SN_POISSON_STATIC_MAX_DOUBLES, where B = min(ceil(nr * nz / 1024), 4 * SM count) blocks per member and NL = 9 / 17 /
+ * 33 / 65 for lmax <= 8 / 16 / 32 / 64.  On a B200 (148 SMs) a single grid of any size fits at every lmax; large
+ * grids fit up to 12 / 6 / 3 / 1 members per call.  A request beyond either limit returns -1 with the numbers in
+ * sn_poisson_last_error; nothing is launched.  Other returns: 0 = enqueued, -1 = bad argument, -2 = CUDA error.
+ *
+ * Sharing.  All calls on one GPU use the same array, and it keeps the previous call's contents; the function clears the
+ * part that has to start at zero itself (on `stream`), so back-to-back calls on ONE stream are safe.  Two calls whose
+ * kernels can overlap on the GPU -- different streams, or different host threads without ordering between them --
+ * race on the scratch and give wrong moments; serialise them (same stream, or an event).
+ *
+ * First call.  The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that
+ * device current) and caches it; make that first call in ordinary, non-capturing code, before any stream capture is
+ * begun on the device.  Later calls do no set-up. */
+#define SN_POISSON_STATIC_MAX_BATCH 64
+#define SN_POISSON_STATIC_MAX_DOUBLES 65536
+int sn_poisson_moments_static(const double* rho, int nbatch, int nr, int nz, double dr, double dz, int symmetry,
+                              int lmax, double* M_out, double* maxf_out, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

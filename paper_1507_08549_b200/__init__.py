@@ -6,7 +6,7 @@ from .binding import (EXPORTS, EXPORTS_LEVELSET, EXPORTS_WENO, sn_weno_create, s
                       sn_weno_get_stat, sn_weno_last_error, sn_weno_max_speeds, sn_weno_rhs, sn_weno_rhs_host, sn_weno_step, sn_levelset_create, sn_levelset_destroy, sn_levelset_get_stat,
                       sn_levelset_last_error, sn_levelset_reinit, sn_levelset_reinit_host, LIB_PATH, SnPoissonError, load, sn_poisson_create, sn_poisson_destroy,
                       sn_poisson_get_boundary, sn_poisson_get_history, sn_poisson_get_moments,
-                      sn_poisson_get_omega, sn_poisson_get_stat, sn_poisson_gravity, sn_poisson_last_error,
+                      sn_poisson_get_omega, sn_poisson_get_stat, sn_poisson_moments_static, sn_poisson_gravity, sn_poisson_last_error,
                       sn_poisson_result,
                       sn_poisson_set_boundary, sn_poisson_set_omega, sn_poisson_set_stop_rule, sn_poisson_solve_gravity, sn_poisson_solve_mg, sn_poisson_solve_mg_batch, sn_poisson_solve_mg_host, sn_poisson_set_option, sn_poisson_solve,
                       sn_poisson_solve_batch, sn_poisson_solve_batch_host, sn_poisson_solve_host,

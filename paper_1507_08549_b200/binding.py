@@ -19,7 +19,7 @@ EXPORTS = (
     "sn_poisson_set_stop_rule", "sn_poisson_solve_gravity", "sn_poisson_solve_mg", "sn_poisson_solve_mg_host", "sn_poisson_solve_mg_batch",
     "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
-    "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version",
+    "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version", "sn_poisson_moments_static",
 )
 
 
@@ -114,6 +114,9 @@ def load():
     lib.sn_poisson_last_error.argtypes = []
     lib.sn_poisson_version.restype = C.c_char_p
     lib.sn_poisson_version.argtypes = []
+    lib.sn_poisson_moments_static.restype = C.c_int
+    lib.sn_poisson_moments_static.argtypes = [_vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
+                                              _vp, _vp, _vp]
     lib.sn_levelset_create.restype = _vp
     lib.sn_levelset_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]
     lib.sn_levelset_reinit.restype = C.c_int64
@@ -276,6 +279,16 @@ def sn_poisson_get_moments(h, lmax):
     M = np.zeros(lmax + 1)
     _check(load().sn_poisson_get_moments(h, M.ctypes.data_as(_dp)), "sn_poisson_get_moments")
     return M
+
+
+def sn_poisson_moments_static(rho_ptr, nbatch, nr, nz, dr, dz, symmetry, lmax, m_out_ptr, maxf_out_ptr=0, stream=0) -> int:
+    """Multipole moments for hosts that may not allocate device memory (all of it handed to their own pool, or a
+    time-step loop that cannot take a cudaMalloc stall): no handle, scratch in an array built into the library.
+    DEVICE addresses: rho [nbatch][nz][nr], m_out [nbatch][lmax + 1], maxf_out [nbatch] or 0.  Enqueues on `stream`
+    and returns; sizes beyond the fixed scratch raise.  Calls that overlap on the GPU race (include/sn_poisson.h)."""
+    return _check(load().sn_poisson_moments_static(rho_ptr, int(nbatch), int(nr), int(nz), float(dr), float(dz),
+                                                   int(symmetry), int(lmax), m_out_ptr, maxf_out_ptr or None,
+                                                   stream or None), "sn_poisson_moments_static")
 
 
 def sn_poisson_set_boundary(h, bE, bN, bS=None):

@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstring>
 #include <algorithm>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1575,3 +1576,128 @@ int sn_poisson_get_stat(sn_poisson* h, const char* key, double* out) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// sn_poisson_moments_static: the multipole moments (step a-1) for callers that must not allocate device memory.
+//
+// k_moments reduces in two stages and needs global scratch between them: one row of NL partial sums per block, plus a
+// per-member Ctl block whose `maxf` word collects max|4 pi rho| by atomicMax.  Everywhere else in this library that
+// scratch comes from cudaMalloc inside a handle.  Here it is a fixed array that is part of the loaded module instead,
+// so the entry point below needs no handle and makes no allocating call of any kind.
+//
+// The array exists once per GPU that loads this library and stays until the process exits (kStaticBytes = 520 KiB each).
+// All calls on one GPU share it.  Layout: [0, kStaticCtlBytes) = Ctl[kStaticMaxBatch]; then kStaticPartialDoubles doubles.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticMaxBatch = SN_POISSON_STATIC_MAX_BATCH;
+constexpr size_t kStaticCtlBytes = 8192;
+constexpr size_t kStaticPartialDoubles = SN_POISSON_STATIC_MAX_DOUBLES;
+constexpr size_t kStaticBytes = kStaticCtlBytes + kStaticPartialDoubles * sizeof(double);
+static_assert(sizeof(Ctl) * kStaticMaxBatch <= kStaticCtlBytes, "Ctl area of the static scratch too small");
+static_assert(kStaticCtlBytes % 256 == 0, "partials must stay 256-byte aligned");
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+// In host code `g_static_scratch` is only a stand-in the runtime uses to look the array up; it is NOT a device address
+// and must never be handed to a kernel or a memset.  The real address differs per GPU and is fetched once per device,
+// with that device current, by cudaGetSymbolAddress below.
+constexpr int kStaticMaxDevices = 64;
+struct StaticDev {
+    bool ready = false;
+    unsigned char* base = nullptr;   // device address of g_static_scratch on this GPU
+    int num_sms = 0;
+};
+std::mutex g_static_mu;
+StaticDev g_static_dev[kStaticMaxDevices];
+
+// Second stage: fixed-order sum of the block partials (the order k_boundary uses, so the bits agree with the handle
+// path when the block count is the same), symmetry rule, result straight into the caller's arrays.  grid = nbatch.
+__global__ void __launch_bounds__(128) k_moments_static_finish(int lmax, int symmetry, int NL, int nblocks,
+                                                               const double* __restrict__ partial,
+                                                               const Ctl* __restrict__ ctl, double* __restrict__ M_out,
+                                                               double* __restrict__ maxf_out) {
+    const int b = blockIdx.x;
+    for (int l = threadIdx.x; l <= lmax; l += blockDim.x) {
+        double v = 0.0;
+        for (int k = 0; k < nblocks; ++k) v += partial[((size_t)b * nblocks + k) * NL + l];
+        if (symmetry == 1) v = (l & 1) ? 0.0 : 2.0 * v;
+        M_out[(size_t)b * (lmax + 1) + l] = v;
+    }
+    if (maxf_out && threadIdx.x == 0) maxf_out[b] = ctl[b].maxf;
+}
+
+// One-time set-up of the current device: architecture check, SM count, device address of the scratch array.
+int static_setup(StaticDev** out) {
+    int dev = 0;
+    CU_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) { set_err("device ordinal %d outside [0, %d)", dev, kStaticMaxDevices); return -1; }
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticDev& d = g_static_dev[dev];
+    if (!d.ready) {
+        int major = 0, sms = 0;
+        CU_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (major != 10) { set_err("device %d is not sm_10x; this library is built for sm_100a only (no fallback)", dev); return -1; }
+        unsigned char* base = nullptr;
+        CU_TRY(cudaGetSymbolAddress((void**)&base, g_static_scratch));
+        if (!base) { set_err("cudaGetSymbolAddress returned a NULL address"); return -2; }
+        d.base = base;
+        d.num_sms = sms;
+        d.ready = true;
+    }
+    *out = &d;
+    return 0;
+}
+
+}  // namespace
+
+extern "C" int sn_poisson_moments_static(const double* rho, int nbatch, int nr, int nz, double dr, double dz,
+                                         int symmetry, int lmax, double* M_out, double* maxf_out, void* stream) {
+    g_err.clear();
+    if (!rho || !M_out) { set_err("NULL argument"); return -1; }
+    if (nr < 2 || nz < 2) { set_err("nr, nz must be >= 2"); return -1; }
+    if (!(dr > 0) || !(dz > 0) || !std::isfinite(dr) || !std::isfinite(dz)) { set_err("dr, dz must be finite and > 0"); return -1; }
+    if (symmetry != 0 && symmetry != 1) { set_err("symmetry must be 0 or 1"); return -1; }
+    if (lmax < 0 || lmax > kMaxL) { set_err("lmax must be in [0, %d]", kMaxL); return -1; }
+    if ((long long)nr * nz > (1ll << 31) - 1) { set_err("grid too large"); return -1; }
+    if (nbatch < 1 || nbatch > kStaticMaxBatch) {
+        set_err("nbatch = %d: the static scratch holds control blocks for 1..%d members", nbatch, kStaticMaxBatch);
+        return -1;
+    }
+    StaticDev* d = nullptr;
+    if (int rc = static_setup(&d)) return rc;
+    // same template choice and block count as a handle makes in sn_poisson_create, so both paths sum in the same order
+    const int NL = lmax <= 8 ? 9 : lmax <= 16 ? 17 : lmax <= 32 ? 33 : 65;
+    const size_t ncell = (size_t)nr * nz;
+    size_t blocks = (ncell + kMomThreads * 4 - 1) / (kMomThreads * 4);
+    const size_t cap = (size_t)d->num_sms * 4;
+    blocks = blocks < 1 ? 1 : blocks > cap ? cap : blocks;
+    const size_t need = (size_t)nbatch * blocks * NL;
+    if (need > kStaticPartialDoubles) {
+        set_err("this call needs %zu doubles of scratch (nbatch %d x %zu blocks x %d sums); the static area holds %zu -- "
+                "use fewer members per call, or a handle (sn_poisson_create), which allocates what it needs",
+                need, nbatch, blocks, NL, kStaticPartialDoubles);
+        return -1;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    Ctl* ctl = reinterpret_cast<Ctl*>(d->base);
+    double* partial = reinterpret_cast<double*>(d->base + kStaticCtlBytes);
+    // The array keeps whatever the previous call left.  The partials are overwritten in full by every launch (each
+    // block stores all NL of its sums), but `maxf` is accumulated with atomicMax and has to start from zero.
+    CU_TRY(cudaMemsetAsync(ctl, 0, sizeof(Ctl) * nbatch, st));
+    Geom g{};
+    g.nr = nr; g.nz = nz; g.symmetry = symmetry; g.lmax = lmax; g.dr = dr; g.dz = dz;
+    const double L0 = nr * dr;
+    dim3 grid((unsigned)blocks, nbatch);
+    switch (NL) {
+        case 9: k_moments<9><<<grid, kMomThreads, 0, st>>>(rho, g, L0, partial, ctl); break;
+        case 17: k_moments<17><<<grid, kMomThreads, 0, st>>>(rho, g, L0, partial, ctl); break;
+        case 33: k_moments<33><<<grid, kMomThreads, 0, st>>>(rho, g, L0, partial, ctl); break;
+        default: k_moments<65><<<grid, kMomThreads, 0, st>>>(rho, g, L0, partial, ctl); break;
+    }
+    CU_TRY(cudaGetLastError());
+    k_moments_static_finish<<<nbatch, 128, 0, st>>>(lmax, symmetry, NL, (int)blocks, partial, ctl, M_out, maxf_out);
+    CU_TRY(cudaGetLastError());
+    return 0;
+}
