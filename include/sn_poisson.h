@@ -73,8 +73,10 @@ sn_poisson_result sn_poisson_solve(sn_poisson* h, const double* rho, double* phi
 sn_poisson_result sn_poisson_solve_host(sn_poisson* h, const double* rho_host, double* phi_inout_host,
                                         double tol, int max_sweeps, void* stream);
 
-/* Limits: max_sweeps <= 4194304 (2^22) and max_sweeps x nbatch <= 2^26 -- the handle keeps 32 bytes of per-sweep
- * bookkeeping (maxima slots, R_k history) per member; larger values are rejected with status -1. */
+/* Limits: max_sweeps <= 4194304 (2^22) and max_sweeps x nbatch <= 2^26 -- the handle keeps 44 bytes of per-sweep
+ * bookkeeping per member (maxima slots 16 + 8, equator-row slots of stop rule 1 8 + 4, R_k history 8), i.e. up to
+ * 2.75 GiB at the limit, allocated for the largest max_sweeps x nbatch a handle has seen; larger values are rejected
+ * with status -1. */
 
 /* nbatch independent solves on the same grid geometry ([CFG 4a]).  rho, phi_inout: DEVICE pointers to nbatch
  * consecutive grids (member b at offset b*nr*nz).  out: HOST array of nbatch results.
@@ -85,7 +87,8 @@ int sn_poisson_solve_batch(sn_poisson* h, int nbatch, const double* rho, double*
 /* sn_poisson_solve_batch with HOST buffers (pageable or pinned; layout as above).  rho is uploaded on `stream`,
  * phi's upload overlaps the moment / boundary kernels on an internal copy stream, phi's download is enqueued right
  * behind the relaxation; ONE stream synchronisation per call.  sn_poisson_solve_host is the nbatch = 1 case.
- * Device staging is grown on demand and kept on the handle.  Returns 0 or a negative status. */
+ * Device staging is grown on demand and kept on the handle.  Also on a negative return every copy the call enqueued
+ * has finished.  Returns 0 or a negative status. */
 int sn_poisson_solve_batch_host(sn_poisson* h, int nbatch, const double* rho_host, double* phi_inout_host,
                                 double tol, int max_sweeps, void* stream, sn_poisson_result* out);
 
@@ -97,7 +100,11 @@ int sn_poisson_solve_batch_host(sn_poisson* h, int nbatch, const double* rho_hos
  *   out             [nsteps]         HOST array of results
  * Copy-compute overlap: rho_{t+1} is uploaded on an internal copy stream while solve t runs, and phi_t is downloaded
  * from a device snapshot while solve t+1 runs (moments are recomputed every step).  Stops early (returning 0) at the
- * first step whose status is < 0; later entries of `out` are then untouched.  Returns 0 or a negative status. */
+ * first step t whose status is < 0; later entries of `out` are then untouched, phi_seq_host[0..t-1] are complete,
+ * phi_seq_host[t..] are not written and phi_inout_host receives phi of the failed step as the device holds it (what
+ * sn_poisson_solve leaves behind for that status; the last good potential is phi_seq_host[t-1]).  However the call
+ * ends -- all steps, an early stop, or a negative return -- both the caller's stream and the internal copy stream have
+ * been synchronised: no copy still reads or writes the host buffers afterwards.  Returns 0 or a negative status. */
 int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_seq_host, double* phi_inout_host,
                                    double* phi_seq_host, double tol, int max_sweeps, void* stream,
                                    sn_poisson_result* out);
@@ -133,7 +140,8 @@ int sn_poisson_gravity(sn_poisson* h, int nbatch, const double* phi, double* gr,
  * differences the patch of phi it still holds in registers right after its final store (neighbours outside the patch
  * from the stored result, after one grid barrier); on the blocked / streaming paths the standalone gravity kernel is
  * enqueued right behind the last sweep.  Bit-identical to sn_poisson_gravity on the returned phi.  gr, gz, phi_inout
- * must not alias.  Returns 0 or a negative status. */
+ * must not alias.  gr / gz need only be 8-byte aligned: when either is not 16-byte aligned the resident path skips its
+ * fused epilogue and the standalone kernel (scalar stores) runs behind it.  Returns 0 or a negative status. */
 int sn_poisson_solve_gravity(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double* gr, double* gz,
                              double tol, int max_sweeps, void* stream, sn_poisson_result* out);
 

@@ -65,9 +65,10 @@ struct ResPlan {
     int shape = -1, halo = 0, ds = 0, ring = 0, ll = 0, m = 0, Q = 0, ntx = 0, nty = 0, ow = 0, oh = 0, ntiles = 0;
     double cost = 0;
 };
-// Limits of the per-sweep bookkeeping (maxima slots + history: 32 B per sweep and member).
+// Limits of the per-sweep bookkeeping (ensure_ws: d_slots 16 + d_slots_f 8 + d_slots0 8 + d_slots0_f 4 + d_hist 8 = 44 B
+// per sweep and member).
 constexpr int kMaxSweepsLimit = 1 << 22;                 // per solve
-constexpr long long kMaxSweepSlots = 1ll << 26;          // max_sweeps x nbatch (2 GiB of slots)
+constexpr long long kMaxSweepSlots = 1ll << 26;          // max_sweeps x nbatch (2.75 GiB of bookkeeping)
 }  // namespace
 
 struct sn_poisson {
@@ -764,11 +765,17 @@ int solve_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, double
         return -1;
     }
     if (pl.shape >= 0) {
+        // the fused epilogue stores gr / gz as double2: it needs them 16-byte aligned (rho / phi are, or the resident path
+        // would not have been planned).  Output arrays that are only 8-byte aligned get the standalone kernel instead,
+        // which picks its scalar variant -- same values, bit for bit.
+        const bool fused = io && io->gr && ((((uintptr_t)io->gr | (uintptr_t)io->gz) & 15) == 0);
         for (int m0 = 0; m0 < nbatch; m0 += group)
             if (int rc = run_resident(h, g, pl, std::min(group, nbatch - m0), rho, phi, max_sweeps, st, m0,
-                                      io ? io->gr : nullptr, io ? io->gz : nullptr)) return rc;
+                                      fused ? io->gr : nullptr, fused ? io->gz : nullptr)) return rc;
         h->st_group = group;
         h->st_ctas = (double)pl.ntiles * group;
+        if (io && io->gr && !fused)
+            if (int rc = launch_gravity(h, g, nbatch, phi, io->gr, io->gz, st)) return rc;
     } else {
         if (bp.shape >= 0) {
             if (int rc = run_blocked(h, g, bp, nbatch, rho, phi, max_sweeps, st)) return rc;
@@ -861,7 +868,34 @@ int mg_num_levels(int nr, int nz) {                                  // M1
     return n;
 }
 
+// Releases the level arrays of the multigrid workspace and marks it as not built (the stream and the pinned history
+// buffer are independent of the level layout and stay).
+void free_mg_levels(sn_poisson* h) {
+    auto& W = h->mg;
+    if (W.exec) { cudaGraphExecDestroy(W.exec); W.exec = nullptr; }
+    for (auto* v : {&W.cE, &W.cW, &W.phi, &W.f}) {
+        for (double* p : *v) cudaFree(p);
+        v->clear();
+    }
+    cudaFree(W.slots); W.slots = nullptr;
+    cudaFree(W.d_ptrs); W.d_ptrs = nullptr;
+    W.nlev = 0;
+    W.cap_batch = 0;
+    W.key = {};
+}
+
+int ensure_mg_levels(sn_poisson* h, int nbatch);
+
+// Builds / grows the multigrid workspace.  A failure half way (out of memory while growing for a larger batch, or
+// during the first build) would leave level pointers NULL under a non-zero nlev / cap_batch, or leak the levels already
+// allocated: on any failure everything is released and the next call rebuilds from scratch.
 int ensure_mg(sn_poisson* h, int nbatch) {
+    const int rc = ensure_mg_levels(h, nbatch);
+    if (rc) free_mg_levels(h);
+    return rc;
+}
+
+int ensure_mg_levels(sn_poisson* h, int nbatch) {
     auto& W = h->mg;
     if (W.nlev && nbatch > W.cap_batch) {        // grow the per-member arrays (the captured cycle holds their addresses)
         if (W.exec) { cudaGraphExecDestroy(W.exec); W.exec = nullptr; }
@@ -1152,6 +1186,14 @@ int solve_mg_impl(sn_poisson* h, int nbatch, const double* rho, double* phi, dou
     return 0;
 }
 
+// Failure tail of the host-buffer entry points: wait for the caller's stream and the handle's copy stream, so that no
+// copy enqueued by the failed call still reads or writes the caller's host memory after it returns.  Keeps the message
+// of the original failure.
+void drain_host_io(sn_poisson* h, cudaStream_t st) {
+    cudaStreamSynchronize(st);
+    if (h->st_copy) cudaStreamSynchronize(h->st_copy);
+}
+
 }  // namespace
 
 extern "C" {
@@ -1295,6 +1337,7 @@ sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host
         cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, h->st_copy) != cudaSuccess ||
         cudaEventRecord(h->ev_io[1], h->st_copy) != cudaSuccess) {
         set_err("host staging failed: %s", cudaGetErrorString(cudaGetLastError()));
+        drain_host_io(h, st);
         return fail(-2);
     }
     HostIO io;
@@ -1302,7 +1345,7 @@ sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host
     io.d2h_dst = phi_inout_host; io.d2h_src = h->d_phi_stage; io.d2h_bytes = bytes;
     sn_poisson_result out = {0, 0, 0.0};
     const int rc = solve_mg_impl(h, 1, h->d_rho_stage, h->d_phi_stage, tol, max_cycles, st, &out, &io);
-    if (rc) return fail(rc);
+    if (rc) { drain_host_io(h, st); return fail(rc); }
     return out;
 }
 
@@ -1327,7 +1370,9 @@ int sn_poisson_solve_batch_host(sn_poisson* h, int nbatch, const double* rho_hos
     HostIO io;
     io.wait_before_relax = h->ev_io[1];
     io.d2h_dst = phi_inout_host; io.d2h_src = h->d_phi_stage; io.d2h_bytes = bytes;
-    return solve_impl(h, nbatch, h->d_rho_stage, h->d_phi_stage, tol, max_sweeps, st, out, &io);
+    const int rc = solve_impl(h, nbatch, h->d_rho_stage, h->d_phi_stage, tol, max_sweeps, st, out, &io);
+    if (rc) drain_host_io(h, st);        // a failed call may have left the uploads in flight: not past the return
+    return rc;
 }
 
 int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_seq_host, double* phi_inout_host,
@@ -1348,6 +1393,10 @@ int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_
     }
     cudaEvent_t ev_h2d[2] = {h->ev_io[0], h->ev_io[1]}, ev_snap[2] = {h->ev_io[2], h->ev_io[3]},
                 ev_d2h[2] = {h->ev_io[4], h->ev_io[5]};
+    // Everything that touches the caller's host buffers is enqueued inside `run`; whatever way it ends (all steps, a
+    // failed step, a CUDA error), the tail below drains both streams before the call returns, so no DMA is still
+    // reading rho_seq_host or writing phi_seq_host / phi_inout_host when the caller gets control back.
+    auto run = [&]() -> int {
     CU_TRY(cudaMemcpyAsync(h->d_rho_stage, rho_seq_host, bytes, cudaMemcpyHostToDevice, st));
     CU_TRY(cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, st));
     CU_TRY(cudaEventRecord(ev_h2d[0], st));
@@ -1364,7 +1413,7 @@ int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_
         }
         if (t > 0) CU_TRY(cudaStreamWaitEvent(st, ev_h2d[cur], 0));
         if (int rc = solve_impl(h, 1, h->d_rho_stage + (size_t)cur * n, h->d_phi_stage, tol, max_sweeps, st, out + t)) return rc;
-        if (out[t].status < 0) return 0;                                // the caller sees which step failed
+        if (out[t].status < 0) break;                                   // the caller sees which step failed
         if (phi_seq_host) {
             // snapshot on the caller's stream (the next solve updates phi in place), download on the copy stream
             // while solve t+1 runs
@@ -1377,10 +1426,17 @@ int sn_poisson_solve_sequence_host(sn_poisson* h, int nsteps, const double* rho_
             d2h_pending[cur] = true;
         }
     }
+    // after the last step -- or after a failed one: phi as the device holds it, like sn_poisson_solve leaves it
     CU_TRY(cudaMemcpyAsync(phi_inout_host, h->d_phi_stage, bytes, cudaMemcpyDeviceToHost, st));
-    CU_TRY(cudaStreamSynchronize(st));
-    CU_TRY(cudaStreamSynchronize(h->st_copy));
     return 0;
+    };
+    int rc = run();
+    const cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(h->st_copy);
+    if (rc == 0 && (e1 != cudaSuccess || e2 != cudaSuccess)) {
+        set_err("stream synchronisation failed: %s", cudaGetErrorString(e1 != cudaSuccess ? e1 : e2));
+        rc = -2;
+    }
+    return rc;
 }
 
 int sn_poisson_solve_gravity(sn_poisson* h, int nbatch, const double* rho, double* phi_inout, double* gr, double* gz,

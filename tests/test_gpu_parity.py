@@ -648,6 +648,46 @@ def test_batch_host_and_sequence_host_equal_device_solves(P, torch_cuda, oracle)
                 assert np.array_equal(phi_all[t], want_phi[t]), t
 
 
+def test_sequence_host_early_stop_leaves_no_copy_in_flight(P, torch_cuda):
+    """A NaN in rho of step 2 of a 5-step sequence, PINNED host buffers (the copies are truly asynchronous): the call
+    returns 0 with status -3 at step 2 and the later entries untouched; when it returns, the potentials of the steps
+    before the failed one are complete (equal to a clean 2-step run, bit for bit), phi_inout holds the device's phi of
+    the failed step, and nothing of step 3 onwards was written."""
+    torch = torch_cuda
+    seq = W.cfg3(128, nsteps=5)
+    w = seq.first
+    rhos, r_t = [w.rho], w.rho
+    for t in range(1, 5):
+        r_t = seq.step(r_t, t)
+        rhos.append(r_t)
+    n = w.rho.size
+    s = P.PoissonSolver.for_workload(w)
+    rho_seq = torch.from_numpy(np.stack(rhos)).pin_memory()
+    rho_seq[2, 17, 5] = float("nan")
+    want_phi = torch.zeros((2,) + w.rho.shape, dtype=torch.float64).pin_memory()
+    phi_io = torch.zeros(w.rho.shape, dtype=torch.float64).pin_memory()
+    st = torch.cuda.current_stream().cuda_stream
+    clean = P.sn_poisson_solve_sequence_host(s.h, 2, rho_seq.data_ptr(), phi_io.data_ptr(), want_phi.data_ptr(), w.tol,
+                                             w.max_sweeps, st)
+    assert [r.status for r in clean] == [0, 0]
+    for rep in range(3):
+        phi_all = torch.full((5,) + w.rho.shape, -7.0, dtype=torch.float64).pin_memory()
+        phi_io.zero_()
+        got = P.sn_poisson_solve_sequence_host(s.h, 5, rho_seq.data_ptr(), phi_io.data_ptr(), phi_all.data_ptr(), w.tol,
+                                               w.max_sweeps, st)
+        # no synchronisation here on purpose: the call itself must have drained its streams
+        assert [r.status for r in got] == [0, 0, -3, -1, -1]
+        assert (got[0].sweeps, got[1].sweeps) == (clean[0].sweeps, clean[1].sweeps)
+        assert torch.equal(phi_all[:2], want_phi)
+        assert torch.all(phi_all[2:] == -7.0)
+        assert not torch.all(torch.isfinite(phi_io))          # the failed step's iterate, as the device holds it
+    # the handle is still usable
+    phi_io.zero_()
+    again = P.sn_poisson_solve_sequence_host(s.h, 2, rho_seq.data_ptr(), phi_io.data_ptr(), 0, w.tol, w.max_sweeps, st)
+    assert [(r.sweeps, r.status) for r in again] == [(r.sweeps, r.status) for r in clean]
+    assert torch.equal(phi_io, want_phi[1])
+
+
 def test_limits_and_stale_ghosts_are_rejected(P, torch_cuda):
     """max_sweeps beyond the documented bookkeeping limit -> -1 (no allocation attempt); gravity for more members than
     the last solve covered -> error."""
@@ -936,3 +976,34 @@ def test_fused_gravity_epilogue_bit_exact(P, torch_cuda, oracle, symmetry, opts)
         bnd = oracle.boundary(m.nr, m.nz, m.dr, m.dz, symmetry, m.lmax, M)
         want_r, want_z = oracle.gravity(pb[b].cpu().numpy(), m.dr, m.dz, symmetry, *bnd)
         assert relmax(grb[b].cpu().numpy(), want_r) <= REL and relmax(gzb[b].cpu().numpy(), want_z) <= REL
+
+
+@pytest.mark.parametrize("opts", [{"path": 2, "halo": 0}, {"path": 2, "halo": 1, "ds": 0, "shape": 4}])
+@pytest.mark.parametrize("shift", [(1, 0), (0, 1), (1, 1)])
+def test_fused_gravity_with_8_byte_aligned_outputs(P, torch_cuda, oracle, opts, shift):
+    """gr / gz that are only 8-byte aligned (an odd-offset view of a larger buffer) while rho / phi are 16-byte aligned:
+    the solve still takes the resident path, and the field equals the aligned call's and the oracle's bit for bit (the
+    double2 stores of the fused epilogue would fault on such pointers; the library falls back to its scalar kernel)."""
+    torch = torch_cuda
+    w = W.random_smooth(128, 104, 1, seed=951, lmax=6)
+    s = P.PoissonSolver(w.nr, w.nz, w.dr, w.dz, 1, w.lmax)
+    for k, v in opts.items():
+        s.set_option(k, v)
+    rho = torch.from_numpy(w.rho).cuda()
+    phi0 = torch.zeros_like(rho)
+    _, gr0, gz0 = s.solve_gravity(rho, phi0, 0.0, 40)
+    n = rho.numel()
+    bufr, bufz = torch.zeros(n + 2, dtype=torch.float64, device="cuda"), torch.zeros(n + 2, dtype=torch.float64, device="cuda")
+    gr, gz = bufr[shift[0]:shift[0] + n].view_as(rho), bufz[shift[1]:shift[1] + n].view_as(rho)
+    assert gr.data_ptr() % 16 == 8 * shift[0] and gz.data_ptr() % 16 == 8 * shift[1]
+    phi = torch.zeros_like(rho)
+    res = P.sn_poisson_solve_gravity(s.h, 1, rho.data_ptr(), phi.data_ptr(), gr.data_ptr(), gz.data_ptr(), 0.0, 40,
+                                     torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert res[0].status in (0, 1) and res[0].sweeps == 40 and s.stat("path") == 2
+    assert torch.equal(phi, phi0) and torch.equal(gr, gr0) and torch.equal(gz, gz0)
+    want_r, want_z = oracle.gravity(phi.cpu().numpy(), w.dr, w.dz, 1, *s.boundary())
+    assert np.array_equal(gr.cpu().numpy(), want_r) and np.array_equal(gz.cpu().numpy(), want_z)
+    # nothing written outside the views
+    assert bufr[0] == 0 or shift[0] == 0
+    assert bufr[n + 1] == 0 and bufz[n + 1] == 0
