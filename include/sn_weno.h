@@ -45,8 +45,10 @@ int sn_weno_rhs(sn_weno* h, const double* U, double* L, double alpha_r, double a
  * (may be NULL) receives the step; the call synchronises `stream` only if dt_host != NULL. */
 int sn_weno_step(sn_weno* h, double* U, double cfl, double* dt_host, void* stream);
 
-/* March from t = 0 to t_end (the last step is shortened to land on it), at most max_steps steps.  Returns the number
- * of steps (>= 0) or an error code (< 0).  Synchronises `stream`. */
+/* March from t = 0 to t_end (the last step is shortened to land on it), at most max_steps steps.  The time and the
+ * step, including the shortened last one, are formed on the device from the maxima the first stage computes anyway;
+ * the host reads (dt, t, last-step flag) back once per step to decide whether to go on.  Returns the number of steps
+ * (>= 0) or an error code (< 0).  Synchronises `stream`. */
 int sn_weno_evolve(sn_weno* h, double* U, double cfl, double t_end, int max_steps, void* stream);
 
 /* Same as sn_weno_rhs with HOST buffers (H2D of U, D2H of L inside the call). */

@@ -136,6 +136,24 @@ __global__ void k_weno_dt(WenoGeom g, const double* __restrict__ alpha, double c
     if (threadIdx.x == 0 && blockIdx.x == 0) *dt = cfl / (alpha[0] / g.dr + alpha[1] / g.dz);
 }
 
+// The step of sn_weno_evolve, decided on the device: the Courant step, shortened if it would pass t_end -- the same
+// expressions, in the same order, as the host loop they replace (and as the oracle's march): use = (t_end - t) / dt_full
+// * cfl for the last step, dt = use / (alpha_r/dr + alpha_z/dz).  tstate[0] = t (advanced here), tstate[1] = 1 if this
+// was the shortened last step.
+__global__ void k_weno_dt_evolve(WenoGeom g, const double* __restrict__ alpha, double cfl, double t_end,
+                                 double* __restrict__ dt, double* __restrict__ tstate) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        const double s = alpha[0] / g.dr + alpha[1] / g.dz;
+        const double t = tstate[0];
+        const double dt_full = cfl / s;
+        const double use = t + dt_full > t_end ? (t_end - t) / dt_full * cfl : cfl;
+        const double d = use / s;
+        *dt = d;
+        tstate[0] = t + d;
+        tstate[1] = use != cfl ? 1.0 : 0.0;
+    }
+}
+
 struct RhsParams {
     WenoGeom g;
     const double* U;         // stage input (stencil source)
@@ -279,12 +297,14 @@ int launch_rhs(sn_weno* h, int mode, const double* U, const double* U0, double* 
     return 0;
 }
 
-// one SSP-RK3 step, everything enqueued on st; the step ends up in d_scal[6]
-int enqueue_step(sn_weno* h, double* U, double cfl, cudaStream_t st) {
+// one SSP-RK3 step, everything enqueued on st; the step ends up in d_scal[6].  march = true (sn_weno_evolve): the step
+// is clamped to t_end on the device and the time in d_scal[8] / the last-step flag in d_scal[9] are advanced.
+int enqueue_step(sn_weno* h, double* U, double cfl, cudaStream_t st, bool march = false, double t_end = 0.0) {
     double* a = h->d_scal;
     WN_TRY(cudaMemsetAsync(a, 0, 6 * sizeof(double), st));
     if (int rc = launch_speeds(h, U, a, st)) return rc;
-    k_weno_dt<<<1, 32, 0, st>>>(h->g, a, cfl, a + 6);
+    if (march) k_weno_dt_evolve<<<1, 32, 0, st>>>(h->g, a, cfl, t_end, a + 6, a + 8);
+    else k_weno_dt<<<1, 32, 0, st>>>(h->g, a, cfl, a + 6);
     WN_TRY(cudaGetLastError());
     h->st_launches += 1;
     if (int rc = launch_rhs(h, 1, U, nullptr, h->d_stage[0], a, a + 6, 0.0, 1.0, st)) return rc;
@@ -411,20 +431,21 @@ int sn_weno_evolve(sn_weno* h, double* U, double cfl, double t_end, int max_step
     double t = 0.0;
     int steps = 0;
     double launches = 0;
+    // t and the last-step flag live on the device (d_scal[8], [9]); the step, clamped to t_end, is formed there from the
+    // maxima the first stage needs anyway.  One read-back per step (dt, t, flag) decides whether to go on.
+    const double zero[2] = {0.0, 0.0};
+    WN_TRY(cudaMemcpyAsync(h->d_scal + 8, zero, sizeof zero, cudaMemcpyHostToDevice, st));    // pageable: staged before return
     while (t < t_end && steps < max_steps) {
-        // the step the full Courant number would take, to decide whether this is the (shortened) last one
-        double a[2];
-        if (int rc = sn_weno_max_speeds(h, U, a, stream)) return rc;
+        h->st_launches = 0;
+        if (int rc = enqueue_step(h, U, cfl, st, true, t_end)) return rc;
         launches += h->st_launches;
-        const double dt_full = cfl / (a[0] / h->g.dr + a[1] / h->g.dz);
-        const double use = t + dt_full > t_end ? (t_end - t) / dt_full * cfl : cfl;
-        double dt = 0.0;
-        if (int rc = sn_weno_step(h, U, use, &dt, stream)) return rc;
-        launches += h->st_launches;
-        if (!(dt > 0.0)) { wn_err("non-positive or non-finite time step at step %d", steps); return -2; }
-        t += dt;
+        double back[4] = {0.0, 0.0, 0.0, 0.0};                       // d_scal[6..9] = dt, (unused), t, last-step flag
+        WN_TRY(cudaMemcpyAsync(back, h->d_scal + 6, sizeof back, cudaMemcpyDeviceToHost, st));
+        WN_TRY(cudaStreamSynchronize(st));
+        if (!(back[0] > 0.0)) { wn_err("non-positive or non-finite time step at step %d", steps); return -2; }
+        t = back[2];
         ++steps;
-        if (use != cfl) break;
+        if (back[3] != 0.0) break;
     }
     h->st_launches = launches;
     return steps;

@@ -155,16 +155,20 @@ def test_weno_argument_errors(P, torch_cuda):
     w.close()
 
 
-def test_paper_test1_at_the_papers_resolution(P, torch_cuda, oracle):
-    """PAPER.md:402 "2000 computing cells": test 1 of Table 3 evolved to t0 = 0.2 on both sides, bit for bit (the oracle
-    needs ~20 s; its distance to the exact Riemann solution at this resolution is pinned in tests/test_weno_pins.py)."""
+@pytest.mark.parametrize("test", [1, 2, 3, 4])
+def test_paper_tubes_at_the_papers_resolution(P, torch_cuda, oracle, test):
+    """PAPER.md:402 "2000 computing cells": every test of Table 3 evolved to its t0 on both sides, bit for bit, with the
+    same number of steps (tests 3 and 4 are the strong-shock ones; the oracle needs 20-60 s per tube; its distance to the
+    exact Riemann solution is pinned in tests/test_weno_pins.py)."""
     torch = torch_cuda
-    row = table3()[0]
+    row = table3()[test - 1]
+    t0 = 0.15 if test == 2 else row[1]                   # reading W9
     n = 2000
     U, dx = W.shock_tube(*row[3:9], x0=row[2], n=n)
-    ref, steps_ref = oracle.weno_evolve(U, dx, 1.0e30, GAMMA, [0, 0, 0, 0], 0.5, row[1])
+    ref, steps_ref = oracle.weno_evolve(U, dx, 1.0e30, GAMMA, [0, 0, 0, 0], 0.5, t0)
     w = P.Weno(n, 1, dx, 1.0e30, GAMMA, [0, 0, 0, 0])
     Ud = torch.from_numpy(U).cuda()
-    assert w.evolve(Ud, 0.5, row[1]) == steps_ref
+    assert w.evolve(Ud, 0.5, t0) == steps_ref
     assert np.array_equal(Ud.cpu().numpy(), ref)
+    assert w.stat("launches") == 7 * steps_ref           # no separate maxima pass per step: 3 x (maxima + rhs) + dt
     w.close()
