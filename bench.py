@@ -54,8 +54,28 @@ FP64_LANE_INSTR_PER_S = 148 * 64 * 1.965e9        # fp64 pipe: 64 lanes per cloc
 LS_FP64_PER_PAIR = 5.0                            # level-set distance kernel: fp64 instructions per node-crossing pair
 WENO_FP64_PER_CELL = 2750.0                       # flux reconstruction: fp64 instructions per cell, no redundant faces (profiles/r02_weno500_rhs.md)
 DEFAULT_WORKLOAD = "cfg3seq100"
-PER_CONFIG = ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "sweep128", "sweep256", "sweep512", "sweep1024", "sweep2048",
-              "sweep4096"]
+PER_CONFIG = ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "paper500", "sweep128", "sweep256", "sweep512", "sweep1024",
+              "sweep2048", "sweep4096"]
+
+
+def mg_alg_bytes_per_cycle(nr, nz, nlev, nu1=1, nu2=1, nc=12):
+    """Algorithmic bytes of one V(nu1, nu2) cycle (readings M3-M8, DESIGN.md section 6 'Multigrid roofline'), every pass
+    counted as one stream over its level with 8 B per fp64 read or written and nothing re-read:
+      smoothing sweep           24 B / cell   (read phi, read f, write phi -- the SOR sweep's figure)
+      residual + restriction    16 B / cell + 8 B / coarse cell   (read phi, f; write the coarse right-hand side)
+      coarse initial guess       8 B / coarse cell                 (phi_c = 0)
+      prolongation + correction 16 B / cell + 8 B / coarse cell   (read, write phi; read the coarse phi)
+      stopping ratio            16 B / level-0 cell                (true residual of the new iterate: read phi, f)
+    the coarsest level runs nc sweeps; a single-level grid runs nu1 + nu2 sweeps plus the stopping pass."""
+    total = 0.0
+    for l in range(nlev):
+        n = (nr >> l) * (nz >> l)
+        if l == nlev - 1:
+            total += 24.0 * n * ((nu1 + nu2) if nlev == 1 else nc)
+        else:
+            nc_cells = (nr >> (l + 1)) * (nz >> (l + 1))
+            total += 24.0 * n * (nu1 + nu2) + 16.0 * n + 8.0 * nc_cells + 8.0 * nc_cells + 16.0 * n + 8.0 * nc_cells
+    return total + 16.0 * nr * nz
 
 
 def make_workload(name: str):
@@ -73,6 +93,13 @@ def make_workload(name: str):
         n = int(name[7:] or 100)
         return (f"cfg3 sequence: {n} warm-started solves on 1024x2048 (rho evolves by seeded 0.1 % perturbations), "
                 f"lmax=32, tol=1e-10"), [W.cfg3(nsteps=n)]
+    if name == "paper500":
+        # the paper's own solver settings on its own grid (PAPER.md:99 Roche boundary = lmax 0, "relative changes of all
+        # grids reach below 1e-8" = stop rule 1; PAPER.md:476 500 x 500): the Table-2 workload, seeded WD as the star
+        w = W.wd_half_plane(500, 3.0, 20, seed=2, lmax=0, tol=1e-8, max_sweeps=20000, name="paper500")
+        w.meta["stop_rule"] = 1
+        return ("paper500: 500x500 half-plane n=3 WD + 20 bubbles, lmax=0 (Roche), paper-literal relative-change rule, "
+                "tol=1e-8, cold start"), [w]
     if name == "cfg4a":
         return "cfg4a: batch of 64 x 512x512 half-plane WDs, lmax=16, tol=1e-10, cold start", W.cfg4a(64)
     if name.startswith("sweep"):
@@ -238,6 +265,8 @@ class Bench:
         solver = P.PoissonSolver.for_workload(w0)
         if self.path:
             solver.set_option("path", self.path)
+        if w0.meta.get("stop_rule"):
+            solver.set_stop_rule(w0.meta["stop_rule"])
         rho_h = np.stack([m.rho for m in mine]) if nb > 1 else w0.rho
         if seq is not None:
             rhos, r_t = [w0.rho], w0.rho
@@ -326,6 +355,7 @@ class Bench:
         path = int(solver.stat("path"))
         info = {
             "name": name, "cells": cells, "nb": nb, "grid": [w0.nr, w0.nz], "lmax": w0.lmax, "tol": w0.tol,
+            "stop_rule": int(w0.meta.get("stop_rule", 0)),
             "step_ms": step_ms, "sweep_ms": sweep_ms, "setup_ms": setup_ms, "launches": launches,
             "sweep_launches": sweep_launches, "updates": updates, "results": results, "region_s": region_s,
             "clocks": clocks, "e2e_ms": e2e_ms, "e2e_upd": e2e_upd, "e2e_api": api, "h2d": h2d, "d2h": d2h,
@@ -369,7 +399,8 @@ class Bench:
     def config_of(info, label, scaling="weak", world=1):
         path = info["path"]
         return {"workload": label, "grid": info["grid"], "batch_per_gpu": info["nb"], "lmax": info["lmax"],
-                "tol": info["tol"], "l2": "flushed between timed solves (256 MiB write)",
+                "tol": info["tol"], "stop_rule": info.get("stop_rule", 0),
+                "l2": "flushed between timed solves (256 MiB write)",
                 "path": {1: "streaming", 2: "resident", 3: "blocked"}.get(path, str(path)),
                 "tblock": info["tblock"], "ctas": info["ctas"],
                 "mode": (("cluster-halo" if info["ds"] else "halo") if info["halo"] else "block") if path == 2 else None,
@@ -377,7 +408,7 @@ class Bench:
                 "parallelism": "replicas" if scaling == "weak" else f"batch sharded x{world}, no collective"}
 
 
-def next_rows(torch, P, flush):
+def next_rows(torch, P, flush, peaks):
     """The NEXT rows of SURVEY.md section 8f that are built (level-set re-initialisation, WENO-5 / LF flux
     reconstruction), each on its paper-sized synthetic input (500 x 500) with its own roofline: both are
     bound by plain fp64 ALU work, so `frac` is fp64 instructions per second against the fp64 pipe's issue peak."""
@@ -450,7 +481,21 @@ def next_rows(torch, P, flush):
                          "h2d_bytes_per_step": U.nbytes, "d2h_bytes_per_step": U.nbytes}})
     wn.close()
     # ---- NEXT-4: multigrid variant on the same stencil (time to the same residual tolerance, next to the SOR path)
-    for name in ("cfg1", "cfg2", "cfg3"):
+    def mg_roofline(w0, nb, levels, cycles_total, solve_ms, opts=(1, 1, 12)):
+        """Whole solve (moments, boundary, every launch of every cycle) against the bandwidth that bounds a streaming
+        V-cycle: L2 while phi + f of all members fit it (the rule of Bench.roofline), else HBM."""
+        per_cycle = mg_alg_bytes_per_cycle(w0.nr, w0.nz, levels, *opts)
+        ach = per_cycle * cycles_total / (solve_ms * 1e-3) / 1e9
+        if 16.0 * w0.cells * nb > 100e6:
+            bound, peak, src = "hbm", peaks["hbm"], peaks["hbm_src"]
+        else:
+            bound, peak, src = "l2", peaks["l2"]["copy"], "sn_poisson_probe_l2 (L2-resident copy, measured live in this run)"
+        return {"bound": bound, "kernel": "all launches of the V-cycles (k_mg_halfsweep, k_mg_residual_restrict, k_mg_prolong, k_mg_tail)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                "alg_bytes_per_cycle": per_cycle, "cycles": cycles_total, "peak_source": src,
+                "frac_of_hbm_peak": ach / peaks["hbm"]}
+
+    for name in ("cfg1", "cfg2", "cfg3", "paper500"):
         lab, mem = make_workload(name)
         w0 = mem[0]
         sv = P.PoissonSolver.for_workload(w0)
@@ -467,8 +512,14 @@ def next_rows(torch, P, flush):
         # cells touched per V(1,1) cycle on level 0: 2 sweeps + 2 residual passes + 1 prolongation; x 4/3 for the coarse levels
         rows.append({"workload": "mg_" + name, "label": "NEXT-4: multigrid V(1,1) on " + lab, "metric": "time_to_residual_ms",
                      "value": ms - zero_ms, "cycles": r.sweeps, "final_residual": r.residual, "levels": int(sv.stat("mg_levels")),
+                     "status": r.status, "converged": r.status == 0,
+                     # 500 = 4 x 125 coarsens twice only; 12 Gauss-Seidel sweeps do not solve the 125 x 125 coarsest level
+                     # and the cycle stalls (the oracle needs "mg_nc" ~ 1500 to reach 1e-8 in 17 cycles): on this grid the
+                     # SOR path (per_config `paper500`) is the solver, this row records that the variant does not help
+                     **({"note": "not converged in 60 cycles: the grid coarsens to 125 x 125 only"} if r.status != 0 else {}),
                      "higher_is_better": False, "gpu_launches_per_step": launches,
                      "fine_cell_updates_per_s": 2.0 * r.sweeps * w0.cells / ((ms - zero_ms) * 1e-3),
+                     "roofline": mg_roofline(w0, 1, int(sv.stat("mg_levels")), r.sweeps, ms - zero_ms),
                      "e2e": {"value": e2e_ms, "unit": "ms", "api": "sn_poisson_solve_mg_host",
                              "h2d_bytes_per_step": 2 * w0.rho.nbytes, "d2h_bytes_per_step": w0.rho.nbytes}})
         sv.close()
@@ -484,9 +535,15 @@ def next_rows(torch, P, flush):
     rows.append({"workload": "mg_cfg4a", "label": "NEXT-4: multigrid V(1,1) on " + lab, "metric": "time_to_residual_ms",
                  "value": ms - zero_ms, "cycles": [r.sweeps for r in res][:8], "max_cycles": max(r.sweeps for r in res),
                  "higher_is_better": False, "gpu_launches_per_step": int(sv.stat("launches")),
-                 "e2e": {"value": None, "api": None}})
+                 # members that have stopped drop out of the later cycles: the cycles actually run are the sum
+                 "roofline": mg_roofline(w0, len(mem), int(sv.stat("mg_levels")), sum(r.sweeps for r in res), ms - zero_ms)})
+    rho_pin = torch.from_numpy(np.stack([m.rho for m in mem])).pin_memory()
+    phi_pin = torch.zeros(rho_pin.shape, dtype=torch.float64).pin_memory()
+    e2e_ms = wall(lambda: (phi_pin.zero_(), sv.solve_mg_host(rho_pin.numpy(), phi_pin.numpy(), w0.tol, 60)), 2)
+    rows[-1]["e2e"] = {"value": e2e_ms, "unit": "ms", "api": "sn_poisson_solve_mg_batch_host",
+                       "h2d_bytes_per_step": 2 * rho_pin.numel() * 8, "d2h_bytes_per_step": rho_pin.numel() * 8}
     sv.close()
-    del rho, phi
+    del rho, phi, rho_pin, phi_pin
     # the [CFG 3] workload itself (warm-started sequence, here its first 20 solves) through the multigrid variant
     seq = W.cfg3(nsteps=20)
     w0 = seq.first
@@ -507,7 +564,20 @@ def next_rows(torch, P, flush):
     ms = timed(run_seq, 3, warm=1)
     rows.append({"workload": "mg_cfg3seq20", "label": "NEXT-4: multigrid V(1,1) on the first 20 warm-started solves of [CFG 3]",
                  "metric": "time_to_residual_ms", "value": ms / seq.nsteps, "sequence_ms": ms, "cycles": list(cyc),
-                 "higher_is_better": False, "e2e": {"value": None, "api": None}})
+                 "higher_is_better": False,
+                 "roofline": mg_roofline(w0, 1, int(sv.stat("mg_levels")), sum(cyc), ms)})
+    # end to end: the same 20 warm-started solves from pinned host arrays, one sn_poisson_solve_mg_host call per step
+    # (rho_t and the previous potential go up, the new potential comes back, every step)
+    rho_pin = rho_d.cpu().pin_memory()
+    phi_pin = torch.zeros((w0.nz, w0.nr), dtype=torch.float64).pin_memory()
+
+    def run_seq_host():
+        phi_pin.zero_()
+        for t in range(seq.nsteps):
+            sv.solve_mg_host(rho_pin[t].numpy(), phi_pin.numpy(), w0.tol, 60)
+    e2e_ms = wall(run_seq_host, 2)
+    rows[-1]["e2e"] = {"value": e2e_ms / seq.nsteps, "unit": "ms", "api": "sn_poisson_solve_mg_host (one call per step)",
+                       "h2d_bytes_per_step": 2 * w0.rho.nbytes, "d2h_bytes_per_step": w0.rho.nbytes}
     sv.close()
     return rows
 
@@ -644,7 +714,7 @@ def main():
                                  "h2d_bytes_per_step": inf["h2d"], "d2h_bytes_per_step": inf["d2h"]},
                          "gpu_launches_per_step": inf["launches"] // max(1, len(inf["step_ms"]))})
         out["per_config"] = rows
-        out["next_rows"] = next_rows(torch, P, bench.flush)
+        out["next_rows"] = next_rows(torch, P, bench.flush, bench.peaks)
     if not args.no_cpu_baseline and world == 1:
         v, sample = oracle_rate([mine[0].first] if hasattr(mine[0], "first") else mine)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,

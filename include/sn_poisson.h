@@ -228,6 +228,12 @@ int sn_poisson_solve_mg_batch(sn_poisson* h, int nbatch, const double* rho, doub
 /* The same as sn_poisson_solve_mg with HOST buffers (H2D of rho and phi, D2H of phi inside the call). */
 sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
                                            int max_cycles, void* stream);
+/* sn_poisson_solve_mg_batch with HOST buffers (pageable or pinned; layout as sn_poisson_solve_batch_host): rho goes up
+ * on `stream`, phi's upload overlaps the moment / boundary kernels on the internal copy stream, phi comes back behind
+ * the last cycle; one stream synchronisation.  sn_poisson_solve_mg_host is the nbatch = 1 case.  Also on a negative
+ * return every copy the call enqueued has finished.  Returns 0 or a negative status. */
+int sn_poisson_solve_mg_batch_host(sn_poisson* h, int nbatch, const double* rho_host, double* phi_inout_host, double tol,
+                                   int max_cycles, void* stream, sn_poisson_result* out);
 
 /* ---- Multipole moments without any device allocation ----------------------------------------------------------------
  * Who this is for.  Every other entry point works through a handle, and a handle gets its workspace from cudaMalloc

@@ -8,7 +8,7 @@ from .binding import (EXPORTS, EXPORTS_LEVELSET, EXPORTS_WENO, sn_weno_create, s
                       sn_poisson_get_boundary, sn_poisson_get_history, sn_poisson_get_moments,
                       sn_poisson_get_omega, sn_poisson_get_stat, sn_poisson_moments_static, sn_poisson_gravity, sn_poisson_last_error,
                       sn_poisson_result,
-                      sn_poisson_set_boundary, sn_poisson_set_omega, sn_poisson_set_stop_rule, sn_poisson_solve_gravity, sn_poisson_solve_mg, sn_poisson_solve_mg_batch, sn_poisson_solve_mg_host, sn_poisson_set_option, sn_poisson_solve,
+                      sn_poisson_set_boundary, sn_poisson_set_omega, sn_poisson_set_stop_rule, sn_poisson_solve_gravity, sn_poisson_solve_mg, sn_poisson_solve_mg_batch, sn_poisson_solve_mg_batch_host, sn_poisson_solve_mg_host, sn_poisson_set_option, sn_poisson_solve,
                       sn_poisson_solve_batch, sn_poisson_solve_batch_host, sn_poisson_solve_host,
                       sn_poisson_solve_sequence_host, sn_poisson_probe_l2, sn_poisson_version)
 from .solver import LevelSet, PoissonSolver, Weno

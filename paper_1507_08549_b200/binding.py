@@ -10,7 +10,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("SN_POISSON_LIB") or os.path.join(_HERE, "libsn_poisson.so")   # override: A/B builds
+LIB_PATH = os.path.join(_HERE, "libsn_poisson.so")       # the in-tree build, always (no environment override)
 
 # every symbol include/sn_poisson.h declares
 EXPORTS = (
@@ -19,7 +19,7 @@ EXPORTS = (
     "sn_poisson_set_stop_rule", "sn_poisson_solve_gravity", "sn_poisson_solve_mg", "sn_poisson_solve_mg_host", "sn_poisson_solve_mg_batch",
     "sn_poisson_destroy", "sn_poisson_gravity", "sn_poisson_set_omega", "sn_poisson_get_omega", "sn_poisson_get_moments",
     "sn_poisson_set_boundary", "sn_poisson_get_boundary", "sn_poisson_get_history", "sn_poisson_set_option",
-    "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version", "sn_poisson_moments_static",
+    "sn_poisson_get_stat", "sn_poisson_last_error", "sn_poisson_version", "sn_poisson_moments_static", "sn_poisson_solve_mg_batch_host",
 )
 
 
@@ -72,6 +72,9 @@ def load():
     lib.sn_poisson_solve_mg.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
     lib.sn_poisson_solve_mg_batch.restype = C.c_int
     lib.sn_poisson_solve_mg_batch.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, C.c_int, _vp, C.POINTER(sn_poisson_result)]
+    lib.sn_poisson_solve_mg_batch_host.restype = C.c_int
+    lib.sn_poisson_solve_mg_batch_host.argtypes = [_vp, C.c_int, _vp, _vp, C.c_double, C.c_int, _vp,
+                                                   C.POINTER(sn_poisson_result)]
     lib.sn_poisson_solve_mg_host.restype = sn_poisson_result
     lib.sn_poisson_solve_mg_host.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp]
     lib.sn_poisson_solve_batch.restype = C.c_int
@@ -192,6 +195,16 @@ def sn_poisson_solve_mg_batch(h, nbatch, rho_ptr, phi_ptr, tol, max_cycles, stre
     rc = load().sn_poisson_solve_mg_batch(h, int(nbatch), rho_ptr, phi_ptr, float(tol), int(max_cycles), stream or None, out)
     if rc != 0:
         raise SnPoissonError(f"sn_poisson_solve_mg_batch failed ({rc}): " + sn_poisson_last_error())
+    return list(out)
+
+
+def sn_poisson_solve_mg_batch_host(h, nbatch, rho_ptr, phi_ptr, tol, max_cycles, stream=0):
+    """Multigrid variant, nbatch independent solves, HOST addresses; returns a list of sn_poisson_result."""
+    out = (sn_poisson_result * int(nbatch))()
+    rc = load().sn_poisson_solve_mg_batch_host(h, int(nbatch), rho_ptr, phi_ptr, float(tol), int(max_cycles),
+                                               stream or None, out)
+    if rc != 0:
+        raise SnPoissonError(f"sn_poisson_solve_mg_batch_host failed ({rc}): " + sn_poisson_last_error())
     return list(out)
 
 

@@ -18,7 +18,6 @@ NVCC_FLAGS = [
     "-fmad=false",                              # pinned fp64 expression trees (R10)
     "-Xcompiler", "-fPIC,-ffp-contract=off,-O2",
 ]
-NVCC_FLAGS += os.environ.get("SN_NVCC_EXTRA", "").split()      # e.g. -DSNP_GROUP_ROWS_ROOMY=2 for an A/B build
 SHAPE_TUS = list(range(11)) + [100, 200]        # csrc/shapes.cuh: kNumResShapes resident shapes, blocked, dispatch
 
 
@@ -43,9 +42,12 @@ def _stale(target: str) -> bool:
     return any(os.path.getmtime(d) > t for d in _deps())
 
 
-def build(force: bool = False, verbose: bool = False, only=None) -> str:
-    """`only`: iterable of SNP_TU numbers to recompile (development shortcut; everything else must be up to date)."""
-    if not force and only is None and not _stale(LIB):
+def build(force: bool = False, verbose: bool = False, only=None, extra_flags=()) -> str:
+    """`only`: iterable of SNP_TU numbers to recompile (development shortcut; everything else must be up to date).
+    `extra_flags`: additional nvcc flags (A/B builds such as -DSNP_GROUP_ROWS_ROOMY=2).  Only the command line below
+    passes any -- from SN_NVCC_EXTRA --; the library callers (`__graft_entry__.build()`, the tests) never do, so the
+    environment cannot change what they build."""
+    if not force and only is None and not extra_flags and not _stale(LIB):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(OBJ, exist_ok=True)
@@ -57,7 +59,7 @@ def build(force: bool = False, verbose: bool = False, only=None) -> str:
                 continue
         elif not force and not _stale(obj):
             continue
-        todo.append([nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *extra, "-c", src, "-o", obj])
+        todo.append([nvcc, *NVCC_FLAGS, *extra_flags, *(["-Xptxas", "-v"] if verbose else []), *extra, "-c", src, "-o", obj])
 
     def run(cmd):
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -74,4 +76,5 @@ def build(force: bool = False, verbose: bool = False, only=None) -> str:
 
 if __name__ == "__main__":
     only = [a.split("=")[1].split(",") for a in sys.argv if a.startswith("--only=")]
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, only=only[0] if only else None))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, only=only[0] if only else None,
+                extra_flags=tuple(os.environ.get("SN_NVCC_EXTRA", "").split())))

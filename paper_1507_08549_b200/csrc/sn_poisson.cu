@@ -1322,30 +1322,45 @@ int sn_poisson_solve_mg_batch(sn_poisson* h, int nbatch, const double* rho, doub
     return solve_mg_impl(h, nbatch, rho, phi_inout, tol, max_cycles, (cudaStream_t)stream, out);
 }
 
+int sn_poisson_solve_mg_batch_host(sn_poisson* h, int nbatch, const double* rho_host, double* phi_inout_host, double tol,
+                                   int max_cycles, void* stream, sn_poisson_result* out) {
+    g_err.clear();
+    if (nbatch < 1 || !out) { set_err("nbatch < 1 or NULL out"); return -1; }
+    if (nbatch > 65535) { set_err("nbatch > 65535"); return -1; }
+    if (!check_solve_args(h, rho_host, phi_inout_host, tol, max_cycles, nbatch)) return -1;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)h->nr * h->nz * nbatch, bytes = sizeof(double) * n;
+    CU_TRY(cudaSetDevice(h->device));
+    if (int rc = ensure_stage(h, n)) return rc;
+    // rho on the caller's stream (the moments need it first), phi on the copy stream behind the moment / boundary
+    // kernels, waited for just before the first cycle; phi's download behind the last cycle, before the one sync
+    auto upload = [&]() -> int {
+        CU_TRY(cudaEventRecord(h->ev_io[0], st));
+        CU_TRY(cudaStreamWaitEvent(h->st_copy, h->ev_io[0], 0));
+        CU_TRY(cudaMemcpyAsync(h->d_rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st));
+        CU_TRY(cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, h->st_copy));
+        CU_TRY(cudaEventRecord(h->ev_io[1], h->st_copy));
+        return 0;
+    };
+    int rc = upload();
+    if (rc == 0) {
+        HostIO io;
+        io.wait_before_relax = h->ev_io[1];
+        io.d2h_dst = phi_inout_host; io.d2h_src = h->d_phi_stage; io.d2h_bytes = bytes;
+        rc = solve_mg_impl(h, nbatch, h->d_rho_stage, h->d_phi_stage, tol, max_cycles, st, out, &io);
+    }
+    if (rc) drain_host_io(h, st);        // a failed call may have left the uploads in flight: not past the return
+    return rc;
+}
+
 sn_poisson_result sn_poisson_solve_mg_host(sn_poisson* h, const double* rho_host, double* phi_inout_host, double tol,
                                            int max_cycles, void* stream) {
     g_err.clear();
     sn_poisson_result r = {0, -1, 0.0};
     if (!check_solve_args(h, rho_host, phi_inout_host, tol, max_cycles)) return r;
-    cudaStream_t st = (cudaStream_t)stream;
-    const size_t n = (size_t)h->nr * h->nz, bytes = sizeof(double) * n;
-    auto fail = [&](int rc) { r.status = rc; return r; };
-    if (cudaSetDevice(h->device) != cudaSuccess) { set_err("cudaSetDevice failed"); return fail(-2); }
-    if (int rc = ensure_stage(h, n)) return fail(rc);
-    if (cudaEventRecord(h->ev_io[0], st) != cudaSuccess || cudaStreamWaitEvent(h->st_copy, h->ev_io[0], 0) != cudaSuccess ||
-        cudaMemcpyAsync(h->d_rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaMemcpyAsync(h->d_phi_stage, phi_inout_host, bytes, cudaMemcpyHostToDevice, h->st_copy) != cudaSuccess ||
-        cudaEventRecord(h->ev_io[1], h->st_copy) != cudaSuccess) {
-        set_err("host staging failed: %s", cudaGetErrorString(cudaGetLastError()));
-        drain_host_io(h, st);
-        return fail(-2);
-    }
-    HostIO io;
-    io.wait_before_relax = h->ev_io[1];
-    io.d2h_dst = phi_inout_host; io.d2h_src = h->d_phi_stage; io.d2h_bytes = bytes;
     sn_poisson_result out = {0, 0, 0.0};
-    const int rc = solve_mg_impl(h, 1, h->d_rho_stage, h->d_phi_stage, tol, max_cycles, st, &out, &io);
-    if (rc) { drain_host_io(h, st); return fail(rc); }
+    const int rc = sn_poisson_solve_mg_batch_host(h, 1, rho_host, phi_inout_host, tol, max_cycles, stream, &out);
+    if (rc) { r.status = rc; return r; }
     return out;
 }
 

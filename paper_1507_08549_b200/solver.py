@@ -84,7 +84,16 @@ class PoissonSolver:
         return r
 
     def solve_mg_host(self, rho_np, phi_np, tol, max_cycles=60):
+        """HOST arrays, (nz, nr) -> one result, or (nbatch, nz, nr) -> a list (sn_poisson_solve_mg_batch_host)."""
         import torch
+        if getattr(rho_np, "ndim", 0) == 3:
+            nb = rho_np.shape[0]
+            self._check_host(rho_np, (nb, self.nz, self.nr))
+            self._check_host(phi_np, (nb, self.nz, self.nr), writeable=True)
+            res = B.sn_poisson_solve_mg_batch_host(self.h, nb, rho_np.ctypes.data, phi_np.ctypes.data, tol, max_cycles,
+                                                   torch.cuda.current_stream().cuda_stream)
+            self._raise_if_failed(res, "sn_poisson_solve_mg_batch_host")
+            return res
         self._check_host(rho_np, (self.nz, self.nr))
         self._check_host(phi_np, (self.nz, self.nr), writeable=True)
         r = B.sn_poisson_solve_mg_host(self.h, rho_np.ctypes.data, phi_np.ctypes.data, tol, max_cycles,

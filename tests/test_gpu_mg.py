@@ -157,6 +157,15 @@ def test_batch_members_equal_single_solves_and_the_oracle(P, torch_cuda, oracle)
     phi3 = torch.zeros_like(rho)
     res3 = s.solve_mg(rho, phi3, w0.tol, 3)
     assert all(r.sweeps == 3 and r.status == 1 for r in res3)
+    # the HOST-buffer batch entry (sn_poisson_solve_mg_batch_host, what bench.py's e2e of mg_cfg4a times): same bits,
+    # from pageable and from pinned arrays
+    rho_h = np.stack([m.rho for m in members])
+    for pin in (False, True):
+        rho_in = torch.from_numpy(rho_h).pin_memory().numpy() if pin else rho_h
+        phi_h = torch.zeros(rho_h.shape, dtype=torch.float64).pin_memory().numpy() if pin else np.zeros_like(rho_h)
+        res_h = s.solve_mg_host(rho_in, phi_h, w0.tol, 60)
+        assert [(r.sweeps, r.status, r.residual) for r in res_h] == [(r.sweeps, r.status, r.residual) for r in res]
+        assert np.array_equal(phi_h, got)
     s.close()
 
 

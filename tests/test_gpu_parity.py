@@ -929,6 +929,9 @@ def test_paper_literal_configuration(P, torch_cuda, oracle):
     phi = torch_cuda.zeros_like(rho)
     r = s.solve(rho, phi, 1e-8, 20000)
     assert r.status == 0 and ref["status"] == 0
+    # 500 = 4 x 125: only the box shapes with 4- or 2-row patches divide it; the planner must still keep phi on chip
+    # (bench.py's `paper500` row times exactly this solve)
+    assert s.stat("path") in (2, 3), s.stat("path")
     assert r.sweeps == ref["sweeps"] and abs(r.residual - ref["residual"]) <= 1e-6 * ref["residual"]
     assert relmax(phi.cpu().numpy(), ref["phi"]) <= REL
     ws = [W.cfg4a_member(b, 128) for b in range(4)]
