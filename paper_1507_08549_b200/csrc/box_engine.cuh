@@ -83,7 +83,19 @@ struct PollCtx {
     int* g_info;                 // Ctl::panic_tile, panic_arg
     int tile;
 };
-constexpr unsigned kPollBudget = 1u << 21;      // polls (each an L2 round trip or a nanosleep): ~1 s
+// The bound has two stages.  A poll count alone is a poor clock (a poll is an L2 round trip on an idle GPU but can be
+// far slower under a profiler's replay, a debugger or a time-sliced GPU), so the count only decides WHEN to start
+// looking at the clock: after kPollBudget polls (~1 s on an idle GPU) the wait notes %globaltimer and from then on
+// gives up only once kWatchdogMs more wall-clock milliseconds (2^20 ns units) have passed without the awaited word.
+constexpr unsigned kPollBudget = 1u << 21;
+constexpr unsigned kWatchdogMs = 20000;
+constexpr unsigned kPollTimed = 0x80000000u;    // top bit of the poll counter: stage two, low 31 bits = start time
+
+__device__ __forceinline__ unsigned watchdog_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return (unsigned)(t >> 20) & 0x7fffffffu;
+}
 
 __device__ __forceinline__ void trip_watchdog(const PollCtx& c, int code, int arg) {
     if (atomicCAS(c.g_panic, 0, code) == 0) {
@@ -95,9 +107,14 @@ __device__ __forceinline__ void trip_watchdog(const PollCtx& c, int code, int ar
 // true: stop waiting
 __device__ __forceinline__ bool poll_giveup(const PollCtx& c, unsigned& n, int code, int arg) {
     if (*c.quit || *c.s_panic) return true;
+    if (n & kPollTimed) {                                    // stage two: bounded by the clock (rare, slow path)
+        if (*(volatile int*)c.g_panic) { *c.s_panic = 1; return true; }
+        if (((watchdog_now() - n) & 0x7fffffffu) > kWatchdogMs) { trip_watchdog(c, code, arg); return true; }
+        return false;
+    }
     if ((++n & 63u) == 0u) {
         if (*(volatile int*)c.g_panic) { *c.s_panic = 1; return true; }
-        if (n > kPollBudget) { trip_watchdog(c, code, arg); return true; }
+        if (n > kPollBudget) n = kPollTimed | watchdog_now();
     }
     return false;
 }
